@@ -1,0 +1,291 @@
+/*
+ * asr_oracle.c -- CPU ORACLE (test infrastructure, NOT the product).
+ * See asr_oracle.h for the rules that govern this directory.
+ *
+ * Every function follows the passage it cites, in the paper's order, with no
+ * blocking, fusion or fast-forwarding: the simulator steps ONE engine
+ * iteration at a time and the selector is "sort everything, take k".
+ */
+#define _GNU_SOURCE
+#include "asr_oracle.h"
+
+#include <stdlib.h>
+#include <string.h>
+
+typedef __int128 i128;
+
+/* ------------------------------------------------------------------ */
+/* c1. comparator (readings S2-S6)                           */
+/* ------------------------------------------------------------------ */
+
+static int64_t est_of(const orc_req_t *r) {
+    /* PAPER.md:260  estimated_output = max(1, int(duration_s * kappa)) */
+    return r->est < 1 ? 1 : (int64_t)r->est;
+}
+
+static int64_t wait_of(const orc_req_t *r, int64_t now) {
+    /* PAPER.md:281  wait = now - req.arrival_time (never negative here) */
+    int64_t w = now - r->arrival_us;
+    return w < 0 ? 0 : w;
+}
+
+/* (arrival_us, idx) ascending: FCFS and every tie-break */
+static int earlier(const orc_req_t *a, int64_t ia, const orc_req_t *b,
+                   int64_t ib) {
+    if (a->arrival_us != b->arrival_us) return a->arrival_us < b->arrival_us;
+    return ia < ib;
+}
+
+int orc_better(const orc_req_t *a, int64_t ia, const orc_req_t *b, int64_t ib,
+               int policy, int64_t now) {
+    if (policy == ORC_FCFS) return earlier(a, ia, b, ib);
+    if (policy == ORC_SJF) {
+        /* PAPER.md:270,277 key (estimated_output_tokens, arrival_time,
+         * request_id); "earlier arrivals are prioritized" */
+        int64_t ea = est_of(a), eb = est_of(b);
+        if (ea != eb) return ea < eb;
+        return earlier(a, ia, b, ib);
+    }
+    /* HRRN: ratio (wait + est) / est, highest first.
+     * (wa+ea)/ea > (wb+eb)/eb  <=>  wa*eb > wb*ea   (all positive),
+     * evaluated exactly in 128-bit integers. */
+    i128 lhs = (i128)wait_of(a, now) * (i128)est_of(b);
+    i128 rhs = (i128)wait_of(b, now) * (i128)est_of(a);
+    if (lhs != rhs) return lhs > rhs;
+    return earlier(a, ia, b, ib);
+}
+
+typedef struct {
+    const orc_req_t *q;
+    int policy;
+    int64_t now;
+} sort_ctx_t;
+
+static int cmp_pos(const void *pa, const void *pb, void *vctx) {
+    const sort_ctx_t *c = (const sort_ctx_t *)vctx;
+    int64_t ia = *(const int64_t *)pa, ib = *(const int64_t *)pb;
+    if (ia == ib) return 0;
+    return orc_better(&c->q[ia], ia, &c->q[ib], ib, c->policy, c->now) ? -1 : 1;
+}
+
+/* Select = sort all n positions by the total order, output the first k. */
+int orc_select(const orc_req_t *q, int64_t n, int policy, int64_t now,
+               int32_t k, int32_t *out_idx) {
+    if (n < 0 || k < 0 || policy < 0 || policy > 2) return -1;
+    int64_t *pos = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
+    if (!pos) return -2;
+    for (int64_t i = 0; i < n; i++) pos[i] = i;
+    sort_ctx_t c = {q, policy, now};
+    qsort_r(pos, (size_t)n, sizeof(int64_t), cmp_pos, &c);
+    for (int32_t j = 0; j < k; j++) out_idx[j] = j < n ? (int32_t)pos[j] : -1;
+    free(pos);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* c2. simulator                                                       */
+/* ------------------------------------------------------------------ */
+
+int64_t orc_tokens(const orc_cost_t *cm, int32_t dur_ms) {
+    /* BASELINE.json configs[0]: tokens = 1 + 4*dur_ms/1000 (floor);
+     * 5 tokens per second of audio in the toy */
+    int64_t t = (int64_t)cm->tok_base +
+                ((int64_t)cm->tok_per_s * (int64_t)dur_ms) / 1000;
+    return t < 1 ? 1 : t;
+}
+
+int64_t orc_enc_cost(const orc_cost_t *cm, int32_t dur_ms) {
+    /* PAPER.md:51 near-constant encoder time per segment (+ linear term of
+     * BASELINE.json configs[0]: 20,000 + 2*dur_ms us) */
+    return cm->enc_base_us + cm->enc_per_ms_us * (int64_t)dur_ms;
+}
+
+/* order the waiting positions by the total order, at one fixed `now` */
+typedef struct {
+    const orc_req_t *trace;
+    int policy;
+    int64_t now;
+} wait_ctx_t;
+
+static int cmp_wait(const void *pa, const void *pb, void *vctx) {
+    const wait_ctx_t *c = (const wait_ctx_t *)vctx;
+    int64_t ia = *(const int64_t *)pa, ib = *(const int64_t *)pb;
+    if (ia == ib) return 0;
+    return orc_better(&c->trace[ia], ia, &c->trace[ib], ib, c->policy, c->now)
+               ? -1
+               : 1;
+}
+
+int orc_simulate(const orc_req_t *trace, int64_t n, int policy,
+                 const orc_cost_t *cm, int32_t slots, int64_t *lat,
+                 int64_t *ttft, int64_t *first_arrival_us,
+                 int64_t *last_done_us) {
+    if (n < 0 || slots < 1 || policy < 0 || policy > 2 || !cm) return -1;
+    if (first_arrival_us) *first_arrival_us = n > 0 ? trace[0].arrival_us : 0;
+    if (last_done_us) *last_done_us = 0;
+    if (n == 0) return 0;
+
+    int64_t *W = (int64_t *)malloc(sizeof(int64_t) * (size_t)n); /* waiting */
+    int64_t *R = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots); /* running idx */
+    int64_t *rem = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots);
+    if (!W || !R || !rem) {
+        free(W); free(R); free(rem);
+        return -2;
+    }
+    int64_t nW = 0, nR = 0, p = 0, done = 0, t = 0;
+
+    while (done < n) {
+        /* 1. ingest: arrivals at or before the iteration boundary (S13) */
+        while (p < n && trace[p].arrival_us <= t) W[nW++] = p++;
+        /* 2. idle server: clock jumps exactly to the next arrival (S14) */
+        if (nR == 0 && nW == 0) {
+            t = trace[p].arrival_us;
+            continue;
+        }
+        /* 3. admit the k best waiting requests into the free slots (S6:
+         *    one `now` = t for the whole step) */
+        int64_t free_slots = (int64_t)slots - nR;
+        int64_t k = free_slots < nW ? free_slots : nW;
+        int64_t enc_sum = 0;
+        int64_t first_new = nR;
+        if (k > 0) {
+            wait_ctx_t c = {trace, policy, t};
+            qsort_r(W, (size_t)nW, sizeof(int64_t), cmp_wait, &c);
+            for (int64_t j = 0; j < k; j++) {
+                int64_t i = W[j];
+                R[nR] = i;
+                rem[nR] = orc_tokens(cm, trace[i].dur_ms);
+                nR++;
+                enc_sum += orc_enc_cost(cm, trace[i].dur_ms); /* S15 */
+            }
+            memmove(W, W + k, sizeof(int64_t) * (size_t)(nW - k));
+            nW -= k;
+        }
+        /* 4. one engine iteration (PAPER.md:31 iteration-level scheduling):
+         *    encoders of the admitted + one decode step for everyone (S16) */
+        t += enc_sum + cm->iter_base_us + cm->iter_per_running_us * nR;
+        for (int64_t s = 0; s < nR; s++) rem[s] -= 1;
+        /* 5. record: first token of the admitted (S9), finished requests */
+        for (int64_t s = first_new; s < nR; s++)
+            ttft[R[s]] = t - trace[R[s]].arrival_us;
+        int64_t keep = 0;
+        for (int64_t s = 0; s < nR; s++) {
+            if (rem[s] == 0) {
+                lat[R[s]] = t - trace[R[s]].arrival_us; /* PAPER.md:100 E2EL */
+                done++;
+            } else {
+                R[keep] = R[s];
+                rem[keep] = rem[s];
+                keep++;
+            }
+        }
+        nR = keep;
+    }
+    if (last_done_us) *last_done_us = t;
+    free(W); free(R); free(rem);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* c3. nearest-rank percentile (S8)            */
+/* ------------------------------------------------------------------ */
+
+static int cmp_i64(const void *a, const void *b) {
+    int64_t x = *(const int64_t *)a, y = *(const int64_t *)b;
+    return (x > y) - (x < y);
+}
+
+int64_t orc_percentile(const int64_t *v, int64_t n, int32_t p) {
+    if (n <= 0 || p < 1 || p > 100) return -1;
+    int64_t *s = (int64_t *)malloc(sizeof(int64_t) * (size_t)n);
+    if (!s) return -1;
+    memcpy(s, v, sizeof(int64_t) * (size_t)n);
+    qsort(s, (size_t)n, sizeof(int64_t), cmp_i64);
+    /* 1-based rank ceil(p*n/100) */
+    int64_t rank = ((int64_t)p * n + 99) / 100;
+    int64_t r = s[rank - 1];
+    free(s);
+    return r;
+}
+
+/* ------------------------------------------------------------------ */
+/* c4. counter-based trace generator        */
+/* ------------------------------------------------------------------ */
+
+uint64_t orc_fmix64(uint64_t z) {
+    /* the output function of splitmix64 (Steele, Lea, Flood 2014) */
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+uint64_t orc_mix64(uint64_t seed, uint32_t stream, uint64_t i) {
+    /* a splitmix64 stream whose start state is a hash of (seed, stream);
+     * draw i is the (i+1)-th output of that stream */
+    uint64_t base = orc_fmix64(orc_fmix64(seed + 0x2545F4914F6CDD1DULL) +
+                               (uint64_t)stream * 0xD1B54A32D192ED03ULL);
+    return orc_fmix64(base + (i + 1) * 0x9E3779B97F4A7C15ULL);
+}
+
+/* T[hi] + ((T[hi+1]-T[hi]) * fr >> 32): 12-bit cell, 32-bit fraction */
+static uint64_t interp_tab(const uint32_t *T, uint64_t u) {
+    uint64_t hi = u >> 52;
+    uint64_t fr = (u >> 20) & 0xFFFFFFFFULL;
+    uint64_t lo_v = T[hi], hi_v = T[hi + 1];
+    return lo_v + (((hi_v - lo_v) * fr) >> 32);
+}
+
+static int clz64(uint64_t x) { /* x != 0 */
+    int c = 0;
+    while (!(x >> 63)) {
+        x <<= 1;
+        c++;
+    }
+    return c;
+}
+
+static int32_t draw_duration(uint64_t u, int32_t dist, const uint32_t *ln_dur) {
+    if (dist == ORC_DIST_UNIFORM) /* integer ms, uniform on [1000, 35000] */
+        return (int32_t)(1000 + (((u >> 32) * 34001ULL) >> 32));
+    return (int32_t)interp_tab(ln_dur, u); /* clipped lognormal quantile */
+}
+
+int orc_gen_trace(uint64_t seed, int32_t rate_mhz, int32_t dist, int64_t n,
+                  const uint32_t *ln_dur, const uint32_t *exp_t,
+                  orc_req_t *out) {
+    if (rate_mhz < 1 || n < 0 || dist < 0 || dist > 1) return -1;
+    /* Poisson process: exponential inter-arrival gaps */
+    uint64_t mean_gap_us = 1000000000ULL / (uint64_t)rate_mhz;
+    uint64_t ln2_q32 = exp_t[4096];
+    int64_t t = 0;
+    for (int64_t i = 0; i < n; i++) {
+        uint64_t u0 = orc_mix64(seed, 0, (uint64_t)i);
+        uint64_t u1 = orc_mix64(seed, 1, (uint64_t)i);
+        uint64_t u2 = orc_mix64(seed, 2, (uint64_t)i);
+        /* unit exponential in Q32: E = G*ln2 + E', G geometric(1/2),
+         * E' exponential truncated to [0, ln 2) by inverse CDF */
+        uint64_t e_q32 = (uint64_t)clz64(u0 | 1ULL) * ln2_q32 + interp_tab(exp_t, u1);
+        uint64_t gap = (uint64_t)(((unsigned __int128)e_q32 * mean_gap_us) >> 32);
+        t += (int64_t)gap; /* S18: first arrival = first gap after t = 0 */
+        out[i].arrival_us = t;
+        out[i].dur_ms = draw_duration(u2, dist, ln_dur);
+        out[i].est = out[i].dur_ms; /* S7: configs set est = dur_ms */
+    }
+    return 0;
+}
+
+/* config-5 queues: arrival uniform in [0, now), unsorted; lognormal dur */
+int orc_gen_queue(uint64_t seed, int64_t first, int64_t n, int64_t now,
+                  const uint32_t *ln_dur, orc_req_t *out) {
+    if (n < 0 || now < 1 || first < 0) return -1;
+    for (int64_t j = 0; j < n; j++) {
+        uint64_t i = (uint64_t)(first + j);
+        uint64_t u2 = orc_mix64(seed, 2, i);
+        uint64_t u3 = orc_mix64(seed, 3, i);
+        out[j].arrival_us =
+            (int64_t)(((unsigned __int128)u3 * (uint64_t)now) >> 64);
+        out[j].dur_ms = draw_duration(u2, ORC_DIST_LOGNORMAL, ln_dur);
+        out[j].est = out[j].dur_ms;
+    }
+    return 0;
+}

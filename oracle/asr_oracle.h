@@ -1,0 +1,87 @@
+/*
+ * asr_oracle.h -- CPU ORACLE (test infrastructure, NOT the product).
+ *
+ * A plain, slow, obviously-correct restatement of what the hot path computes,
+ * written from /root/reference/PAPER.md (arxiv 2603.11273) and the readings
+ * listed in DESIGN.md.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, link, import or run
+ * anything in this directory.  It shares no code, header, table generator or
+ * constant with the CUDA path under paper_2603_11273_b200/.
+ *
+ * All time is integer microseconds; every result is exact (no tolerance).
+ *
+ * Parity pins (tests/test_oracle_*.py, run with -m "not gpu"):
+ *   orc_better / orc_select   : pinned (brute force, invariants, hand ties)
+ *   orc_simulate              : pinned (Fig. 1 toy, brute force
+ *                               over orderings, closed forms, invariants)
+ *   orc_percentile            : pinned (textbook nearest-rank example)
+ *   orc_fmix64 / orc_mix64    : pinned (published splitmix64 known answers)
+ *   orc_gen_trace/orc_gen_queue: moments pinned to closed forms; the exact
+ *                               bit stream is a recipe of this repo
+ *                                -- the paper fixes
+ *                               only "Poisson, burstiness 1.0".
+ *   The paper's Table 1/2 trends: PARITY UNPINNED (real-system measurements).
+ */
+#ifndef ASR_ORACLE_H
+#define ASR_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* one request: PAPER.md:57-59 (Eq. 1: est = d * kappa) */
+typedef struct {
+    int64_t arrival_us; /* arrival time, integer microseconds */
+    int32_t dur_ms;     /* audio duration: drives the TRUE cost */
+    int32_t est;        /* scheduler's job-length estimate */
+} orc_req_t;
+
+/* cost model: PAPER.md:51-53 (encoder ~constant, decode linear in tokens) */
+typedef struct {
+    int64_t enc_base_us;
+    int64_t enc_per_ms_us;
+    int64_t iter_base_us;
+    int64_t iter_per_running_us;
+    int32_t tok_base;
+    int32_t tok_per_s;
+} orc_cost_t;
+
+enum { ORC_FCFS = 0, ORC_SJF = 1, ORC_HRRN = 2 };
+enum { ORC_DIST_LOGNORMAL = 0, ORC_DIST_UNIFORM = 1 };
+
+/* 1 if request a (at position ia) is strictly better than b (at ib). */
+int orc_better(const orc_req_t *a, int64_t ia, const orc_req_t *b, int64_t ib,
+               int policy, int64_t now);
+
+/* sort all n by orc_better, write the first min(k,n) positions, pad -1 */
+int orc_select(const orc_req_t *q, int64_t n, int policy, int64_t now,
+               int32_t k, int32_t *out_idx);
+
+/* iteration-level continuous-batching simulator, one iteration at a time */
+int orc_simulate(const orc_req_t *trace, int64_t n, int policy,
+                 const orc_cost_t *cm, int32_t slots, int64_t *lat,
+                 int64_t *ttft, int64_t *first_arrival_us,
+                 int64_t *last_done_us);
+
+/* nearest-rank percentile, p in [1,100]; n == 0 -> -1 */
+int64_t orc_percentile(const int64_t *v, int64_t n, int32_t p);
+
+/* tokens and encoder cost of one request (exposed for closed-form pins) */
+int64_t orc_tokens(const orc_cost_t *cm, int32_t dur_ms);
+int64_t orc_enc_cost(const orc_cost_t *cm, int32_t dur_ms);
+
+/* counter-based generator */
+uint64_t orc_fmix64(uint64_t z);
+uint64_t orc_mix64(uint64_t seed, uint32_t stream, uint64_t i);
+int orc_gen_trace(uint64_t seed, int32_t rate_mhz, int32_t dist, int64_t n,
+                  const uint32_t *ln_dur /*[4097]*/,
+                  const uint32_t *exp_t /*[4097]*/, orc_req_t *out);
+int orc_gen_queue(uint64_t seed, int64_t first, int64_t n, int64_t now,
+                  const uint32_t *ln_dur /*[4097]*/, orc_req_t *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
