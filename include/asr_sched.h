@@ -1,0 +1,234 @@
+/*
+ * asr_sched.h -- C ABI of the B200-native duration-aware ASR scheduling hot path
+ * (arxiv 2603.11273, "Duration Aware Scheduling for ASR Serving under Workload
+ * Drift").  Citations are /root/reference/PAPER.md:<line>.
+ *
+ * The library holds hand-written sm_100a CUDA kernels for
+ *   a1  trace generation          (Poisson arrivals; durations PAPER.md:80,96)
+ *   a2  priority keys             (FCFS PAPER.md:13; SJF PAPER.md:63,270,277;
+ *                                  HRRN PAPER.md:67-72,279-282)
+ *   a3  batched top-k select      (the paper's heap pop / O(n) scan)
+ *   a4  continuous-batching simulator step (iteration-level scheduling, PAPER.md:31;
+ *                                  encoder ~constant + decode linear in tokens)
+ *   a5  per-request E2E latency and TTFT
+ *   a6  segmented nearest-rank percentiles + throughput inputs
+ *
+ * CONVENTIONS (apply to every call unless the call says otherwise)
+ *  - Pointers marked DEVICE are device addresses allocated and owned by the
+ *    caller; pointers marked HOST are ordinary host addresses read during the
+ *    call.  The library never allocates or frees caller-visible memory; scratch
+ *    comes from the caller-supplied DEVICE `workspace` (size it with
+ *    asr_sched_workspace_bytes; its contents need no initialisation).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *    Calls only enqueue work on it and return without synchronising; outputs
+ *    are valid once the caller has synchronised the stream.  The *_host entry
+ *    points are the exception: they are synchronous and take HOST buffers.
+ *  - Return value: 0 success; -1 invalid argument (null pointer, negative size,
+ *    unknown policy, slots < 1, workspace too small); -2 CUDA runtime error
+ *    (text via asr_sched_last_error); -3 unsupported shape (exceeds a limit
+ *    stated at the call).  No exception crosses the ABI, nothing is printed.
+ *  - There is no CPU fallback: without a CUDA device every compute call
+ *    returns -2.
+ *  - All times are integer microseconds.  Documented preconditions (not
+ *    checked on the device): 0 <= arrival_us < 2^38, now < 2^38, est <= 2^24,
+ *    so that wait * est < 2^62 fits int64.  est < 1 is read as 1
+ *    (PAPER.md:260 max(1, .)); arrival_us > now is read as wait = 0.
+ *
+ * TOTAL ORDER better(a, b, now) used by select and by the simulator's admit
+ * step (exactly one correct answer everywhere; idx = position in the input):
+ *   FCFS  (arrival_us, idx) ascending
+ *   SJF   (max(est,1), arrival_us, idx) ascending
+ *   HRRN  wait_a*est_b > wait_b*est_a, wait = max(now-arrival_us,0), exact in
+ *         int64 (equivalent to comparing (wait+est)/est);
+ *         equal products -> (arrival_us, idx) ascending
+ */
+#ifndef ASR_SCHED_H
+#define ASR_SCHED_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ASR_SCHED_VERSION 100
+
+enum { ASR_FCFS = 0, ASR_SJF = 1, ASR_HRRN = 2 };
+enum { ASR_DIST_LOGNORMAL = 0, ASR_DIST_UNIFORM = 1 };
+enum { ASR_OK = 0, ASR_EINVAL = -1, ASR_ECUDA = -2, ASR_EUNSUPPORTED = -3 };
+
+/* one request, 16 bytes, read with one 128-bit load */
+typedef struct {
+    int64_t arrival_us; /* arrival time */
+    int32_t dur_ms;     /* audio duration: drives the TRUE cost (tokens, encoder) */
+    int32_t est;        /* scheduler's job-length estimate, est = max(1,int(d*kappa)) */
+} asr_req_t;
+
+/* cost of serving:  tokens(d) = max(1, tok_base + tok_per_s*d/1000),
+ * admission costs enc_base_us + enc_per_ms_us*d once, an engine iteration costs
+ * iter_base_us + iter_per_running_us*|running| and emits one token per running request */
+typedef struct {
+    int64_t enc_base_us;
+    int64_t enc_per_ms_us;
+    int64_t iter_base_us;
+    int64_t iter_per_running_us;
+    int32_t tok_base;
+    int32_t tok_per_s;
+} asr_cost_model_t; /* 40 bytes */
+
+/* one replica of a batched simulation, 32 bytes */
+typedef struct {
+    int64_t trace_off; /* first record of this replica's trace in `traces` */
+    int64_t out_off;   /* first element of this replica in out_lat/out_ttft  */
+    int32_t n;         /* requests in the trace (sorted by arrival_us)       */
+    int32_t policy;    /* ASR_FCFS / ASR_SJF / ASR_HRRN                     */
+    int32_t slots;     /* continuous-batching slots, 1..256                 */
+    int32_t cm_id;     /* index into `cms`                                  */
+} asr_replica_t;
+
+/* per-replica summary, 56 bytes; throughput = n_done*1e6/(last_done_us-first_arrival_us)
+ * is left to the caller so the ABI stays integer */
+typedef struct {
+    int64_t p50_e2e_us, p90_e2e_us;   /* nearest-rank */
+    int64_t p50_ttft_us, p90_ttft_us;
+    int64_t first_arrival_us, last_done_us;
+    int64_t n_done;                   /* -1: the replica descriptor was invalid */
+} asr_summary_t;
+
+/* one trace to generate, 16 bytes */
+typedef struct {
+    uint64_t seed;
+    int32_t rate_mhz; /* arrival rate in milli-requests/s; mean gap = 1e9/rate_mhz us */
+    int32_t dist;     /* ASR_DIST_* */
+} asr_trace_spec_t;
+
+/* quantile tables the generator interpolates (inputs, built by the caller):
+ * ln_dur[j] = duration quantile (ms) at probability j/4096;
+ * exp_t[j]  = round(-ln(1 - j/8192) * 2^32), exp_t[4096] = ln 2 in Q32 */
+typedef struct {
+    uint32_t ln_dur[4097];
+    uint32_t exp_t[4097];
+} asr_tables_t;
+
+/* ------------------------------------------------------------------ */
+/* a2+a3  priority keys and top-k select                               */
+/* ------------------------------------------------------------------ */
+
+/* One queue of n records.  Writes k indices (positions in `keys`), best
+ * first; if k > n the tail is -1.
+ *   keys DEVICE [n]; out_idx DEVICE [k]; workspace DEVICE.
+ * Limits: 0 <= k <= 32 (else -3); n < 2^31. */
+int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy, int64_t now,
+                     int32_t k, int32_t *out_idx, void *workspace,
+                     size_t workspace_bytes, void *stream);
+
+/* n_queues independent queues; queue q is keys[q*q_len .. q*q_len+q_len) of
+ * which the first q_count[q] (or q_len if q_count is NULL) records are valid.
+ * Indices are local to the queue; out_idx[q*k + j] is the j-th best, -1 padded.
+ * now_per_queue (nullable) overrides `now` per queue.
+ *   keys DEVICE [n_queues*q_len]; q_count, now_per_queue DEVICE [n_queues] or NULL;
+ *   out_idx DEVICE [n_queues*k].  Limits: 0 <= k <= 32, q_len < 2^31. */
+int asr_sched_select_batched(const asr_req_t *keys, int32_t n_queues, int32_t q_len,
+                             const int32_t *q_count, int32_t policy, int64_t now,
+                             const int64_t *now_per_queue, int32_t k, int32_t *out_idx,
+                             void *stream);
+
+/* ------------------------------------------------------------------ */
+/* a4+a5+a6  simulator                                                 */
+/* ------------------------------------------------------------------ */
+
+/* One replica.  trace DEVICE [n] sorted by arrival_us non-decreasing
+ * (precondition); cm HOST; out_lat/out_ttft DEVICE [n] or NULL; out_summary
+ * DEVICE [1] or NULL; workspace DEVICE.  slots in 1..256 (else -3). */
+int asr_sched_simulate(const asr_req_t *trace, int64_t n, int32_t policy,
+                       const asr_cost_model_t *cm, int32_t slots, int64_t *out_lat,
+                       int64_t *out_ttft, asr_summary_t *out_summary, void *workspace,
+                       size_t workspace_bytes, void *stream);
+
+/* n_replicas independent replicas (seed x rate x policy), one warp each.
+ *   traces DEVICE; replicas DEVICE [n_replicas]; cms DEVICE [n_cms];
+ *   out_lat/out_ttft DEVICE [total_requests] indexed by replica.out_off, or both
+ *   NULL for summary-only mode (the arrays then live in the workspace);
+ *   out_summary DEVICE [n_replicas] or NULL.
+ * total_requests = max over replicas of out_off + n (HOST value; the regions
+ * [out_off, out_off+n) must be disjoint); max_slots = an upper bound of
+ * replica.slots (HOST value, 1..256, picks the kernel instantiation).  A
+ * replica with an invalid descriptor (or slots > max_slots) gets n_done = -1
+ * and no other output.  Further preconditions: dur_ms <= 2^24, every cost
+ * >= 0 and one engine iteration < 2^31 us. */
+int asr_sched_simulate_batched(const asr_req_t *traces, const asr_replica_t *replicas,
+                               int32_t n_replicas, const asr_cost_model_t *cms,
+                               int32_t n_cms, int64_t total_requests, int32_t max_slots,
+                               int64_t *out_lat, int64_t *out_ttft,
+                               asr_summary_t *out_summary, void *workspace,
+                               size_t workspace_bytes, void *stream);
+
+/* Segmented nearest-rank percentiles: segment s is values[seg_off[s] ..
+ * seg_off[s+1]); out[s*n_pct + j] = element of rank ceil(pcts[j]*N/100) of the
+ * sorted segment, -1 for an empty segment.  `values` is not modified.
+ *   values DEVICE; seg_off DEVICE [n_seg+1]; pcts HOST [n_pct], each 1..100,
+ *   n_pct <= 8; out DEVICE [n_seg*n_pct]. */
+int asr_sched_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg,
+                          const int32_t *pcts, int32_t n_pct, int64_t *out,
+                          void *workspace, size_t workspace_bytes, void *stream);
+
+/* ------------------------------------------------------------------ */
+/* a1  integer-only counter-based trace generator                      */
+/* ------------------------------------------------------------------ */
+
+/* Poisson arrivals (exponential gaps, inclusive prefix sum) and durations
+ * (table quantile or uniform integer ms on [1000, 35000]); est = dur_ms.
+ *   tables DEVICE; out DEVICE [n]. */
+int asr_sched_gen_trace(uint64_t seed, int32_t rate_mhz, int32_t dist, int64_t n,
+                        const asr_tables_t *tables, asr_req_t *out, void *stream);
+
+/* n_traces traces of n_per_trace records each; trace t is written at
+ * out[t*n_per_trace ..).  specs DEVICE [n_traces]. */
+int asr_sched_gen_trace_batched(const asr_trace_spec_t *specs, int32_t n_traces,
+                                int64_t n_per_trace, const asr_tables_t *tables,
+                                asr_req_t *out, void *stream);
+
+/* Unsorted waiting queues of the standalone select workload: record i (global
+ * counter first+i) has arrival_us uniform in [0, now), dur_ms from ln_dur. */
+int asr_sched_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now,
+                         const asr_tables_t *tables, asr_req_t *out, void *stream);
+
+/* ------------------------------------------------------------------ */
+/* synchronous HOST-buffer entry points (the end-to-end calls)         */
+/* ------------------------------------------------------------------ */
+
+/* Replica sweep from host descriptors: generates n_traces traces, simulates
+ * every trace under each of the n_policies policies (replica index =
+ * t*n_policies + j) with one cost model and slot count, and returns the
+ * per-replica summaries.  All pointers HOST.  Device scratch is allocated and
+ * released inside the call. */
+int asr_sched_sweep_host(const asr_trace_spec_t *specs, int32_t n_traces,
+                         int64_t n_per_trace, const asr_tables_t *tables,
+                         const int32_t *policies, int32_t n_policies, int32_t slots,
+                         const asr_cost_model_t *cm, asr_summary_t *out_summary);
+
+/* asr_sched_select_batched with HOST keys / out_idx (q_count, now_per_queue
+ * not supported: pass full queues). */
+int asr_sched_select_host(const asr_req_t *keys, int32_t n_queues, int32_t q_len,
+                          int32_t policy, int64_t now, int32_t k, int32_t *out_idx);
+
+/* ------------------------------------------------------------------ */
+/* helpers                                                             */
+/* ------------------------------------------------------------------ */
+
+enum { ASR_OP_SELECT = 0, ASR_OP_SIMULATE = 1, ASR_OP_PERCENTILES = 2 };
+/* Workspace bytes needed.  SELECT: a = n, b = k.  SIMULATE: a = total_requests,
+ * b = n_replicas, c = 1 if summary-only (out_lat/out_ttft NULL) else 0.
+ * PERCENTILES: a = total values, b = n_seg.  Returns 0 for an unknown op. */
+size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c);
+
+const char *asr_sched_last_error(void); /* thread-local, never NULL */
+int asr_sched_version(void);
+/* number of kernels this library has launched in this process (monotonic) */
+int64_t asr_sched_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ASR_SCHED_H */

@@ -1,0 +1,323 @@
+// api.cu -- C ABI of libasr_sched (include/asr_sched.h): argument checks,
+// workspace carving, launch sequencing.  No compute happens on the host.
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "launchers.cuh"
+
+namespace asr {
+
+static thread_local char g_err[512] = "";
+static std::atomic<long long> g_launches{0};
+
+void set_error(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int check_launch(const char *what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        set_error("%s: %s", what, cudaGetErrorString(e));
+        return ASR_ECUDA;
+    }
+    return ASR_OK;
+}
+
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct SimWorkspace {
+    size_t bm_off_bytes, bitmap_bytes, lat_bytes, total;
+};
+
+static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summary_only) {
+    SimWorkspace w;
+    w.bm_off_bytes = align_up(sizeof(int64_t) * (size_t)(n_replicas + 1));
+    w.bitmap_bytes = align_up(sizeof(uint32_t) * (size_t)(total_requests / 32 + 2 * n_replicas + 2));
+    w.lat_bytes = summary_only ? align_up(sizeof(int64_t) * (size_t)total_requests) : 0;
+    w.total = w.bm_off_bytes + w.bitmap_bytes + 2 * w.lat_bytes;
+    return w;
+}
+
+}  // namespace asr
+
+using namespace asr;
+
+#define CUDA_TRY(expr, what)                                         \
+    do {                                                             \
+        cudaError_t _e = (expr);                                     \
+        if (_e != cudaSuccess) {                                     \
+            set_error("%s: %s", what, cudaGetErrorString(_e));       \
+            return ASR_ECUDA;                                        \
+        }                                                            \
+    } while (0)
+
+extern "C" const char *asr_sched_last_error(void) { return g_err; }
+extern "C" int asr_sched_version(void) { return ASR_SCHED_VERSION; }
+extern "C" int64_t asr_sched_launch_count(void) { return (int64_t)g_launches.load(); }
+
+extern "C" size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c) {
+    if (a < 0 || b < 0) return 0;
+    switch (op) {
+        case ASR_OP_SELECT: return select_workspace_bytes(a, b);
+        case ASR_OP_SIMULATE: return sim_ws(a, b, c != 0).total + 512;   // + descriptors of the single-replica call
+        case ASR_OP_PERCENTILES: return 0;
+    }
+    return 0;
+}
+
+extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_replica_t *replicas,
+                                          int32_t n_replicas, const asr_cost_model_t *cms, int32_t n_cms,
+                                          int64_t total_requests, int32_t max_slots, int64_t *out_lat,
+                                          int64_t *out_ttft, asr_summary_t *out_summary, void *workspace,
+                                          size_t workspace_bytes, void *stream) {
+    if (n_replicas < 0 || n_cms < 1 || total_requests < 0 || max_slots < 1) {
+        set_error("simulate_batched: bad argument (n_replicas=%d n_cms=%d total=%lld max_slots=%d)", n_replicas,
+                  n_cms, (long long)total_requests, max_slots);
+        return ASR_EINVAL;
+    }
+    if (max_slots > 256) {
+        set_error("simulate_batched: max_slots=%d exceeds the limit 256", max_slots);
+        return ASR_EUNSUPPORTED;
+    }
+    if (n_replicas == 0) return ASR_OK;
+    if (!replicas || !cms || (!traces && total_requests > 0) || ((out_lat == nullptr) != (out_ttft == nullptr))) {
+        set_error("simulate_batched: null pointer (out_lat and out_ttft must both be given or both be NULL)");
+        return ASR_EINVAL;
+    }
+    const bool summary_only = out_lat == nullptr;
+    if (summary_only && !out_summary) {
+        set_error("simulate_batched: nothing to output");
+        return ASR_EINVAL;
+    }
+    const SimWorkspace w = sim_ws(total_requests, n_replicas, summary_only);
+    if (!workspace || workspace_bytes < w.total) {
+        set_error("simulate_batched: workspace too small (%zu < %zu)", workspace_bytes, w.total);
+        return ASR_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    int64_t *bm_off = (int64_t *)ws;
+    uint32_t *bitmap = (uint32_t *)(ws + w.bm_off_bytes);
+    if (summary_only) {
+        out_lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes);
+        out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.lat_bytes);
+    }
+    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, st);
+    if (rc) return rc;
+    SimArgs a{traces, replicas, cms, bm_off, bitmap, out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms};
+    rc = launch_simulate(a, max_slots, st);
+    if (rc) return rc;
+    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
+    return rc;
+}
+
+extern "C" int asr_sched_simulate(const asr_req_t *trace, int64_t n, int32_t policy, const asr_cost_model_t *cm,
+                                  int32_t slots, int64_t *out_lat, int64_t *out_ttft, asr_summary_t *out_summary,
+                                  void *workspace, size_t workspace_bytes, void *stream) {
+    if (n < 0 || n >= (1ll << 31) || policy < 0 || policy > 2 || slots < 1 || !cm) {
+        set_error("simulate: bad argument (n=%lld policy=%d slots=%d)", (long long)n, policy, slots);
+        return ASR_EINVAL;
+    }
+    if (slots > 256) {
+        set_error("simulate: slots=%d exceeds the limit 256", slots);
+        return ASR_EUNSUPPORTED;
+    }
+    // the single-replica call is the batched call with descriptors staged in the workspace
+    const size_t head = 256 + 256;   // asr_replica_t + asr_cost_model_t, each in its own 256 B line
+    const bool summary_only = out_lat == nullptr;
+    const size_t need = head + sim_ws(n, 1, summary_only).total;
+    if (!workspace || workspace_bytes < need) {
+        set_error("simulate: workspace too small (%zu < %zu)", workspace_bytes, need);
+        return ASR_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    asr_replica_t rep;
+    rep.trace_off = 0;
+    rep.out_off = 0;
+    rep.n = (int32_t)n;
+    rep.policy = policy;
+    rep.slots = slots;
+    rep.cm_id = 0;
+    char *ws = (char *)workspace;
+    CUDA_TRY(cudaMemcpyAsync(ws, &rep, sizeof(rep), cudaMemcpyHostToDevice, st), "simulate: upload replica");
+    CUDA_TRY(cudaMemcpyAsync(ws + 256, cm, sizeof(*cm), cudaMemcpyHostToDevice, st), "simulate: upload cost model");
+    // rep/cm are stack temporaries: pageable copies are staged before the call returns
+    return asr_sched_simulate_batched(trace, (const asr_replica_t *)ws, 1, (const asr_cost_model_t *)(ws + 256), 1,
+                                      n, slots, out_lat, out_ttft, out_summary, ws + head, workspace_bytes - head,
+                                      stream);
+}
+
+extern "C" int asr_sched_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg,
+                                     const int32_t *pcts, int32_t n_pct, int64_t *out, void *workspace,
+                                     size_t workspace_bytes, void *stream) {
+    (void)workspace;
+    (void)workspace_bytes;
+    if (n_seg < 0 || n_pct < 0 || (n_pct > 0 && !pcts)) {
+        set_error("percentiles: bad argument (n_seg=%d n_pct=%d)", n_seg, n_pct);
+        return ASR_EINVAL;
+    }
+    if (n_pct > 8) {
+        set_error("percentiles: n_pct=%d exceeds the limit 8", n_pct);
+        return ASR_EUNSUPPORTED;
+    }
+    for (int j = 0; j < n_pct; ++j)
+        if (pcts[j] < 1 || pcts[j] > 100) {
+            set_error("percentiles: pcts[%d]=%d outside 1..100", j, pcts[j]);
+            return ASR_EINVAL;
+        }
+    if (n_seg == 0 || n_pct == 0) return ASR_OK;
+    if (!seg_off || !out) {
+        set_error("percentiles: null pointer");
+        return ASR_EINVAL;
+    }
+    return launch_percentiles(values, seg_off, n_seg, pcts, n_pct, out, (cudaStream_t)stream);
+}
+
+extern "C" int asr_sched_gen_trace(uint64_t seed, int32_t rate_mhz, int32_t dist, int64_t n,
+                                   const asr_tables_t *tables, asr_req_t *out, void *stream) {
+    if (rate_mhz < 1 || dist < 0 || dist > 1 || n < 0 || !tables || (!out && n > 0)) {
+        set_error("gen_trace: bad argument (rate_mhz=%d dist=%d n=%lld)", rate_mhz, dist, (long long)n);
+        return ASR_EINVAL;
+    }
+    asr_trace_spec_t one{seed, rate_mhz, dist};
+    return launch_gen_trace(nullptr, one, 1, n, tables, out, (cudaStream_t)stream);
+}
+
+extern "C" int asr_sched_gen_trace_batched(const asr_trace_spec_t *specs, int32_t n_traces, int64_t n_per_trace,
+                                           const asr_tables_t *tables, asr_req_t *out, void *stream) {
+    if (n_traces < 0 || n_per_trace < 0 || !tables || ((!specs || !out) && n_traces > 0 && n_per_trace > 0)) {
+        set_error("gen_trace_batched: bad argument (n_traces=%d n_per_trace=%lld)", n_traces, (long long)n_per_trace);
+        return ASR_EINVAL;
+    }
+    asr_trace_spec_t none{0, 0, 0};
+    return launch_gen_trace(specs, none, n_traces, n_per_trace, tables, out, (cudaStream_t)stream);
+}
+
+extern "C" int asr_sched_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now,
+                                    const asr_tables_t *tables, asr_req_t *out, void *stream) {
+    if (first < 0 || n < 0 || now < 1 || !tables || (!out && n > 0)) {
+        set_error("gen_queues: bad argument (first=%lld n=%lld now=%lld)", (long long)first, (long long)n,
+                  (long long)now);
+        return ASR_EINVAL;
+    }
+    return launch_gen_queues(seed, first, n, now, tables, out, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------
+// synchronous HOST-buffer entry points
+// ---------------------------------------------------------------------------
+namespace {
+struct DevBuf {
+    void *p = nullptr;
+    ~DevBuf() {
+        if (p) cudaFree(p);
+    }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 1); }
+};
+
+__global__ void build_sweep_replicas_kernel(asr_replica_t *rep, int32_t n_traces, int64_t n_per_trace,
+                                            int32_t n_policies, int32_t slots, const int32_t *policies) {
+    const int64_t total = (int64_t)n_traces * n_policies;
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < total; r += (int64_t)gridDim.x * blockDim.x) {
+        asr_replica_t x;
+        x.trace_off = (r / n_policies) * n_per_trace;
+        x.out_off = r * n_per_trace;
+        x.n = (int32_t)n_per_trace;
+        x.policy = policies[r % n_policies];
+        x.slots = slots;
+        x.cm_id = 0;
+        rep[r] = x;
+    }
+}
+}  // namespace
+
+extern "C" int asr_sched_sweep_host(const asr_trace_spec_t *specs, int32_t n_traces, int64_t n_per_trace,
+                                    const asr_tables_t *tables, const int32_t *policies, int32_t n_policies,
+                                    int32_t slots, const asr_cost_model_t *cm, asr_summary_t *out_summary) {
+    if (n_traces < 0 || n_per_trace < 0 || n_per_trace >= (1ll << 31) || n_policies < 1 || n_policies > 16 ||
+        slots < 1 || !specs || !tables || !policies || !cm || !out_summary) {
+        set_error("sweep_host: bad argument");
+        return ASR_EINVAL;
+    }
+    if (slots > 256) {
+        set_error("sweep_host: slots=%d exceeds the limit 256", slots);
+        return ASR_EUNSUPPORTED;
+    }
+    if (n_traces == 0) return ASR_OK;
+    const int64_t n_rep = (int64_t)n_traces * n_policies;
+    const int64_t total = n_rep * n_per_trace;
+    if (n_rep >= (1ll << 31)) {
+        set_error("sweep_host: too many replicas");
+        return ASR_EUNSUPPORTED;
+    }
+    DevBuf d_specs, d_tables, d_traces, d_rep, d_cm, d_pol, d_sum, d_ws;
+    const size_t ws_bytes = sim_ws(total, n_rep, true).total;
+    CUDA_TRY(d_specs.alloc(sizeof(asr_trace_spec_t) * (size_t)n_traces), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_tables.alloc(sizeof(asr_tables_t)), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_traces.alloc(sizeof(asr_req_t) * (size_t)n_traces * (size_t)n_per_trace), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_rep.alloc(sizeof(asr_replica_t) * (size_t)n_rep), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_cm.alloc(sizeof(asr_cost_model_t)), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_pol.alloc(sizeof(int32_t) * (size_t)n_policies), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_sum.alloc(sizeof(asr_summary_t) * (size_t)n_rep), "sweep_host: cudaMalloc");
+    CUDA_TRY(d_ws.alloc(ws_bytes), "sweep_host: cudaMalloc workspace");
+    cudaStream_t st = nullptr;
+    CUDA_TRY(cudaMemcpyAsync(d_specs.p, specs, sizeof(asr_trace_spec_t) * (size_t)n_traces, cudaMemcpyHostToDevice, st),
+             "sweep_host: H2D specs");
+    CUDA_TRY(cudaMemcpyAsync(d_tables.p, tables, sizeof(asr_tables_t), cudaMemcpyHostToDevice, st), "sweep_host: H2D tables");
+    CUDA_TRY(cudaMemcpyAsync(d_cm.p, cm, sizeof(asr_cost_model_t), cudaMemcpyHostToDevice, st), "sweep_host: H2D cm");
+    CUDA_TRY(cudaMemcpyAsync(d_pol.p, policies, sizeof(int32_t) * (size_t)n_policies, cudaMemcpyHostToDevice, st),
+             "sweep_host: H2D policies");
+    int rc = asr_sched_gen_trace_batched((const asr_trace_spec_t *)d_specs.p, n_traces, n_per_trace,
+                                         (const asr_tables_t *)d_tables.p, (asr_req_t *)d_traces.p, st);
+    if (rc) return rc;
+    build_sweep_replicas_kernel<<<(int)((n_rep + 255) / 256 < 1184 ? (n_rep + 255) / 256 : 1184), 256, 0, st>>>(
+        (asr_replica_t *)d_rep.p, n_traces, n_per_trace, n_policies, slots, (const int32_t *)d_pol.p);
+    count_launch();
+    rc = check_launch("build_sweep_replicas_kernel");
+    if (rc) return rc;
+    rc = asr_sched_simulate_batched((const asr_req_t *)d_traces.p, (const asr_replica_t *)d_rep.p, (int32_t)n_rep,
+                                    (const asr_cost_model_t *)d_cm.p, 1, total, slots, nullptr, nullptr,
+                                    (asr_summary_t *)d_sum.p, d_ws.p, ws_bytes, st);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out_summary, d_sum.p, sizeof(asr_summary_t) * (size_t)n_rep, cudaMemcpyDeviceToHost, st),
+             "sweep_host: D2H summaries");
+    CUDA_TRY(cudaStreamSynchronize(st), "sweep_host: synchronize");
+    return ASR_OK;
+}
+
+extern "C" int asr_sched_select_host(const asr_req_t *keys, int32_t n_queues, int32_t q_len, int32_t policy,
+                                     int64_t now, int32_t k, int32_t *out_idx) {
+    if (n_queues < 0 || q_len < 0 || k < 0 || policy < 0 || policy > 2) {
+        set_error("select_host: bad argument");
+        return ASR_EINVAL;
+    }
+    if (k > 32) {
+        set_error("select_host: k=%d exceeds the limit 32", k);
+        return ASR_EUNSUPPORTED;
+    }
+    if (n_queues == 0 || k == 0) return ASR_OK;
+    if ((!keys && q_len > 0) || !out_idx) {
+        set_error("select_host: null pointer");
+        return ASR_EINVAL;
+    }
+    DevBuf d_keys, d_out;
+    const size_t kb = sizeof(asr_req_t) * (size_t)n_queues * (size_t)q_len;
+    const size_t ob = sizeof(int32_t) * (size_t)n_queues * (size_t)k;
+    CUDA_TRY(d_keys.alloc(kb), "select_host: cudaMalloc");
+    CUDA_TRY(d_out.alloc(ob), "select_host: cudaMalloc");
+    cudaStream_t st = nullptr;
+    if (kb) CUDA_TRY(cudaMemcpyAsync(d_keys.p, keys, kb, cudaMemcpyHostToDevice, st), "select_host: H2D keys");
+    int rc = asr_sched_select_batched((const asr_req_t *)d_keys.p, n_queues, q_len, nullptr, policy, now, nullptr, k,
+                                      (int32_t *)d_out.p, st);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out_idx, d_out.p, ob, cudaMemcpyDeviceToHost, st), "select_host: D2H indices");
+    CUDA_TRY(cudaStreamSynchronize(st), "select_host: synchronize");
+    return ASR_OK;
+}

@@ -1,0 +1,102 @@
+// common.cuh -- device helpers shared by the sm_100a kernels of libasr_sched.
+// Product code: shares nothing with the CPU checker used by the tests.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "asr_sched.h"
+
+#define ASR_FULL_MASK 0xFFFFFFFFu
+
+namespace asr {
+
+// ---- host-side error plumbing (api.cu) ------------------------------------
+void set_error(const char *fmt, ...);
+int check_launch(const char *what);   // cudaGetLastError -> ASR_OK / ASR_ECUDA
+void count_launch(int n = 1);
+
+// ---- 128-bit record access -------------------------------------------------
+struct __align__(16) Rec {
+    int64_t arrival_us;
+    int32_t dur_ms;
+    int32_t est;
+};
+static_assert(sizeof(Rec) == sizeof(asr_req_t), "record layout");
+
+// streaming load: read once, keep out of L1
+__device__ __forceinline__ Rec ld_stream(const asr_req_t *p) {
+    int4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p));
+    Rec r;
+    r.arrival_us = (int64_t)(((uint64_t)(uint32_t)v.y << 32) | (uint32_t)v.x);
+    r.dur_ms = v.z;
+    r.est = v.w;
+    return r;
+}
+
+// cached load (trace windows that are re-read by the simulator)
+__device__ __forceinline__ Rec ld_cached(const asr_req_t *p) {
+    int4 v = __ldg(reinterpret_cast<const int4 *>(p));
+    Rec r;
+    r.arrival_us = (int64_t)(((uint64_t)(uint32_t)v.y << 32) | (uint32_t)v.x);
+    r.dur_ms = v.z;
+    r.est = v.w;
+    return r;
+}
+
+// ---- the total order (asr_sched.h "TOTAL ORDER") -----------------------------
+// a2: priority keys.  FCFS PAPER.md:13; SJF PAPER.md:277; HRRN PAPER.md:282.
+__device__ __forceinline__ int64_t est_of(int32_t est) { return est < 1 ? 1 : (int64_t)est; }
+
+__device__ __forceinline__ int64_t wait_of(int64_t arrival_us, int64_t now) {
+    int64_t w = now - arrival_us;
+    return w < 0 ? 0 : w;
+}
+
+__device__ __forceinline__ bool earlier(int64_t arr_a, int32_t idx_a, int64_t arr_b, int32_t idx_b) {
+    return arr_a != arr_b ? arr_a < arr_b : idx_a < idx_b;
+}
+
+template <int POLICY>
+__device__ __forceinline__ bool better(int64_t arr_a, int32_t est_a, int32_t idx_a, int64_t arr_b,
+                                       int32_t est_b, int32_t idx_b, int64_t now) {
+    if (POLICY == ASR_FCFS) return earlier(arr_a, idx_a, arr_b, idx_b);
+    if (POLICY == ASR_SJF) {
+        int64_t ea = est_of(est_a), eb = est_of(est_b);
+        if (ea != eb) return ea < eb;
+        return earlier(arr_a, idx_a, arr_b, idx_b);
+    }
+    // HRRN: (wa+ea)/ea > (wb+eb)/eb  <=>  wa*eb > wb*ea ; products < 2^62 under
+    // the documented bounds (wait < 2^38, est <= 2^24)
+    int64_t lhs = wait_of(arr_a, now) * est_of(est_b);
+    int64_t rhs = wait_of(arr_b, now) * est_of(est_a);
+    if (lhs != rhs) return lhs > rhs;
+    return earlier(arr_a, idx_a, arr_b, idx_b);
+}
+
+__device__ __forceinline__ bool better_rt(int policy, int64_t arr_a, int32_t est_a, int32_t idx_a,
+                                          int64_t arr_b, int32_t est_b, int32_t idx_b, int64_t now) {
+    if (policy == ASR_FCFS) return better<ASR_FCFS>(arr_a, est_a, idx_a, arr_b, est_b, idx_b, now);
+    if (policy == ASR_SJF) return better<ASR_SJF>(arr_a, est_a, idx_a, arr_b, est_b, idx_b, now);
+    return better<ASR_HRRN>(arr_a, est_a, idx_a, arr_b, est_b, idx_b, now);
+}
+
+// ---- warp helpers -----------------------------------------------------------
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+__device__ __forceinline__ int64_t shfl64(int64_t v, int src) {
+    int lo = __shfl_sync(ASR_FULL_MASK, (int)(uint32_t)v, src);
+    int hi = __shfl_sync(ASR_FULL_MASK, (int)(v >> 32), src);
+    return (int64_t)(((uint64_t)(uint32_t)hi << 32) | (uint32_t)lo);
+}
+
+__device__ __forceinline__ uint64_t shfl64_xor(uint64_t v, int m) {
+    uint32_t lo = __shfl_xor_sync(ASR_FULL_MASK, (uint32_t)v, m);
+    uint32_t hi = __shfl_xor_sync(ASR_FULL_MASK, (uint32_t)(v >> 32), m);
+    return ((uint64_t)hi << 32) | lo;
+}
+
+}  // namespace asr

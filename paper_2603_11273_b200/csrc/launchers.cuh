@@ -1,0 +1,33 @@
+// launchers.cuh -- host-side launch interfaces between api.cu and the kernel files.
+#pragma once
+#include "common.cuh"
+
+namespace asr {
+
+struct SimArgs {
+    const asr_req_t *traces;
+    const asr_replica_t *replicas;
+    const asr_cost_model_t *cms;
+    const int64_t *bm_off;    // [n_replicas] first bitmap word of each replica
+    uint32_t *bitmap;
+    int64_t *out_lat;
+    int64_t *out_ttft;
+    asr_summary_t *out_summary;  // nullable
+    int64_t total_requests;
+    int32_t n_replicas;
+    int32_t n_cms;
+};
+
+int launch_simulate(const SimArgs &a, int max_slots, cudaStream_t st);
+int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, cudaStream_t st);
+int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg, const int32_t *pcts,
+                       int32_t n_pct, int64_t *out, cudaStream_t st);
+int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
+                               const int64_t *ttft, asr_summary_t *out_summary, cudaStream_t st);
+int launch_gen_trace(const asr_trace_spec_t *specs, asr_trace_spec_t one, int32_t n_traces, int64_t n_per_trace,
+                     const asr_tables_t *tables, asr_req_t *out, cudaStream_t st);
+int launch_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now, const asr_tables_t *tables,
+                      asr_req_t *out, cudaStream_t st);
+size_t select_workspace_bytes(int64_t n, int64_t k);
+
+}  // namespace asr

@@ -1,0 +1,362 @@
+// simulate.cu -- a4 simulator step + a5 per-request outputs, sm_100a.
+//
+// One warp owns one replica (seed x rate x policy).  Lane L holds batch slots
+// L, L+32, ... in registers (remaining tokens, request index, arrival), so the
+// per-iteration work of the paper's engine (PAPER.md:31 iteration-level
+// scheduling; PAPER.md:51-53 encoder + linear decode) is a handful of
+// warp-wide instructions: redux.min for the next completion, ballots for
+// arrivals and finishes.
+//
+// Exact fast-forward.  Between two events (an admission opportunity or a
+// completion) every engine iteration is identical: cost c = iter_base +
+// iter_per_running*|R| and one token for everyone.  The kernel jumps j such
+// iterations at once, j = min(iterations to the first completion, iterations
+// to the first boundary at or after the next arrival when a slot is free),
+// which is bit-identical to stepping them one by one.
+//
+// Waiting queue.  Requests are ingested in trace order, so the waiting set is
+// {i in [lo, p) : not admitted(i)}.  While it is a dense range (always for
+// FCFS, and whenever everything waiting is admitted at once) no queue storage
+// is touched at all.  Otherwise a per-replica bitmap in the workspace marks
+// admitted requests and the admit step scans the trace window [lo, p) with
+// coalesced 128-bit loads, applying the exact comparator of asr_sched.h.
+#include "launchers.cuh"
+
+namespace asr {
+
+constexpr int SIM_WARPS = 4;
+constexpr int32_t REM_FREE = 0x7FFFFFFF;
+
+__device__ __forceinline__ int64_t ceil_div_pos(int64_t g, int64_t c) {
+    // g > 0, c > 0; 32-bit divide whenever both operands fit
+    if ((((uint64_t)g | (uint64_t)c) >> 32) == 0) {
+        const uint32_t q = (uint32_t)g / (uint32_t)c;
+        return (int64_t)q + ((uint32_t)g - q * (uint32_t)c != 0u ? 1 : 0);
+    }
+    const uint64_t q = (uint64_t)g / (uint64_t)c;
+    return (int64_t)q + ((uint64_t)g - q * (uint64_t)c != 0ull ? 1 : 0);
+}
+
+__device__ __forceinline__ int32_t tokens_of(const asr_cost_model_t &cm, int32_t dur_ms) {
+    int64_t t = (int64_t)cm.tok_base + ((int64_t)cm.tok_per_s * (int64_t)dur_ms) / 1000;
+    t = t < 1 ? 1 : t;
+    return t > 0x7FFFFFFE ? 0x7FFFFFFE : (int32_t)t;
+}
+
+// sum over the warp of a non-negative 32-bit value per lane, exact in 64 bits
+__device__ __forceinline__ int64_t warp_sum_u32(uint32_t v) {
+    uint32_t lo = __reduce_add_sync(ASR_FULL_MASK, v & 0xFFFFu);
+    uint32_t hi = __reduce_add_sync(ASR_FULL_MASK, v >> 16);
+    return ((int64_t)hi << 16) + (int64_t)lo;
+}
+
+template <int SPL>
+__global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
+    const int lane = lane_id();
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const int r = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
+    if (r >= a.n_replicas) return;
+
+    const asr_replica_t rep = a.replicas[r];
+    const int n = rep.n;
+    const int slots = rep.slots;
+    const int policy = rep.policy;
+    const bool ok = n >= 0 && slots >= 1 && slots <= 32 * SPL && policy >= 0 && policy <= 2 &&
+                    rep.cm_id >= 0 && rep.cm_id < a.n_cms && rep.trace_off >= 0 && rep.out_off >= 0 &&
+                    rep.out_off + (int64_t)n <= a.total_requests;
+    if (!ok) {
+        if (a.out_summary && lane == 0) {
+            asr_summary_t s;
+            s.p50_e2e_us = s.p90_e2e_us = s.p50_ttft_us = s.p90_ttft_us = -1;
+            s.first_arrival_us = s.last_done_us = 0;
+            s.n_done = -1;
+            a.out_summary[r] = s;
+        }
+        return;
+    }
+    const asr_cost_model_t cm = a.cms[rep.cm_id];
+    const asr_req_t *trace = a.traces + rep.trace_off;
+    int64_t *lat = a.out_lat + rep.out_off;
+    int64_t *ttft = a.out_ttft + rep.out_off;
+    uint32_t *bm = a.bitmap + a.bm_off[r];
+
+    // running set: slot id = s*32 + lane
+    int32_t rem[SPL];
+    int32_t ridx[SPL];
+    int64_t rarr[SPL];
+#pragma unroll
+    for (int s = 0; s < SPL; ++s) {
+        rem[s] = REM_FREE;
+        ridx[s] = -1;
+        rarr[s] = 0;
+    }
+
+    int64_t t = 0;
+    int p = 0;        // next request to ingest
+    int lo = 0;       // every request below lo has been admitted
+    int nW = 0;       // waiting requests
+    int nR = 0;       // running requests
+    int done = 0;
+    bool sparse = false;  // bitmap in use for [lo, bm_hi)
+    int bm_hi = 0;
+
+    // arrival stamps of the trace chunk [cbase, cbase+32)
+    int cbase = 0;
+    int64_t carr = (lane < n) ? trace[lane].arrival_us : 0;
+    const int64_t first_arrival = n > 0 ? shfl64(carr, 0) : 0;
+
+    while (done < n) {
+        // ---- 1. ingest arrivals <= t (at the iteration boundary)
+        while (p < n) {
+            if (p >= cbase + 32) {
+                cbase = p & ~31;
+                carr = (cbase + lane < n) ? trace[cbase + lane].arrival_us : 0;
+            }
+            const int i = cbase + lane;
+            uint32_t m = __ballot_sync(ASR_FULL_MASK, i >= p && i < n && carr <= t);
+            int cnt = __popc(m);
+            p += cnt;
+            nW += cnt;
+            if (cnt == 0 || p < cbase + 32) break;
+        }
+        if (p < n && p >= cbase + 32) {
+            cbase = p & ~31;
+            carr = (cbase + lane < n) ? trace[cbase + lane].arrival_us : 0;
+        }
+        // ---- 2. idle server: jump to the next arrival
+        if (nR == 0 && nW == 0) {
+            t = shfl64(carr, p - cbase);
+            continue;
+        }
+        // ---- 3. admit the k best waiting requests into the free slots
+        const int free_slots = slots - nR;
+        const int k = free_slots < nW ? free_slots : nW;
+        uint32_t newly = 0;        // bit s: my slot s was admitted in this step
+        uint32_t dur_sum_part = 0; // my share of sum(dur_ms) of the admitted
+        if (k > 0) {
+            const bool take_all = (k == nW);
+            if (!sparse && (take_all || policy == ASR_FCFS)) {
+                // dense window: admit requests lo .. lo+k-1 (their order is irrelevant
+                // to every time; only the set matters, S15)
+                int before = 0;
+#pragma unroll
+                for (int s = 0; s < SPL; ++s) {
+                    const bool is_free = (s * 32 + lane < slots) && rem[s] == REM_FREE;
+                    const uint32_t fm = __ballot_sync(ASR_FULL_MASK, is_free);
+                    const int rank = before + __popc(fm & lt_mask);
+                    if (is_free && rank < k) {
+                        const Rec q = ld_cached(trace + lo + rank);
+                        rem[s] = tokens_of(cm, q.dur_ms);
+                        ridx[s] = lo + rank;
+                        rarr[s] = q.arrival_us;
+                        dur_sum_part += (uint32_t)q.dur_ms;
+                        newly |= 1u << s;
+                    }
+                    before += __popc(fm);
+                }
+                lo += k;
+                nW -= k;
+            } else {
+                // sparse window: bitmap marks the admitted requests of [lo, p)
+                if (!sparse) {
+                    for (int w = (lo >> 5) + lane; w <= ((p - 1) >> 5); w += 32) bm[w] = 0u;
+                    sparse = true;
+                    bm_hi = p;
+                    __syncwarp();
+                } else if (bm_hi < p) {
+                    // clear the bits of the newly ingested requests [bm_hi, p)
+                    const int w0 = bm_hi >> 5, w1 = (p - 1) >> 5;
+                    for (int w = w0 + lane; w <= w1; w += 32) {
+                        if (w == w0) {
+                            if (bm_hi & 31) bm[w] &= (1u << (bm_hi & 31)) - 1u;
+                            else bm[w] = 0u;
+                        } else {
+                            bm[w] = 0u;
+                        }
+                    }
+                    bm_hi = p;
+                    __syncwarp();
+                }
+                for (int round = 0; round < k; ++round) {
+                    // lane-local best over the window, then warp argmax
+                    int64_t b_arr = 0;
+                    int32_t b_est = 0, b_dur = 0, b_idx = -1;
+                    for (int c = lo & ~31; c < p; c += 32) {
+                        const uint32_t word = bm[c >> 5];
+                        const int i = c + lane;
+                        if (i >= lo && i < p && !((word >> lane) & 1u)) {
+                            const Rec q = ld_cached(trace + i);
+                            if (b_idx < 0 ||
+                                better_rt(policy, q.arrival_us, q.est, i, b_arr, b_est, b_idx, t)) {
+                                b_arr = q.arrival_us;
+                                b_est = q.est;
+                                b_dur = q.dur_ms;
+                                b_idx = i;
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int j = 16; j > 0; j >>= 1) {
+                        const int64_t o_arr = (int64_t)shfl64_xor((uint64_t)b_arr, j);
+                        const int32_t o_est = __shfl_xor_sync(ASR_FULL_MASK, b_est, j);
+                        const int32_t o_dur = __shfl_xor_sync(ASR_FULL_MASK, b_dur, j);
+                        const int32_t o_idx = __shfl_xor_sync(ASR_FULL_MASK, b_idx, j);
+                        if (o_idx >= 0 &&
+                            (b_idx < 0 || better_rt(policy, o_arr, o_est, o_idx, b_arr, b_est, b_idx, t))) {
+                            b_arr = o_arr;
+                            b_est = o_est;
+                            b_dur = o_dur;
+                            b_idx = o_idx;
+                        }
+                    }
+                    // b_* now uniform: the winner.  Mark it and seat it in the first free slot.
+                    if (lane == 0) bm[b_idx >> 5] |= 1u << (b_idx & 31);
+                    bool seated = false;
+#pragma unroll
+                    for (int s = 0; s < SPL; ++s) {
+                        const bool is_free = (s * 32 + lane < slots) && rem[s] == REM_FREE;
+                        const uint32_t fm = __ballot_sync(ASR_FULL_MASK, is_free);
+                        if (!seated && fm != 0u) {
+                            if (lane == __ffs(fm) - 1) {
+                                rem[s] = tokens_of(cm, b_dur);
+                                ridx[s] = b_idx;
+                                rarr[s] = b_arr;
+                                dur_sum_part += (uint32_t)b_dur;
+                                newly |= 1u << s;
+                            }
+                            seated = true;
+                        }
+                    }
+                    __syncwarp();
+                }
+                nW -= k;
+                if (nW == 0) {
+                    lo = p;
+                    sparse = false;
+                } else {
+                    // advance lo past admitted requests
+                    while (lo < p) {
+                        uint32_t word = ~bm[lo >> 5] & ~((1u << (lo & 31)) - 1u);
+                        if (word) {
+                            lo = (lo & ~31) + __ffs(word) - 1;
+                            break;
+                        }
+                        lo = (lo & ~31) + 32;
+                    }
+                    if (lo > p) lo = p;
+                }
+            }
+            nR += k;
+        }
+        // ---- 4. one engine iteration with the encoders of the admitted ...
+        const int64_t c = cm.iter_base_us + cm.iter_per_running_us * (int64_t)nR;
+        int64_t t1 = t + c;
+        if (k > 0) {
+            const int64_t dur_sum = warp_sum_u32(dur_sum_part);
+            t1 += cm.enc_base_us * (int64_t)k + cm.enc_per_ms_us * dur_sum;
+#pragma unroll
+            for (int s = 0; s < SPL; ++s)
+                if ((newly >> s) & 1u) ttft[ridx[s]] = t1 - rarr[s];   // first token (S9)
+        }
+        // ---- ... then fast-forward over identical iterations to the next event
+        int32_t my_min = rem[0];
+#pragma unroll
+        for (int s = 1; s < SPL; ++s) my_min = rem[s] < my_min ? rem[s] : my_min;
+        const int32_t m = __reduce_min_sync(ASR_FULL_MASK, my_min);   // >= 1, nR >= 1 here
+        int64_t j = 1;
+        if (m > 1) {
+            if (nR == slots || p >= n || c <= 0) {
+                j = m;   // nothing can be admitted before the first completion
+            } else {
+                const int64_t g = shfl64(carr, p - cbase) - t1;
+                if (g <= 0) j = 1;
+                else if (g > (int64_t)(m - 2) * c) j = m;
+                else j = 1 + ceil_div_pos(g, c);
+            }
+        }
+        t = t1 + (j - 1) * c;
+        // ---- 5. tokens, completions (a5: E2E latency)
+        int fin = 0;
+#pragma unroll
+        for (int s = 0; s < SPL; ++s) {
+            if (rem[s] != REM_FREE) {
+                rem[s] -= (int32_t)j;
+                if (rem[s] == 0) {
+                    lat[ridx[s]] = t - rarr[s];
+                    rem[s] = REM_FREE;
+                    fin++;
+                }
+            }
+        }
+        const int nfin = __reduce_add_sync(ASR_FULL_MASK, fin);
+        nR -= nfin;
+        done += nfin;
+    }
+    if (a.out_summary && lane == 0) {
+        asr_summary_t *s = a.out_summary + r;
+        s->first_arrival_us = first_arrival;
+        s->last_done_us = t;
+        s->n_done = done;
+    }
+}
+
+// exclusive prefix sum of the per-replica bitmap sizes (words), one CTA
+__global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *replicas, int32_t n_replicas,
+                                                           int64_t *bm_off) {
+    __shared__ int64_t warp_tot[32];
+    __shared__ int64_t carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    for (int base = 0; base < n_replicas; base += 1024) {
+        const int r = base + threadIdx.x;
+        int64_t v = 0;
+        if (r < n_replicas) {
+            int n = replicas[r].n;
+            v = (int64_t)((n < 0 ? 0 : n) >> 5) + 2;   // ceil(n/32) + slack word
+        }
+        int64_t x = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int64_t y = (int64_t)shfl64(x, lane >= d ? lane - d : lane);
+            if (lane >= d) x += y;
+        }
+        if (lane == 31) warp_tot[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            int64_t w = warp_tot[lane];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                int64_t y = (int64_t)shfl64(w, lane >= d ? lane - d : lane);
+                if (lane >= d) w += y;
+            }
+            warp_tot[lane] = w;   // inclusive over warps
+        }
+        __syncthreads();
+        const int64_t carry = carry_s;
+        const int64_t incl = carry + (warp > 0 ? warp_tot[warp - 1] : 0) + x;
+        if (r < n_replicas) bm_off[r] = incl - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = incl;
+        __syncthreads();
+    }
+}
+
+int launch_simulate(const SimArgs &a, int max_slots, cudaStream_t st) {
+    if (a.n_replicas <= 0) return ASR_OK;
+    const int grid = (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS;
+    if (max_slots <= 32) sim_warp_kernel<1><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    else if (max_slots <= 64) sim_warp_kernel<2><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    else if (max_slots <= 128) sim_warp_kernel<4><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    else sim_warp_kernel<8><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    count_launch();
+    return check_launch("sim_warp_kernel");
+}
+
+int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, cudaStream_t st) {
+    sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, bm_off);
+    count_launch();
+    return check_launch("sim_prepare_kernel");
+}
+
+}  // namespace asr

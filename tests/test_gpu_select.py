@@ -1,0 +1,91 @@
+"""-m gpu: the CUDA select (a2+a3) against the oracle, bit-exact, through the C ABI."""
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+POL = (orc.FCFS, orc.SJF, orc.HRRN)
+
+
+@pytest.fixture(scope="module")
+def asr():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2603_11273_b200 as asr
+    return asr
+
+
+def gpu_select_batched(asr, q2d, policy, now, k, q_count=None, now_pq=None):
+    import torch
+    nq, ql = q2d.shape
+    d = asr.to_device(q2d)
+    dc = None if q_count is None else torch.from_numpy(np.asarray(q_count, dtype=np.int32)).cuda()
+    dn = None if now_pq is None else torch.from_numpy(np.asarray(now_pq, dtype=np.int64)).cuda()
+    out = asr.select_batched(d, nq, ql, policy, now, k, q_count=dc, now_per_queue=dn)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+@pytest.mark.parametrize("kind", ["random", "six", "proportional", "identical", "few_arrivals", "future", "est_edge"])
+@pytest.mark.parametrize("policy", POL)
+def test_batched_stress_kinds(asr, kind, policy):
+    now = 10**9
+    for ql, k, nq in [(1, 4, 3), (31, 32, 5), (32, 32, 5), (33, 7, 5), (257, 32, 9), (700, 32, 17), (4096, 32, 6),
+                      (5000, 1, 3)]:
+        q = np.stack([wl.stress_queue(kind, ql, 1000 * ql + i, now) for i in range(nq)])
+        got = gpu_select_batched(asr, q, policy, now, k)
+        for i in range(nq):
+            assert np.array_equal(got[i], orc.select(q[i], policy, now, k)), (kind, policy, ql, k, i)
+
+
+@pytest.mark.parametrize("policy", POL)
+def test_ragged_counts_and_per_queue_now(asr, policy):
+    rng = np.random.default_rng(policy)
+    nq, ql, k = 40, 600, 32
+    now = 10**8
+    q = np.stack([wl.stress_queue("random" if i % 2 else "few_arrivals", ql, 77 + i, now) for i in range(nq)])
+    counts = rng.integers(0, ql + 1, size=nq)
+    counts[:4] = [0, 1, ql, 31]
+    nows = rng.integers(1, 2 * now, size=nq)
+    got = gpu_select_batched(asr, q, policy, now, k, q_count=counts, now_pq=nows)
+    for i in range(nq):
+        assert np.array_equal(got[i], orc.select(q[i][:counts[i]], policy, int(nows[i]), k)), i
+
+
+@pytest.mark.parametrize("policy", POL)
+@pytest.mark.parametrize("n", [0, 1, 4096, 4097, 20000, 300000])
+def test_single_queue_any_length(asr, policy, n):
+    import torch
+    now = 10**10
+    q = wl.stress_queue("random" if n != 20000 else "six", n, n + 1, now)
+    d = asr.to_device(q) if n else torch.zeros(16, dtype=torch.uint8, device="cuda")
+    for k in (1, 32):
+        out = asr.select(d, n, policy, now, k)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), orc.select(q, policy, now, k)), (policy, n, k)
+
+
+def test_generated_config5_queues_small(asr, tables):
+    """config-5 recipe at oracle-friendly size: 96 queues x 4096, k = 32, seed 5."""
+    import torch
+    cfg = wl.config5(n_queues=96)
+    d_tab = asr.tables_to_device(*tables)
+    dq = asr.gen_queues(cfg["seed"], 0, cfg["n_queues"] * cfg["q_len"], cfg["now"], d_tab)
+    torch.cuda.synchronize()
+    q = dq.cpu().numpy().view(asr.REQ_DTYPE).reshape(cfg["n_queues"], cfg["q_len"])
+    ref = orc.gen_queue(cfg["seed"], 0, q.size, cfg["now"], tables[0]).reshape(q.shape)
+    assert np.array_equal(q.view(np.uint8), ref.view(np.uint8))
+    for pol in cfg["policies"]:
+        got = asr.select_batched(dq, cfg["n_queues"], cfg["q_len"], pol, cfg["now"], cfg["k"]).cpu().numpy()
+        for i in range(cfg["n_queues"]):
+            assert np.array_equal(got[i], orc.select(ref[i], pol, cfg["now"], cfg["k"])), (pol, i)
+
+
+def test_select_host_entry(asr):
+    now = 10**9
+    q = np.stack([wl.stress_queue("random", 300, i, now) for i in range(8)])
+    got = asr.select_host(q, 8, 300, orc.HRRN, now, 16)
+    for i in range(8):
+        assert np.array_equal(got[i], orc.select(q[i], orc.HRRN, now, 16))
