@@ -228,6 +228,16 @@ int asr_sched_version(void);
 /* number of kernels this library has launched in this process (monotonic) */
 int64_t asr_sched_launch_count(void);
 
+/* Per-kernel timing (the library's own tracing aid).  While enabled, every
+ * kernel launch is bracketed by a CUDA-event pair recorded on the launching
+ * stream.  asr_sched_timing_read synchronises those events and returns the
+ * summed device time and launch count of kernel `kernel_id` since the last
+ * reset; asr_sched_kernel_name(id) names the ids 0.. (NULL past the end). */
+int asr_sched_timing_enable(int on);
+int asr_sched_timing_reset(void);
+int asr_sched_timing_read(int32_t kernel_id, double *total_ms, int64_t *launches);
+const char *asr_sched_kernel_name(int32_t kernel_id);
+
 #ifdef __cplusplus
 }
 #endif

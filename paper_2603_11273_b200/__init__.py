@@ -11,5 +11,5 @@ from .binding import (  # noqa: F401
     REPLICA_DTYPE, COST_DTYPE, AsrSchedError, lib, lib_path, version, last_error, launch_count,
     workspace_bytes, to_device, tables_to_device, select, select_batched, simulate,
     simulate_batched, percentiles, gen_trace, gen_trace_batched, gen_queues, sweep_host,
-    select_host, make_tables, make_replicas, make_cost,
+    select_host, make_tables, make_replicas, make_cost, timing_enable, timing_reset, timing_read,
 )

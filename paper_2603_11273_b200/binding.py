@@ -31,7 +31,8 @@ EXPORTS = (
     "asr_sched_select", "asr_sched_select_batched", "asr_sched_simulate", "asr_sched_simulate_batched",
     "asr_sched_percentiles", "asr_sched_gen_trace", "asr_sched_gen_trace_batched", "asr_sched_gen_queues",
     "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_workspace_bytes", "asr_sched_last_error",
-    "asr_sched_version", "asr_sched_launch_count",
+    "asr_sched_version", "asr_sched_launch_count", "asr_sched_timing_enable", "asr_sched_timing_reset",
+    "asr_sched_timing_read", "asr_sched_kernel_name",
 )
 
 
@@ -73,6 +74,10 @@ def lib():
         L.asr_sched_last_error.restype = C.c_char_p
         L.asr_sched_version.restype = C.c_int
         L.asr_sched_launch_count.restype = i64
+        L.asr_sched_timing_enable.argtypes = [C.c_int]
+        L.asr_sched_timing_read.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(i64)]
+        L.asr_sched_kernel_name.argtypes = [i32]
+        L.asr_sched_kernel_name.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -87,6 +92,27 @@ def last_error() -> str:
 
 def launch_count() -> int:
     return int(lib().asr_sched_launch_count())
+
+
+def timing_enable(on: bool):
+    lib().asr_sched_timing_enable(1 if on else 0)
+
+
+def timing_reset():
+    lib().asr_sched_timing_reset()
+
+
+def timing_read() -> dict:
+    """-> {kernel name: (total device ms, launches)} since the last reset (synchronises)."""
+    out, kid = {}, 0
+    while True:
+        name = lib().asr_sched_kernel_name(kid)
+        if name is None:
+            return out
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        _check(lib().asr_sched_timing_read(kid, C.byref(ms), C.byref(n)), "asr_sched_timing_read")
+        out[name.decode()] = (ms.value, int(n.value))
+        kid += 1
 
 
 def workspace_bytes(op: int, a: int, b: int, c: int = 0) -> int:

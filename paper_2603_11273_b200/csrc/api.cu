@@ -4,6 +4,8 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
+#include <vector>
 
 #include "launchers.cuh"
 
@@ -29,6 +31,47 @@ int check_launch(const char *what) {
 }
 
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+// ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
+static const char *const g_kernel_names[KID_COUNT] = {
+    "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "summary_percentiles_kernel",
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel"};
+struct TimedLaunch {
+    int kid;
+    cudaEvent_t start, stop;
+};
+static std::mutex g_timing_mu;
+static bool g_timing_on = false;
+static std::vector<TimedLaunch> g_timed;      // recorded launches since the last reset
+static std::vector<cudaEvent_t> g_event_pool; // recycled events
+
+static cudaEvent_t take_event() {
+    if (!g_event_pool.empty()) {
+        cudaEvent_t e = g_event_pool.back();
+        g_event_pool.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+KernelTimer::KernelTimer(int kid, cudaStream_t st) : kid_(kid), st_(st), slot_(-1) {
+    count_launch();
+    std::lock_guard<std::mutex> g(g_timing_mu);
+    if (!g_timing_on) return;
+    TimedLaunch t{kid, take_event(), take_event()};
+    if (!t.start || !t.stop) return;
+    cudaEventRecord(t.start, st);
+    g_timed.push_back(t);
+    slot_ = (int)g_timed.size() - 1;
+}
+
+KernelTimer::~KernelTimer() {
+    if (slot_ < 0) return;
+    std::lock_guard<std::mutex> g(g_timing_mu);
+    if (slot_ < (int)g_timed.size()) cudaEventRecord(g_timed[slot_].stop, st_);
+}
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -61,6 +104,51 @@ using namespace asr;
 extern "C" const char *asr_sched_last_error(void) { return g_err; }
 extern "C" int asr_sched_version(void) { return ASR_SCHED_VERSION; }
 extern "C" int64_t asr_sched_launch_count(void) { return (int64_t)g_launches.load(); }
+
+extern "C" int asr_sched_timing_enable(int on) {
+    std::lock_guard<std::mutex> g(g_timing_mu);
+    g_timing_on = on != 0;
+    return ASR_OK;
+}
+
+extern "C" int asr_sched_timing_reset(void) {
+    std::lock_guard<std::mutex> g(g_timing_mu);
+    for (auto &t : g_timed) {
+        g_event_pool.push_back(t.start);
+        g_event_pool.push_back(t.stop);
+    }
+    g_timed.clear();
+    return ASR_OK;
+}
+
+extern "C" const char *asr_sched_kernel_name(int32_t kernel_id) {
+    return kernel_id >= 0 && kernel_id < KID_COUNT ? g_kernel_names[kernel_id] : nullptr;
+}
+
+extern "C" int asr_sched_timing_read(int32_t kernel_id, double *total_ms, int64_t *launches) {
+    if (kernel_id < 0 || kernel_id >= KID_COUNT || !total_ms || !launches) {
+        set_error("timing_read: bad argument");
+        return ASR_EINVAL;
+    }
+    std::lock_guard<std::mutex> g(g_timing_mu);
+    double ms = 0.0;
+    int64_t n = 0;
+    for (auto &t : g_timed) {
+        if (t.kid != kernel_id) continue;
+        cudaError_t e = cudaEventSynchronize(t.stop);
+        float f = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&f, t.start, t.stop);
+        if (e != cudaSuccess) {
+            set_error("timing_read: %s", cudaGetErrorString(e));
+            return ASR_ECUDA;
+        }
+        ms += f;
+        n++;
+    }
+    *total_ms = ms;
+    *launches = n;
+    return ASR_OK;
+}
 
 extern "C" size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c) {
     if (a < 0 || b < 0) return 0;
@@ -277,9 +365,11 @@ extern "C" int asr_sched_sweep_host(const asr_trace_spec_t *specs, int32_t n_tra
     int rc = asr_sched_gen_trace_batched((const asr_trace_spec_t *)d_specs.p, n_traces, n_per_trace,
                                          (const asr_tables_t *)d_tables.p, (asr_req_t *)d_traces.p, st);
     if (rc) return rc;
-    build_sweep_replicas_kernel<<<(int)((n_rep + 255) / 256 < 1184 ? (n_rep + 255) / 256 : 1184), 256, 0, st>>>(
-        (asr_replica_t *)d_rep.p, n_traces, n_per_trace, n_policies, slots, (const int32_t *)d_pol.p);
-    count_launch();
+    {
+        KernelTimer kt(KID_SWEEP_REPLICAS, st);
+        build_sweep_replicas_kernel<<<(int)((n_rep + 255) / 256 < 1184 ? (n_rep + 255) / 256 : 1184), 256, 0, st>>>(
+            (asr_replica_t *)d_rep.p, n_traces, n_per_trace, n_policies, slots, (const int32_t *)d_pol.p);
+    }
     rc = check_launch("build_sweep_replicas_kernel");
     if (rc) return rc;
     rc = asr_sched_simulate_batched((const asr_req_t *)d_traces.p, (const asr_replica_t *)d_rep.p, (int32_t)n_rep,

@@ -16,6 +16,21 @@ void set_error(const char *fmt, ...);
 int check_launch(const char *what);   // cudaGetLastError -> ASR_OK / ASR_ECUDA
 void count_launch(int n = 1);
 
+// kernel ids of the per-kernel CUDA-event timing facility (asr_sched_timing_*)
+enum KernelId {
+    KID_SELECT = 0, KID_SIM_PREPARE, KID_SIMULATE, KID_SUMMARY_PCT, KID_PERCENTILES, KID_GEN_TRACE,
+    KID_GEN_QUEUES, KID_SWEEP_REPLICAS, KID_COUNT
+};
+// RAII: counts the launch and, when timing is enabled, brackets it with an
+// event pair recorded on the launching stream.
+struct KernelTimer {
+    KernelTimer(int kid, cudaStream_t st);
+    ~KernelTimer();
+    int kid_;
+    cudaStream_t st_;
+    int slot_;
+};
+
 // ---- 128-bit record access -------------------------------------------------
 struct __align__(16) Rec {
     int64_t arrival_us;

@@ -115,8 +115,10 @@ int launch_gen_trace(const asr_trace_spec_t *specs, asr_trace_spec_t one, int32_
                      const asr_tables_t *tables, asr_req_t *out, cudaStream_t st) {
     if (n_traces <= 0 || n_per_trace <= 0) return ASR_OK;
     int grid = n_traces < 148 * 64 ? n_traces : 148 * 64;
-    gen_trace_kernel<<<grid, GEN_THREADS, 0, st>>>(specs, one, n_traces, n_per_trace, tables, out);
-    count_launch();
+    {
+        KernelTimer kt(KID_GEN_TRACE, st);
+        gen_trace_kernel<<<grid, GEN_THREADS, 0, st>>>(specs, one, n_traces, n_per_trace, tables, out);
+    }
     return check_launch("gen_trace_kernel");
 }
 
@@ -125,8 +127,10 @@ int launch_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now, cons
     if (n <= 0) return ASR_OK;
     int64_t want = (n + GEN_THREADS - 1) / GEN_THREADS;
     int grid = (int)(want < 148 * 16 ? want : 148 * 16);
-    gen_queues_kernel<<<grid, GEN_THREADS, 0, st>>>(seed, first, n, now, tables, out);
-    count_launch();
+    {
+        KernelTimer kt(KID_GEN_QUEUES, st);
+        gen_queues_kernel<<<grid, GEN_THREADS, 0, st>>>(seed, first, n, now, tables, out);
+    }
     return check_launch("gen_queues_kernel");
 }
 

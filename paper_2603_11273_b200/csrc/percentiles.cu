@@ -188,8 +188,10 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
         attr = true;
     }
     const int grid = pct_grid(n_seg, (const void *)percentiles_kernel);
-    percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(values, seg_off, n_seg, pl, out);
-    count_launch();
+    {
+        KernelTimer kt(KID_PERCENTILES, st);
+        percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(values, seg_off, n_seg, pl, out);
+    }
     return check_launch("percentiles_kernel");
 }
 
@@ -205,8 +207,10 @@ int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas
     int gx = pct_grid(n_replicas, (const void *)summary_percentiles_kernel);
     gx = gx > 1 ? (gx + 1) / 2 : 1;
     dim3 grid(gx, 2);
-    summary_percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary);
-    count_launch();
+    {
+        KernelTimer kt(KID_SUMMARY_PCT, st);
+        summary_percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary);
+    }
     return check_launch("summary_percentiles_kernel");
 }
 

@@ -298,8 +298,10 @@ static int launch_one(const SelArgs &a, cudaStream_t st) {
     int64_t want = ((int64_t)a.n_queues + SEL_WARPS - 1) / SEL_WARPS;
     int64_t cap = (int64_t)n_sm * blocks_per_sm;
     int grid = (int)(want < cap ? want : cap);
-    select_topk_kernel<POLICY, INDIRECT><<<grid, SEL_WARPS * 32, 0, st>>>(a);
-    count_launch();
+    {
+        KernelTimer kt(KID_SELECT, st);
+        select_topk_kernel<POLICY, INDIRECT><<<grid, SEL_WARPS * 32, 0, st>>>(a);
+    }
     return check_launch("select_topk_kernel");
 }
 

@@ -345,17 +345,21 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
 int launch_simulate(const SimArgs &a, int max_slots, cudaStream_t st) {
     if (a.n_replicas <= 0) return ASR_OK;
     const int grid = (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS;
-    if (max_slots <= 32) sim_warp_kernel<1><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-    else if (max_slots <= 64) sim_warp_kernel<2><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-    else if (max_slots <= 128) sim_warp_kernel<4><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-    else sim_warp_kernel<8><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-    count_launch();
+    {
+        KernelTimer kt(KID_SIMULATE, st);
+        if (max_slots <= 32) sim_warp_kernel<1><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+        else if (max_slots <= 64) sim_warp_kernel<2><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+        else if (max_slots <= 128) sim_warp_kernel<4><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+        else sim_warp_kernel<8><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    }
     return check_launch("sim_warp_kernel");
 }
 
 int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, cudaStream_t st) {
-    sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, bm_off);
-    count_launch();
+    {
+        KernelTimer kt(KID_SIM_PREPARE, st);
+        sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, bm_off);
+    }
     return check_launch("sim_prepare_kernel");
 }
 
