@@ -1,0 +1,427 @@
+#!/usr/bin/env python
+"""bench.py -- simulated requests/s on the replica sweep (BASELINE.json configs[2])
+and priority-select GB/s on config 5 (configs[4]), on N B200s of one node.
+
+  python bench.py --gpus 1 --steps 5 --warmup 3
+  python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+      --master-port P bench.py --gpus N --steps K --warmup W
+  python bench.py --impl reference        # the CPU oracle, as it stands, on the host cores
+
+One step = one pass of the whole hot path over one batch: a1 generate the
+32,768 traces -> a4/a5 simulate 98,304 replicas (a2/a3 inside the admit step)
+-> a6 per-replica p50/p90 + throughput inputs.  The standalone batched select
+(config 5) is timed in its own region of the same run.  Rank r of an N-GPU run
+takes seeds [r*4096, (r+1)*4096) and its own 65,536 queues: weak scaling, no
+data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "simulated requests/sec (replica sweep)"
+UNIT = "requests/s"
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
+# issue-slot peak: 148 SMs x 4 schedulers x 1 warp-instruction/clk x 1.965 GHz
+ALU_PEAK_WARP_INSTR_PER_S = 148 * 4 * 1.965e9
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def load_profile_constants():
+    """per-launch DRAM traffic and warp instructions per request, from the committed ncu summaries"""
+    p = os.path.join(ROOT, "profiles", "roofline_constants.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p))
+        except Exception:
+            pass
+    return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=f,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            try:
+                self.proc.kill()
+            except Exception:
+                pass
+        try:
+            sm, mx, reasons = [], [], set()
+            for line in open(self.path):
+                t = [x.strip() for x in line.split(",")]
+                if len(t) < 9:
+                    continue
+                try:
+                    sm.append(float(t[1]))
+                    mx.append(float(t[2]))
+                except ValueError:
+                    continue
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"),
+                                   t[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            if sm:
+                out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                       "samples": len(sm)}
+            os.unlink(self.path)
+        except Exception:
+            pass
+        return out
+
+
+# ---------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of the default run, and --impl reference)
+# ---------------------------------------------------------------------------
+
+def oracle_sweep_sample(n_replicas: int, n: int, seed0: int, threads: int):
+    """Run the oracle on `n_replicas` replicas spread evenly over the sweep
+    (generate -> simulate -> p50/p90).  -> (requests, seconds)"""
+    import concurrent.futures as cf
+    import oracle as orc
+    cfg = wl.config3(n=n, seed0=seed0)
+    ln_dur, exp_t = wl.ln_dur_table(), wl.exp_table()
+    total = cfg["n_seeds"] * len(cfg["rates_mhz"]) * len(cfg["policies"])
+    picks = np.unique(np.linspace(0, total - 1, n_replicas).astype(np.int64))
+    cm = orc.cost(*cfg["cost"])
+    orc.lib()
+
+    def one(r):
+        t, pol = divmod(int(r), 3)
+        s, ri = divmod(t, 8)
+        dist = 1 if s >= cfg["n_seeds"] // 2 else 0
+        tr = orc.gen_trace(seed0 + s, cfg["rates_mhz"][ri], dist, n, ln_dur, exp_t)
+        lat, ttft, _, _ = orc.simulate(tr, cfg["policies"][pol], cm, cfg["slots"])
+        return (orc.percentile(lat, 50), orc.percentile(lat, 90), orc.percentile(ttft, 50), orc.percentile(ttft, 90))
+
+    t0 = time.perf_counter()
+    with cf.ThreadPoolExecutor(max_workers=threads) as ex:   # ctypes releases the GIL
+        list(ex.map(one, picks))
+    return len(picks) * n, time.perf_counter() - t0
+
+
+def oracle_select_sample(n_queues: int, q_len: int, threads: int):
+    import concurrent.futures as cf
+    import oracle as orc
+    cfg = wl.config5(q_len=q_len)
+    ln_dur = wl.ln_dur_table()
+    qs = orc.gen_queue(cfg["seed"], 0, n_queues * q_len, cfg["now"], ln_dur).reshape(n_queues, q_len)
+
+    def one(i):
+        for pol in cfg["policies"]:
+            orc.select(qs[i], pol, cfg["now"], cfg["k"])
+
+    t0 = time.perf_counter()
+    with cf.ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(one, range(n_queues)))
+    dt = time.perf_counter() - t0
+    return n_queues * q_len * 16 * len(cfg["policies"]) / dt / 1e9, dt
+
+
+def cpu_baseline(n: int, target_s: float = 12.0):
+    cores = os.cpu_count() or 1
+    req, dt = oracle_sweep_sample(cores, n, 0, cores)          # pilot: one replica per core
+    per_replica = dt / max(1, req // n) * cores
+    count = int(max(cores, min(4096, target_s * cores / max(per_replica, 1e-6))))
+    req, dt = oracle_sweep_sample(count, n, 0, cores)
+    sel_gbs, sel_dt = oracle_select_sample(max(cores * 8, 64), 4096, cores)
+    return {"value": req / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%d of the 98,304 config-3 replicas (evenly spaced over seeds x rates x policies, "
+                      "n=%d each; generate+simulate+p50/p90), %.1f s wall on %d threads" % (req // n, n, dt, cores),
+            "select_gbs": sel_gbs,
+            "select_sample": "%d config-5 queues x 4096, HRRN+SJF full sort, %.1f s" % (max(cores * 8, 64), sel_dt)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    per_step = max(cores, args.ref_replicas)
+    for _ in range(args.warmup):
+        oracle_sweep_sample(cores, args.n, 0, cores)
+    req_total, t_total = 0, 0.0
+    for s in range(args.steps):
+        req, dt = oracle_sweep_sample(per_step, args.n, 0, cores)
+        req_total += req
+        t_total += dt
+    value = req_total / t_total
+    sample = "%d config-3 replicas per step (evenly spaced over the sweep), n=%d" % (per_step, args.n)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / max(1, args.steps),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
+            "data": "synthetic",
+            "config": {"workload": "config3 replica sweep (sampled): seeds x 8 rates x 3 policies, "
+                                   "%d requests per replica, 32 slots" % args.n, "timing": "host wall clock"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------
+
+def run_ours(args):
+    import torch
+    import paper_2603_11273_b200 as asr
+    from paper_2603_11273_b200 import dist as D
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    rank, world, local = D.init()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    hbm_peak, peak_src = load_peaks()
+    consts = load_profile_constants()
+
+    # ---- inputs, resident in HBM before any timed region ------------------
+    cfg3 = wl.config3(n_seeds=args.seeds, n=args.n, seed0=D.seed_block(rank, args.seeds))
+    seeds, rates, dist = wl.config3_traces(cfg3)
+    n_traces, n, n_pol = len(seeds), cfg3["n"], len(cfg3["policies"])
+    n_rep = n_traces * n_pol
+    total = n_rep * n
+    specs = np.zeros(n_traces, dtype=asr.SPEC_DTYPE)
+    specs["seed"], specs["rate_mhz"], specs["dist"] = seeds, rates, dist
+    rep = asr.make_replicas(np.repeat(np.arange(n_traces, dtype=np.int64) * n, n_pol),
+                            np.arange(n_rep, dtype=np.int64) * n, n,
+                            np.tile(np.asarray(cfg3["policies"], dtype=np.int32), n_traces), cfg3["slots"], 0)
+    tables_h = asr.make_tables(wl.ln_dur_table(), wl.exp_table())
+    cost_h = asr.make_cost(*cfg3["cost"])
+    d_tables, d_specs, d_rep, d_cost = (asr.to_device(x, dev) for x in (tables_h, specs, rep, cost_h))
+    d_traces = torch.empty(n_traces * n * 16, dtype=torch.uint8, device=dev)
+    d_sum = torch.zeros(n_rep * asr.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    from paper_2603_11273_b200 import binding as B
+    d_ws = torch.empty(asr.workspace_bytes(B.OP_SIMULATE, total, n_rep, 1), dtype=torch.uint8, device=dev)
+
+    def sweep_step():
+        asr.gen_trace_batched(d_specs, n_traces, n, d_tables, out=d_traces)
+        asr.simulate_batched(d_traces, d_rep, n_rep, d_cost, 1, total, cfg3["slots"], None, None, d_sum, workspace=d_ws)
+
+    cfg5 = wl.config5(n_queues=args.queues)
+    nq, ql, k5, now5 = cfg5["n_queues"], cfg5["q_len"], cfg5["k"], cfg5["now"]
+    d_queues = asr.gen_queues(cfg5["seed"], rank * nq * ql, nq * ql, now5, d_tables)
+    d_idx = torch.empty((nq, k5), dtype=torch.int32, device=dev)
+
+    def select_step():
+        for pol in cfg5["policies"]:
+            asr.select_batched(d_queues, nq, ql, pol, now5, k5, out_idx=d_idx)
+
+    torch.cuda.synchronize()
+    for _ in range(args.warmup):
+        sweep_step()
+        select_step()
+    torch.cuda.synchronize()
+
+    # ---- timed regions ------------------------------------------------------
+    sampler = ClockSampler(local)
+    sampler.start()
+    asr.timing_enable(True)
+    asr.timing_reset()
+    launches0 = asr.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    D.barrier()
+    torch.cuda.synchronize()
+    ev[0].record()
+    for _ in range(args.steps):
+        sweep_step()
+    ev[1].record()
+    torch.cuda.synchronize()
+    D.barrier()
+    sweep_ms = D.max_over_ranks(ev[0].elapsed_time(ev[1]))
+    D.barrier()
+    torch.cuda.synchronize()
+    ev[2].record()
+    for _ in range(args.steps):
+        select_step()
+    ev[3].record()
+    torch.cuda.synchronize()
+    D.barrier()
+    select_ms = D.max_over_ranks(ev[2].elapsed_time(ev[3]))
+    launches = asr.launch_count() - launches0
+    ktimes = asr.timing_read()
+    asr.timing_enable(False)
+    clocks = sampler.stop()
+
+    summ = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
+    assert int((summ["n_done"] == n).sum()) == n_rep, "replicas did not finish"
+
+    value = world * total * args.steps / (sweep_ms / 1e3)
+    sel_bytes = nq * ql * 16 + nq * k5 * 4
+    select_gbs = world * sel_bytes * len(cfg5["policies"]) * args.steps / (select_ms / 1e3) / 1e9
+
+    def per_launch(name):
+        ms, cnt = ktimes.get(name, (0.0, 0))
+        return (ms / cnt if cnt else None), cnt, ms
+
+    sel_avg, sel_cnt, sel_tot = per_launch("select_topk_kernel")
+    sim_avg, sim_cnt, sim_tot = per_launch("sim_warp_kernel")
+    gen_avg, _, gen_tot = per_launch("gen_trace_kernel")
+    pct_avg, _, pct_tot = per_launch("summary_percentiles_kernel")
+    rooflines = {}
+    if sel_avg:
+        a = sel_bytes / (sel_avg / 1e3) / 1e9
+        rooflines["select_topk_kernel"] = {
+            "bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak,
+            "traffic": consts.get("select_dram_bytes_per_launch"), "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": sel_bytes, "avg_launch_ms": sel_avg, "frac_of_nominal_8TBs": a / 8000.0}
+    if sim_avg:
+        wi = consts.get("sim_warp_instr_per_request")
+        a = (wi * total / (sim_avg / 1e3)) if wi else None
+        rooflines["sim_warp_kernel"] = {
+            "bound": "alu", "achieved": a, "peak": ALU_PEAK_WARP_INSTR_PER_S, "unit": "warp-instr/s",
+            "frac": (a / ALU_PEAK_WARP_INSTR_PER_S) if a else None, "traffic": consts.get("sim_dram_bytes_per_launch"),
+            "warp_instr_per_request": wi, "avg_launch_ms": sim_avg,
+            "peak_source": "148 SMs x 4 schedulers x 1.965 GHz (DESIGN.md)"}
+    if gen_avg:
+        a = n_traces * n * 16 / (gen_avg / 1e3) / 1e9
+        rooflines["gen_trace_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
+                                         "frac": a / hbm_peak, "traffic": None, "avg_launch_ms": gen_avg}
+    if pct_avg:
+        a = 2 * total * 8 / (pct_avg / 1e3) / 1e9
+        rooflines["summary_percentiles_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
+                                                   "frac": a / hbm_peak, "traffic": None, "avg_launch_ms": pct_avg}
+    stage_ms = {"gen_trace_kernel": gen_tot, "sim_warp_kernel": sim_tot, "summary_percentiles_kernel": pct_tot}
+    dominant = max(stage_ms, key=lambda k_: stage_ms[k_] or 0.0)
+    roofline = dict(rooflines.get(dominant, {}), kernel=dominant,
+                    share_of_step=(stage_ms[dominant] / sweep_ms) if sweep_ms else None)
+
+    # ---- end to end through the host-buffer C-ABI calls ---------------------
+    e2e = None
+    if not args.no_e2e:
+        pol_h = np.asarray(cfg3["policies"], dtype=np.int32)
+        out_h = np.zeros(n_rep, dtype=asr.SUMMARY_DTYPE)
+        asr.sweep_host(specs, n, tables_h, pol_h, cfg3["slots"], cost_h, out_h)      # warm-up
+        D.barrier()
+        t0 = time.perf_counter()
+        e2e_steps = max(1, min(args.steps, 3))
+        for _ in range(e2e_steps):
+            asr.sweep_host(specs, n, tables_h, pol_h, cfg3["slots"], cost_h, out_h)
+        e2e_s = D.max_over_ranks(time.perf_counter() - t0)
+        assert np.array_equal(out_h.view(np.uint8), summ.view(np.uint8)), "host-buffer sweep disagrees"
+        h2d = specs.nbytes + tables_h.nbytes + cost_h.nbytes + pol_h.nbytes
+        e2e = {"value": world * total * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(out_h.nbytes), "steps": e2e_steps,
+               "call": "asr_sched_sweep_host (host specs/tables in, host summaries out; device scratch "
+                       "allocated inside the call)"}
+        # select with host records: pinned host keys in, host indices out
+        try:
+            h_keys = torch.empty(nq * ql * 16, dtype=torch.uint8, pin_memory=True)
+            h_keys.copy_(d_queues)
+            h_idx = torch.empty((nq, k5), dtype=torch.int32, pin_memory=True)
+            torch.cuda.synchronize()
+            asr.select_host(h_keys, nq, ql, cfg5["policies"][0], now5, k5, h_idx)   # warm-up
+            t0 = time.perf_counter()
+            for pol in cfg5["policies"]:
+                asr.select_host(h_keys, nq, ql, pol, now5, k5, h_idx)
+            dt = D.max_over_ranks(time.perf_counter() - t0)
+            e2e["select_gbs"] = world * sel_bytes * len(cfg5["policies"]) / dt / 1e9
+            e2e["select_h2d_bytes_per_call"] = int(nq * ql * 16)
+            e2e["select_d2h_bytes_per_call"] = int(nq * k5 * 4)
+            del h_keys
+        except Exception as exc:  # pinned allocation can fail on a small host
+            e2e["select_error"] = str(exc)[:200]
+
+    base = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        base = cpu_baseline(n)
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sweep_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+            "config": {
+                "workload": "config3 replica sweep: %d seeds x 8 rates x 3 policies = %d replicas x %d requests "
+                            "per GPU, 32 slots, config-1 cost model; half lognormal, half uniform durations"
+                            % (args.seeds, n_rep, n),
+                "select_workload": "config5: %d queues x %d records, now=1e10, k=32, HRRN+SJF" % (nq, ql),
+                "l2": "inputs_larger_than_l2 (traces %.2f GB, queues %.2f GB per GPU; L2 126 MB)"
+                      % (n_traces * n * 16 / 1e9, nq * ql * 16 / 1e9),
+                "parallelism": "replicas/queues sharded over %d GPU(s), no collective" % world,
+                "step": "gen_trace_batched -> simulate_batched(summary-only: simulate + p50/p90)"},
+            "select": {"metric": "priority-select GB/s vs HBM peak", "value": select_gbs, "unit": "GB/s",
+                       "ms_per_step": select_ms / args.steps, "policies": ["hrrn", "sjf"],
+                       "frac_of_measured_peak": select_gbs / world / hbm_peak,
+                       "frac_of_nominal_8TBs": select_gbs / world / 8000.0},
+            "roofline": roofline, "rooflines": rooflines, "clocks": clocks, "e2e": e2e,
+            "gpu_launches": int(launches), "cpu_baseline": base,
+            "kernel_ms_total": {k_: v[0] for k_, v in ktimes.items() if v[1]},
+        }
+        print(json.dumps(line), flush=True)
+    D.finalize()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--seeds", type=int, default=4096, help="config-3 seeds per GPU (4096 = the full config)")
+    ap.add_argument("--n", type=int, default=10000, help="requests per replica")
+    ap.add_argument("--queues", type=int, default=65536, help="config-5 queues per GPU")
+    ap.add_argument("--ref-replicas", type=int, default=256, help="--impl reference: replicas per step")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
