@@ -1,312 +1,423 @@
 // select.cu -- a2 priority keys + a3 batched top-k select (k <= 32), sm_100a.
 //
-// One warp owns one queue and STREAMS it from HBM exactly once with 128-bit
-// loads (8 independent loads per lane in flight, next tile prefetched).  The
-// exact k best so far live as a sorted list across the 32 lanes ("kept").
-// A record is looked at closely only if a cheap, conservative proxy test says
-// it might beat the current k-th best; such candidates are parked in a small
-// shared-memory buffer and merged into the kept list 32 at a time with a
-// bitonic sort + bitonic merge over warp shuffles.  Expected candidates per
-// queue are ~k(1+ln(n/k)), so the merge work is O(k log^2 k ln n) while the
-// stream is O(n): the kernel is HBM-bound by design (16 B per record).
+// One warp owns one queue at a time and STREAMS it from HBM exactly once.  The
+// queue is cut into chunks of SEL_CHUNK records (4 KB); lane 0 of the warp
+// moves each chunk into the warp's private ring of shared-memory stages with
+// one TMA bulk copy (cp.async.bulk, completion on an mbarrier), SEL_STAGES
+// chunks ahead of the consumer and across queue boundaries, so the data path
+// costs one instruction per 4 KB and no registers.  The 32 lanes then read the
+// stage with conflict-free 128-bit shared loads.
 //
-// Exactness.  Ordering inside the sort uses a 57-bit monotone surrogate key
-// (exact for FCFS/SJF up to the arrival resolution, a truncated fp64 ratio
-// for HRRN); whenever two surrogate keys are closer than the surrogate's
-// resolution the full integer comparator of asr_sched.h (int64
-// cross-multiplication for HRRN) decides, so the result is the
-// exact total order -- never an approximation of it.
+// Per record the warp runs ONE cheap, conservative, integer test against a
+// threshold record T ("could this record be among the k best?"):
+//   FCFS  arrival <= T.arrival
+//   SJF   (est, arrival) <= (T.est, T.arrival)
+//   HRRN  wait*T.est >= T.wait*est  in int64
+// Survivors (a few per cent) are appended to a small candidate buffer in
+// shared memory.  When the buffer fills, an exact quickselect over the buffer
+// (random pivot, full comparator of asr_sched.h incl. the (arrival, idx)
+// tie-break) keeps the best k..2k candidates and makes the worst kept one the
+// new T.  At the end of the queue the buffer is cut to exactly the k best and
+// sorted across the lanes with a bitonic network on the exact comparator.
+// Every decision that affects the output is taken by the exact integer
+// comparator, so the result is the unique total order -- never an approximation.
+// HBM-bound by design: 16 B read per record, 4k B written per queue.
 #include "launchers.cuh"
 
 namespace asr {
 
-constexpr int SEL_WARPS = 8;   // warps (= queues in flight) per CTA
-constexpr int SEL_TILE = 8;    // chunks of 32 records per tile: 8 x 16 B per lane in flight
-constexpr int SEL_PEND = 64;   // pending-candidate capacity per warp
-constexpr int SEL_SLOTS = 32 + SEL_PEND;
-constexpr uint64_t SEL_INF = ~0ull;  // "no element": key 2^57-1, slot 127
+constexpr int SEL_WARPS = 12;                   // warps (= queues in flight) per CTA, one CTA per SM
+constexpr int SEL_CHUNK = 256;                  // records per staged chunk (4 KB)
+constexpr int SEL_STAGES = 3;                   // TMA ring depth per warp
+constexpr int SEL_ROWS = 5;                     // candidate buffer: rows of 32
+constexpr int SEL_BUFCAP = SEL_ROWS * 32;       // 160 candidates
+constexpr int SEL_FLUSH_AT = SEL_BUFCAP - 32;   // cut the buffer once it holds more than this
+constexpr int SEL_UNROLL = 4;                   // records per lane between buffer checks
 
-struct __align__(16) SelWarpSmem {
-    int4 rec[SEL_SLOTS];       // (arrival lo, arrival hi, est, idx); 0..31 kept bank, 32.. pending
-    uint64_t pkey[SEL_PEND];   // surrogate key of each pending candidate
+struct __align__(128) SelWarpSmem {
+    int4 stage[SEL_STAGES][SEL_CHUNK];   // raw records (arrival lo, arrival hi, dur_ms | src idx, est)
+    int4 buf[SEL_BUFCAP];                // candidates (arrival lo, arrival hi, max(est,1), idx)
+    uint64_t full[SEL_STAGES];           // mbarriers: chunk landed
 };
+constexpr size_t SEL_SMEM_BYTES = sizeof(SelWarpSmem) * SEL_WARPS;
+
+// ---- TMA bulk copy + mbarrier (PTX) -------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
 
 __device__ __forceinline__ int64_t rec_arr(const int4 &r) {
     return (int64_t)(((uint64_t)(uint32_t)r.y << 32) | (uint32_t)r.x);
 }
 
-// 57-bit surrogate key, smaller = better.  Guarantee used below:
-//   key(a) + MARGIN < key(b)  ==>  a is strictly better than b.
-template <int POLICY>
-struct Surrogate;
-template <>
-struct Surrogate<ASR_FCFS> {
-    static constexpr uint64_t MARGIN = 0;
-    __device__ static uint64_t key(int64_t arr, int32_t, int64_t) {
-        return (uint64_t)arr & ((1ull << 57) - 1);
-    }
-};
-template <>
-struct Surrogate<ASR_SJF> {
-    static constexpr uint64_t MARGIN = 0;
-    __device__ static uint64_t key(int64_t arr, int32_t est, int64_t) {
-        // est < 2^25, arrival < 2^38: (est, arrival >> 6) packed
-        return ((uint64_t)est_of(est) << 32) | (((uint64_t)arr >> 6) & 0xFFFFFFFFull);
-    }
-};
-template <>
-struct Surrogate<ASR_HRRN> {
-    // fp64 quotient is within 2^-53 of wait/est; dropping 7 bits leaves 2^-45
-    // resolution, so keys two or more units apart are ordered with certainty.
-    static constexpr uint64_t MARGIN = 1;
-    __device__ static uint64_t key(int64_t arr, int32_t est, int64_t now) {
-        double q = __ll2double_rn(wait_of(arr, now)) / __ll2double_rn(est_of(est));
-        return (~(uint64_t)__double_as_longlong(q)) >> 7;
-    }
+// ---- threshold record T and the conservative per-record test -------------------
+struct Thr {
+    int64_t t64;
+    int32_t t32;
 };
 
-// a before b in the exact total order; a, b are packed (key << 7 | slot)
 template <int POLICY>
-__device__ __forceinline__ bool packed_less(uint64_t a, uint64_t b, const int4 *rec, int64_t now) {
-    uint64_t ka = a >> 7, kb = b >> 7;
-    uint64_t d = ka > kb ? ka - kb : kb - ka;
-    if (d > Surrogate<POLICY>::MARGIN || a == SEL_INF || b == SEL_INF) return a < b;
-    int4 ra = rec[a & 127], rb = rec[b & 127];
-    return better<POLICY>(rec_arr(ra), ra.z, ra.w, rec_arr(rb), rb.z, rb.w, now);
+__device__ __forceinline__ Thr thr_pass_all() {
+    Thr t;
+    if (POLICY == ASR_HRRN) {
+        t.t64 = 0;   // T.wait
+        t.t32 = 0;   // T.est = 0: 0 >= 0 passes everything
+    } else {
+        t.t64 = INT64_MAX;
+        t.t32 = INT32_MAX;
+    }
+    return t;
 }
 
+// T := candidate p (arrival lo, hi, est >= 1, idx)
 template <int POLICY>
-__device__ __forceinline__ uint64_t cmp_exchange(uint64_t v, int j, bool keep_min, const int4 *rec,
-                                                 int64_t now) {
-    uint64_t o = shfl64_xor(v, j);
-    bool v_less = packed_less<POLICY>(v, o, rec, now);
-    return (keep_min == v_less) ? v : o;
+__device__ __forceinline__ Thr thr_from(const int4 &p, int64_t now) {
+    Thr t;
+    if (POLICY == ASR_HRRN) {
+        t.t64 = wait_of(rec_arr(p), now);
+        t.t32 = t.t64 == 0 ? 0 : p.z;   // a zero-wait threshold ties with every clamped wait: pass all
+    } else {
+        t.t64 = rec_arr(p);
+        t.t32 = p.z;
+    }
+    return t;
 }
 
-// Merge up to 32 pending candidates (batch b) into the kept list K.
+// true for every record that is better than or ties with T (a superset is fine)
 template <int POLICY>
-__device__ __forceinline__ uint64_t merge_batch(uint64_t K, SelWarpSmem &sm, int b, int nP, int64_t now) {
+__device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr &t, int64_t now) {
+    if (POLICY == ASR_FCFS) return arr <= t.t64;
+    const int32_t e = est_raw < 1 ? 1 : est_raw;
+    if (POLICY == ASR_SJF) return e < t.t32 || (e == t.t32 && arr <= t.t64);
+    // HRRN: the signed wait is not clamped here: a negative wait fails unless T.est == 0
+    const int64_t w = now - arr;
+    return w * (int64_t)t.t32 >= t.t64 * (int64_t)e;
+}
+
+// ---- exact quickselect over the candidate buffer --------------------------------
+// Keeps the c+1 best candidates where c in [c_lo, c_hi] is the rank of an
+// accepted pivot (number of candidates strictly better than it); the pivot is
+// the worst kept candidate.  Precondition: c_lo < cnt.  Returns the new count.
+template <int POLICY>
+__device__ __forceinline__ int buffer_cut(int4 *buf, int cnt, int c_lo, int c_hi, int64_t now, uint32_t &seed,
+                                          int4 &pivot) {
     const int lane = lane_id();
-    const int pi = b * 32 + lane;
-    uint64_t P = pi < nP ? ((sm.pkey[pi] << 7) | (uint64_t)(32 + pi)) : SEL_INF;
-    // bitonic sort of P, ascending across lanes
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    int4 E[SEL_ROWS];
+    uint32_t alive = 0, keep = 0;
+#pragma unroll
+    for (int j = 0; j < SEL_ROWS; ++j) {
+        E[j] = buf[j * 32 + lane];
+        if (j * 32 + lane < cnt) alive |= 1u << j;
+    }
+    int base = 0;
+    int4 P = make_int4(0, 0, 1, -1);
+    for (;;) {
+        // uniform random pivot among the alive candidates: max of a per-candidate hash
+        seed = seed * 1664525u + 1013904223u;
+        uint32_t best = 0;
+#pragma unroll
+        for (int j = 0; j < SEL_ROWS; ++j) {
+            const uint32_t i = (uint32_t)(j * 32 + lane);
+            uint32_t h = (i + 1u) * 2654435761u ^ seed;
+            h ^= h >> 15;
+            h = (h * 2246822519u) | 0x80000000u;
+            h = (h & 0xFFFFFF00u) | i;
+            if ((alive >> j) & 1u) best = h > best ? h : best;
+        }
+        const uint32_t win = __reduce_max_sync(ASR_FULL_MASK, best);
+        if (win == 0u) break;   // nothing alive (cannot happen under the precondition)
+        const int pi = (int)(win & 0xFFu);
+        P = buf[pi];
+        const uint32_t pflag = (pi & 31) == lane ? (1u << (pi >> 5)) : 0u;
+        const int64_t p_arr = rec_arr(P);
+        uint32_t bflags = 0;
+        int c_alive = 0;
+#pragma unroll
+        for (int j = 0; j < SEL_ROWS; ++j) {
+            const bool b = ((alive >> j) & 1u) &&
+                           better<POLICY>(rec_arr(E[j]), E[j].z, E[j].w, p_arr, P.z, P.w, now);
+            c_alive += __popc(__ballot_sync(ASR_FULL_MASK, b));
+            bflags |= b ? (1u << j) : 0u;
+        }
+        const int c = base + c_alive;
+        if (c < c_lo) {            // pivot too good: it and everything better are certainly kept
+            const uint32_t mv = alive & (bflags | pflag);
+            keep |= mv;
+            alive &= ~mv;
+            base = c + 1;
+        } else if (c > c_hi) {     // pivot too lax: it and everything worse are dropped
+            alive &= bflags;
+        } else {
+            keep |= alive & (bflags | pflag);
+            break;
+        }
+    }
+    __syncwarp();
+    int off = 0;
+#pragma unroll
+    for (int j = 0; j < SEL_ROWS; ++j) {
+        const bool kp = (keep >> j) & 1u;
+        const uint32_t m = __ballot_sync(ASR_FULL_MASK, kp);
+        if (kp) buf[off + __popc(m & lt_mask)] = E[j];
+        off += __popc(m);
+    }
+    __syncwarp();
+    pivot = P;
+    return off;
+}
+
+// exact bitonic sort of one candidate per lane, best first; idx < 0 = empty (sorts last)
+template <int POLICY>
+__device__ __forceinline__ int4 sort32(int4 v, int64_t now) {
+    const int lane = lane_id();
 #pragma unroll
     for (int k = 2; k <= 32; k <<= 1) {
 #pragma unroll
         for (int j = k >> 1; j > 0; j >>= 1) {
-            bool up = (lane & k) == 0;
-            bool lower = (lane & j) == 0;
-            P = cmp_exchange<POLICY>(P, j, lower == up, sm.rec, now);
+            int4 o;
+            o.x = __shfl_xor_sync(ASR_FULL_MASK, v.x, j);
+            o.y = __shfl_xor_sync(ASR_FULL_MASK, v.y, j);
+            o.z = __shfl_xor_sync(ASR_FULL_MASK, v.z, j);
+            o.w = __shfl_xor_sync(ASR_FULL_MASK, v.w, j);
+            const bool up = (lane & k) == 0 || k == 32;
+            const bool want_min = ((lane & j) == 0) == up;
+            const bool v_less = v.w >= 0 && (o.w < 0 || better<POLICY>(rec_arr(v), v.z, v.w, rec_arr(o), o.z, o.w, now));
+            if (want_min != v_less) v = o;
         }
     }
-    // K ascending, reversed P descending -> element-wise min is the 32 best, bitonic
-    uint64_t Pr;
-    {
-        uint32_t lo = __shfl_sync(ASR_FULL_MASK, (uint32_t)P, 31 - lane);
-        uint32_t hi = __shfl_sync(ASR_FULL_MASK, (uint32_t)(P >> 32), 31 - lane);
-        Pr = ((uint64_t)hi << 32) | lo;
-    }
-    K = packed_less<POLICY>(K, Pr, sm.rec, now) ? K : Pr;
-#pragma unroll
-    for (int j = 16; j > 0; j >>= 1) K = cmp_exchange<POLICY>(K, j, (lane & j) == 0, sm.rec, now);
-    // move the survivors' payload into the kept bank, slot = lane
-    int4 r = make_int4(0, 0, 0, -1);
-    if (K != SEL_INF) r = sm.rec[K & 127];
-    __syncwarp();
-    sm.rec[lane] = r;
-    if (K != SEL_INF) K = (K & ~127ull) | (uint64_t)lane;
-    __syncwarp();
-    return K;
+    return v;
 }
 
 struct SelArgs {
     const asr_req_t *keys;
-    const int32_t *src_idx;     // INDIRECT: positions into keys (-1 = hole), else nullptr
-    const int32_t *q_count;     // nullable
+    const int32_t *src_idx;        // INDIRECT: positions into keys, else nullptr
+    const int32_t *q_count;        // nullable
     const int64_t *now_per_queue;  // nullable
     int32_t *out_idx;
     int64_t now;
-    int64_t total;              // total records (ragged last queue) or -1
+    int64_t total;                 // total records (ragged last queue) or -1
     int32_t n_queues;
     int32_t q_len;
     int32_t k;
-    int32_t global_idx;         // report q*q_len + j instead of j
+    int32_t global_idx;            // report q*q_len + j instead of j
 };
 
+__device__ __forceinline__ int sel_count(const SelArgs &a, int q) {
+    int count = a.q_count ? a.q_count[q] : a.q_len;
+    if (a.total >= 0) {
+        const int64_t left = a.total - (int64_t)q * a.q_len;
+        count = (int)(left < (int64_t)count ? (left < 0 ? 0 : left) : count);
+    }
+    return count < 0 ? 0 : (count > a.q_len ? a.q_len : count);
+}
+
+// per-queue selection state of one warp
+template <int POLICY>
+struct SelState {
+    Thr thr;
+    int cnt;
+    uint32_t seed;
+};
+
+// scan one staged chunk: `nvalid` records, the first one is record `rec0` of the queue
 template <int POLICY, bool INDIRECT>
-__global__ void __launch_bounds__(SEL_WARPS * 32) select_topk_kernel(SelArgs a) {
-    __shared__ SelWarpSmem smem[SEL_WARPS];
+__device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 *buf, int rec0, int nvalid,
+                                           int32_t idx_base, int k, int64_t now, SelState<POLICY> &s) {
+    const int lane = lane_id();
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const bool full = nvalid == SEL_CHUNK;
+#pragma unroll 1
+    for (int i = 0; i < SEL_CHUNK / 32; i += SEL_UNROLL) {
+        if (!full && i * 32 >= nvalid) break;
+        int4 r[SEL_UNROLL];
+        bool p[SEL_UNROLL];
+#pragma unroll
+        for (int u = 0; u < SEL_UNROLL; ++u) r[u] = stage[(i + u) * 32 + lane];
+#pragma unroll
+        for (int u = 0; u < SEL_UNROLL; ++u) {
+            p[u] = may_beat<POLICY>(rec_arr(r[u]), r[u].w, s.thr, now);
+            if (!full) p[u] = p[u] && ((i + u) * 32 + lane < nvalid);
+        }
+#pragma unroll
+        for (int u = 0; u < SEL_UNROLL; ++u) {
+            const uint32_t m = __ballot_sync(ASR_FULL_MASK, p[u]);
+            if (m == 0u) continue;
+            if (p[u]) {
+                const int32_t idx = INDIRECT ? r[u].z : idx_base + rec0 + (i + u) * 32 + lane;
+                buf[s.cnt + __popc(m & lt_mask)] = make_int4(r[u].x, r[u].y, r[u].w < 1 ? 1 : r[u].w, idx);
+            }
+            s.cnt += __popc(m);
+            if (s.cnt > SEL_FLUSH_AT) {
+                int4 pv;
+                const int slack = k > 16 ? k : 16;
+                s.cnt = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1 + slack, now, s.seed, pv);
+                s.thr = thr_from<POLICY>(pv, now);
+            }
+        }
+    }
+}
+
+// cut to the k best, sort them, write the indices of queue q
+template <int POLICY>
+__device__ __forceinline__ void finish_queue(int4 *buf, int32_t *out, int k, int64_t now, SelState<POLICY> &s) {
+    const int lane = lane_id();
+    __syncwarp();
+    if (s.cnt > k) {
+        int4 pv;
+        s.cnt = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1, now, s.seed, pv);
+    }
+    int4 v = lane < s.cnt ? buf[lane] : make_int4(0, 0, 1, -1);
+    v = sort32<POLICY>(v, now);
+    if (lane < k) out[lane] = v.w;
+    __syncwarp();
+}
+
+template <int POLICY, bool INDIRECT>
+__global__ void __launch_bounds__(SEL_WARPS * 32, 1) select_topk_kernel(SelArgs a) {
+    extern __shared__ __align__(128) unsigned char sel_dyn_smem[];
+    SelWarpSmem *smem = reinterpret_cast<SelWarpSmem *>(sel_dyn_smem);
     const int lane = lane_id();
     const int warp = threadIdx.x >> 5;
     SelWarpSmem &sm = smem[warp];
-    const uint32_t lt_mask = (1u << lane) - 1u;
     const int k = a.k;
+    const int gw = blockIdx.x * SEL_WARPS + warp;
+    const int GW = gridDim.x * SEL_WARPS;
 
-    for (int q = blockIdx.x * SEL_WARPS + warp; q < a.n_queues; q += gridDim.x * SEL_WARPS) {
-        const int64_t qbase = (int64_t)q * a.q_len;
-        int count = a.q_count ? a.q_count[q] : a.q_len;
-        if (a.total >= 0) {
-            int64_t left = a.total - qbase;
-            count = (int)(left < (int64_t)count ? (left < 0 ? 0 : left) : count);
+    if (!INDIRECT) {
+        if (threadIdx.x == 0) {
+            for (int w = 0; w < SEL_WARPS; ++w)
+                for (int s = 0; s < SEL_STAGES; ++s) mbar_init(&smem[w].full[s], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
-        count = count < 0 ? 0 : (count > a.q_len ? a.q_len : count);
+        __syncthreads();
+    }
+
+    // producer cursor: the next chunk to fetch is chunk pc of queue pq (pq >= n_queues: no more)
+    int pq = gw - GW, pc = 0, pn = 0, pcnt = 0;
+    auto next_chunk = [&]() {   // move to the next chunk that exists, skipping empty queues
+        while (pc >= pn) {
+            pq += GW;
+            if (pq >= a.n_queues) return;
+            pcnt = sel_count(a, pq);
+            pn = (pcnt + SEL_CHUNK - 1) / SEL_CHUNK;
+            pc = 0;
+        }
+    };
+    auto produce = [&](uint32_t g) {
+        if (pq >= a.n_queues) return;
+        const int st = (int)(g % SEL_STAGES);
+        const int left = pcnt - pc * SEL_CHUNK;
+        const uint32_t bytes = (uint32_t)(left < SEL_CHUNK ? left : SEL_CHUNK) * 16u;
+        if (lane == 0) {
+            mbar_expect_tx(&sm.full[st], bytes);
+            bulk_g2s(sm.stage[st], a.keys + (int64_t)pq * a.q_len + (int64_t)pc * SEL_CHUNK, bytes, &sm.full[st]);
+        }
+        pc++;
+        next_chunk();
+    };
+
+    uint32_t gp = 0, gc = 0;
+    if (!INDIRECT) {
+        next_chunk();
+#pragma unroll 1
+        for (int s = 0; s < SEL_STAGES; ++s) produce(gp++);
+    }
+
+    for (int q = gw; q < a.n_queues; q += GW) {
+        const int count = sel_count(a, q);
         const int64_t now = a.now_per_queue ? a.now_per_queue[q] : a.now;
-        const asr_req_t *base = a.keys + (INDIRECT ? 0 : qbase);
+        const int64_t qbase = (int64_t)q * a.q_len;
         const int32_t idx_base = a.global_idx ? (int32_t)qbase : 0;
-
-        uint64_t K = SEL_INF;   // kept list, lane i = i-th best so far (packed)
-        int nP = 0;             // pending candidates
-        // threshold record T = current k-th best (valid once k records are kept)
-        bool t_valid = false;
-        uint64_t t_key = 0;
-        int64_t t_arr = 0;
-        int32_t t_est = 0, t_idx = 0;
-        float t_qf = -1.0f;     // HRRN proxy: pass if wait_up >= t_qf * est
-
-        auto refresh_threshold = [&]() {
-            uint64_t Kk = (uint64_t)shfl64((int64_t)K, k - 1);
-            t_valid = Kk != SEL_INF;
-            if (t_valid) {
-                int4 r = sm.rec[Kk & 127];
-                t_key = Kk >> 7;
-                t_arr = rec_arr(r);
-                t_est = r.z;
-                t_idx = r.w;
-                if (POLICY == ASR_HRRN) {
-                    double q = __ll2double_rn(wait_of(t_arr, now)) / __ll2double_rn(est_of(t_est));
-                    float f = __double2float_rd(q);
-                    // one fp32 ulp of slack covers the fp64 rounding and the key margin
-                    t_qf = f > 0.0f ? __int_as_float(__float_as_int(f) - 1) : -1.0f;
-                }
-            }
-        };
-
-        auto flush = [&]() {
-            __syncwarp();
-            for (int b = 0; b * 32 < nP; ++b) K = merge_batch<POLICY>(K, sm, b, nP, now);
-            nP = 0;
-            if (k > 0) refresh_threshold();
-        };
-
-        auto consider = [&](const Rec &r, int32_t idx, bool valid) {
-            // cheap conservative proxy: a superset of {key <= t_key + MARGIN}
-            bool pass = valid;
-            if (t_valid) {
-                if (POLICY == ASR_FCFS) pass = pass && r.arrival_us <= t_arr;
-                if (POLICY == ASR_SJF) pass = pass && est_of(r.est) <= est_of(t_est);
-                if (POLICY == ASR_HRRN) {
-                    float w_up = __ll2float_ru(wait_of(r.arrival_us, now));
-                    float e_dn = __ll2float_rd(est_of(r.est));
-                    pass = pass && w_up >= __fmul_rd(t_qf, e_dn);
-                }
-            }
-            if (__ballot_sync(ASR_FULL_MASK, pass) == 0u) return;
-            uint64_t key = 0;
-            if (pass) {
-                key = Surrogate<POLICY>::key(r.arrival_us, r.est, now);
-                if (t_valid) {
-                    if (key > t_key + Surrogate<POLICY>::MARGIN) {
-                        pass = false;
-                    } else if (key + Surrogate<POLICY>::MARGIN >= t_key) {
-                        // too close for the surrogate: the integer comparator decides
-                        pass = better<POLICY>(r.arrival_us, r.est, idx, t_arr, t_est, t_idx, now);
-                    }
-                }
-            }
-            uint32_t m = __ballot_sync(ASR_FULL_MASK, pass);
-            if (m == 0u) return;
-            if (pass) {
-                int pos = nP + __popc(m & lt_mask);
-                sm.rec[32 + pos] = make_int4((int)(uint32_t)r.arrival_us, (int)(r.arrival_us >> 32),
-                                             r.est, idx);
-                sm.pkey[pos] = key;
-            }
-            nP += __popc(m);
-            if (nP >= 32) flush();
-        };
-
-        auto fetch = [&](int j, Rec &r, int32_t &idx, bool &valid) {
-            valid = j < count;
-            r.arrival_us = 0;
-            r.dur_ms = 0;
-            r.est = 1;
-            idx = idx_base + j;
+        SelState<POLICY> s;
+        s.thr = thr_pass_all<POLICY>();
+        s.cnt = 0;
+        s.seed = 0x9E3779B9u * (uint32_t)(q + 1);
+        const int nch = (count + SEL_CHUNK - 1) / SEL_CHUNK;
+#pragma unroll 1
+        for (int c = 0; c < nch; ++c) {
+            const int left = count - c * SEL_CHUNK;
+            const int nvalid = left < SEL_CHUNK ? left : SEL_CHUNK;
             if (INDIRECT) {
-                if (valid) {
-                    int32_t s = a.src_idx[qbase + j];
-                    valid = s >= 0;
-                    idx = s;
-                    if (valid) r = ld_cached(base + s);
+                __syncwarp();
+                for (int j = lane; j < nvalid; j += 32) {
+                    const int32_t src = a.src_idx[qbase + (int64_t)c * SEL_CHUNK + j];
+                    const int4 v = __ldg(reinterpret_cast<const int4 *>(a.keys + src));
+                    sm.stage[0][j] = make_int4(v.x, v.y, src, v.w);
                 }
-            } else if (valid) {
-                r = ld_stream(base + j);
-            }
-        };
-
-        const int ntiles = (count + SEL_TILE * 32 - 1) / (SEL_TILE * 32);
-        Rec cur[SEL_TILE];
-        int32_t cidx[SEL_TILE];
-        bool cval[SEL_TILE];
-        if (ntiles > 0) {
-#pragma unroll
-            for (int c = 0; c < SEL_TILE; ++c) fetch(c * 32 + lane, cur[c], cidx[c], cval[c]);
-        }
-        for (int t = 0; t < ntiles; ++t) {
-            Rec nxt[SEL_TILE];
-            int32_t nidx[SEL_TILE];
-            bool nval[SEL_TILE];
-            if (t + 1 < ntiles) {
-#pragma unroll
-                for (int c = 0; c < SEL_TILE; ++c)
-                    fetch((t + 1) * SEL_TILE * 32 + c * 32 + lane, nxt[c], nidx[c], nval[c]);
-            }
-#pragma unroll
-            for (int c = 0; c < SEL_TILE; ++c) consider(cur[c], cidx[c], cval[c]);
-            if (t + 1 < ntiles) {
-#pragma unroll
-                for (int c = 0; c < SEL_TILE; ++c) {
-                    cur[c] = nxt[c];
-                    cidx[c] = nidx[c];
-                    cval[c] = nval[c];
-                }
+                __syncwarp();
+                scan_chunk<POLICY, true>(sm.stage[0], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+            } else {
+                const int st = (int)(gc % SEL_STAGES);
+                mbar_wait(&sm.full[st], (gc / SEL_STAGES) & 1u);
+                scan_chunk<POLICY, false>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                __syncwarp();          // every lane is done reading the stage: refill it
+                produce(gp++);
+                gc++;
             }
         }
-        if (nP > 0) flush();
-        __syncwarp();
-        if (lane < k) {
-            int32_t o = -1;
-            if (K != SEL_INF) o = sm.rec[K & 127].w;
-            a.out_idx[(int64_t)q * k + lane] = o;
-        }
-        __syncwarp();
+        finish_queue<POLICY>(sm.buf, a.out_idx + (int64_t)q * k, k, now, s);
     }
 }
 
 template <int POLICY, bool INDIRECT>
 static int launch_one(const SelArgs &a, cudaStream_t st) {
     if (a.n_queues <= 0 || a.k <= 0) return ASR_OK;
-    static int blocks_per_sm = 0, n_sm = 0;
-    if (blocks_per_sm == 0) {
+    static int n_sm = 0;
+    static bool attr_set = false;
+    if (n_sm == 0) {
         int dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, select_topk_kernel<POLICY, INDIRECT>,
-                                                      SEL_WARPS * 32, 0);
-        if (blocks_per_sm < 1) blocks_per_sm = 1;
         if (n_sm < 1) n_sm = 148;
     }
-    int64_t want = ((int64_t)a.n_queues + SEL_WARPS - 1) / SEL_WARPS;
-    int64_t cap = (int64_t)n_sm * blocks_per_sm;
-    int grid = (int)(want < cap ? want : cap);
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(select_topk_kernel<POLICY, INDIRECT>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM_BYTES);
+        if (e != cudaSuccess) {
+            set_error("select_topk_kernel: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+            cudaGetLastError();
+            return ASR_ECUDA;
+        }
+        attr_set = true;
+    }
+    // persistent: one CTA of SEL_WARPS queue-streams per SM
+    const int64_t want = ((int64_t)a.n_queues + SEL_WARPS - 1) / SEL_WARPS;
+    const int grid = (int)(want < (int64_t)n_sm ? want : (int64_t)n_sm);
     {
         KernelTimer kt(KID_SELECT, st);
-        select_topk_kernel<POLICY, INDIRECT><<<grid, SEL_WARPS * 32, 0, st>>>(a);
+        select_topk_kernel<POLICY, INDIRECT><<<grid, SEL_WARPS * 32, SEL_SMEM_BYTES, st>>>(a);
     }
     return check_launch("select_topk_kernel");
 }
 
 int launch_select(const SelArgs &a, int policy, cudaStream_t st) {
     const bool ind = a.src_idx != nullptr;
+    if (!ind && (reinterpret_cast<uintptr_t>(a.keys) & 15u) != 0) {
+        set_error("select: keys must be 16-byte aligned");
+        return ASR_EINVAL;
+    }
     switch (policy) {
         case ASR_FCFS: return ind ? launch_one<ASR_FCFS, true>(a, st) : launch_one<ASR_FCFS, false>(a, st);
         case ASR_SJF: return ind ? launch_one<ASR_SJF, true>(a, st) : launch_one<ASR_SJF, false>(a, st);
@@ -358,6 +469,12 @@ static size_t select_ws_bytes(int64_t n, int64_t k) {
     return ints * sizeof(int32_t) + 256;
 }
 
+// valid prefix of a level array: every segment but the last reports k indices
+static int64_t level_valid(int64_t len, int64_t segs, int64_t k) {
+    const int64_t last = len - (segs - 1) * SEL_SEG;
+    return (segs - 1) * k + (last < k ? last : k);
+}
+
 extern "C" int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy, int64_t now, int32_t k,
                                 int32_t *out_idx, void *workspace, size_t workspace_bytes, void *stream) {
     if (n < 0 || k < 0 || policy < 0 || policy > 2 || n >= (1ll << 31)) {
@@ -390,17 +507,20 @@ extern "C" int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy
         int rc = launch_select(a, policy, st);
         if (rc) return rc;
     }
-    // further levels: select among the reported candidates (holes are -1)
-    int64_t len = segs * k;
+    // further levels: select among the reported candidates (the -1 padding of a
+    // short last segment sits at the very end of the level, outside `len`)
+    int64_t len = level_valid(n, segs, k);
+    int64_t stride = segs * k;
     while (true) {
         int64_t nsegs = (len + SEL_SEG - 1) / SEL_SEG;
-        int32_t *dst = nsegs == 1 ? out_idx : level + len;
+        int32_t *dst = nsegs == 1 ? out_idx : level + stride;
         SelArgs a{keys, level, nullptr, nullptr, dst, now, len, (int32_t)nsegs, (int32_t)SEL_SEG, k, 0};
         int rc = launch_select(a, policy, st);
         if (rc) return rc;
         if (nsegs == 1) break;
         level = dst;
-        len = nsegs * k;
+        len = level_valid(len, nsegs, k);
+        stride = nsegs * k;
     }
     return ASR_OK;
 }
