@@ -29,10 +29,10 @@ namespace asr {
 constexpr int SEL_WARPS = 12;                   // warps (= queues in flight) per CTA, one CTA per SM
 constexpr int SEL_CHUNK = 256;                  // records per staged chunk (4 KB)
 constexpr int SEL_STAGES = 3;                   // TMA ring depth per warp
-constexpr int SEL_ROWS = 5;                     // candidate buffer: rows of 32
-constexpr int SEL_BUFCAP = SEL_ROWS * 32;       // 160 candidates
-constexpr int SEL_FLUSH_AT = SEL_BUFCAP - 32;   // cut the buffer once it holds more than this
 constexpr int SEL_UNROLL = 4;                   // records per lane between buffer checks
+constexpr int SEL_ROWS = 8;                     // candidate buffer: rows of 32
+constexpr int SEL_BUFCAP = SEL_ROWS * 32;       // 256 candidates
+constexpr int SEL_FLUSH_AT = SEL_BUFCAP - 32 * SEL_UNROLL;   // cut the buffer once it holds more than this
 
 struct __align__(128) SelWarpSmem {
     int4 stage[SEL_STAGES][SEL_CHUNK];   // raw records (arrival lo, arrival hi, dur_ms | src idx, est)
@@ -118,49 +118,77 @@ __device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr
 // ---- exact quickselect over the candidate buffer --------------------------------
 // Keeps the c+1 best candidates where c in [c_lo, c_hi] is the rank of an
 // accepted pivot (number of candidates strictly better than it); the pivot is
-// the worst kept candidate.  Precondition: c_lo < cnt.  Returns the new count.
+// the worst kept candidate.  Precondition: c_lo < cnt <= SEL_BUFCAP.
+// Returns (position of the pivot in the compacted buffer << 16) | new count.
 template <int POLICY>
-__device__ __forceinline__ int buffer_cut(int4 *buf, int cnt, int c_lo, int c_hi, int64_t now, uint32_t &seed,
-                                          int4 &pivot) {
+__device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_hi, int64_t now, uint32_t seed) {
     const int lane = lane_id();
     const uint32_t lt_mask = (1u << lane) - 1u;
+    const int nrows = (cnt + 31) >> 5;
     int4 E[SEL_ROWS];
+    int64_t W[SEL_ROWS];      // HRRN: clamped wait of each candidate
+    uint32_t pri[SEL_ROWS];   // random priority (23 bits) | 0x100 | position
     uint32_t alive = 0, keep = 0;
 #pragma unroll
     for (int j = 0; j < SEL_ROWS; ++j) {
-        E[j] = buf[j * 32 + lane];
-        if (j * 32 + lane < cnt) alive |= 1u << j;
-    }
-    int base = 0;
-    int4 P = make_int4(0, 0, 1, -1);
-    for (;;) {
-        // uniform random pivot among the alive candidates: max of a per-candidate hash
-        seed = seed * 1664525u + 1013904223u;
-        uint32_t best = 0;
-#pragma unroll
-        for (int j = 0; j < SEL_ROWS; ++j) {
+        if (j < nrows) {
             const uint32_t i = (uint32_t)(j * 32 + lane);
+            E[j] = buf[i];
+            if ((int)i < cnt) alive |= 1u << j;
+            if (POLICY == ASR_HRRN) W[j] = wait_of(rec_arr(E[j]), now);
             uint32_t h = (i + 1u) * 2654435761u ^ seed;
             h ^= h >> 15;
-            h = (h * 2246822519u) | 0x80000000u;
-            h = (h & 0xFFFFFF00u) | i;
-            if ((alive >> j) & 1u) best = h > best ? h : best;
+            h *= 2246822519u;
+            pri[j] = (h & 0xFFFFFE00u) | 0x100u | i;
         }
+    }
+    int base = 0;
+    int pi = 0;
+    for (;;) {
+        // uniform random pivot among the alive candidates
+        seed = seed * 1664525u + 1013904223u;
+        const uint32_t sx = seed & 0xFFFFFE00u;
+        uint32_t best = 0;
+#pragma unroll
+        for (int j = 0; j < SEL_ROWS; ++j)
+            if (j < nrows) {
+                const uint32_t h = pri[j] ^ sx;
+                if ((alive >> j) & 1u) best = h > best ? h : best;
+            }
         const uint32_t win = __reduce_max_sync(ASR_FULL_MASK, best);
         if (win == 0u) break;   // nothing alive (cannot happen under the precondition)
-        const int pi = (int)(win & 0xFFu);
-        P = buf[pi];
+        pi = (int)(win & 0xFFu);
+        const int4 P = buf[pi];
         const uint32_t pflag = (pi & 31) == lane ? (1u << (pi >> 5)) : 0u;
         const int64_t p_arr = rec_arr(P);
+        const int64_t p_w = wait_of(p_arr, now);
         uint32_t bflags = 0;
         int c_alive = 0;
 #pragma unroll
-        for (int j = 0; j < SEL_ROWS; ++j) {
-            const bool b = ((alive >> j) & 1u) &&
-                           better<POLICY>(rec_arr(E[j]), E[j].z, E[j].w, p_arr, P.z, P.w, now);
-            c_alive += __popc(__ballot_sync(ASR_FULL_MASK, b));
-            bflags |= b ? (1u << j) : 0u;
-        }
+        for (int j = 0; j < SEL_ROWS; ++j)
+            if (j < nrows) {
+                const bool a = (alive >> j) & 1u;
+                bool gt, tie;
+                if (POLICY == ASR_HRRN) {
+                    const int64_t lhs = W[j] * (int64_t)P.z, rhs = p_w * (int64_t)E[j].z;
+                    gt = lhs > rhs;
+                    tie = lhs == rhs;
+                } else if (POLICY == ASR_SJF) {
+                    gt = E[j].z < P.z;
+                    tie = E[j].z == P.z;
+                } else {
+                    gt = false;
+                    tie = true;
+                }
+                if (POLICY == ASR_FCFS) {
+                    gt = earlier(rec_arr(E[j]), E[j].w, p_arr, P.w);
+                } else if (__any_sync(ASR_FULL_MASK, a && tie)) {   // rare: the (arrival, idx) tie-break
+                    if (tie) gt = earlier(rec_arr(E[j]), E[j].w, p_arr, P.w);
+                }
+                const bool bt = a && gt;
+                c_alive += __popc(__ballot_sync(ASR_FULL_MASK, bt));
+                bflags |= bt ? (1u << j) : 0u;
+            }
         const int c = base + c_alive;
         if (c < c_lo) {            // pivot too good: it and everything better are certainly kept
             const uint32_t mv = alive & (bflags | pflag);
@@ -176,16 +204,22 @@ __device__ __forceinline__ int buffer_cut(int4 *buf, int cnt, int c_lo, int c_hi
     }
     __syncwarp();
     int off = 0;
+    uint32_t ppos = 0;
 #pragma unroll
-    for (int j = 0; j < SEL_ROWS; ++j) {
-        const bool kp = (keep >> j) & 1u;
-        const uint32_t m = __ballot_sync(ASR_FULL_MASK, kp);
-        if (kp) buf[off + __popc(m & lt_mask)] = E[j];
-        off += __popc(m);
-    }
+    for (int j = 0; j < SEL_ROWS; ++j)
+        if (j < nrows) {
+            const bool kp = (keep >> j) & 1u;
+            const uint32_t m = __ballot_sync(ASR_FULL_MASK, kp);
+            if (kp) {
+                const int pos = off + __popc(m & lt_mask);
+                buf[pos] = E[j];
+                if (j * 32 + lane == pi) ppos = (uint32_t)pos;
+            }
+            off += __popc(m);
+        }
+    ppos = __reduce_max_sync(ASR_FULL_MASK, ppos);
     __syncwarp();
-    pivot = P;
-    return off;
+    return (ppos << 16) | (uint32_t)off;
 }
 
 // exact bitonic sort of one candidate per lane, best first; idx < 0 = empty (sorts last)
@@ -242,39 +276,44 @@ struct SelState {
 };
 
 // scan one staged chunk: `nvalid` records, the first one is record `rec0` of the queue
-template <int POLICY, bool INDIRECT>
+template <int POLICY, bool INDIRECT, bool FULL>
 __device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 *buf, int rec0, int nvalid,
                                            int32_t idx_base, int k, int64_t now, SelState<POLICY> &s) {
     const int lane = lane_id();
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const bool full = nvalid == SEL_CHUNK;
 #pragma unroll 1
     for (int i = 0; i < SEL_CHUNK / 32; i += SEL_UNROLL) {
-        if (!full && i * 32 >= nvalid) break;
+        if (!FULL && i * 32 >= nvalid) break;
         int4 r[SEL_UNROLL];
+        uint32_t m[SEL_UNROLL];
         bool p[SEL_UNROLL];
 #pragma unroll
         for (int u = 0; u < SEL_UNROLL; ++u) r[u] = stage[(i + u) * 32 + lane];
+        uint32_t many = 0;
 #pragma unroll
         for (int u = 0; u < SEL_UNROLL; ++u) {
             p[u] = may_beat<POLICY>(rec_arr(r[u]), r[u].w, s.thr, now);
-            if (!full) p[u] = p[u] && ((i + u) * 32 + lane < nvalid);
+            if (!FULL) p[u] = p[u] && ((i + u) * 32 + lane < nvalid);
+            m[u] = __ballot_sync(ASR_FULL_MASK, p[u]);
+            many |= m[u];
         }
+        if (many == 0u) continue;
 #pragma unroll
         for (int u = 0; u < SEL_UNROLL; ++u) {
-            const uint32_t m = __ballot_sync(ASR_FULL_MASK, p[u]);
-            if (m == 0u) continue;
+            if (m[u] == 0u) continue;
             if (p[u]) {
                 const int32_t idx = INDIRECT ? r[u].z : idx_base + rec0 + (i + u) * 32 + lane;
-                buf[s.cnt + __popc(m & lt_mask)] = make_int4(r[u].x, r[u].y, r[u].w < 1 ? 1 : r[u].w, idx);
+                buf[s.cnt + __popc(m[u] & lt_mask)] = make_int4(r[u].x, r[u].y, r[u].w < 1 ? 1 : r[u].w, idx);
             }
-            s.cnt += __popc(m);
-            if (s.cnt > SEL_FLUSH_AT) {
-                int4 pv;
-                const int slack = k > 16 ? k : 16;
-                s.cnt = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1 + slack, now, s.seed, pv);
-                s.thr = thr_from<POLICY>(pv, now);
-            }
+            s.cnt += __popc(m[u]);
+        }
+        if (s.cnt > SEL_FLUSH_AT) {
+            const int slack = k > 16 ? k : 16;
+            s.seed = s.seed * 747796405u + 2891336453u;
+            __syncwarp();
+            const uint32_t rc = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1 + slack, now, s.seed);
+            s.cnt = (int)(rc & 0xFFFFu);
+            s.thr = thr_from<POLICY>(buf[rc >> 16], now);
         }
     }
 }
@@ -285,8 +324,8 @@ __device__ __forceinline__ void finish_queue(int4 *buf, int32_t *out, int k, int
     const int lane = lane_id();
     __syncwarp();
     if (s.cnt > k) {
-        int4 pv;
-        s.cnt = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1, now, s.seed, pv);
+        s.seed = s.seed * 747796405u + 2891336453u;
+        s.cnt = (int)(buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1, now, s.seed) & 0xFFFFu);
     }
     int4 v = lane < s.cnt ? buf[lane] : make_int4(0, 0, 1, -1);
     v = sort32<POLICY>(v, now);
@@ -367,11 +406,14 @@ __global__ void __launch_bounds__(SEL_WARPS * 32, 1) select_topk_kernel(SelArgs 
                     sm.stage[0][j] = make_int4(v.x, v.y, src, v.w);
                 }
                 __syncwarp();
-                scan_chunk<POLICY, true>(sm.stage[0], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                scan_chunk<POLICY, true, false>(sm.stage[0], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
             } else {
                 const int st = (int)(gc % SEL_STAGES);
                 mbar_wait(&sm.full[st], (gc / SEL_STAGES) & 1u);
-                scan_chunk<POLICY, false>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                if (nvalid == SEL_CHUNK)
+                    scan_chunk<POLICY, false, true>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                else
+                    scan_chunk<POLICY, false, false>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
                 __syncwarp();          // every lane is done reading the stage: refill it
                 produce(gp++);
                 gc++;
