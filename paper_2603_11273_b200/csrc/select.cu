@@ -26,13 +26,13 @@
 
 namespace asr {
 
-constexpr int SEL_WARPS = 12;                   // warps (= queues in flight) per CTA, one CTA per SM
+constexpr int SEL_WARPS = 20;                   // warps (= queues in flight) per CTA, one CTA per SM
 constexpr int SEL_CHUNK = 256;                  // records per staged chunk (4 KB)
-constexpr int SEL_STAGES = 3;                   // TMA ring depth per warp
-constexpr int SEL_UNROLL = 4;                   // records per lane between buffer checks
-constexpr int SEL_ROWS = 8;                     // candidate buffer: rows of 32
-constexpr int SEL_BUFCAP = SEL_ROWS * 32;       // 256 candidates
-constexpr int SEL_FLUSH_AT = SEL_BUFCAP - 32 * SEL_UNROLL;   // cut the buffer once it holds more than this
+constexpr int SEL_STAGES = 2;                   // TMA ring depth per warp
+constexpr int SEL_UNROLL = 2;                   // records per lane loaded and tested together
+constexpr int SEL_ROWS = 6;                     // candidate buffer: rows of 32
+constexpr int SEL_BUFCAP = SEL_ROWS * 32;       // 192 candidates
+constexpr int SEL_FLUSH_AT = SEL_BUFCAP - 64;   // cut the buffer once it holds more than this (checked every 64 records)
 
 struct __align__(128) SelWarpSmem {
     int4 stage[SEL_STAGES][SEL_CHUNK];   // raw records (arrival lo, arrival hi, dur_ms | src idx, est)
@@ -104,6 +104,14 @@ __device__ __forceinline__ Thr thr_from(const int4 &p, int64_t now) {
     return t;
 }
 
+// a * b for |a| < 2^62 / b: one wide multiply + one multiply-add (the compiler's
+// generic 64x64 product costs twice that)
+__device__ __forceinline__ int64_t mul64x32(int64_t a, uint32_t b) {
+    const uint64_t lo = (uint64_t)(uint32_t)a * b;
+    const uint32_t hi = (uint32_t)(lo >> 32) + (uint32_t)(a >> 32) * b;
+    return (int64_t)(((uint64_t)hi << 32) | (uint32_t)lo);
+}
+
 // true for every record that is better than or ties with T (a superset is fine)
 template <int POLICY>
 __device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr &t, int64_t now) {
@@ -112,7 +120,7 @@ __device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr
     if (POLICY == ASR_SJF) return e < t.t32 || (e == t.t32 && arr <= t.t64);
     // HRRN: the signed wait is not clamped here: a negative wait fails unless T.est == 0
     const int64_t w = now - arr;
-    return w * (int64_t)t.t32 >= t.t64 * (int64_t)e;
+    return mul64x32(w, (uint32_t)t.t32) >= mul64x32(t.t64, (uint32_t)e);
 }
 
 // ---- exact quickselect over the candidate buffer --------------------------------
@@ -125,17 +133,19 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
     const int lane = lane_id();
     const uint32_t lt_mask = (1u << lane) - 1u;
     const int nrows = (cnt + 31) >> 5;
-    int4 E[SEL_ROWS];
-    int64_t W[SEL_ROWS];      // HRRN: clamped wait of each candidate
+    // per candidate, in registers: only what the common-case comparison needs
+    int64_t A[SEL_ROWS];      // HRRN: clamped wait; FCFS: arrival
+    int32_t Z[SEL_ROWS];      // HRRN, SJF: est; FCFS: idx
     uint32_t pri[SEL_ROWS];   // random priority (23 bits) | 0x100 | position
     uint32_t alive = 0, keep = 0;
 #pragma unroll
     for (int j = 0; j < SEL_ROWS; ++j) {
         if (j < nrows) {
             const uint32_t i = (uint32_t)(j * 32 + lane);
-            E[j] = buf[i];
+            const int4 e = buf[i];
             if ((int)i < cnt) alive |= 1u << j;
-            if (POLICY == ASR_HRRN) W[j] = wait_of(rec_arr(E[j]), now);
+            A[j] = POLICY == ASR_HRRN ? wait_of(rec_arr(e), now) : rec_arr(e);
+            Z[j] = POLICY == ASR_FCFS ? e.w : e.z;
             uint32_t h = (i + 1u) * 2654435761u ^ seed;
             h ^= h >> 15;
             h *= 2246822519u;
@@ -162,33 +172,41 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
         const uint32_t pflag = (pi & 31) == lane ? (1u << (pi >> 5)) : 0u;
         const int64_t p_arr = rec_arr(P);
         const int64_t p_w = wait_of(p_arr, now);
-        uint32_t bflags = 0;
-        int c_alive = 0;
+        uint32_t bflags = 0, tflags = 0;
 #pragma unroll
         for (int j = 0; j < SEL_ROWS; ++j)
             if (j < nrows) {
-                const bool a = (alive >> j) & 1u;
                 bool gt, tie;
                 if (POLICY == ASR_HRRN) {
-                    const int64_t lhs = W[j] * (int64_t)P.z, rhs = p_w * (int64_t)E[j].z;
+                    const int64_t lhs = mul64x32(A[j], (uint32_t)P.z), rhs = mul64x32(p_w, (uint32_t)Z[j]);
                     gt = lhs > rhs;
-                    tie = lhs == rhs;
+                    tie = (uint32_t)lhs == (uint32_t)rhs;   // necessary for equality; settled below
                 } else if (POLICY == ASR_SJF) {
-                    gt = E[j].z < P.z;
-                    tie = E[j].z == P.z;
+                    gt = Z[j] < P.z;
+                    tie = Z[j] == P.z;
                 } else {
-                    gt = false;
-                    tie = true;
+                    gt = earlier(A[j], Z[j], p_arr, P.w);
+                    tie = false;
                 }
-                if (POLICY == ASR_FCFS) {
-                    gt = earlier(rec_arr(E[j]), E[j].w, p_arr, P.w);
-                } else if (__any_sync(ASR_FULL_MASK, a && tie)) {   // rare: the (arrival, idx) tie-break
-                    if (tie) gt = earlier(rec_arr(E[j]), E[j].w, p_arr, P.w);
-                }
-                const bool bt = a && gt;
-                c_alive += __popc(__ballot_sync(ASR_FULL_MASK, bt));
-                bflags |= bt ? (1u << j) : 0u;
+                bflags |= gt ? (1u << j) : 0u;
+                tflags |= tie ? (1u << j) : 0u;
             }
+        tflags &= alive;
+        if (POLICY != ASR_FCFS && __any_sync(ASR_FULL_MASK, tflags != 0u)) {
+            // rare: equal keys -- the full comparator with its (arrival, idx) tie-break decides
+#pragma unroll
+            for (int j = 0; j < SEL_ROWS; ++j)
+                if (j < nrows && ((tflags >> j) & 1u)) {
+                    const int4 e = buf[j * 32 + lane];
+                    const bool bt = better<POLICY>(rec_arr(e), e.z, e.w, p_arr, P.z, P.w, now);
+                    bflags = (bflags & ~(1u << j)) | (bt ? (1u << j) : 0u);
+                }
+        }
+        bflags &= alive;
+        int c_alive = 0;
+#pragma unroll
+        for (int j = 0; j < SEL_ROWS; ++j)
+            if (j < nrows) c_alive += __popc(__ballot_sync(ASR_FULL_MASK, (bflags >> j) & 1u));
         const int c = base + c_alive;
         if (c < c_lo) {            // pivot too good: it and everything better are certainly kept
             const uint32_t mv = alive & (bflags | pflag);
@@ -202,6 +220,7 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
             break;
         }
     }
+    // in-place compaction, row by row: row j only writes positions <= its own
     __syncwarp();
     int off = 0;
     uint32_t ppos = 0;
@@ -209,10 +228,12 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
     for (int j = 0; j < SEL_ROWS; ++j)
         if (j < nrows) {
             const bool kp = (keep >> j) & 1u;
+            const int4 e = buf[j * 32 + lane];
             const uint32_t m = __ballot_sync(ASR_FULL_MASK, kp);
+            __syncwarp();
             if (kp) {
                 const int pos = off + __popc(m & lt_mask);
-                buf[pos] = E[j];
+                buf[pos] = e;
                 if (j * 32 + lane == pi) ppos = (uint32_t)pos;
             }
             off += __popc(m);
@@ -299,21 +320,24 @@ __device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 
         }
         if (many == 0u) continue;
 #pragma unroll
-        for (int u = 0; u < SEL_UNROLL; ++u) {
-            if (m[u] == 0u) continue;
-            if (p[u]) {
-                const int32_t idx = INDIRECT ? r[u].z : idx_base + rec0 + (i + u) * 32 + lane;
-                buf[s.cnt + __popc(m[u] & lt_mask)] = make_int4(r[u].x, r[u].y, r[u].w < 1 ? 1 : r[u].w, idx);
+        for (int half = 0; half < SEL_UNROLL; half += 2) {
+            if ((m[half] | m[half + 1]) == 0u) continue;
+#pragma unroll
+            for (int u = half; u < half + 2; ++u) {
+                if (p[u]) {
+                    const int32_t idx = INDIRECT ? r[u].z : idx_base + rec0 + (i + u) * 32 + lane;
+                    buf[s.cnt + __popc(m[u] & lt_mask)] = make_int4(r[u].x, r[u].y, r[u].w < 1 ? 1 : r[u].w, idx);
+                }
+                s.cnt += __popc(m[u]);
             }
-            s.cnt += __popc(m[u]);
-        }
-        if (s.cnt > SEL_FLUSH_AT) {
-            const int slack = k > 16 ? k : 16;
-            s.seed = s.seed * 747796405u + 2891336453u;
-            __syncwarp();
-            const uint32_t rc = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1 + slack, now, s.seed);
-            s.cnt = (int)(rc & 0xFFFFu);
-            s.thr = thr_from<POLICY>(buf[rc >> 16], now);
+            if (s.cnt > SEL_FLUSH_AT) {
+                const int slack = k > 16 ? k : 16;
+                s.seed = s.seed * 747796405u + 2891336453u;
+                __syncwarp();
+                const uint32_t rc = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1 + slack, now, s.seed);
+                s.cnt = (int)(rc & 0xFFFFu);
+                s.thr = thr_from<POLICY>(buf[rc >> 16], now);
+            }
         }
     }
 }
