@@ -146,7 +146,11 @@ int asr_sched_simulate(const asr_req_t *trace, int64_t n, int32_t policy,
                        int64_t *out_ttft, asr_summary_t *out_summary, void *workspace,
                        size_t workspace_bytes, void *stream);
 
-/* n_replicas independent replicas (seed x rate x policy), one warp each.
+/* n_replicas independent replicas (seed x rate x policy).  Batches of at least
+ * ASR_OPT_SIM_LANE_MIN_REPLICAS replicas with max_slots <= 32 run one THREAD
+ * per replica until a replica has to choose among waiting requests under
+ * SJF/HRRN; such replicas, and every other batch, run one WARP per replica.
+ * The results do not depend on which kernel ran.
  *   traces DEVICE; replicas DEVICE [n_replicas]; cms DEVICE [n_cms];
  *   out_lat/out_ttft DEVICE [total_requests] indexed by replica.out_off, or both
  *   NULL for summary-only mode (the arrays then live in the workspace);
@@ -222,6 +226,13 @@ enum { ASR_OP_SELECT = 0, ASR_OP_SIMULATE = 1, ASR_OP_PERCENTILES = 2 };
  * b = n_replicas, c = 1 if summary-only (out_lat/out_ttft NULL) else 0.
  * PERCENTILES: a = total values, b = n_seg.  Returns 0 for an unknown op. */
 size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c);
+
+/* Process-wide tuning options (never change any result).
+ * ASR_OPT_SIM_LANE_MIN_REPLICAS: smallest batch that asr_sched_simulate_batched
+ * runs thread-per-replica (default 1024; 1 = always when max_slots <= 32;
+ * INT32_MAX = never). */
+enum { ASR_OPT_SIM_LANE_MIN_REPLICAS = 0 };
+int asr_sched_set_option(int32_t option, int64_t value);
 
 const char *asr_sched_last_error(void); /* thread-local, never NULL */
 int asr_sched_version(void);

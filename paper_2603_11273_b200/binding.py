@@ -32,7 +32,7 @@ EXPORTS = (
     "asr_sched_percentiles", "asr_sched_gen_trace", "asr_sched_gen_trace_batched", "asr_sched_gen_queues",
     "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_workspace_bytes", "asr_sched_last_error",
     "asr_sched_version", "asr_sched_launch_count", "asr_sched_timing_enable", "asr_sched_timing_reset",
-    "asr_sched_timing_read", "asr_sched_kernel_name",
+    "asr_sched_timing_read", "asr_sched_kernel_name", "asr_sched_set_option",
 )
 
 
@@ -78,6 +78,8 @@ def lib():
         L.asr_sched_timing_read.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(i64)]
         L.asr_sched_kernel_name.argtypes = [i32]
         L.asr_sched_kernel_name.restype = C.c_char_p
+        L.asr_sched_set_option.argtypes = [i32, i64]
+        L.asr_sched_set_option.restype = C.c_int
         _lib = L
     return _lib
 
@@ -92,6 +94,13 @@ def last_error() -> str:
 
 def launch_count() -> int:
     return int(lib().asr_sched_launch_count())
+
+
+OPT_SIM_LANE_MIN_REPLICAS = 0
+
+
+def set_option(option: int, value: int):
+    _check(lib().asr_sched_set_option(option, value), "asr_sched_set_option")
 
 
 def timing_enable(on: bool):

@@ -1,6 +1,7 @@
 // api.cu -- C ABI of libasr_sched (include/asr_sched.h): argument checks,
 // workspace carving, launch sequencing.  No compute happens on the host.
 #include <atomic>
+#include <climits>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -34,7 +35,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
-    "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "summary_percentiles_kernel",
+    "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
     "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel"};
 struct TimedLaunch {
     int kid;
@@ -76,15 +77,19 @@ KernelTimer::~KernelTimer() {
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct SimWorkspace {
-    size_t bm_off_bytes, bitmap_bytes, lat_bytes, total;
+    size_t bm_off_bytes, bitmap_bytes, defer_bytes, lat_bytes, total;
 };
+
+// asr_sched_set_option values
+static std::atomic<int> g_opt_lane_min{1024};
 
 static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summary_only) {
     SimWorkspace w;
     w.bm_off_bytes = align_up(sizeof(int64_t) * (size_t)(n_replicas + 1));
     w.bitmap_bytes = align_up(sizeof(uint32_t) * (size_t)(total_requests / 32 + 2 * n_replicas + 2));
+    w.defer_bytes = align_up(sizeof(int32_t) * (size_t)(n_replicas + 64));   // [0]: counter, [64..]: list
     w.lat_bytes = summary_only ? align_up(sizeof(int64_t) * (size_t)total_requests) : 0;
-    w.total = w.bm_off_bytes + w.bitmap_bytes + 2 * w.lat_bytes;
+    w.total = w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + 2 * w.lat_bytes;
     return w;
 }
 
@@ -104,6 +109,17 @@ using namespace asr;
 extern "C" const char *asr_sched_last_error(void) { return g_err; }
 extern "C" int asr_sched_version(void) { return ASR_SCHED_VERSION; }
 extern "C" int64_t asr_sched_launch_count(void) { return (int64_t)g_launches.load(); }
+
+extern "C" int asr_sched_set_option(int32_t option, int64_t value) {
+    switch (option) {
+        case ASR_OPT_SIM_LANE_MIN_REPLICAS:
+            if (value < 1 || value > INT32_MAX) break;
+            g_opt_lane_min.store((int)value);
+            return ASR_OK;
+    }
+    set_error("set_option: bad option %d or value %lld", option, (long long)value);
+    return ASR_EINVAL;
+}
 
 extern "C" int asr_sched_timing_enable(int on) {
     std::lock_guard<std::mutex> g(g_timing_mu);
@@ -193,14 +209,18 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     char *ws = (char *)workspace;
     int64_t *bm_off = (int64_t *)ws;
     uint32_t *bitmap = (uint32_t *)(ws + w.bm_off_bytes);
+    int32_t *defer = (int32_t *)(ws + w.bm_off_bytes + w.bitmap_bytes);
     if (summary_only) {
-        out_lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes);
-        out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.lat_bytes);
+        out_lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes);
+        out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + w.lat_bytes);
     }
-    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, st);
+    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
     if (rc) return rc;
-    SimArgs a{traces, replicas, cms, bm_off, bitmap, out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms};
-    rc = launch_simulate(a, max_slots, st);
+    SimArgs a{traces, replicas, cms,      bm_off,         bitmap,     defer + 64, defer,
+              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms};
+    // many small replicas: one thread each; few or wide ones: one warp each
+    const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
+    rc = launch_simulate(a, max_slots, use_lane, st);
     if (rc) return rc;
     if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
     return rc;

@@ -10,6 +10,8 @@ struct SimArgs {
     const asr_cost_model_t *cms;
     const int64_t *bm_off;    // [n_replicas] first bitmap word of each replica
     uint32_t *bitmap;
+    int32_t *defer_list;      // [n_replicas] replicas handed from the lane kernel to the warp kernel
+    int32_t *defer_count;     // [1]
     int64_t *out_lat;
     int64_t *out_ttft;
     asr_summary_t *out_summary;  // nullable
@@ -18,8 +20,9 @@ struct SimArgs {
     int32_t n_cms;
 };
 
-int launch_simulate(const SimArgs &a, int max_slots, cudaStream_t st);
-int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, cudaStream_t st);
+int launch_simulate(const SimArgs &a, int max_slots, bool use_lane, cudaStream_t st);
+int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,
+                       cudaStream_t st);
 int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg, const int32_t *pcts,
                        int32_t n_pct, int64_t *out, cudaStream_t st);
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,

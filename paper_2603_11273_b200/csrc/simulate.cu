@@ -50,28 +50,34 @@ __device__ __forceinline__ int64_t warp_sum_u32(uint32_t v) {
     return ((int64_t)hi << 16) + (int64_t)lo;
 }
 
+// true if the descriptor of replica r can be simulated with `max_slots` slots per replica
+__device__ __forceinline__ bool replica_ok(const SimArgs &a, const asr_replica_t &rep, int max_slots) {
+    return rep.n >= 0 && rep.slots >= 1 && rep.slots <= max_slots && rep.policy >= 0 && rep.policy <= 2 &&
+           rep.cm_id >= 0 && rep.cm_id < a.n_cms && rep.trace_off >= 0 && rep.out_off >= 0 &&
+           rep.out_off + (int64_t)rep.n <= a.total_requests;
+}
+
+__device__ __forceinline__ void flag_invalid(const SimArgs &a, int r) {
+    if (!a.out_summary) return;
+    asr_summary_t s;
+    s.p50_e2e_us = s.p90_e2e_us = s.p50_ttft_us = s.p90_ttft_us = -1;
+    s.first_arrival_us = s.last_done_us = 0;
+    s.n_done = -1;
+    a.out_summary[r] = s;
+}
+
+// one warp simulates replica r from start to end
 template <int SPL>
-__global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
+__device__ __forceinline__ void sim_warp_replica(const SimArgs &a, const int r) {
     const int lane = lane_id();
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const int r = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
-    if (r >= a.n_replicas) return;
 
     const asr_replica_t rep = a.replicas[r];
     const int n = rep.n;
     const int slots = rep.slots;
     const int policy = rep.policy;
-    const bool ok = n >= 0 && slots >= 1 && slots <= 32 * SPL && policy >= 0 && policy <= 2 &&
-                    rep.cm_id >= 0 && rep.cm_id < a.n_cms && rep.trace_off >= 0 && rep.out_off >= 0 &&
-                    rep.out_off + (int64_t)n <= a.total_requests;
-    if (!ok) {
-        if (a.out_summary && lane == 0) {
-            asr_summary_t s;
-            s.p50_e2e_us = s.p90_e2e_us = s.p50_ttft_us = s.p90_ttft_us = -1;
-            s.first_arrival_us = s.last_done_us = 0;
-            s.n_done = -1;
-            a.out_summary[r] = s;
-        }
+    if (!replica_ok(a, rep, 32 * SPL)) {
+        if (lane == 0) flag_invalid(a, r);
         return;
     }
     const asr_cost_model_t cm = a.cms[rep.cm_id];
@@ -300,12 +306,166 @@ __global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
     }
 }
 
+// warp-per-replica kernel.  Direct mode: warp w of the grid simulates replica w.
+// Worklist mode (a.defer_list != nullptr): the warps share the replicas that the
+// lane kernel below handed over, defer_list[0 .. *defer_count).
+template <int SPL>
+__global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
+    const int gw = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
+    if (a.defer_list == nullptr) {
+        if (gw < a.n_replicas) sim_warp_replica<SPL>(a, gw);
+        return;
+    }
+    const int cnt = *a.defer_count;
+    for (int w = gw; w < cnt; w += gridDim.x * SIM_WARPS) sim_warp_replica<SPL>(a, a.defer_list[w]);
+}
+
+// ---------------------------------------------------------------------------
+// lane-per-replica kernel: ONE THREAD simulates one replica.
+//
+// At the loads of the replica sweep (0.5-4 req/s against a capacity of 10-27
+// req/s) a replica has a handful of running requests, so a warp-wide running
+// set leaves most lanes idle.  Here every lane runs its own event loop: the
+// running set is a compact array of (finish iteration, request index) pairs
+// in shared memory, laid out [slot][thread] so that lane accesses never
+// conflict; the trace is read with 16-byte loads.  "Finish iteration" is the
+// engine-iteration counter at which the request emits its last token
+// (counter at admission + tokens), kept modulo 2^32: remaining = fin - it is
+// exact because remaining < 2^31.  The fast-forward is the one of the warp
+// kernel.  The three policy replicas of one trace sit in adjacent lanes and
+// read the same addresses.
+//
+// Only the uncontended regime is handled here: as soon as SJF/HRRN must CHOOSE
+// (more waiting than free slots), the thread appends its replica to defer_list
+// and stops; the warp kernel then simulates that replica from the start with
+// its coalesced window scan.  Results are identical either way.
+// ---------------------------------------------------------------------------
+constexpr int LANE_THREADS = 128;
+constexpr int LANE_CAP = 32;   // slots per replica handled by the lane kernel
+
+__device__ __forceinline__ int64_t ld_arrival(const asr_req_t *p) {
+    return __ldg(reinterpret_cast<const long long *>(p));
+}
+
+__global__ void __launch_bounds__(LANE_THREADS) sim_lane_kernel(SimArgs a) {
+    __shared__ uint32_t s_fin[LANE_CAP * LANE_THREADS];
+    __shared__ int32_t s_idx[LANE_CAP * LANE_THREADS];
+    const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
+    if (r >= a.n_replicas) return;
+    const asr_replica_t rep = a.replicas[r];
+    if (!replica_ok(a, rep, LANE_CAP)) {
+        flag_invalid(a, r);
+        return;
+    }
+    uint32_t *fin = s_fin + threadIdx.x;
+    int32_t *sidx = s_idx + threadIdx.x;
+    const int n = rep.n, slots = rep.slots, policy = rep.policy;
+    const asr_cost_model_t *cmp = a.cms + rep.cm_id;
+    const int64_t enc_base = __ldg(&cmp->enc_base_us), enc_per_ms = __ldg(&cmp->enc_per_ms_us);
+    const int64_t iter_base = __ldg(&cmp->iter_base_us), iter_per = __ldg(&cmp->iter_per_running_us);
+    const int64_t tok_base = __ldg(&cmp->tok_base), tok_per_s = __ldg(&cmp->tok_per_s);
+    const asr_req_t *trace = a.traces + rep.trace_off;
+    int64_t *lat = a.out_lat + rep.out_off;
+    int64_t *ttft = a.out_ttft + rep.out_off;
+
+    int64_t t = 0;
+    int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
+    uint32_t it = 0;   // engine iterations so far, mod 2^32
+    int64_t next_arr = n > 0 ? ld_arrival(trace) : INT64_MAX;
+    const int64_t first_arrival = n > 0 ? next_arr : 0;
+    bool deferred = false;
+
+    while (done < n) {
+        // idle server: the clock jumps to the next arrival (S14)
+        if (nR == 0 && nW == 0 && next_arr > t) t = next_arr;
+        // 1. ingest arrivals <= t
+        while (next_arr <= t) {
+            ++p;
+            ++nW;
+            next_arr = p < n ? ld_arrival(trace + p) : INT64_MAX;
+        }
+        // 3. admit
+        const int free_slots = slots - nR;
+        const int k = free_slots < nW ? free_slots : nW;
+        int64_t t1 = t + iter_base + iter_per * (int64_t)(nR + k);
+        if (k > 0) {
+            if (policy != ASR_FCFS && k < nW) {   // a real choice: hand over to the warp kernel
+                deferred = true;
+                break;
+            }
+            int64_t dur_sum = 0;
+            for (int q = 0; q < k; ++q) {
+                const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo + q));
+                int64_t tok = tok_base + (tok_per_s * (int64_t)v.z) / 1000;
+                tok = tok < 1 ? 1 : (tok > 0x7FFFFFFE ? 0x7FFFFFFE : tok);
+                fin[(nR + q) * LANE_THREADS] = it + (uint32_t)tok;
+                sidx[(nR + q) * LANE_THREADS] = lo + q;
+                dur_sum += (int64_t)v.z;
+            }
+            t1 += enc_base * (int64_t)k + enc_per_ms * dur_sum;
+            for (int q = 0; q < k; ++q) ttft[lo + q] = t1 - ld_arrival(trace + lo + q);   // first token (S9)
+            lo += k;
+            nW -= k;
+            nR += k;
+        }
+        // 4. fast-forward over identical iterations to the next event
+        uint32_t m = 0xFFFFFFFFu;
+        for (int s = 0; s < nR; ++s) {
+            const uint32_t left = fin[s * LANE_THREADS] - it;
+            m = left < m ? left : m;
+        }
+        const int64_t c = iter_base + iter_per * (int64_t)nR;
+        int64_t j = 1;
+        if (m > 1u) {
+            if (nR == slots || p >= n || c <= 0) {
+                j = m;
+            } else {
+                const int64_t g = next_arr - t1;
+                if (g <= 0) j = 1;
+                else if (g > (int64_t)(m - 2u) * c) j = m;
+                else j = 1 + ceil_div_pos(g, c);
+            }
+        }
+        t = t1 + (j - 1) * c;
+        it += (uint32_t)j;
+        // 5. completions
+        if ((uint32_t)j == m) {
+            for (int s = 0; s < nR;) {
+                if (fin[s * LANE_THREADS] == it) {
+                    const int32_t i = sidx[s * LANE_THREADS];
+                    lat[i] = t - ld_arrival(trace + i);
+                    --nR;
+                    fin[s * LANE_THREADS] = fin[nR * LANE_THREADS];
+                    sidx[s * LANE_THREADS] = sidx[nR * LANE_THREADS];
+                    ++done;
+                } else {
+                    ++s;
+                }
+            }
+        }
+    }
+    if (deferred) {
+        const int pos = atomicAdd(a.defer_count, 1);
+        a.defer_list[pos] = r;
+        return;
+    }
+    if (a.out_summary) {
+        asr_summary_t *s = a.out_summary + r;
+        s->first_arrival_us = first_arrival;
+        s->last_done_us = t;
+        s->n_done = done;
+    }
+}
+
 // exclusive prefix sum of the per-replica bitmap sizes (words), one CTA
 __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *replicas, int32_t n_replicas,
-                                                           int64_t *bm_off) {
+                                                           int64_t *bm_off, int32_t *defer_count) {
     __shared__ int64_t warp_tot[32];
     __shared__ int64_t carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
+    if (threadIdx.x == 0) {
+        carry_s = 0;
+        *defer_count = 0;
+    }
     __syncthreads();
     const int lane = lane_id(), warp = threadIdx.x >> 5;
     for (int base = 0; base < n_replicas; base += 1024) {
@@ -342,23 +502,46 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
     }
 }
 
-int launch_simulate(const SimArgs &a, int max_slots, cudaStream_t st) {
-    if (a.n_replicas <= 0) return ASR_OK;
-    const int grid = (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS;
-    {
-        KernelTimer kt(KID_SIMULATE, st);
-        if (max_slots <= 32) sim_warp_kernel<1><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-        else if (max_slots <= 64) sim_warp_kernel<2><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-        else if (max_slots <= 128) sim_warp_kernel<4><<<grid, SIM_WARPS * 32, 0, st>>>(a);
-        else sim_warp_kernel<8><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+template <int SPL>
+static void launch_warp(const SimArgs &a, int grid, cudaStream_t st) {
+    KernelTimer kt(KID_SIMULATE, st);
+    sim_warp_kernel<SPL><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+}
+
+static void launch_warp_any(const SimArgs &a, int max_slots, int grid, cudaStream_t st) {
+    if (max_slots <= 32) launch_warp<1>(a, grid, st);
+    else if (max_slots <= 64) launch_warp<2>(a, grid, st);
+    else if (max_slots <= 128) launch_warp<4>(a, grid, st);
+    else launch_warp<8>(a, grid, st);
+}
+
+// use_lane: thread-per-replica kernel first (slots <= 32), then the warp kernel
+// on the replicas it handed over; else the warp kernel on everything.
+int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStream_t st) {
+    if (a_in.n_replicas <= 0) return ASR_OK;
+    SimArgs a = a_in;
+    if (use_lane && max_slots <= LANE_CAP) {
+        {
+            KernelTimer kt(KID_SIM_LANE, st);
+            sim_lane_kernel<<<(a.n_replicas + LANE_THREADS - 1) / LANE_THREADS, LANE_THREADS, 0, st>>>(a);
+        }
+        int rc = check_launch("sim_lane_kernel");
+        if (rc) return rc;
+        // worklist pass: empty (and a few microseconds) when nothing was handed over
+        const int want = (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS;
+        launch_warp_any(a, max_slots, want < 148 * 8 ? want : 148 * 8, st);
+        return check_launch("sim_warp_kernel");
     }
+    a.defer_list = nullptr;
+    launch_warp_any(a, max_slots, (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS, st);
     return check_launch("sim_warp_kernel");
 }
 
-int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, cudaStream_t st) {
+int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,
+                       cudaStream_t st) {
     {
         KernelTimer kt(KID_SIM_PREPARE, st);
-        sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, bm_off);
+        sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, bm_off, defer_count);
     }
     return check_launch("sim_prepare_kernel");
 }

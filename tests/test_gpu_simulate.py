@@ -11,11 +11,21 @@ POL = (orc.FCFS, orc.SJF, orc.HRRN)
 
 
 @pytest.fixture(scope="module")
-def asr():
+def asr_mod():
     import torch
     assert torch.cuda.is_available()
     import paper_2603_11273_b200 as asr
     return asr
+
+
+@pytest.fixture(params=["warp", "lane"])
+def asr(asr_mod, request):
+    """every test runs twice: warp-per-replica only, and thread-per-replica first
+    (with hand-over to the warp kernel where SJF/HRRN must choose)"""
+    big = 2**31 - 1
+    asr_mod.set_option(asr_mod.OPT_SIM_LANE_MIN_REPLICAS, 1 if request.param == "lane" else big)
+    yield asr_mod
+    asr_mod.set_option(asr_mod.OPT_SIM_LANE_MIN_REPLICAS, 1024)
 
 
 def test_fig1_toy(asr):
