@@ -52,6 +52,10 @@ __device__ __forceinline__ Rec ld_stream(const asr_req_t *p) {
     return r;
 }
 
+__device__ __forceinline__ int64_t rec_arrival(const int4 &v) {
+    return (int64_t)(((uint64_t)(uint32_t)v.y << 32) | (uint32_t)v.x);
+}
+
 // cached load (trace windows that are re-read by the simulator)
 __device__ __forceinline__ Rec ld_cached(const asr_req_t *p) {
     int4 v = __ldg(reinterpret_cast<const int4 *>(p));

@@ -340,14 +340,22 @@ __global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
 // and stops; the warp kernel then simulates that replica from the start with
 // its coalesced window scan.  Results are identical either way.
 // ---------------------------------------------------------------------------
-constexpr int LANE_THREADS = 128;
+constexpr int LANE_THREADS = 64;
+constexpr int LANE_BLOCKS_PER_SM = 12;
 constexpr int LANE_CAP = 32;   // slots per replica handled by the lane kernel
 
 __device__ __forceinline__ int64_t ld_arrival(const asr_req_t *p) {
     return __ldg(reinterpret_cast<const long long *>(p));
 }
 
-__global__ void __launch_bounds__(LANE_THREADS) sim_lane_kernel(SimArgs a) {
+__device__ __forceinline__ uint32_t lane_tokens(int64_t tok_base, int64_t tok_per_s, int32_t dur_ms) {
+    const int64_t prod = tok_per_s * (int64_t)dur_ms;
+    int64_t tok = tok_base + (((uint64_t)prod >> 32) == 0 ? (int64_t)((uint32_t)prod / 1000u) : prod / 1000);
+    tok = tok < 1 ? 1 : (tok > 0x7FFFFFFE ? 0x7FFFFFFE : tok);
+    return (uint32_t)tok;
+}
+
+__global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
     __shared__ uint32_t s_fin[LANE_CAP * LANE_THREADS];
     __shared__ int32_t s_idx[LANE_CAP * LANE_THREADS];
     const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
@@ -371,18 +379,44 @@ __global__ void __launch_bounds__(LANE_THREADS) sim_lane_kernel(SimArgs a) {
     int64_t t = 0;
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
     uint32_t it = 0;   // engine iterations so far, mod 2^32
-    int64_t next_arr = n > 0 ? ld_arrival(trace) : INT64_MAX;
-    const int64_t first_arrival = n > 0 ? next_arr : 0;
+    // look-ahead window over the trace: record p and record p+1 are in registers, so
+    // the load of a record is issued two ingests before its arrival stamp is tested
+    int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, last_arr = 0;
+    int32_t dur0 = 0, dur1 = 0, last_dur = 0;
+    if (n > 0) {
+        const int4 v = __ldg(reinterpret_cast<const int4 *>(trace));
+        arr0 = rec_arrival(v);
+        dur0 = v.z;
+    }
+    if (n > 1) {
+        const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + 1));
+        arr1 = rec_arrival(v);
+        dur1 = v.z;
+    }
+    const int64_t first_arrival = n > 0 ? arr0 : 0;
+    // E2E latency store deferred by one completion: the arrival stamp it needs is
+    // loaded at completion and consumed at the next one
+    int64_t pend_t = 0, pend_arr = 0;
+    int32_t pend_i = -1;
     bool deferred = false;
 
     while (done < n) {
         // idle server: the clock jumps to the next arrival (S14)
-        if (nR == 0 && nW == 0 && next_arr > t) t = next_arr;
+        if (nR == 0 && nW == 0 && arr0 > t) t = arr0;
         // 1. ingest arrivals <= t
-        while (next_arr <= t) {
+        while (arr0 <= t) {
+            last_arr = arr0;
+            last_dur = dur0;
             ++p;
             ++nW;
-            next_arr = p < n ? ld_arrival(trace + p) : INT64_MAX;
+            arr0 = arr1;
+            dur0 = dur1;
+            arr1 = INT64_MAX;
+            if (p + 1 < n) {
+                const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + p + 1));
+                arr1 = rec_arrival(v);
+                dur1 = v.z;
+            }
         }
         // 3. admit
         const int free_slots = slots - nR;
@@ -393,26 +427,45 @@ __global__ void __launch_bounds__(LANE_THREADS) sim_lane_kernel(SimArgs a) {
                 deferred = true;
                 break;
             }
-            int64_t dur_sum = 0;
-            for (int q = 0; q < k; ++q) {
-                const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo + q));
-                int64_t tok = tok_base + (tok_per_s * (int64_t)v.z) / 1000;
-                tok = tok < 1 ? 1 : (tok > 0x7FFFFFFE ? 0x7FFFFFFE : tok);
-                fin[(nR + q) * LANE_THREADS] = it + (uint32_t)tok;
-                sidx[(nR + q) * LANE_THREADS] = lo + q;
-                dur_sum += (int64_t)v.z;
+            if (k == 1) {
+                int64_t arr = last_arr;
+                int32_t dur = last_dur;
+                if (lo != p - 1) {
+                    const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo));
+                    arr = rec_arrival(v);
+                    dur = v.z;
+                }
+                fin[nR * LANE_THREADS] = it + lane_tokens(tok_base, tok_per_s, dur);
+                sidx[nR * LANE_THREADS] = lo;
+                t1 += enc_base + enc_per_ms * (int64_t)dur;
+                ttft[lo] = t1 - arr;   // first token (S9)
+            } else {
+                int64_t dur_sum = 0;
+                for (int q = 0; q < k; ++q) {
+                    const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo + q));
+                    fin[(nR + q) * LANE_THREADS] = it + lane_tokens(tok_base, tok_per_s, v.z);
+                    sidx[(nR + q) * LANE_THREADS] = lo + q;
+                    dur_sum += (int64_t)v.z;
+                }
+                t1 += enc_base * (int64_t)k + enc_per_ms * dur_sum;
+                for (int q = 0; q < k; ++q) ttft[lo + q] = t1 - ld_arrival(trace + lo + q);
             }
-            t1 += enc_base * (int64_t)k + enc_per_ms * dur_sum;
-            for (int q = 0; q < k; ++q) ttft[lo + q] = t1 - ld_arrival(trace + lo + q);   // first token (S9)
             lo += k;
             nW -= k;
             nR += k;
         }
         // 4. fast-forward over identical iterations to the next event
         uint32_t m = 0xFFFFFFFFu;
+        int s_min = 0, ties = 0;
         for (int s = 0; s < nR; ++s) {
             const uint32_t left = fin[s * LANE_THREADS] - it;
-            m = left < m ? left : m;
+            if (left < m) {
+                m = left;
+                s_min = s;
+                ties = 1;
+            } else if (left == m) {
+                ++ties;
+            }
         }
         const int64_t c = iter_base + iter_per * (int64_t)nR;
         int64_t j = 1;
@@ -420,7 +473,7 @@ __global__ void __launch_bounds__(LANE_THREADS) sim_lane_kernel(SimArgs a) {
             if (nR == slots || p >= n || c <= 0) {
                 j = m;
             } else {
-                const int64_t g = next_arr - t1;
+                const int64_t g = arr0 - t1;
                 if (g <= 0) j = 1;
                 else if (g > (int64_t)(m - 2u) * c) j = m;
                 else j = 1 + ceil_div_pos(g, c);
@@ -428,22 +481,28 @@ __global__ void __launch_bounds__(LANE_THREADS) sim_lane_kernel(SimArgs a) {
         }
         t = t1 + (j - 1) * c;
         it += (uint32_t)j;
-        // 5. completions
+        // 5. completions: slot s_min, plus (rarely) later slots that finish in the same iteration
         if ((uint32_t)j == m) {
-            for (int s = 0; s < nR;) {
+            int s = s_min;
+            do {
                 if (fin[s * LANE_THREADS] == it) {
                     const int32_t i = sidx[s * LANE_THREADS];
-                    lat[i] = t - ld_arrival(trace + i);
+                    if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
+                    pend_i = i;
+                    pend_t = t;
+                    pend_arr = ld_arrival(trace + i);
                     --nR;
                     fin[s * LANE_THREADS] = fin[nR * LANE_THREADS];
                     sidx[s * LANE_THREADS] = sidx[nR * LANE_THREADS];
                     ++done;
+                    --ties;
                 } else {
                     ++s;
                 }
-            }
+            } while (ties > 0);
         }
     }
+    if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
     if (deferred) {
         const int pos = atomicAdd(a.defer_count, 1);
         a.defer_list[pos] = r;
