@@ -355,6 +355,24 @@ __device__ __forceinline__ uint32_t lane_tokens(int64_t tok_base, int64_t tok_pe
     return (uint32_t)tok;
 }
 
+// insert (it + tokens, idx) into the sorted ring of nR entries starting at `head`
+__device__ __forceinline__ void lane_insert(uint32_t *fin, int32_t *sidx, int head, int nR, uint32_t it,
+                                            uint32_t tokens, int32_t idx) {
+    int h = nR;
+    while (h > 0) {
+        const int prev = ((head + h - 1) & (LANE_CAP - 1)) * LANE_THREADS;
+        const uint32_t f = fin[prev];
+        if (f - it <= tokens) break;
+        const int cur = ((head + h) & (LANE_CAP - 1)) * LANE_THREADS;
+        fin[cur] = f;
+        sidx[cur] = sidx[prev];
+        --h;
+    }
+    const int cur = ((head + h) & (LANE_CAP - 1)) * LANE_THREADS;
+    fin[cur] = it + tokens;
+    sidx[cur] = idx;
+}
+
 __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
     __shared__ uint32_t s_fin[LANE_CAP * LANE_THREADS];
     __shared__ int32_t s_idx[LANE_CAP * LANE_THREADS];
@@ -378,20 +396,21 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
 
     int64_t t = 0;
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
+    int head = 0;      // running set = ring positions head .. head+nR-1, sorted by finish iteration
     uint32_t it = 0;   // engine iterations so far, mod 2^32
     // look-ahead window over the trace: record p and record p+1 are in registers, so
     // the load of a record is issued two ingests before its arrival stamp is tested
     int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, last_arr = 0;
     int32_t dur0 = 0, dur1 = 0, last_dur = 0;
+    // (two loads per record on purpose: a 128-bit load would leave the unused est word
+    // as a dead destination register that the allocator reuses while the load is in flight)
     if (n > 0) {
-        const int4 v = __ldg(reinterpret_cast<const int4 *>(trace));
-        arr0 = rec_arrival(v);
-        dur0 = v.z;
+        arr0 = ld_arrival(trace);
+        dur0 = __ldg(&trace[0].dur_ms);
     }
     if (n > 1) {
-        const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + 1));
-        arr1 = rec_arrival(v);
-        dur1 = v.z;
+        arr1 = ld_arrival(trace + 1);
+        dur1 = __ldg(&trace[1].dur_ms);
     }
     const int64_t first_arrival = n > 0 ? arr0 : 0;
     // E2E latency store deferred by one completion: the arrival stamp it needs is
@@ -413,9 +432,8 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             dur0 = dur1;
             arr1 = INT64_MAX;
             if (p + 1 < n) {
-                const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + p + 1));
-                arr1 = rec_arrival(v);
-                dur1 = v.z;
+                arr1 = ld_arrival(trace + p + 1);
+                dur1 = __ldg(&trace[p + 1].dur_ms);
             }
         }
         // 3. admit
@@ -431,20 +449,17 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 int64_t arr = last_arr;
                 int32_t dur = last_dur;
                 if (lo != p - 1) {
-                    const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo));
-                    arr = rec_arrival(v);
-                    dur = v.z;
+                    arr = ld_arrival(trace + lo);
+                    dur = __ldg(&trace[lo].dur_ms);
                 }
-                fin[nR * LANE_THREADS] = it + lane_tokens(tok_base, tok_per_s, dur);
-                sidx[nR * LANE_THREADS] = lo;
+                lane_insert(fin, sidx, head, nR, it, lane_tokens(tok_base, tok_per_s, dur), lo);
                 t1 += enc_base + enc_per_ms * (int64_t)dur;
                 ttft[lo] = t1 - arr;   // first token (S9)
             } else {
                 int64_t dur_sum = 0;
                 for (int q = 0; q < k; ++q) {
                     const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo + q));
-                    fin[(nR + q) * LANE_THREADS] = it + lane_tokens(tok_base, tok_per_s, v.z);
-                    sidx[(nR + q) * LANE_THREADS] = lo + q;
+                    lane_insert(fin, sidx, head, nR + q, it, lane_tokens(tok_base, tok_per_s, v.z), lo + q);
                     dur_sum += (int64_t)v.z;
                 }
                 t1 += enc_base * (int64_t)k + enc_per_ms * dur_sum;
@@ -455,18 +470,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             nR += k;
         }
         // 4. fast-forward over identical iterations to the next event
-        uint32_t m = 0xFFFFFFFFu;
-        int s_min = 0, ties = 0;
-        for (int s = 0; s < nR; ++s) {
-            const uint32_t left = fin[s * LANE_THREADS] - it;
-            if (left < m) {
-                m = left;
-                s_min = s;
-                ties = 1;
-            } else if (left == m) {
-                ++ties;
-            }
-        }
+        const uint32_t m = fin[head * LANE_THREADS] - it;   // the running set is sorted: its head finishes first
         const int64_t c = iter_base + iter_per * (int64_t)nR;
         int64_t j = 1;
         if (m > 1u) {
@@ -481,25 +485,18 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         }
         t = t1 + (j - 1) * c;
         it += (uint32_t)j;
-        // 5. completions: slot s_min, plus (rarely) later slots that finish in the same iteration
+        // 5. completions: pop the head while it finishes in this iteration
         if ((uint32_t)j == m) {
-            int s = s_min;
             do {
-                if (fin[s * LANE_THREADS] == it) {
-                    const int32_t i = sidx[s * LANE_THREADS];
-                    if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
-                    pend_i = i;
-                    pend_t = t;
-                    pend_arr = ld_arrival(trace + i);
-                    --nR;
-                    fin[s * LANE_THREADS] = fin[nR * LANE_THREADS];
-                    sidx[s * LANE_THREADS] = sidx[nR * LANE_THREADS];
-                    ++done;
-                    --ties;
-                } else {
-                    ++s;
-                }
-            } while (ties > 0);
+                const int32_t i = sidx[head * LANE_THREADS];
+                if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
+                pend_i = i;
+                pend_t = t;
+                pend_arr = ld_arrival(trace + i);
+                head = (head + 1) & (LANE_CAP - 1);
+                --nR;
+                ++done;
+            } while (nR > 0 && fin[head * LANE_THREADS] == it);
         }
     }
     if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
