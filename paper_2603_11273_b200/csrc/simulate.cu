@@ -413,10 +413,6 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         dur1 = __ldg(&trace[1].dur_ms);
     }
     const int64_t first_arrival = n > 0 ? arr0 : 0;
-    // E2E latency store deferred by one completion: the arrival stamp it needs is
-    // loaded at completion and consumed at the next one
-    int64_t pend_t = 0, pend_arr = 0;
-    int32_t pend_i = -1;
     bool deferred = false;
 
     while (done < n) {
@@ -445,25 +441,25 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 deferred = true;
                 break;
             }
-            if (k == 1) {
-                int64_t arr = last_arr;
-                int32_t dur = last_dur;
-                if (lo != p - 1) {
-                    arr = ld_arrival(trace + lo);
-                    dur = __ldg(&trace[lo].dur_ms);
-                }
-                lane_insert(fin, sidx, head, nR, it, lane_tokens(tok_base, tok_per_s, dur), lo);
-                t1 += enc_base + enc_per_ms * (int64_t)dur;
-                ttft[lo] = t1 - arr;   // first token (S9)
+            if (k == 1 && lo == p - 1) {
+                // the request ingested last: everything needed is in registers
+                lane_insert(fin, sidx, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
+                t1 += enc_base + enc_per_ms * (int64_t)last_dur;
+                ttft[lo] = t1 - last_arr;   // first token (S9)
+                lat[lo] = -last_arr;        // E2E = completion time - arrival: the completion adds its time
             } else {
                 int64_t dur_sum = 0;
                 for (int q = 0; q < k; ++q) {
-                    const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + lo + q));
-                    lane_insert(fin, sidx, head, nR + q, it, lane_tokens(tok_base, tok_per_s, v.z), lo + q);
-                    dur_sum += (int64_t)v.z;
+                    const int32_t dur = __ldg(&trace[lo + q].dur_ms);
+                    lane_insert(fin, sidx, head, nR + q, it, lane_tokens(tok_base, tok_per_s, dur), lo + q);
+                    dur_sum += (int64_t)dur;
                 }
                 t1 += enc_base * (int64_t)k + enc_per_ms * dur_sum;
-                for (int q = 0; q < k; ++q) ttft[lo + q] = t1 - ld_arrival(trace + lo + q);
+                for (int q = 0; q < k; ++q) {
+                    const int64_t arr = ld_arrival(trace + lo + q);
+                    ttft[lo + q] = t1 - arr;
+                    lat[lo + q] = -arr;
+                }
             }
             lo += k;
             nW -= k;
@@ -485,21 +481,19 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         }
         t = t1 + (j - 1) * c;
         it += (uint32_t)j;
-        // 5. completions: pop the head while it finishes in this iteration
+        // 5. completions: pop the head while it finishes in this iteration.  lat[i] holds
+        // -arrival since admission; a fire-and-forget reduction adds the completion time, so
+        // no load sits on the critical path
         if ((uint32_t)j == m) {
             do {
                 const int32_t i = sidx[head * LANE_THREADS];
-                if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
-                pend_i = i;
-                pend_t = t;
-                pend_arr = ld_arrival(trace + i);
+                atomicAdd(reinterpret_cast<unsigned long long *>(lat + i), (unsigned long long)t);
                 head = (head + 1) & (LANE_CAP - 1);
                 --nR;
                 ++done;
             } while (nR > 0 && fin[head * LANE_THREADS] == it);
         }
     }
-    if (pend_i >= 0) lat[pend_i] = pend_t - pend_arr;
     if (deferred) {
         const int pos = atomicAdd(a.defer_count, 1);
         a.defer_list[pos] = r;
