@@ -1,10 +1,21 @@
 // percentiles.cu -- a6 segmented nearest-rank percentiles, sm_100a.
 //
-// One CTA per segment.  The segment is read from HBM once (staged into shared
-// memory when it fits), reduced to its min/max, and each requested rank is
-// found by an MSB-first radix select over (value - min): 8-bit digits, a
-// 256-bin shared-memory histogram per pass, only as many passes as the value
-// range needs (a 2 s latency spread in microseconds is 21 bits = 3 passes).
+// One CTA per segment, the segment read from HBM exactly once.
+//
+// Register path (segments of up to 10,240 values whose high 32-bit words are
+// all equal -- every latency below 71 minutes): each thread keeps the low
+// words of 40 values in registers and the ranks are found by an MSB-first
+// radix select WITHOUT shared-memory atomics (2 cycles per lane on this part,
+// which made the histogram the bottleneck): every lane counts into its own
+// private byte counters, laid out [warp][bin][lane] with a 36-byte bin stride
+// so that both the counting and the column sums are free of systematic bank
+// conflicts; the column sums use dp4a.  One counting pass over all values
+// serves all requested ranks; each rank then continues on the few hundred
+// values of its own bin, compacted into shared memory.
+//
+// General path (anything else): min/max, then MSB-first radix select over
+// (value - min) with 8-bit digits and a 256-bin shared-memory histogram, only
+// as many passes as the value range needs.
 // Nearest rank (asr_sched.h): element of 1-based rank
 // ceil(p*N/100) of the sorted segment; an empty segment gives -1.
 #include "launchers.cuh"
@@ -49,7 +60,7 @@ __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, co
         for (int j = 0; j < pl.n_pct; ++j) results[j] = -1;
         return;
     }
-    const bool staged = N <= PCT_SMEM_VALUES;
+    const bool staged = smem_vals != nullptr && N <= PCT_SMEM_VALUES;
     int64_t mn = INT64_MAX, mx = INT64_MIN;
     for (int64_t i = threadIdx.x; i < N; i += PCT_THREADS) {
         int64_t x = v[i];
@@ -117,26 +128,249 @@ __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, co
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(PCT_THREADS) percentiles_kernel(const int64_t *values, const int64_t *seg_off,
+
+// ---------------------------------------------------------------------------
+// register path
+// ---------------------------------------------------------------------------
+constexpr int PCT_VPT = 40;                                  // values per thread
+constexpr int PCT_REG_MAX = PCT_THREADS * PCT_VPT;           // 10,240 values
+constexpr int PCT_DIG = 7;                                   // digit width of a counting pass
+constexpr int PCT_BINS = 1 << PCT_DIG;
+constexpr int PCT_BIN_STRIDE = 36;                           // bytes: 32 lane counters + 4 padding
+constexpr int PCT_TAB_BYTES = PCT_BINS * PCT_BIN_STRIDE;     // per warp
+constexpr int PCT_CAND = 1024;                               // candidates finished in shared memory
+
+struct PctRegSmem {
+    unsigned char tab[PCT_THREADS / 32][PCT_TAB_BYTES];      // private byte counters
+    uint32_t part[2][PCT_BINS];                              // column sums of warps 0-3 / 4-7
+    uint32_t cand[PCT_CAND];
+    uint32_t hist[256];
+    uint32_t warp_or[PCT_THREADS / 32];
+    uint32_t sel_digit[PCT_MAX], sel_below[PCT_MAX], sel_pop[PCT_MAX];
+    uint32_t n_cand;
+};
+
+// One counting pass over the register-resident keys.  Counts digit
+// (key >> new_shift) & (2^width - 1) of every valid key with key >> shift ==
+// prefix (no filter when shift >= 32), then resolves every rank kk[t] of the
+// targets [t0, t1): sel_digit/sel_below/sel_pop.
+__device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], int N, int shift, int new_shift,
+                                               uint32_t prefix, const uint32_t *kk, int t0, int t1,
+                                               PctRegSmem &sm) {
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    const uint32_t mask = (1u << (shift - new_shift)) - 1u;
+    // zero the private counters
+    {
+        uint4 *z = reinterpret_cast<uint4 *>(&sm.tab[0][0]);
+        constexpr int n16 = (PCT_THREADS / 32) * PCT_TAB_BYTES / 16;
+        for (int i = threadIdx.x; i < n16; i += PCT_THREADS) z[i] = make_uint4(0, 0, 0, 0);
+    }
+    __syncthreads();
+    unsigned char *mine = &sm.tab[warp][lane];
+#pragma unroll
+    for (int j = 0; j < PCT_VPT; ++j) {
+        const int i = j * PCT_THREADS + threadIdx.x;
+        const bool in = i < N && (shift >= 32 || (key[j] >> shift) == prefix);
+        if (in) {
+            unsigned char *c = mine + ((key[j] >> new_shift) & mask) * PCT_BIN_STRIDE;
+            *c = (unsigned char)(*c + 1);
+        }
+    }
+    __syncthreads();
+    // column sums: thread (half, bin) adds the 32 lane counters of 4 warps
+    {
+        const int bin = threadIdx.x & (PCT_BINS - 1), half = threadIdx.x >> PCT_DIG;
+        uint32_t tot = 0;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const uint32_t *row = reinterpret_cast<const uint32_t *>(&sm.tab[half * 4 + w][bin * PCT_BIN_STRIDE]);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) tot = __dp4a(row[q], 0x01010101u, tot);
+        }
+        sm.part[half][bin] = tot;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        // lane L owns bins 4L .. 4L+3
+        uint32_t c[4], tot = 0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            c[b] = sm.part[0][lane * 4 + b] + sm.part[1][lane * 4 + b];
+            tot += c[b];
+        }
+        uint32_t incl = tot;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+            if (lane >= d) incl += y;
+        }
+        const uint32_t excl = incl - tot;
+        for (int t = t0; t < t1; ++t) {
+            const uint32_t k = kk[t];
+            if (excl < k && k <= incl) {
+                uint32_t run = excl;
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    if (run < k && k <= run + c[b]) {
+                        sm.sel_digit[t] = (uint32_t)(lane * 4 + b);
+                        sm.sel_below[t] = run;
+                        sm.sel_pop[t] = c[b];
+                    }
+                    run += c[b];
+                }
+            }
+        }
+    }
+    __syncthreads();
+}
+
+// Returns false (nothing written) when the segment does not qualify.
+__device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N64, const PctList &pl,
+                                        int64_t *results, PctRegSmem &sm) {
+    if (N64 <= 0 || N64 > PCT_REG_MAX) return false;
+    const int N = (int)N64;
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    uint32_t key[PCT_VPT];
+    const uint32_t hi0 = (uint32_t)((uint64_t)__ldg(reinterpret_cast<const long long *>(v)) >> 32);
+    uint32_t hi_diff = 0, or_all = 0;
+#pragma unroll
+    for (int j = 0; j < PCT_VPT; ++j) {
+        const int i = j * PCT_THREADS + threadIdx.x;
+        uint64_t x = (uint64_t)hi0 << 32;
+        if (i < N) x = (uint64_t)__ldcs(reinterpret_cast<const long long *>(v + i));   // read once: streaming
+        key[j] = (uint32_t)x;
+        hi_diff |= (uint32_t)(x >> 32) ^ hi0;
+        or_all |= (uint32_t)x;
+    }
+    if (__syncthreads_or(hi_diff != 0u)) return false;
+    or_all = __reduce_or_sync(ASR_FULL_MASK, or_all);
+    if (lane == 0) sm.warp_or[warp] = or_all;
+    __syncthreads();
+    or_all = 0;
+#pragma unroll
+    for (int w = 0; w < PCT_THREADS / 32; ++w) or_all |= sm.warp_or[w];
+    const int bits = or_all == 0u ? 0 : 32 - __clz((int)or_all);
+
+    uint32_t kk[PCT_MAX], prefix[PCT_MAX];
+#pragma unroll
+    for (int t = 0; t < PCT_MAX; ++t) {
+        kk[t] = t < pl.n_pct ? (uint32_t)(((uint64_t)pl.pct[t] * (uint64_t)N + 99) / 100) : 0u;   // 1-based rank
+        prefix[t] = 0;
+    }
+    if (bits > 0) {
+        // first pass: all targets at once, no filter (every key >> bits is 0)
+        const int sh1 = bits > PCT_DIG ? bits - PCT_DIG : 0;
+        reg_count_pass(key, N, 32, sh1, 0u, kk, 0, pl.n_pct, sm);
+        uint32_t pop[PCT_MAX];
+#pragma unroll
+        for (int t = 0; t < PCT_MAX; ++t)
+            if (t < pl.n_pct) {
+                prefix[t] = sm.sel_digit[t];
+                kk[t] -= sm.sel_below[t];
+                pop[t] = sm.sel_pop[t];
+            }
+        __syncthreads();
+        for (int t = 0; t < pl.n_pct; ++t) {
+            int shift = sh1;
+            // more counting passes while the bin is too crowded for the candidate buffer
+            while (shift > 0 && pop[t] > (uint32_t)PCT_CAND) {
+                const int ns = shift > PCT_DIG ? shift - PCT_DIG : 0;
+                reg_count_pass(key, N, shift, ns, prefix[t], kk, t, t + 1, sm);
+                prefix[t] = (prefix[t] << (shift - ns)) | sm.sel_digit[t];
+                kk[t] -= sm.sel_below[t];
+                pop[t] = sm.sel_pop[t];
+                shift = ns;
+                __syncthreads();
+            }
+            if (shift == 0) continue;
+            // compact the keys of the selected bin into shared memory
+            if (threadIdx.x == 0) sm.n_cand = 0;
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < PCT_VPT; ++j) {
+                const int i = j * PCT_THREADS + threadIdx.x;
+                const bool in = i < N && (key[j] >> shift) == prefix[t];
+                const uint32_t m = __ballot_sync(ASR_FULL_MASK, in);
+                if (m != 0u) {
+                    uint32_t base = 0;
+                    if (lane == 0) base = atomicAdd(&sm.n_cand, (uint32_t)__popc(m));
+                    base = __shfl_sync(ASR_FULL_MASK, base, 0);
+                    if (in) sm.cand[base + __popc(m & ((1u << lane) - 1u))] = key[j];
+                }
+            }
+            __syncthreads();
+            const int C = (int)sm.n_cand;   // == pop[t]
+            // finish on the candidates: 8-bit digits, shared-memory histogram (few values)
+            while (shift > 0) {
+                const int ns = shift > 8 ? shift - 8 : 0;
+                const uint32_t mask = (1u << (shift - ns)) - 1u;
+                sm.hist[threadIdx.x] = 0;   // PCT_THREADS == 256
+                __syncthreads();
+                for (int i = threadIdx.x; i < C; i += PCT_THREADS) {
+                    const uint32_t x = sm.cand[i];
+                    if ((x >> shift) == prefix[t]) atomicAdd(&sm.hist[(x >> ns) & mask], 1u);
+                }
+                __syncthreads();
+                if (warp == 0) {
+                    uint32_t c[8], tot = 0;
+#pragma unroll
+                    for (int b = 0; b < 8; ++b) {
+                        c[b] = sm.hist[lane * 8 + b];
+                        tot += c[b];
+                    }
+                    uint32_t incl = tot;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+                        if (lane >= d) incl += y;
+                    }
+                    const uint32_t excl = incl - tot, k = kk[t];
+                    if (excl < k && k <= incl) {
+                        uint32_t run = excl;
+#pragma unroll
+                        for (int b = 0; b < 8; ++b) {
+                            if (run < k && k <= run + c[b]) {
+                                sm.sel_digit[t] = (uint32_t)(lane * 8 + b);
+                                sm.sel_below[t] = run;
+                            }
+                            run += c[b];
+                        }
+                    }
+                }
+                __syncthreads();
+                prefix[t] = (prefix[t] << (shift - ns)) | sm.sel_digit[t];
+                kk[t] -= sm.sel_below[t];
+                shift = ns;
+                __syncthreads();
+            }
+        }
+    }
+    for (int t = 0; t < pl.n_pct; ++t) results[t] = (int64_t)(((uint64_t)hi0 << 32) | prefix[t]);
+    __syncthreads();
+    return true;
+}
+
+__global__ void __launch_bounds__(PCT_THREADS, 3) percentiles_kernel(const int64_t *values, const int64_t *seg_off,
                                                                   int32_t n_seg, PctList pl, int64_t *out) {
     extern __shared__ __align__(16) unsigned char dyn_smem[];
-    int64_t *smem_vals = reinterpret_cast<int64_t *>(dyn_smem);
+    PctRegSmem &sm = *reinterpret_cast<PctRegSmem *>(dyn_smem);
     for (int s = blockIdx.x; s < n_seg; s += gridDim.x) {
         const int64_t b = seg_off[s], e = seg_off[s + 1];
         int64_t res[PCT_MAX];
-        segment_percentiles(values + b, e - b, pl, res, smem_vals);
+        if (!segment_percentiles_reg(values + b, e - b, pl, res, sm))
+            segment_percentiles(values + b, e - b, pl, res, nullptr);
         if (threadIdx.x == 0)
             for (int j = 0; j < pl.n_pct; ++j) out[(int64_t)s * pl.n_pct + j] = res[j];
     }
 }
 
 // p50/p90 of E2E latency (blockIdx.y = 0) and TTFT (blockIdx.y = 1) of every replica
-__global__ void __launch_bounds__(PCT_THREADS) summary_percentiles_kernel(const asr_replica_t *replicas,
+__global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(const asr_replica_t *replicas,
                                                                           int32_t n_replicas, const int64_t *lat,
                                                                           const int64_t *ttft,
                                                                           asr_summary_t *out_summary) {
     extern __shared__ __align__(16) unsigned char dyn_smem[];
-    int64_t *smem_vals = reinterpret_cast<int64_t *>(dyn_smem);
+    PctRegSmem &sm = *reinterpret_cast<PctRegSmem *>(dyn_smem);
     PctList pl;
     pl.n_pct = 2;
     pl.pct[0] = 50;
@@ -146,7 +380,8 @@ __global__ void __launch_bounds__(PCT_THREADS) summary_percentiles_kernel(const 
         if (out_summary[r].n_done < 0) continue;   // invalid descriptor, flagged by the simulator
         const asr_replica_t rep = replicas[r];
         int64_t res[PCT_MAX];
-        segment_percentiles(vals + rep.out_off, rep.n, pl, res, smem_vals);
+        if (!segment_percentiles_reg(vals + rep.out_off, rep.n, pl, res, sm))
+            segment_percentiles(vals + rep.out_off, rep.n, pl, res, nullptr);
         if (threadIdx.x == 0) {
             if (blockIdx.y == 0) {
                 out_summary[r].p50_e2e_us = res[0];
@@ -159,7 +394,7 @@ __global__ void __launch_bounds__(PCT_THREADS) summary_percentiles_kernel(const 
     }
 }
 
-static constexpr size_t PCT_DYN_SMEM = (size_t)PCT_SMEM_VALUES * sizeof(int64_t);
+static constexpr size_t PCT_DYN_SMEM = sizeof(PctRegSmem);
 
 static int pct_grid(int n_units, const void *fn) {
     static int n_sm = 0;
