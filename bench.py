@@ -306,7 +306,6 @@ def run_ours(args):
         return (ms / cnt if cnt else None), cnt, ms
 
     sel_avg, sel_cnt, sel_tot = per_launch("select_topk_kernel")
-    sim_avg, sim_cnt, sim_tot = per_launch("sim_warp_kernel")
     gen_avg, _, gen_tot = per_launch("gen_trace_kernel")
     pct_avg, _, pct_tot = per_launch("summary_percentiles_kernel")
     rooflines = {}
@@ -316,23 +315,34 @@ def run_ours(args):
             "bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak,
             "traffic": consts.get("select_dram_bytes_per_launch"), "peak_source": peak_src,
             "algorithmic_bytes_per_launch": sel_bytes, "avg_launch_ms": sel_avg, "frac_of_nominal_8TBs": a / 8000.0}
-    if sim_avg:
-        wi = consts.get("sim_warp_instr_per_request")
-        a = (wi * total / (sim_avg / 1e3)) if wi else None
-        rooflines["sim_warp_kernel"] = {
+    stage_ms = {"gen_trace_kernel": gen_tot, "summary_percentiles_kernel": pct_tot}
+    for kname in ("sim_lane_kernel", "sim_warp_kernel"):
+        k_avg, k_cnt, k_tot = per_launch(kname)
+        if not k_avg:
+            continue
+        stage_ms[kname] = k_tot
+        # ALU/issue-bound: achieved = warp instructions issued per second; the per-request
+        # instruction count is the ncu figure committed in profiles/roofline_constants.json
+        wi = consts.get(kname + "_warp_instr_per_request")
+        a = (wi * total / (k_avg / 1e3)) if wi else None
+        rooflines[kname] = {
             "bound": "alu", "achieved": a, "peak": ALU_PEAK_WARP_INSTR_PER_S, "unit": "warp-instr/s",
-            "frac": (a / ALU_PEAK_WARP_INSTR_PER_S) if a else None, "traffic": consts.get("sim_dram_bytes_per_launch"),
-            "warp_instr_per_request": wi, "avg_launch_ms": sim_avg,
+            "frac": (a / ALU_PEAK_WARP_INSTR_PER_S) if a else None,
+            "traffic": consts.get(kname + "_dram_bytes_per_launch"),
+            "warp_instr_per_request": wi, "avg_launch_ms": k_avg,
             "peak_source": "148 SMs x 4 schedulers x 1.965 GHz (DESIGN.md)"}
     if gen_avg:
         a = n_traces * n * 16 / (gen_avg / 1e3) / 1e9
         rooflines["gen_trace_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
-                                         "frac": a / hbm_peak, "traffic": None, "avg_launch_ms": gen_avg}
+                                         "frac": a / hbm_peak, "traffic": consts.get("gen_trace_dram_bytes_per_launch"),
+                                         "algorithmic_bytes_per_launch": n_traces * n * 16, "avg_launch_ms": gen_avg}
     if pct_avg:
         a = 2 * total * 8 / (pct_avg / 1e3) / 1e9
         rooflines["summary_percentiles_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
-                                                   "frac": a / hbm_peak, "traffic": None, "avg_launch_ms": pct_avg}
-    stage_ms = {"gen_trace_kernel": gen_tot, "sim_warp_kernel": sim_tot, "summary_percentiles_kernel": pct_tot}
+                                                   "frac": a / hbm_peak,
+                                                   "traffic": consts.get("summary_percentiles_dram_bytes_per_launch"),
+                                                   "algorithmic_bytes_per_launch": 2 * total * 8,
+                                                   "avg_launch_ms": pct_avg}
     dominant = max(stage_ms, key=lambda k_: stage_ms[k_] or 0.0)
     roofline = dict(rooflines.get(dominant, {}), kernel=dominant,
                     share_of_step=(stage_ms[dominant] / sweep_ms) if sweep_ms else None)
