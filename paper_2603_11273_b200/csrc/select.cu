@@ -19,6 +19,14 @@
 // tie-break) keeps the best k..2k candidates and makes the worst kept one the
 // new T.  At the end of the queue the buffer is cut to exactly the k best and
 // sorted across the lanes with a bitonic network on the exact comparator.
+// Carried threshold.  Consecutive queues of a batch usually look alike, so a
+// warp starts a queue with the threshold of rank ~2k that it found in its
+// previous queue instead of "pass everything": ~2k records survive, no cut
+// happens before the end of the queue, and the exact work per queue is one
+// quickselect over ~2k candidates.  The pass set of any threshold is closed
+// upwards in the total order, so it holds the k best whenever it holds at
+// least k records; if it holds fewer (the carried threshold was too strict for
+// this queue) the warp re-reads the queue with "pass everything".
 // Every decision that affects the output is taken by the exact integer
 // comparator, so the result is the unique total order -- never an approximation.
 // HBM-bound by design: 16 B read per record, 4k B written per queue.
@@ -38,6 +46,9 @@ struct __align__(128) SelWarpSmem {
     int4 stage[SEL_STAGES][SEL_CHUNK];   // raw records (arrival lo, arrival hi, dur_ms | src idx, est)
     int4 buf[SEL_BUFCAP];                // candidates (arrival lo, arrival hi, max(est,1), idx)
     uint64_t full[SEL_STAGES];           // mbarriers: chunk landed
+    int64_t carry_t64;                   // threshold carried to this warp's next queue (valid if carry_ok)
+    int32_t carry_t32;
+    int32_t carry_ok;
 };
 constexpr size_t SEL_SMEM_BYTES = sizeof(SelWarpSmem) * SEL_WARPS;
 
@@ -293,11 +304,13 @@ template <int POLICY>
 struct SelState {
     Thr thr;
     int cnt;
+    int cuts;        // quickselect cuts taken inside this queue
     uint32_t seed;
 };
 
-// scan one staged chunk: `nvalid` records, the first one is record `rec0` of the queue
-template <int POLICY, bool INDIRECT, bool FULL>
+// scan one chunk: `nvalid` records, the first one is record `rec0` of the queue.  The chunk
+// sits in a shared-memory stage, or (GUARDED) in global memory, where nothing past nvalid is read.
+template <int POLICY, bool INDIRECT, bool FULL, bool GUARDED = false>
 __device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 *buf, int rec0, int nvalid,
                                            int32_t idx_base, int k, int64_t now, SelState<POLICY> &s) {
     const int lane = lane_id();
@@ -309,7 +322,10 @@ __device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 
         uint32_t m[SEL_UNROLL];
         bool p[SEL_UNROLL];
 #pragma unroll
-        for (int u = 0; u < SEL_UNROLL; ++u) r[u] = stage[(i + u) * 32 + lane];
+        for (int u = 0; u < SEL_UNROLL; ++u) {
+            if (GUARDED) r[u] = (i + u) * 32 + lane < nvalid ? __ldg(stage + (i + u) * 32 + lane) : make_int4(0, 0, 0, 0);
+            else r[u] = stage[(i + u) * 32 + lane];
+        }
         uint32_t many = 0;
 #pragma unroll
         for (int u = 0; u < SEL_UNROLL; ++u) {
@@ -331,22 +347,56 @@ __device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 
                 s.cnt += __popc(m[u]);
             }
             if (s.cnt > SEL_FLUSH_AT) {
-                const int slack = k > 16 ? k : 16;
+                // keep the best 2k .. 2k+16: the survivors of a queue's last cut seed the carried threshold
                 s.seed = s.seed * 747796405u + 2891336453u;
                 __syncwarp();
-                const uint32_t rc = buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1 + slack, now, s.seed);
+                const uint32_t rc = buffer_cut<POLICY>(buf, s.cnt, 2 * k - 1, 2 * k + 15, now, s.seed);
                 s.cnt = (int)(rc & 0xFFFFu);
                 s.thr = thr_from<POLICY>(buf[rc >> 16], now);
+                s.cuts++;
             }
         }
     }
 }
 
-// cut to the k best, sort them, write the indices of queue q
+// second reading of a whole queue straight from global memory with "pass everything" (cold path)
 template <int POLICY>
-__device__ __forceinline__ void finish_queue(int4 *buf, int32_t *out, int k, int64_t now, SelState<POLICY> &s) {
+__device__ __noinline__ void rescan_queue(const int4 *keys, int4 *buf, int count, int32_t idx_base, int k, int64_t now,
+                                          SelState<POLICY> &s) {
+    s.thr = thr_pass_all<POLICY>();
+    s.cnt = 0;
+    for (int c = 0; c * SEL_CHUNK < count; ++c) {
+        const int left = count - c * SEL_CHUNK;
+        scan_chunk<POLICY, false, false, true>(keys + (int64_t)c * SEL_CHUNK, buf, c * SEL_CHUNK,
+                                               left < SEL_CHUNK ? left : SEL_CHUNK, idx_base, k, now, s);
+    }
+}
+
+// cut to the k best, sort them, write the indices of queue q; decide what the next queue starts with
+template <int POLICY>
+__device__ __forceinline__ void finish_queue(SelWarpSmem &sm, int32_t *out, int k, int64_t now, SelState<POLICY> &s,
+                                             bool steady) {
     const int lane = lane_id();
+    int4 *buf = sm.buf;
     __syncwarp();
+    if (steady) {
+        // the carried threshold let s.cnt >= k records through and no cut was needed: keep it
+        // unless it is getting close to letting fewer than k through
+        if (s.cnt < k + (k >> 1) && lane == 0) sm.carry_ok = 0;
+    } else if (s.cnt >= 2 * k) {
+        // calibrate: the record of rank 2k .. 2k+16 of this queue becomes the carried threshold
+        s.seed = s.seed * 747796405u + 2891336453u;
+        const uint32_t rc = buffer_cut<POLICY>(buf, s.cnt, 2 * k - 1, 2 * k + 15, now, s.seed);
+        s.cnt = (int)(rc & 0xFFFFu);
+        const Thr c = thr_from<POLICY>(buf[rc >> 16], now);
+        if (lane == 0) {
+            sm.carry_t64 = c.t64;
+            sm.carry_t32 = c.t32;
+            sm.carry_ok = 1;
+        }
+    } else if (lane == 0) {
+        sm.carry_ok = 0;
+    }
     if (s.cnt > k) {
         s.seed = s.seed * 747796405u + 2891336453u;
         s.cnt = (int)(buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1, now, s.seed) & 0xFFFFu);
@@ -408,42 +458,63 @@ __global__ void __launch_bounds__(SEL_WARPS * 32, 1) select_topk_kernel(SelArgs 
         for (int s = 0; s < SEL_STAGES; ++s) produce(gp++);
     }
 
+    if (lane == 0) sm.carry_ok = 0;   // threshold carried from this warp's previous queue: none yet
+    __syncwarp();
     for (int q = gw; q < a.n_queues; q += GW) {
         const int count = sel_count(a, q);
         const int64_t now = a.now_per_queue ? a.now_per_queue[q] : a.now;
         const int64_t qbase = (int64_t)q * a.q_len;
         const int32_t idx_base = a.global_idx ? (int32_t)qbase : 0;
         SelState<POLICY> s;
+        const bool have_carry = sm.carry_ok != 0;
         s.thr = thr_pass_all<POLICY>();
+        if (have_carry) {
+            s.thr.t64 = sm.carry_t64;
+            s.thr.t32 = sm.carry_t32;
+        }
         s.cnt = 0;
+        s.cuts = 0;
         s.seed = 0x9E3779B9u * (uint32_t)(q + 1);
         const int nch = (count + SEL_CHUNK - 1) / SEL_CHUNK;
+        bool redo = false;
+        for (;;) {
 #pragma unroll 1
-        for (int c = 0; c < nch; ++c) {
-            const int left = count - c * SEL_CHUNK;
-            const int nvalid = left < SEL_CHUNK ? left : SEL_CHUNK;
-            if (INDIRECT) {
-                __syncwarp();
-                for (int j = lane; j < nvalid; j += 32) {
-                    const int32_t src = a.src_idx[qbase + (int64_t)c * SEL_CHUNK + j];
-                    const int4 v = __ldg(reinterpret_cast<const int4 *>(a.keys + src));
-                    sm.stage[0][j] = make_int4(v.x, v.y, src, v.w);
+            for (int c = 0; c < nch; ++c) {
+                const int left = count - c * SEL_CHUNK;
+                const int nvalid = left < SEL_CHUNK ? left : SEL_CHUNK;
+                if (INDIRECT) {
+                    __syncwarp();
+                    for (int j = lane; j < nvalid; j += 32) {
+                        const int32_t src = a.src_idx[qbase + (int64_t)c * SEL_CHUNK + j];
+                        const int4 v = __ldg(reinterpret_cast<const int4 *>(a.keys + src));
+                        sm.stage[0][j] = make_int4(v.x, v.y, src, v.w);
+                    }
+                    __syncwarp();
+                    scan_chunk<POLICY, true, false>(sm.stage[0], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                } else {
+                    const int st = (int)(gc % SEL_STAGES);
+                    mbar_wait(&sm.full[st], (gc / SEL_STAGES) & 1u);
+                    if (nvalid == SEL_CHUNK)
+                        scan_chunk<POLICY, false, true>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                    else
+                        scan_chunk<POLICY, false, false>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
+                    __syncwarp();          // every lane is done reading the stage: refill it
+                    produce(gp++);
+                    gc++;
                 }
-                __syncwarp();
-                scan_chunk<POLICY, true, false>(sm.stage[0], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
-            } else {
-                const int st = (int)(gc % SEL_STAGES);
-                mbar_wait(&sm.full[st], (gc / SEL_STAGES) & 1u);
-                if (nvalid == SEL_CHUNK)
-                    scan_chunk<POLICY, false, true>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
-                else
-                    scan_chunk<POLICY, false, false>(sm.stage[st], sm.buf, c * SEL_CHUNK, nvalid, idx_base, k, now, s);
-                __syncwarp();          // every lane is done reading the stage: refill it
-                produce(gp++);
-                gc++;
             }
+            // a carried threshold that let fewer than min(k, count) records through was too strict
+            // for this queue: read it again with "pass everything"
+            if (redo || !have_carry || s.cuts > 0 || s.cnt >= (k < count ? k : count)) break;
+            redo = true;
+            if (!INDIRECT) {
+                rescan_queue<POLICY>(reinterpret_cast<const int4 *>(a.keys + qbase), sm.buf, count, idx_base, k, now, s);
+                break;
+            }
+            s.thr = thr_pass_all<POLICY>();
+            s.cnt = 0;
         }
-        finish_queue<POLICY>(sm.buf, a.out_idx + (int64_t)q * k, k, now, s);
+        finish_queue<POLICY>(sm, a.out_idx + (int64_t)q * k, k, now, s, have_carry && !redo && s.cuts == 0);
     }
 }
 

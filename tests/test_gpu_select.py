@@ -89,3 +89,45 @@ def test_select_host_entry(asr):
     got = asr.select_host(q, 8, 300, orc.HRRN, now, 16)
     for i in range(8):
         assert np.array_equal(got[i], orc.select(q[i], orc.HRRN, now, 16))
+
+
+@pytest.mark.parametrize("policy", POL)
+@pytest.mark.parametrize("k", [32, 5])
+def test_many_queues_per_warp_with_drifting_distributions(asr, policy, k):
+    """Every warp of the persistent grid serves six queues in a row whose key distributions jump
+    around, so a threshold carried over from the previous queue is in turn well calibrated, far
+    too strict (nothing passes: the queue is read again), far too loose (cuts inside the queue),
+    or meets a queue shorter than k / an empty queue / a queue of identical keys."""
+    import torch
+    now = 10**9
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    gw = sm * 20                       # queues in flight: one per warp of the persistent grid
+    nq, ql = 6 * gw, 128
+    rng = np.random.default_rng(1000 * policy + k)
+    q = np.zeros((nq, ql), dtype=wl.REQ)
+    counts = np.full(nq, ql, dtype=np.int32)
+    kind = (np.arange(nq) // gw + np.arange(nq) % 3) % 6
+    arr = rng.integers(0, now, size=(nq, ql), dtype=np.int64)
+    dur = rng.integers(1000, 35001, size=(nq, ql)).astype(np.int32)
+    late = kind == 1                   # recent arrivals, long jobs: worst under every policy
+    arr[late] = now - rng.integers(0, 1000, size=(int(late.sum()), ql))
+    dur[late] = rng.integers(30000, 35001, size=(int(late.sum()), ql))
+    early = kind == 2                  # old arrivals, short jobs: best under every policy
+    arr[early] = rng.integers(0, 1000, size=(int(early.sum()), ql))
+    dur[early] = rng.integers(1, 50, size=(int(early.sum()), ql))
+    same = kind == 4                   # identical keys: the index decides
+    arr[same] = now // 3
+    dur[same] = 7000
+    q["arrival_us"], q["dur_ms"], q["est"] = arr, dur, dur
+    short = kind == 5                  # shorter than k, or empty
+    counts[short] = rng.integers(0, max(2, k), size=int(short.sum()))
+    got = gpu_select_batched(asr, q, policy, now, k, q_count=counts)
+    pick = np.unique(np.concatenate([np.arange(0, nq, 37), np.arange(gw - 3, nq, gw), np.arange(gw, nq, gw)]))
+    for i in pick:
+        assert np.array_equal(got[i], orc.select(q[i][:counts[i]], policy, now, k)), (policy, k, int(i), int(kind[i]))
+    # every queue: k distinct valid indices, then -1 padding
+    valid = np.minimum(counts, k)
+    for i in range(0, nq, 11):
+        v = got[i][:valid[i]]
+        assert len(set(v.tolist())) == len(v) and (v >= 0).all() and (v < counts[i]).all()
+        assert (got[i][valid[i]:] == -1).all()
