@@ -134,6 +134,29 @@ __device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr
     return mul64x32(w, (uint32_t)t.t32) >= mul64x32(t.t64, (uint32_t)e);
 }
 
+// ---- order scalar ---------------------------------------------------------------
+// A 64-bit scalar that is WEAKLY order-preserving: scalar(a) < scalar(b) implies
+// that a is better than b under the total order; equal scalars say nothing and
+// are settled by the exact comparator.  It makes the common-case comparison of
+// the quickselect and of the final sort one 64-bit compare.
+//   FCFS  arrival
+//   SJF   est (>= 1) above the arrival time in units of 256 us, saturated
+//   HRRN  the IEEE double quotient wait/est, negated: wait < 2^53 and est are exact
+//         in double and the division is correctly rounded, hence monotone in the
+//         exact ratio (a strictly larger double means a strictly larger ratio)
+template <int POLICY>
+__device__ __forceinline__ int64_t order_scalar(const int4 &e, int64_t now) {
+    const int64_t arr = rec_arr(e);
+    if (POLICY == ASR_FCFS) return arr;
+    if (POLICY == ASR_SJF) {
+        int64_t a8 = arr >> 8;
+        a8 = a8 < 0 ? 0 : (a8 > 0xFFFFFFFFll ? 0xFFFFFFFFll : a8);
+        return ((int64_t)e.z << 32) | a8;
+    }
+    const double r = (double)wait_of(arr, now) / (double)e.z;   // e.z = max(est, 1)
+    return INT64_MAX - __double_as_longlong(r);
+}
+
 // ---- exact quickselect over the candidate buffer --------------------------------
 // Keeps the c+1 best candidates where c in [c_lo, c_hi] is the rank of an
 // accepted pivot (number of candidates strictly better than it); the pivot is
@@ -144,19 +167,15 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
     const int lane = lane_id();
     const uint32_t lt_mask = (1u << lane) - 1u;
     const int nrows = (cnt + 31) >> 5;
-    // per candidate, in registers: only what the common-case comparison needs
-    int64_t A[SEL_ROWS];      // HRRN: clamped wait; FCFS: arrival
-    int32_t Z[SEL_ROWS];      // HRRN, SJF: est; FCFS: idx
+    int64_t A[SEL_ROWS];      // order scalar of candidate j*32 + lane
     uint32_t pri[SEL_ROWS];   // random priority (23 bits) | 0x100 | position
     uint32_t alive = 0, keep = 0;
 #pragma unroll
     for (int j = 0; j < SEL_ROWS; ++j) {
         if (j < nrows) {
             const uint32_t i = (uint32_t)(j * 32 + lane);
-            const int4 e = buf[i];
             if ((int)i < cnt) alive |= 1u << j;
-            A[j] = POLICY == ASR_HRRN ? wait_of(rec_arr(e), now) : rec_arr(e);
-            Z[j] = POLICY == ASR_FCFS ? e.w : e.z;
+            A[j] = order_scalar<POLICY>(buf[(int)i < cnt ? i : 0u], now);
             uint32_t h = (i + 1u) * 2654435761u ^ seed;
             h ^= h >> 15;
             h *= 2246822519u;
@@ -179,38 +198,29 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
         const uint32_t win = __reduce_max_sync(ASR_FULL_MASK, best);
         if (win == 0u) break;   // nothing alive (cannot happen under the precondition)
         pi = (int)(win & 0xFFu);
-        const int4 P = buf[pi];
         const uint32_t pflag = (pi & 31) == lane ? (1u << (pi >> 5)) : 0u;
-        const int64_t p_arr = rec_arr(P);
-        const int64_t p_w = wait_of(p_arr, now);
+        // the pivot's scalar comes from the lane that holds it
+        int64_t mine = 0;
+#pragma unroll
+        for (int j = 0; j < SEL_ROWS; ++j)
+            if (j < nrows && (pi >> 5) == j) mine = A[j];
+        const int64_t Kp = shfl64(mine, pi & 31);
         uint32_t bflags = 0, tflags = 0;
 #pragma unroll
         for (int j = 0; j < SEL_ROWS; ++j)
             if (j < nrows) {
-                bool gt, tie;
-                if (POLICY == ASR_HRRN) {
-                    const int64_t lhs = mul64x32(A[j], (uint32_t)P.z), rhs = mul64x32(p_w, (uint32_t)Z[j]);
-                    gt = lhs > rhs;
-                    tie = (uint32_t)lhs == (uint32_t)rhs;   // necessary for equality; settled below
-                } else if (POLICY == ASR_SJF) {
-                    gt = Z[j] < P.z;
-                    tie = Z[j] == P.z;
-                } else {
-                    gt = earlier(A[j], Z[j], p_arr, P.w);
-                    tie = false;
-                }
-                bflags |= gt ? (1u << j) : 0u;
-                tflags |= tie ? (1u << j) : 0u;
+                bflags |= A[j] < Kp ? (1u << j) : 0u;
+                tflags |= A[j] == Kp ? (1u << j) : 0u;
             }
-        tflags &= alive;
-        if (POLICY != ASR_FCFS && __any_sync(ASR_FULL_MASK, tflags != 0u)) {
-            // rare: equal keys -- the full comparator with its (arrival, idx) tie-break decides
+        tflags &= alive & ~pflag;
+        if (__any_sync(ASR_FULL_MASK, tflags != 0u)) {
+            // rare: equal scalars -- the full comparator with its (arrival, idx) tie-break decides
+            const int4 P = buf[pi];
 #pragma unroll
             for (int j = 0; j < SEL_ROWS; ++j)
                 if (j < nrows && ((tflags >> j) & 1u)) {
                     const int4 e = buf[j * 32 + lane];
-                    const bool bt = better<POLICY>(rec_arr(e), e.z, e.w, p_arr, P.z, P.w, now);
-                    bflags = (bflags & ~(1u << j)) | (bt ? (1u << j) : 0u);
+                    if (better<POLICY>(rec_arr(e), e.z, e.w, rec_arr(P), P.z, P.w, now)) bflags |= 1u << j;
                 }
         }
         bflags &= alive;
@@ -254,26 +264,37 @@ __device__ __noinline__ uint32_t buffer_cut(int4 *buf, int cnt, int c_lo, int c_
     return (ppos << 16) | (uint32_t)off;
 }
 
-// exact bitonic sort of one candidate per lane, best first; idx < 0 = empty (sorts last)
+// exact bitonic sort of buf[0 .. cnt), cnt <= 32, one candidate per lane: returns the buffer
+// position of the candidate of rank `lane` (best first), -1 past the end.  Compares order
+// scalars; equal scalars are settled by the exact comparator on the records themselves.
 template <int POLICY>
-__device__ __forceinline__ int4 sort32(int4 v, int64_t now) {
+__device__ __forceinline__ int sort32(const int4 *buf, int cnt, int64_t now) {
     const int lane = lane_id();
+    int pos = lane < cnt ? lane : -1;
+    int64_t K = pos >= 0 ? order_scalar<POLICY>(buf[lane], now) : INT64_MAX;
 #pragma unroll
     for (int k = 2; k <= 32; k <<= 1) {
 #pragma unroll
         for (int j = k >> 1; j > 0; j >>= 1) {
-            int4 o;
-            o.x = __shfl_xor_sync(ASR_FULL_MASK, v.x, j);
-            o.y = __shfl_xor_sync(ASR_FULL_MASK, v.y, j);
-            o.z = __shfl_xor_sync(ASR_FULL_MASK, v.z, j);
-            o.w = __shfl_xor_sync(ASR_FULL_MASK, v.w, j);
+            const int64_t oK = (int64_t)shfl64_xor((uint64_t)K, j);
+            const int opos = __shfl_xor_sync(ASR_FULL_MASK, pos, j);
             const bool up = (lane & k) == 0 || k == 32;
             const bool want_min = ((lane & j) == 0) == up;
-            const bool v_less = v.w >= 0 && (o.w < 0 || better<POLICY>(rec_arr(v), v.z, v.w, rec_arr(o), o.z, o.w, now));
-            if (want_min != v_less) v = o;
+            bool v_less = pos >= 0 && (opos < 0 || K < oK);
+            const bool tie = pos >= 0 && opos >= 0 && K == oK;
+            if (__any_sync(ASR_FULL_MASK, tie)) {
+                if (tie) {
+                    const int4 a = buf[pos], b = buf[opos];
+                    v_less = better<POLICY>(rec_arr(a), a.z, a.w, rec_arr(b), b.z, b.w, now);
+                }
+            }
+            if (want_min != v_less) {
+                K = oK;
+                pos = opos;
+            }
         }
     }
-    return v;
+    return pos;
 }
 
 struct SelArgs {
@@ -401,9 +422,8 @@ __device__ __forceinline__ void finish_queue(SelWarpSmem &sm, int32_t *out, int 
         s.seed = s.seed * 747796405u + 2891336453u;
         s.cnt = (int)(buffer_cut<POLICY>(buf, s.cnt, k - 1, k - 1, now, s.seed) & 0xFFFFu);
     }
-    int4 v = lane < s.cnt ? buf[lane] : make_int4(0, 0, 1, -1);
-    v = sort32<POLICY>(v, now);
-    if (lane < k) out[lane] = v.w;
+    const int pos = sort32<POLICY>(buf, s.cnt, now);
+    if (lane < k) out[lane] = pos >= 0 ? buf[pos].w : -1;
     __syncwarp();
 }
 
