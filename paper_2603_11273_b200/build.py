@@ -33,7 +33,8 @@ def is_stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or is_stale():
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [NVCC] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
+        extra = os.environ.get("ASR_NVCC_EXTRA", "").split()   # e.g. -DSEL_L2_AHEAD=8 for a tuning build
+        cmd = [NVCC] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB

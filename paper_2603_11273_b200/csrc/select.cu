@@ -118,8 +118,10 @@ __device__ __forceinline__ Thr thr_from(const int4 &p, int64_t now) {
 // a * b for |a| < 2^62 / b: one wide multiply + one multiply-add (the compiler's
 // generic 64x64 product costs twice that)
 __device__ __forceinline__ int64_t mul64x32(int64_t a, uint32_t b) {
-    const uint64_t lo = (uint64_t)(uint32_t)a * b;
-    const uint32_t hi = (uint32_t)(lo >> 32) + (uint32_t)(a >> 32) * b;
+    uint64_t lo;
+    uint32_t hi;
+    asm("mul.wide.u32 %0, %1, %2;" : "=l"(lo) : "r"((uint32_t)a), "r"(b));
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(hi) : "r"((uint32_t)(a >> 32)), "r"(b), "r"((uint32_t)(lo >> 32)));
     return (int64_t)(((uint64_t)hi << 32) | (uint32_t)lo);
 }
 
@@ -336,7 +338,7 @@ __device__ __forceinline__ void scan_chunk(const int4 *__restrict__ stage, int4 
                                            int32_t idx_base, int k, int64_t now, SelState<POLICY> &s) {
     const int lane = lane_id();
     const uint32_t lt_mask = (1u << lane) - 1u;
-#pragma unroll 1
+#pragma unroll
     for (int i = 0; i < SEL_CHUNK / 32; i += SEL_UNROLL) {
         if (!FULL && i * 32 >= nvalid) break;
         int4 r[SEL_UNROLL];
