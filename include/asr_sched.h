@@ -149,8 +149,10 @@ int asr_sched_simulate(const asr_req_t *trace, int64_t n, int32_t policy,
 /* n_replicas independent replicas (seed x rate x policy).  Batches of at least
  * ASR_OPT_SIM_LANE_MIN_REPLICAS replicas with max_slots <= 32 run one THREAD
  * per replica until a replica has to choose among waiting requests under
- * SJF/HRRN; such replicas, and every other batch, run one WARP per replica.
- * The results do not depend on which kernel ran.
+ * SJF/HRRN; such replicas, and every other batch, run one WARP per replica; a
+ * replica whose waiting window outgrows ASR_OPT_SIM_ESCALATE_WINDOW requests
+ * (a deep backlog) is handed on to one CTA per replica, which selects from a
+ * candidate pool in shared memory.  The results do not depend on which kernel ran.
  *   traces DEVICE; replicas DEVICE [n_replicas]; cms DEVICE [n_cms];
  *   out_lat/out_ttft DEVICE [total_requests] indexed by replica.out_off, or both
  *   NULL for summary-only mode (the arrays then live in the workspace);
@@ -230,8 +232,11 @@ size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c);
 /* Process-wide tuning options (never change any result).
  * ASR_OPT_SIM_LANE_MIN_REPLICAS: smallest batch that asr_sched_simulate_batched
  * runs thread-per-replica (default 1024; 1 = always when max_slots <= 32;
- * INT32_MAX = never). */
-enum { ASR_OPT_SIM_LANE_MIN_REPLICAS = 0 };
+ * INT32_MAX = never).
+ * ASR_OPT_SIM_ESCALATE_WINDOW: waiting-window length (requests) beyond which the
+ * warp kernel hands a SJF/HRRN replica to the CTA kernel (default 4096; 0 = as
+ * soon as the policy has to choose; INT32_MAX = never). */
+enum { ASR_OPT_SIM_LANE_MIN_REPLICAS = 0, ASR_OPT_SIM_ESCALATE_WINDOW = 1 };
 int asr_sched_set_option(int32_t option, int64_t value);
 
 const char *asr_sched_last_error(void); /* thread-local, never NULL */

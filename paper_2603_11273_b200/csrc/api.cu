@@ -36,7 +36,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
-    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel"};
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel"};
 struct TimedLaunch {
     int kid;
     cudaEvent_t start, stop;
@@ -82,12 +82,13 @@ struct SimWorkspace {
 
 // asr_sched_set_option values
 static std::atomic<int> g_opt_lane_min{1024};
+static std::atomic<int> g_opt_escalate{4096};
 
 static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summary_only) {
     SimWorkspace w;
     w.bm_off_bytes = align_up(sizeof(int64_t) * (size_t)(n_replicas + 1));
     w.bitmap_bytes = align_up(sizeof(uint32_t) * (size_t)(total_requests / 32 + 2 * n_replicas + 2));
-    w.defer_bytes = align_up(sizeof(int32_t) * (size_t)(n_replicas + 64));   // [0]: counter, [64..]: list
+    w.defer_bytes = align_up(sizeof(int32_t) * (size_t)(2 * n_replicas + 64));   // [0], [1]: counters, [64..]: the two lists
     w.lat_bytes = summary_only ? align_up(sizeof(int64_t) * (size_t)total_requests) : 0;
     w.total = w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + 2 * w.lat_bytes;
     return w;
@@ -115,6 +116,10 @@ extern "C" int asr_sched_set_option(int32_t option, int64_t value) {
         case ASR_OPT_SIM_LANE_MIN_REPLICAS:
             if (value < 1 || value > INT32_MAX) break;
             g_opt_lane_min.store((int)value);
+            return ASR_OK;
+        case ASR_OPT_SIM_ESCALATE_WINDOW:
+            if (value < 0 || value > INT32_MAX) break;
+            g_opt_escalate.store((int)value);
             return ASR_OK;
     }
     set_error("set_option: bad option %d or value %lld", option, (long long)value);
@@ -216,8 +221,8 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     }
     int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
     if (rc) return rc;
-    SimArgs a{traces, replicas, cms,      bm_off,         bitmap,     defer + 64, defer,
-              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms};
+    SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
+              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, g_opt_escalate.load()};
     // many small replicas: one thread each; few or wide ones: one warp each
     const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
     rc = launch_simulate(a, max_slots, use_lane, st);

@@ -19,7 +19,7 @@ void count_launch(int n = 1);
 // kernel ids of the per-kernel CUDA-event timing facility (asr_sched_timing_*)
 enum KernelId {
     KID_SELECT = 0, KID_SIM_PREPARE, KID_SIMULATE, KID_SIM_LANE, KID_SUMMARY_PCT, KID_PERCENTILES, KID_GEN_TRACE,
-    KID_GEN_QUEUES, KID_SWEEP_REPLICAS, KID_COUNT
+    KID_GEN_QUEUES, KID_SWEEP_REPLICAS, KID_SIM_CTA, KID_COUNT
 };
 // RAII: counts the launch and, when timing is enabled, brackets it with an
 // event pair recorded on the launching stream.
@@ -101,6 +101,44 @@ __device__ __forceinline__ bool better_rt(int policy, int64_t arr_a, int32_t est
     if (policy == ASR_FCFS) return better<ASR_FCFS>(arr_a, est_a, idx_a, arr_b, est_b, idx_b, now);
     if (policy == ASR_SJF) return better<ASR_SJF>(arr_a, est_a, idx_a, arr_b, est_b, idx_b, now);
     return better<ASR_HRRN>(arr_a, est_a, idx_a, arr_b, est_b, idx_b, now);
+}
+
+// ---- candidate records (arrival lo, arrival hi, max(est,1), idx) and their order scalar ----
+__device__ __forceinline__ int64_t rec_arr(const int4 &r) {
+    return (int64_t)(((uint64_t)(uint32_t)r.y << 32) | (uint32_t)r.x);
+}
+
+// a * b for |a| < 2^62 / b: one wide multiply + one multiply-add (the compiler's
+// generic 64x64 product costs twice that)
+__device__ __forceinline__ int64_t mul64x32(int64_t a, uint32_t b) {
+    uint64_t lo;
+    uint32_t hi;
+    asm("mul.wide.u32 %0, %1, %2;" : "=l"(lo) : "r"((uint32_t)a), "r"(b));
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(hi) : "r"((uint32_t)(a >> 32)), "r"(b), "r"((uint32_t)(lo >> 32)));
+    return (int64_t)(((uint64_t)hi << 32) | (uint32_t)lo);
+}
+
+// ---- order scalar ---------------------------------------------------------------
+// A 64-bit scalar that is WEAKLY order-preserving: scalar(a) < scalar(b) implies
+// that a is better than b under the total order; equal scalars say nothing and
+// are settled by the exact comparator.  It makes the common-case comparison of
+// the quickselect and of the final sort one 64-bit compare.
+//   FCFS  arrival
+//   SJF   est (>= 1) above the arrival time in units of 256 us, saturated
+//   HRRN  the IEEE double quotient wait/est, negated: wait < 2^53 and est are exact
+//         in double and the division is correctly rounded, hence monotone in the
+//         exact ratio (a strictly larger double means a strictly larger ratio)
+template <int POLICY>
+__device__ __forceinline__ int64_t order_scalar(const int4 &e, int64_t now) {
+    const int64_t arr = rec_arr(e);
+    if (POLICY == ASR_FCFS) return arr;
+    if (POLICY == ASR_SJF) {
+        int64_t a8 = arr >> 8;
+        a8 = a8 < 0 ? 0 : (a8 > 0xFFFFFFFFll ? 0xFFFFFFFFll : a8);
+        return ((int64_t)e.z << 32) | a8;
+    }
+    const double r = (double)wait_of(arr, now) / (double)e.z;   // e.z = max(est, 1)
+    return INT64_MAX - __double_as_longlong(r);
 }
 
 // ---- warp helpers -----------------------------------------------------------

@@ -12,15 +12,19 @@ struct SimArgs {
     uint32_t *bitmap;
     int32_t *defer_list;      // [n_replicas] replicas handed from the lane kernel to the warp kernel
     int32_t *defer_count;     // [1]
+    int32_t *defer2_list;     // [n_replicas] replicas handed from the warp kernel to the CTA kernel
+    int32_t *defer2_count;    // [1]
     int64_t *out_lat;
     int64_t *out_ttft;
     asr_summary_t *out_summary;  // nullable
     int64_t total_requests;
     int32_t n_replicas;
     int32_t n_cms;
+    int32_t escalate_window;  // waiting window (requests) beyond which a warp hands its replica to the CTA kernel
 };
 
 int launch_simulate(const SimArgs &a, int max_slots, bool use_lane, cudaStream_t st);
+int launch_simulate_cta(const SimArgs &a, cudaStream_t st);
 int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,
                        cudaStream_t st);
 int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg, const int32_t *pcts,

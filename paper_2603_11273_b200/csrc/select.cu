@@ -78,10 +78,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     } while (!ok);
 }
 
-__device__ __forceinline__ int64_t rec_arr(const int4 &r) {
-    return (int64_t)(((uint64_t)(uint32_t)r.y << 32) | (uint32_t)r.x);
-}
-
 // ---- threshold record T and the conservative per-record test -------------------
 struct Thr {
     int64_t t64;
@@ -115,16 +111,6 @@ __device__ __forceinline__ Thr thr_from(const int4 &p, int64_t now) {
     return t;
 }
 
-// a * b for |a| < 2^62 / b: one wide multiply + one multiply-add (the compiler's
-// generic 64x64 product costs twice that)
-__device__ __forceinline__ int64_t mul64x32(int64_t a, uint32_t b) {
-    uint64_t lo;
-    uint32_t hi;
-    asm("mul.wide.u32 %0, %1, %2;" : "=l"(lo) : "r"((uint32_t)a), "r"(b));
-    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(hi) : "r"((uint32_t)(a >> 32)), "r"(b), "r"((uint32_t)(lo >> 32)));
-    return (int64_t)(((uint64_t)hi << 32) | (uint32_t)lo);
-}
-
 // true for every record that is better than or ties with T (a superset is fine)
 template <int POLICY>
 __device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr &t, int64_t now) {
@@ -134,29 +120,6 @@ __device__ __forceinline__ bool may_beat(int64_t arr, int32_t est_raw, const Thr
     // HRRN: the signed wait is not clamped here: a negative wait fails unless T.est == 0
     const int64_t w = now - arr;
     return mul64x32(w, (uint32_t)t.t32) >= mul64x32(t.t64, (uint32_t)e);
-}
-
-// ---- order scalar ---------------------------------------------------------------
-// A 64-bit scalar that is WEAKLY order-preserving: scalar(a) < scalar(b) implies
-// that a is better than b under the total order; equal scalars say nothing and
-// are settled by the exact comparator.  It makes the common-case comparison of
-// the quickselect and of the final sort one 64-bit compare.
-//   FCFS  arrival
-//   SJF   est (>= 1) above the arrival time in units of 256 us, saturated
-//   HRRN  the IEEE double quotient wait/est, negated: wait < 2^53 and est are exact
-//         in double and the division is correctly rounded, hence monotone in the
-//         exact ratio (a strictly larger double means a strictly larger ratio)
-template <int POLICY>
-__device__ __forceinline__ int64_t order_scalar(const int4 &e, int64_t now) {
-    const int64_t arr = rec_arr(e);
-    if (POLICY == ASR_FCFS) return arr;
-    if (POLICY == ASR_SJF) {
-        int64_t a8 = arr >> 8;
-        a8 = a8 < 0 ? 0 : (a8 > 0xFFFFFFFFll ? 0xFFFFFFFFll : a8);
-        return ((int64_t)e.z << 32) | a8;
-    }
-    const double r = (double)wait_of(arr, now) / (double)e.z;   // e.z = max(est, 1)
-    return INT64_MAX - __double_as_longlong(r);
 }
 
 // ---- exact quickselect over the candidate buffer --------------------------------

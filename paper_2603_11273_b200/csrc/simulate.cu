@@ -20,51 +20,9 @@
 // is touched at all.  Otherwise a per-replica bitmap in the workspace marks
 // admitted requests and the admit step scans the trace window [lo, p) with
 // coalesced 128-bit loads, applying the exact comparator of asr_sched.h.
-#include "launchers.cuh"
+#include "sim_common.cuh"
 
 namespace asr {
-
-constexpr int SIM_WARPS = 4;
-constexpr int32_t REM_FREE = 0x7FFFFFFF;
-
-__device__ __forceinline__ int64_t ceil_div_pos(int64_t g, int64_t c) {
-    // g > 0, c > 0; 32-bit divide whenever both operands fit
-    if ((((uint64_t)g | (uint64_t)c) >> 32) == 0) {
-        const uint32_t q = (uint32_t)g / (uint32_t)c;
-        return (int64_t)q + ((uint32_t)g - q * (uint32_t)c != 0u ? 1 : 0);
-    }
-    const uint64_t q = (uint64_t)g / (uint64_t)c;
-    return (int64_t)q + ((uint64_t)g - q * (uint64_t)c != 0ull ? 1 : 0);
-}
-
-__device__ __forceinline__ int32_t tokens_of(const asr_cost_model_t &cm, int32_t dur_ms) {
-    int64_t t = (int64_t)cm.tok_base + ((int64_t)cm.tok_per_s * (int64_t)dur_ms) / 1000;
-    t = t < 1 ? 1 : t;
-    return t > 0x7FFFFFFE ? 0x7FFFFFFE : (int32_t)t;
-}
-
-// sum over the warp of a non-negative 32-bit value per lane, exact in 64 bits
-__device__ __forceinline__ int64_t warp_sum_u32(uint32_t v) {
-    uint32_t lo = __reduce_add_sync(ASR_FULL_MASK, v & 0xFFFFu);
-    uint32_t hi = __reduce_add_sync(ASR_FULL_MASK, v >> 16);
-    return ((int64_t)hi << 16) + (int64_t)lo;
-}
-
-// true if the descriptor of replica r can be simulated with `max_slots` slots per replica
-__device__ __forceinline__ bool replica_ok(const SimArgs &a, const asr_replica_t &rep, int max_slots) {
-    return rep.n >= 0 && rep.slots >= 1 && rep.slots <= max_slots && rep.policy >= 0 && rep.policy <= 2 &&
-           rep.cm_id >= 0 && rep.cm_id < a.n_cms && rep.trace_off >= 0 && rep.out_off >= 0 &&
-           rep.out_off + (int64_t)rep.n <= a.total_requests;
-}
-
-__device__ __forceinline__ void flag_invalid(const SimArgs &a, int r) {
-    if (!a.out_summary) return;
-    asr_summary_t s;
-    s.p50_e2e_us = s.p90_e2e_us = s.p50_ttft_us = s.p90_ttft_us = -1;
-    s.first_arrival_us = s.last_done_us = 0;
-    s.n_done = -1;
-    a.out_summary[r] = s;
-}
 
 // one warp simulates replica r from start to end
 template <int SPL>
@@ -164,6 +122,12 @@ __device__ __forceinline__ void sim_warp_replica(const SimArgs &a, const int r) 
                 nW -= k;
             } else {
                 // sparse window: bitmap marks the admitted requests of [lo, p)
+                if (p - lo > a.escalate_window) {
+                    // a backlog this deep is re-scanned for every admission: the CTA kernel
+                    // (candidate pool in shared memory) takes the replica over, from the start
+                    if (lane == 0) a.defer2_list[atomicAdd(a.defer2_count, 1)] = r;
+                    return;
+                }
                 if (!sparse) {
                     for (int w = (lo >> 5) + lane; w <= ((p - 1) >> 5); w += 32) bm[w] = 0u;
                     sparse = true;
@@ -514,7 +478,8 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
     __shared__ int64_t carry_s;
     if (threadIdx.x == 0) {
         carry_s = 0;
-        *defer_count = 0;
+        defer_count[0] = 0;   // lane kernel -> warp kernel
+        defer_count[1] = 0;   // warp kernel -> CTA kernel
     }
     __syncthreads();
     const int lane = lane_id(), warp = threadIdx.x >> 5;
@@ -580,11 +545,16 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
         // worklist pass: empty (and a few microseconds) when nothing was handed over
         const int want = (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS;
         launch_warp_any(a, max_slots, want < 148 * 8 ? want : 148 * 8, st);
-        return check_launch("sim_warp_kernel");
+        rc = check_launch("sim_warp_kernel");
+        if (rc) return rc;
+        return launch_simulate_cta(a, st);   // worklist of the warp kernel; empty unless a backlog ran deep
     }
     a.defer_list = nullptr;
     launch_warp_any(a, max_slots, (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS, st);
-    return check_launch("sim_warp_kernel");
+    int rc = check_launch("sim_warp_kernel");
+    if (rc) return rc;
+    a.defer_list = a_in.defer_list;
+    return launch_simulate_cta(a, st);
 }
 
 int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,

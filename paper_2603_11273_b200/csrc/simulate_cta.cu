@@ -1,0 +1,636 @@
+// simulate_cta.cu -- a4 simulator step + a5 outputs for DEEP BACKLOGS: one CTA per replica.
+//
+// The warp-per-replica kernel re-scans the whole waiting window for every
+// admission, which is fine for windows of a few thousand requests and hopeless
+// for the deep-backlog configuration (10^6 requests, ~2*10^5 waiting,
+// PAPER.md:104-118 overload regime; BASELINE.json configs[3]).  A warp whose
+// window outgrows ASR_OPT_SIM_ESCALATE_WINDOW hands its replica to this kernel.
+//
+// Thread s of the CTA owns batch slot s (up to 256, "max batch
+// 256"); the engine step (ingest, admit, iterate with exact fast-forward,
+// record) is the one of simulate.cu with block-wide reductions.
+//
+// Candidate pool.  Admission never looks at the whole waiting set.  A pool of
+// at most POOL_CAP waiting requests in shared memory is guaranteed to contain
+// the k best; the exact k-set is found in the pool with a block-wide
+// quickselect over 64-bit order scalars (common.cuh), ties settled by the
+// exact comparator.  The guarantee:
+//   complete   the pool IS the waiting set (backlogs up to POOL_CAP).
+//   SJF        the order is static: the pool holds every waiting request with
+//              est <= E; it contains the k best while it has k members.
+//   HRRN       the order moves with time, r_x(t) = (t - a_x)/e_x.  Built at t0
+//              with a threshold ratio theta and a horizon H, the pool holds
+//              every request with r_x(t0 + H) >= theta (ratios only grow, so
+//              nobody else can reach theta before t0 + H); G counts the
+//              members with r_x(t0) >= theta ("strong").  While t <= t0 + H and
+//              at least k strong members remain, k pool members have a ratio
+//              >= theta > that of every request outside: the k best are inside.
+// When the guarantee lapses the pool is rebuilt from the waiting window (a
+// histogram over an approximate 32-bit key picks theta; the pool itself is
+// filled by the exact integer tests).  If no pool can be built (massive ties)
+// the step falls back to an exact block-wide arg-best scan of the window.
+#include "sim_common.cuh"
+
+namespace asr {
+
+constexpr int CTA_T = 256;
+constexpr int POOL_CAP = 2048;
+constexpr int POOL_EPT = POOL_CAP / CTA_T;
+constexpr int POOL_TARGET = 1024;      // strong members wanted from a rebuild
+constexpr int HIST_BINS = 2048;
+constexpr int64_t H_MAX = 1ll << 36;   // (2^38 + 2^36) * 2^24 < 2^63
+
+struct CtaSmem {
+    int4 pool[POOL_CAP];       // (arrival lo, arrival hi, max(est,1), trace position)
+    int64_t K[POOL_CAP];       // order scalars of the current step
+    int4 adm[CTA_T];           // requests admitted in this step
+    int4 wbest[CTA_T / 32];    // per-warp winners of the fallback scan
+    uint32_t hist[HIST_BINS];
+    int32_t rep[HIST_BINS];    // one trace position per histogram bin
+    uint16_t tie[POOL_CAP];
+    uint16_t hole[CTA_T], surv[CTA_T];
+    int64_t red64[CTA_T / 32];
+    int32_t red32[CTA_T / 32];
+    int64_t bc64;
+    int32_t pool_n, adm_n, hole_n, surv_n, tie_n, bc32[4];
+};
+
+// ---- block-wide helpers (every thread calls them; every thread gets the result) ----
+__device__ __forceinline__ int block_sum(int v, CtaSmem &sm) {
+    v = __reduce_add_sync(ASR_FULL_MASK, v);
+    __syncthreads();
+    if (lane_id() == 0) sm.red32[threadIdx.x >> 5] = v;
+    __syncthreads();
+    int s = 0;
+#pragma unroll
+    for (int w = 0; w < CTA_T / 32; ++w) s += sm.red32[w];
+    return s;
+}
+__device__ __forceinline__ int block_min(int v, CtaSmem &sm) {
+    v = __reduce_min_sync(ASR_FULL_MASK, v);
+    __syncthreads();
+    if (lane_id() == 0) sm.red32[threadIdx.x >> 5] = v;
+    __syncthreads();
+    int s = sm.red32[0];
+#pragma unroll
+    for (int w = 1; w < CTA_T / 32; ++w) s = sm.red32[w] < s ? sm.red32[w] : s;
+    return s;
+}
+__device__ __forceinline__ int block_max(int v, CtaSmem &sm) { return -block_min(-v, sm); }
+__device__ __forceinline__ int64_t block_sum64(int64_t v, CtaSmem &sm) {
+#pragma unroll
+    for (int j = 16; j > 0; j >>= 1) v += (int64_t)shfl64_xor((uint64_t)v, j);
+    __syncthreads();
+    if (lane_id() == 0) sm.red64[threadIdx.x >> 5] = v;
+    __syncthreads();
+    int64_t s = 0;
+#pragma unroll
+    for (int w = 0; w < CTA_T / 32; ++w) s += sm.red64[w];
+    return s;
+}
+// exclusive rank of this thread among the threads with flag set
+__device__ __forceinline__ int block_rank(bool flag, CtaSmem &sm) {
+    const uint32_t m = __ballot_sync(ASR_FULL_MASK, flag);
+    const int warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane_id() == 0) sm.red32[warp] = __popc(m);
+    __syncthreads();
+    int before = 0;
+#pragma unroll
+    for (int w = 0; w < CTA_T / 32; ++w)
+        if (w < warp) before += sm.red32[w];
+    return before + __popc(m & ((1u << lane_id()) - 1u));
+}
+
+__device__ __forceinline__ int64_t order_scalar_rt(int policy, const int4 &e, int64_t now) {
+    return policy == ASR_SJF ? order_scalar<ASR_SJF>(e, now) : order_scalar<ASR_HRRN>(e, now);
+}
+__device__ __forceinline__ bool cand_better(int policy, const int4 &x, const int4 &y, int64_t now) {
+    return better_rt(policy, rec_arr(x), x.z, x.w, rec_arr(y), y.z, y.w, now);
+}
+__device__ __forceinline__ int4 cand_of(const asr_req_t *trace, int pos) {
+    const int4 v = __ldg(reinterpret_cast<const int4 *>(trace + pos));
+    return make_int4(v.x, v.y, v.w < 1 ? 1 : v.w, pos);
+}
+// the bitmap is updated with atomics (performed in L2): read it past L1
+__device__ __forceinline__ bool is_admitted(const uint32_t *bm, int pos) { return (__ldcg(bm + (pos >> 5)) >> (pos & 31)) & 1u; }
+
+// approximate 32-bit key of a waiting request, smaller = better; only used to pick a threshold
+__device__ __forceinline__ int32_t approx_key(int policy, const int4 &e, int64_t t0) {
+    if (policy == ASR_SJF) return e.z;
+    const float r = (float)wait_of(rec_arr(e), t0) / (float)e.z;
+    return 0x7FFFFFFF - __float_as_int(r);
+}
+
+struct PoolState {
+    int P;             // members
+    bool complete;     // the pool is the whole waiting set
+    bool thr_valid;    // threshold mode: thrW/thrE/t0H describe the membership test
+    int G;             // HRRN: strong members left (lower bound)
+    int64_t thrW;      // HRRN: theta = thrW / thrE
+    int32_t thrE;      // SJF: est bound E
+    int64_t t0H;       // HRRN: the guarantee holds up to this time
+    int64_t t0;
+    int64_t H;
+};
+
+// membership test of the current threshold for a request (threshold mode)
+__device__ __forceinline__ bool pool_pass(int policy, const PoolState &ps, const int4 &e) {
+    if (policy == ASR_SJF) return e.z <= ps.thrE;
+    return mul64x32(ps.t0H - rec_arr(e), (uint32_t)ps.thrE) >= mul64x32(ps.thrW, (uint32_t)e.z);
+}
+
+// ---- rebuild the pool from the waiting window [lo, p) ---------------------------------
+__device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_req_t *trace, const uint32_t *bm,
+                                          int policy, int64_t t, int &lo, int p, int nW, int k) {
+    const int tid = threadIdx.x;
+    // advance lo to the first waiting request
+    for (;;) {
+        const int w = (lo >> 5) + tid;
+        int cand = 0x7FFFFFFF;
+        if ((int64_t)w * 32 < p) {
+            uint32_t inv = ~__ldcg(bm + w);
+            if (w == (lo >> 5)) inv &= ~((1u << (lo & 31)) - 1u);
+            if (inv) cand = w * 32 + __ffs(inv) - 1;
+        }
+        cand = block_min(cand, sm);
+        if (cand != 0x7FFFFFFF) {
+            lo = cand < p ? cand : p;
+            break;
+        }
+        lo = ((lo >> 5) + CTA_T) * 32;
+        if (lo >= p) {
+            lo = p;
+            break;
+        }
+    }
+    if (policy == ASR_HRRN && ps.thr_valid && t > ps.t0H && ps.G >= k && ps.H < H_MAX) ps.H *= 2;   // horizon ran out first
+    ps.thr_valid = false;
+    ps.complete = false;
+    ps.P = 0;
+    ps.G = 0;
+    ps.t0 = t;
+    if (tid == 0) sm.pool_n = 0;
+    __syncthreads();
+    if (nW <= POOL_CAP) {
+        for (int pos = lo + tid; pos < p; pos += CTA_T)
+            if (!is_admitted(bm, pos)) sm.pool[atomicAdd(&sm.pool_n, 1)] = cand_of(trace, pos);
+        __syncthreads();
+        ps.P = sm.pool_n;
+        ps.complete = true;
+        return;
+    }
+    // --- threshold mode: pick theta with a histogram over the approximate key
+    int kmin = 0x7FFFFFFF, kmax = 0;
+    for (int pos = lo + tid; pos < p; pos += CTA_T)
+        if (!is_admitted(bm, pos)) {
+            const int key = approx_key(policy, cand_of(trace, pos), t);
+            kmin = key < kmin ? key : kmin;
+            kmax = key > kmax ? key : kmax;
+        }
+    const int64_t lo_k0 = block_min(kmin, sm), hi_k0 = block_max(kmax, sm);
+    int target = POOL_TARGET;
+  for (int attempt = 0; attempt < 4; ++attempt) {
+    int64_t lo_k = lo_k0, hi_k = hi_k0;
+    int base_above = 0;
+    int theta_pos = -1;
+    for (int level = 0; level < 4 && theta_pos < 0; ++level) {
+        const int64_t width = (hi_k - lo_k + HIST_BINS) / HIST_BINS;   // >= 1
+        for (int b = tid; b < HIST_BINS; b += CTA_T) {
+            sm.hist[b] = 0;
+            sm.rep[b] = -1;
+        }
+        __syncthreads();
+        for (int pos = lo + tid; pos < p; pos += CTA_T)
+            if (!is_admitted(bm, pos)) {
+                const int64_t key = approx_key(policy, cand_of(trace, pos), t);
+                if (key >= lo_k && key <= hi_k) {
+                    const int b = (int)((key - lo_k) / width);
+                    atomicAdd(&sm.hist[b], 1u);
+                    sm.rep[b] = pos;
+                }
+            }
+        __syncthreads();
+        if (tid == 0) {
+            // smallest bin b with base_above + cum(b) >= target
+            int cum = base_above, b = 0, prev = -1;
+            for (; b < HIST_BINS; ++b) {
+                if (cum + (int)sm.hist[b] >= target) break;
+                if (sm.hist[b]) prev = b;
+                cum += (int)sm.hist[b];
+            }
+            int verdict;   // >= 0: trace position of theta; -1: refine inside bin b; -2: give up
+            if (b == HIST_BINS) verdict = prev >= 0 ? sm.rep[prev] : -2;
+            else if (cum + (int)sm.hist[b] <= POOL_CAP / 2 + POOL_CAP / 4) verdict = sm.rep[b];
+            else if (cum >= target / 8 && prev >= 0) verdict = sm.rep[prev];
+            else verdict = width > 1 ? -1 : -2;
+            sm.bc32[0] = verdict;
+            sm.bc32[1] = b;
+            sm.bc32[2] = cum;
+        }
+        __syncthreads();
+        const int verdict = sm.bc32[0];
+        if (verdict >= 0) theta_pos = verdict;
+        else if (verdict == -1) {
+            base_above = sm.bc32[2];
+            lo_k = lo_k + (int64_t)sm.bc32[1] * width;
+            hi_k = lo_k + width - 1;
+        } else {
+            __syncthreads();
+            return;   // no usable threshold (massive ties): the caller scans the window directly
+        }
+        __syncthreads();
+    }
+    if (theta_pos < 0) return;
+    const int4 th = cand_of(trace, theta_pos);
+    ps.thrE = th.z;
+    ps.thrW = wait_of(rec_arr(th), t);
+    // --- fill the pool with the exact tests; shrink the horizon until it fits
+    for (;;) {
+        ps.t0H = t + (policy == ASR_HRRN ? ps.H : 0);
+        if (tid == 0) sm.pool_n = 0;
+        __syncthreads();
+        int strong = 0;
+        for (int pos = lo + tid; pos < p; pos += CTA_T)
+            if (!is_admitted(bm, pos)) {
+                const int4 e = cand_of(trace, pos);
+                if (pool_pass(policy, ps, e)) {
+                    const int at = atomicAdd(&sm.pool_n, 1);
+                    if (at < POOL_CAP) sm.pool[at] = e;
+                    if (policy == ASR_HRRN &&
+                        mul64x32(t - rec_arr(e), (uint32_t)ps.thrE) >= mul64x32(ps.thrW, (uint32_t)e.z))
+                        strong++;
+                }
+            }
+        strong = block_sum(strong, sm);
+        const int cnt = sm.pool_n;
+        if (cnt <= POOL_CAP) {
+            ps.P = cnt;
+            ps.G = strong;
+            ps.thr_valid = true;
+            return;
+        }
+        if (policy == ASR_HRRN && ps.H > 0) {
+            ps.H = ps.H >= 4096 ? ps.H / 4 : 0;
+            continue;
+        }
+        // theta lets too many through (ties, or a crowded histogram bin): aim lower and pick again
+        __syncthreads();
+        if (tid == 0) sm.pool_n = 0;
+        __syncthreads();
+        target = (int)((int64_t)target * (POOL_CAP / 2) / cnt);
+        break;
+    }
+    if (target < 1) return;
+  }
+}
+
+// ---- exact k-set of the pool -> sm.adm[0..k), members removed from the pool ----------------
+__device__ __forceinline__ void pool_select(CtaSmem &sm, PoolState &ps, int policy, int64_t t, int k, uint32_t &seed) {
+    const int tid = threadIdx.x;
+    const int P = ps.P;
+    int64_t Kr[POOL_EPT];
+#pragma unroll
+    for (int e = 0; e < POOL_EPT; ++e) {
+        const int i = e * CTA_T + tid;
+        Kr[e] = INT64_MAX;
+        if (i < P) {
+            Kr[e] = order_scalar_rt(policy, sm.pool[i], t);
+            sm.K[i] = Kr[e];
+        }
+    }
+    if (tid == 0) sm.adm_n = sm.hole_n = sm.surv_n = sm.tie_n = 0;
+    __syncthreads();
+    uint32_t admmask = 0;
+    if (k >= P) {
+#pragma unroll
+        for (int e = 0; e < POOL_EPT; ++e)
+            if (e * CTA_T + tid < P) admmask |= 1u << e;
+    } else {
+        // v = k-th smallest scalar: count_less(v) < k <= count_le(v)
+        int64_t Klo = 0, Khi = 0, v = 0;
+        bool lo_inf = true, hi_inf = true;
+        int cl = 0, ce = 0;
+        for (;;) {
+            int64_t pv = 0;
+            bool ok = false;
+#pragma unroll 1
+            for (int probe = 0; probe < 2 && !ok; ++probe) {
+                seed = seed * 1664525u + 1013904223u;
+                pv = sm.K[(seed >> 8) % (uint32_t)P];
+                ok = (lo_inf || pv > Klo) && (hi_inf || pv < Khi);
+            }
+            if (!ok) {
+                // any scalar inside the bracket (v itself is one)
+                __syncthreads();
+#pragma unroll
+                for (int e = 0; e < POOL_EPT; ++e)
+                    if (e * CTA_T + tid < P && (lo_inf || Kr[e] > Klo) && (hi_inf || Kr[e] < Khi)) sm.bc64 = Kr[e];
+                __syncthreads();
+                pv = sm.bc64;
+            }
+            int c = 0;
+#pragma unroll
+            for (int e = 0; e < POOL_EPT; ++e)
+                if (e * CTA_T + tid < P) c += (Kr[e] < pv ? 1 : 0) + (Kr[e] <= pv ? 0x10000 : 0);
+            c = block_sum(c, sm);
+            cl = c & 0xFFFF;
+            ce = c >> 16;
+            if (cl >= k) {
+                Khi = pv;
+                hi_inf = false;
+            } else if (ce >= k) {
+                v = pv;
+                break;
+            } else {
+                Klo = pv;
+                lo_inf = false;
+            }
+        }
+        const int m = k - cl, T = ce - cl;   // m of the T members with scalar v are admitted
+#pragma unroll
+        for (int e = 0; e < POOL_EPT; ++e)
+            if (e * CTA_T + tid < P && (Kr[e] < v || (T == m && Kr[e] == v))) admmask |= 1u << e;
+        if (T != m) {
+            // equal scalars: the exact comparator ranks the tied members
+#pragma unroll
+            for (int e = 0; e < POOL_EPT; ++e)
+                if (e * CTA_T + tid < P && Kr[e] == v) sm.tie[atomicAdd(&sm.tie_n, 1)] = (uint16_t)(e * CTA_T + tid);
+            __syncthreads();
+#pragma unroll 1
+            for (int e = 0; e < POOL_EPT; ++e)
+                if (e * CTA_T + tid < P && Kr[e] == v) {
+                    const int4 me = sm.pool[e * CTA_T + tid];
+                    int rank = 0;
+                    for (int j = 0; j < T; ++j) {
+                        const int4 o = sm.pool[sm.tie[j]];
+                        if (o.w != me.w && cand_better(policy, o, me, t)) rank++;
+                    }
+                    if (rank < m) admmask |= 1u << e;
+                }
+        }
+    }
+    // publish the admitted, fill their holes with the survivors of the pool's tail
+    const int kk = k < P ? k : P;
+    const int newP = P - kk;
+#pragma unroll
+    for (int e = 0; e < POOL_EPT; ++e) {
+        const int i = e * CTA_T + tid;
+        if (i < P) {
+            if ((admmask >> e) & 1u) {
+                sm.adm[atomicAdd(&sm.adm_n, 1)] = sm.pool[i];
+                if (i < newP) sm.hole[atomicAdd(&sm.hole_n, 1)] = (uint16_t)i;
+            } else if (i >= newP) {
+                sm.surv[atomicAdd(&sm.surv_n, 1)] = (uint16_t)i;
+            }
+        }
+    }
+    __syncthreads();
+    const int h = sm.hole_n;
+    for (int j = tid; j < h; j += CTA_T) sm.pool[sm.hole[j]] = sm.pool[sm.surv[j]];
+    if (tid == 0) sm.pool_n = newP;
+    __syncthreads();
+    ps.P = newP;
+}
+
+// ---- fallback: exact k best of the waiting window by k block-wide arg-best scans ----------------
+__device__ __noinline__ void direct_select(CtaSmem &sm, const asr_req_t *trace, uint32_t *bm, int policy, int64_t t,
+                                           int lo, int p, int k) {
+    const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
+    for (int round = 0; round < k; ++round) {
+        int4 b = make_int4(0, 0, 1, -1);
+        for (int pos = lo + tid; pos < p; pos += CTA_T)
+            if (!is_admitted(bm, pos)) {
+                const int4 e = cand_of(trace, pos);
+                if (b.w < 0 || cand_better(policy, e, b, t)) b = e;
+            }
+#pragma unroll
+        for (int j = 16; j > 0; j >>= 1) {
+            int4 o;
+            o.x = __shfl_xor_sync(ASR_FULL_MASK, b.x, j);
+            o.y = __shfl_xor_sync(ASR_FULL_MASK, b.y, j);
+            o.z = __shfl_xor_sync(ASR_FULL_MASK, b.z, j);
+            o.w = __shfl_xor_sync(ASR_FULL_MASK, b.w, j);
+            if (o.w >= 0 && (b.w < 0 || cand_better(policy, o, b, t))) b = o;
+        }
+        __syncthreads();
+        if (lane == 0) sm.wbest[warp] = b;
+        __syncthreads();
+        if (tid == 0) {
+            int4 w = sm.wbest[0];
+            for (int j = 1; j < CTA_T / 32; ++j) {
+                const int4 o = sm.wbest[j];
+                if (o.w >= 0 && (w.w < 0 || cand_better(policy, o, w, t))) w = o;
+            }
+            sm.adm[round] = w;
+            atomicOr(&bm[w.w >> 5], 1u << (w.w & 31));   // the next round skips it
+            __threadfence_block();
+        }
+        __syncthreads();
+    }
+}
+
+__device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
+    const int tid = threadIdx.x;
+    const asr_replica_t rep = a.replicas[r];
+    const int n = rep.n, slots = rep.slots, policy = rep.policy;
+    if (!replica_ok(a, rep, CTA_T)) {
+        if (tid == 0) flag_invalid(a, r);
+        return;
+    }
+    const asr_cost_model_t cm = a.cms[rep.cm_id];
+    const asr_req_t *trace = a.traces + rep.trace_off;
+    int64_t *lat = a.out_lat + rep.out_off;
+    int64_t *ttft = a.out_ttft + rep.out_off;
+    uint32_t *bm = a.bitmap + a.bm_off[r];
+    for (int w = tid; w <= (n >> 5) + 1; w += CTA_T) bm[w] = 0u;
+    if (tid == 0) sm.pool_n = 0;
+    __syncthreads();
+
+    int32_t rem = REM_FREE, ridx = -1;   // my batch slot
+    int64_t rarr = 0;
+    int64_t t = 0;
+    int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
+    PoolState ps;
+    ps.P = 0;
+    ps.complete = true;   // nothing waits, the empty pool holds it
+    ps.thr_valid = false;
+    ps.G = 0;
+    ps.thrW = 0;
+    ps.thrE = 0;
+    ps.t0H = 0;
+    ps.t0 = 0;
+    ps.H = 1000000;
+    uint32_t seed = 0x9E3779B9u * (uint32_t)(r + 1);
+    int cbase = 0;
+    int64_t carr = tid < n ? __ldg(reinterpret_cast<const long long *>(trace + tid)) : INT64_MAX;
+    const int64_t first_arrival = n > 0 ? __ldg(reinterpret_cast<const long long *>(trace)) : 0;
+
+    while (done < n) {
+        // ---- 1. ingest arrivals <= t
+        for (;;) {
+            const int i = cbase + tid;
+            const bool isnew = i >= p && i < n && carr <= t;
+            const int cnt = __syncthreads_count(isnew);
+            if (cnt > 0 && policy != ASR_FCFS && (ps.complete || ps.thr_valid)) {
+                if (isnew) {
+                    const int4 e = cand_of(trace, i);
+                    if (ps.complete || pool_pass(policy, ps, e)) {
+                        const int at = atomicAdd(&sm.pool_n, 1);
+                        if (at < POOL_CAP) sm.pool[at] = e;
+                    }
+                }
+                __syncthreads();
+                const int np = sm.pool_n;
+                if (np > POOL_CAP) {   // does not fit any more: drop the pool, rebuild on demand
+                    __syncthreads();
+                    if (tid == 0) sm.pool_n = 0;
+                    __syncthreads();
+                    ps.P = 0;
+                    ps.complete = false;
+                    ps.thr_valid = false;
+                    ps.G = 0;
+                } else {
+                    ps.P = np;
+                }
+            }
+            p += cnt;
+            nW += cnt;
+            if (cnt == 0 || p < cbase + CTA_T) break;
+            cbase += CTA_T;
+            carr = cbase + tid < n ? __ldg(reinterpret_cast<const long long *>(trace + cbase + tid)) : INT64_MAX;
+        }
+        // arrival stamp of the next request (p < cbase + CTA_T here)
+        int64_t next_arr = INT64_MAX;
+        if (p < n) {
+            __syncthreads();
+            if (tid == p - cbase) sm.bc64 = carr;
+            __syncthreads();
+            next_arr = sm.bc64;
+        }
+        // ---- 2. idle server
+        if (nR == 0 && nW == 0) {
+            t = next_arr;
+            continue;
+        }
+        // ---- 3. admit
+        const int free_slots = slots - nR;
+        const int k = free_slots < nW ? free_slots : nW;
+        bool newly = false;
+        int32_t my_dur = 0;
+        if (k > 0) {
+            const bool is_free = tid < slots && rem == REM_FREE;
+            if (policy == ASR_FCFS) {
+                const int rank = block_rank(is_free, sm);
+                if (is_free && rank < k) {
+                    const Rec q = ld_cached(trace + lo + rank);
+                    rem = tokens_of(cm, q.dur_ms);
+                    ridx = lo + rank;
+                    rarr = q.arrival_us;
+                    my_dur = q.dur_ms;
+                    newly = true;
+                }
+                lo += k;
+            } else {
+                auto usable = [&]() {
+                    return ps.complete ||
+                           (ps.thr_valid && (policy == ASR_SJF ? ps.P >= k : (ps.G >= k && ps.P >= k && t <= ps.t0H)));
+                };
+                if (!usable()) pool_rebuild(sm, ps, trace, bm, policy, t, lo, p, nW, k);
+                if (usable()) {
+                    pool_select(sm, ps, policy, t, k, seed);
+                    if (!ps.complete) ps.G -= k;
+                } else {
+                    direct_select(sm, trace, bm, policy, t, lo, p, k);
+                    ps.P = 0;
+                    ps.thr_valid = false;
+                    ps.complete = false;
+                    ps.G = 0;
+                    if (tid == 0) sm.pool_n = 0;
+                }
+                const int rank = block_rank(is_free, sm);   // also orders the writes of sm.adm before the reads
+                if (is_free && rank < k) {
+                    const int4 e = sm.adm[rank];
+                    my_dur = __ldg(&trace[e.w].dur_ms);
+                    rem = tokens_of(cm, my_dur);
+                    ridx = e.w;
+                    rarr = rec_arr(e);
+                    newly = true;
+                    atomicOr(&bm[e.w >> 5], 1u << (e.w & 31));
+                }
+            }
+            nW -= k;
+            nR += k;
+        }
+        // ---- 4. one engine iteration with the encoders of the admitted, then the exact fast-forward
+        const int64_t c = cm.iter_base_us + cm.iter_per_running_us * (int64_t)nR;
+        int64_t t1 = t + c;
+        if (k > 0) {
+            const int64_t dur_sum = block_sum64((int64_t)my_dur, sm);
+            t1 += cm.enc_base_us * (int64_t)k + cm.enc_per_ms_us * dur_sum;
+            if (newly) ttft[ridx] = t1 - rarr;   // first token (S9)
+        }
+        const int32_t m = block_min(rem, sm);   // >= 1: nR >= 1 here
+        int64_t j = 1;
+        if (m > 1) {
+            if (nR == slots || p >= n || c <= 0) {
+                j = m;
+            } else {
+                const int64_t g = next_arr - t1;
+                if (g <= 0) j = 1;
+                else if (g > (int64_t)(m - 2) * c) j = m;
+                else j = 1 + ceil_div_pos(g, c);
+            }
+        }
+        t = t1 + (j - 1) * c;
+        // ---- 5. tokens, completions
+        bool fin = false;
+        if (rem != REM_FREE) {
+            rem -= (int32_t)j;
+            if (rem == 0) {
+                lat[ridx] = t - rarr;
+                rem = REM_FREE;
+                fin = true;
+            }
+        }
+        const int nfin = __syncthreads_count(fin);
+        nR -= nfin;
+        done += nfin;
+    }
+    if (a.out_summary && tid == 0) {
+        asr_summary_t *s = a.out_summary + r;
+        s->first_arrival_us = first_arrival;
+        s->last_done_us = t;
+        s->n_done = done;
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(CTA_T) sim_cta_kernel(SimArgs a) {
+    extern __shared__ __align__(16) unsigned char cta_dyn_smem[];
+    CtaSmem &sm = *reinterpret_cast<CtaSmem *>(cta_dyn_smem);
+    const int cnt = *a.defer2_count;
+    for (int w = blockIdx.x; w < cnt; w += gridDim.x) cta_replica(a, a.defer2_list[w], sm);
+}
+
+int launch_simulate_cta(const SimArgs &a, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(sim_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)sizeof(CtaSmem));
+        if (e != cudaSuccess) {
+            set_error("sim_cta_kernel: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+            cudaGetLastError();
+            return ASR_ECUDA;
+        }
+        attr = true;
+    }
+    const int grid = a.n_replicas < 148 * 2 ? a.n_replicas : 148 * 2;
+    {
+        KernelTimer kt(KID_SIM_CTA, st);
+        sim_cta_kernel<<<grid, CTA_T, sizeof(CtaSmem), st>>>(a);
+    }
+    return check_launch("sim_cta_kernel");
+}
+
+}  // namespace asr
