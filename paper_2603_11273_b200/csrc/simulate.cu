@@ -341,24 +341,48 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     __shared__ uint32_t s_fin[LANE_CAP * LANE_THREADS];
     __shared__ int32_t s_idx[LANE_CAP * LANE_THREADS];
     const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
-    if (r >= a.n_replicas) return;
-    const asr_replica_t rep = a.replicas[r];
-    if (!replica_ok(a, rep, LANE_CAP)) {
-        flag_invalid(a, r);
-        return;
+    // every lane of a warp stays in the loop below until the whole warp is done (the loop
+    // re-converges the warp once per admission step); `live` marks the lanes with work
+    bool live = r < a.n_replicas;
+    bool valid = live;
+    asr_replica_t rep;
+    rep.trace_off = rep.out_off = 0;
+    rep.n = 0;
+    rep.policy = rep.cm_id = 0;
+    rep.slots = 1;
+    if (live) {
+        rep = a.replicas[r];
+        if (!replica_ok(a, rep, LANE_CAP)) {
+            flag_invalid(a, r);
+            live = valid = false;
+            rep.cm_id = 0;
+            rep.n = 0;
+        }
     }
     uint32_t *fin = s_fin + threadIdx.x;
     int32_t *sidx = s_idx + threadIdx.x;
     const int n = rep.n, slots = rep.slots, policy = rep.policy;
     const asr_cost_model_t *cmp = a.cms + rep.cm_id;
-    const int64_t enc_base = __ldg(&cmp->enc_base_us), enc_per_ms = __ldg(&cmp->enc_per_ms_us);
-    const int64_t iter_base = __ldg(&cmp->iter_base_us), iter_per = __ldg(&cmp->iter_per_running_us);
+    const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
+    const int64_t iter_base64 = __ldg(&cmp->iter_base_us), iter_per64 = __ldg(&cmp->iter_per_running_us);
     const int64_t tok_base = __ldg(&cmp->tok_base), tok_per_s = __ldg(&cmp->tok_per_s);
+    // this kernel computes iteration costs in 32 bits; any other cost model goes to the warp kernel
+    const int64_t lim31 = (int64_t)1 << 31;
+    const bool small = enc_base64 >= 0 && enc_base64 < lim31 && enc_per64 >= 0 && enc_per64 < lim31 &&
+                       iter_base64 >= 0 && iter_per64 >= 0 && iter_base64 + iter_per64 * LANE_CAP < lim31;
+    bool deferred = false;
+    if (live && !small) {
+        deferred = true;
+        live = false;
+    }
+    const uint32_t enc_base = (uint32_t)enc_base64;
+    const int32_t enc_per = (int32_t)enc_per64;
+    const uint32_t ib = (uint32_t)iter_base64, ip = (uint32_t)iter_per64;
     const asr_req_t *trace = a.traces + rep.trace_off;
     int64_t *lat = a.out_lat + rep.out_off;
     int64_t *ttft = a.out_ttft + rep.out_off;
 
-    int64_t t = 0;
+    int64_t t = 0;     // the current iteration boundary
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
     int head = 0;      // running set = ring positions head .. head+nR-1, sorted by finish iteration
     uint32_t it = 0;   // engine iterations so far, mod 2^32
@@ -368,94 +392,112 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     int32_t dur0 = 0, dur1 = 0, last_dur = 0;
     // (two loads per record on purpose: a 128-bit load would leave the unused est word
     // as a dead destination register that the allocator reuses while the load is in flight)
-    if (n > 0) {
+    if (live && n > 0) {
         arr0 = ld_arrival(trace);
         dur0 = __ldg(&trace[0].dur_ms);
     }
-    if (n > 1) {
+    if (live && n > 1) {
         arr1 = ld_arrival(trace + 1);
         dur1 = __ldg(&trace[1].dur_ms);
     }
     const int64_t first_arrival = n > 0 ? arr0 : 0;
-    bool deferred = false;
+    if (n == 0) live = false;
 
-    while (done < n) {
-        // idle server: the clock jumps to the next arrival (S14)
-        if (nR == 0 && nW == 0 && arr0 > t) t = arr0;
-        // 1. ingest arrivals <= t
-        while (arr0 <= t) {
-            last_arr = arr0;
-            last_dur = dur0;
-            ++p;
-            ++nW;
-            arr0 = arr1;
-            dur0 = dur1;
-            arr1 = INT64_MAX;
-            if (p + 1 < n) {
-                arr1 = ld_arrival(trace + p + 1);
-                dur1 = __ldg(&trace[p + 1].dur_ms);
+    // One trip of the outer loop = one admission step, so that the lanes of a warp (32
+    // different replicas) stay in the same phase: A pops the completions that precede the
+    // step, B moves the clock to its boundary, C ingests, D admits.
+    while (true) {
+        if (live) {
+            // A. completions before the next admission opportunity.  With m iterations to the
+            // head's last token at cost c each, the boundaries t + j*c, j < m, precede it: if a
+            // slot is free and somebody is waiting, or the next arrival falls at or before
+            // t + (m-1)*c, the admission step comes first.
+            bool more = nR > 0;
+            while (more) {
+                const uint32_t f = fin[head * LANE_THREADS];   // sorted: the head finishes first
+                const uint32_t m = f - it;
+                const uint32_t c = ib + ip * (uint32_t)nR;
+                const int64_t lim = t + (int64_t)((uint64_t)(m - 1u) * c);
+                if (m > 0u && nR < slots && (nW > 0 || arr0 <= lim)) {
+                    more = false;
+                } else {
+                    if (m > 0u) {
+                        t = lim + c;
+                        it = f;
+                    }
+                    // lat[i] holds -arrival since admission; a fire-and-forget reduction adds the
+                    // completion time, so no load sits on the critical path
+                    const int32_t i = sidx[head * LANE_THREADS];
+                    atomicAdd(reinterpret_cast<unsigned long long *>(lat + i), (unsigned long long)t);
+                    head = (head + 1) & (LANE_CAP - 1);
+                    --nR;
+                    ++done;
+                    more = nR > 0;
+                }
             }
+            if (done >= n) live = false;
         }
-        // 3. admit
-        const int free_slots = slots - nR;
-        const int k = free_slots < nW ? free_slots : nW;
-        int64_t t1 = t + iter_base + iter_per * (int64_t)(nR + k);
-        if (k > 0) {
+        if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
+        if (live) {
+            // B. the boundary of the admission step
+            if (nW == 0 && arr0 > t) {
+                if (nR == 0) {
+                    t = arr0;   // idle server: the clock jumps to the next arrival (S14)
+                } else {
+                    const uint32_t c = ib + ip * (uint32_t)nR;
+                    const int64_t j = ceil_div_pos(arr0 - t, (int64_t)c);   // c > 0: arr0 <= t + (m-1)*c
+                    t += j * (int64_t)c;
+                    it += (uint32_t)j;
+                }
+            }
+            // C. ingest arrivals <= t
+            while (arr0 <= t) {
+                last_arr = arr0;
+                last_dur = dur0;
+                ++p;
+                ++nW;
+                arr0 = arr1;
+                dur0 = dur1;
+                arr1 = INT64_MAX;
+                if (p + 1 < n) {
+                    arr1 = ld_arrival(trace + p + 1);
+                    dur1 = __ldg(&trace[p + 1].dur_ms);
+                }
+            }
+            // D. admit k >= 1 requests (a slot is free and somebody waits)
+            const int free_slots = slots - nR;
+            const int k = free_slots < nW ? free_slots : nW;
             if (policy != ASR_FCFS && k < nW) {   // a real choice: hand over to the warp kernel
                 deferred = true;
-                break;
-            }
-            if (k == 1 && lo == p - 1) {
-                // the request ingested last: everything needed is in registers
-                lane_insert(fin, sidx, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
-                t1 += enc_base + enc_per_ms * (int64_t)last_dur;
-                ttft[lo] = t1 - last_arr;   // first token (S9)
-                lat[lo] = -last_arr;        // E2E = completion time - arrival: the completion adds its time
+                live = false;
             } else {
-                int64_t dur_sum = 0;
-                for (int q = 0; q < k; ++q) {
-                    const int32_t dur = __ldg(&trace[lo + q].dur_ms);
-                    lane_insert(fin, sidx, head, nR + q, it, lane_tokens(tok_base, tok_per_s, dur), lo + q);
-                    dur_sum += (int64_t)dur;
+                int64_t t1 = t + (int64_t)(ib + ip * (uint32_t)(nR + k));
+                if (k == 1 && lo == p - 1) {
+                    // the request ingested last: everything needed is in registers
+                    lane_insert(fin, sidx, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
+                    t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
+                    ttft[lo] = t1 - last_arr;   // first token (S9)
+                    lat[lo] = -last_arr;        // E2E = completion time - arrival: the completion adds its time
+                } else {
+                    int64_t dur_sum = 0;
+                    for (int q = 0; q < k; ++q) {
+                        const int32_t dur = __ldg(&trace[lo + q].dur_ms);
+                        lane_insert(fin, sidx, head, nR + q, it, lane_tokens(tok_base, tok_per_s, dur), lo + q);
+                        dur_sum += (int64_t)dur;
+                    }
+                    t1 += (int64_t)enc_base * (int64_t)k + (int64_t)enc_per * dur_sum;
+                    for (int q = 0; q < k; ++q) {
+                        const int64_t arr = ld_arrival(trace + lo + q);
+                        ttft[lo + q] = t1 - arr;
+                        lat[lo + q] = -arr;
+                    }
                 }
-                t1 += enc_base * (int64_t)k + enc_per_ms * dur_sum;
-                for (int q = 0; q < k; ++q) {
-                    const int64_t arr = ld_arrival(trace + lo + q);
-                    ttft[lo + q] = t1 - arr;
-                    lat[lo + q] = -arr;
-                }
+                lo += k;
+                nW -= k;
+                nR += k;
+                t = t1;
+                it += 1u;
             }
-            lo += k;
-            nW -= k;
-            nR += k;
-        }
-        // 4. fast-forward over identical iterations to the next event
-        const uint32_t m = fin[head * LANE_THREADS] - it;   // the running set is sorted: its head finishes first
-        const int64_t c = iter_base + iter_per * (int64_t)nR;
-        int64_t j = 1;
-        if (m > 1u) {
-            if (nR == slots || p >= n || c <= 0) {
-                j = m;
-            } else {
-                const int64_t g = arr0 - t1;
-                if (g <= 0) j = 1;
-                else if (g > (int64_t)(m - 2u) * c) j = m;
-                else j = 1 + ceil_div_pos(g, c);
-            }
-        }
-        t = t1 + (j - 1) * c;
-        it += (uint32_t)j;
-        // 5. completions: pop the head while it finishes in this iteration.  lat[i] holds
-        // -arrival since admission; a fire-and-forget reduction adds the completion time, so
-        // no load sits on the critical path
-        if ((uint32_t)j == m) {
-            do {
-                const int32_t i = sidx[head * LANE_THREADS];
-                atomicAdd(reinterpret_cast<unsigned long long *>(lat + i), (unsigned long long)t);
-                head = (head + 1) & (LANE_CAP - 1);
-                --nR;
-                ++done;
-            } while (nR > 0 && fin[head * LANE_THREADS] == it);
         }
     }
     if (deferred) {
@@ -463,7 +505,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         a.defer_list[pos] = r;
         return;
     }
-    if (a.out_summary) {
+    if (valid && a.out_summary) {
         asr_summary_t *s = a.out_summary + r;
         s->first_arrival_us = first_arrival;
         s->last_done_us = t;
