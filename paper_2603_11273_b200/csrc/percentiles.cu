@@ -143,8 +143,9 @@ constexpr int PCT_CAND = 1024;                               // candidates finis
 struct PctRegSmem {
     unsigned char tab[PCT_THREADS / 32][PCT_TAB_BYTES];      // private byte counters
     uint32_t part[2][PCT_BINS];                              // column sums of warps 0-3 / 4-7
-    uint32_t cand[PCT_CAND];
-    uint32_t hist[256];
+    uint32_t cand[2][PCT_CAND];                              // candidates of a pair of targets
+    uint32_t hist[2][256];
+    uint32_t warp_cnt[PCT_THREADS / 32];
     uint32_t warp_or[PCT_THREADS / 32];
     uint32_t sel_digit[PCT_MAX], sel_below[PCT_MAX], sel_pop[PCT_MAX];
     uint32_t n_cand;
@@ -270,6 +271,9 @@ __device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N
                 pop[t] = sm.sel_pop[t];
             }
         __syncthreads();
+        int shiftv[PCT_MAX];
+#pragma unroll
+        for (int t = 0; t < PCT_MAX; ++t) shiftv[t] = sh1;
         for (int t = 0; t < pl.n_pct; ++t) {
             int shift = sh1;
             // more counting passes while the bin is too crowded for the candidate buffer
@@ -282,67 +286,119 @@ __device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N
                 shift = ns;
                 __syncthreads();
             }
-            if (shift == 0) continue;
-            // compact the keys of the selected bin into shared memory
-            if (threadIdx.x == 0) sm.n_cand = 0;
-            __syncthreads();
+            shiftv[t] = shift;
+        }
+        // number of valid values of this thread (value j of a thread is element j*PCT_THREADS + tid)
+        const int nj = N > (int)threadIdx.x ? (N - (int)threadIdx.x + PCT_THREADS - 1) / PCT_THREADS : 0;
+        // targets two at a time: compact the keys of both selected bins into shared memory
+        // (private counts, one block scan, no ballots), then finish both on the candidates
+        for (int t0 = 0; t0 < pl.n_pct; t0 += 2) {
+            const bool two = t0 + 1 < pl.n_pct;
+            const int sa = shiftv[t0], sb = two ? shiftv[t0 + 1] : 0;
+            const uint32_t pa = prefix[t0], pb = two ? prefix[t0 + 1] : 0u;
+            const bool do_a = sa > 0, do_b = two && sb > 0;
+            if (!do_a && !do_b) continue;
+            // an inactive target matches nothing: shift 31 against an impossible prefix (keys < 2^32)
+            const int sha = do_a ? sa : 31, shb = do_b ? sb : 31;
+            const uint32_t pra = do_a ? pa : 2u, prb = do_b ? pb : 2u;
+            uint32_t cnt = 0;   // matches of target a in the low half, of target b in the high half
 #pragma unroll
             for (int j = 0; j < PCT_VPT; ++j) {
-                const int i = j * PCT_THREADS + threadIdx.x;
-                const bool in = i < N && (key[j] >> shift) == prefix[t];
-                const uint32_t m = __ballot_sync(ASR_FULL_MASK, in);
-                if (m != 0u) {
-                    uint32_t base = 0;
-                    if (lane == 0) base = atomicAdd(&sm.n_cand, (uint32_t)__popc(m));
-                    base = __shfl_sync(ASR_FULL_MASK, base, 0);
-                    if (in) sm.cand[base + __popc(m & ((1u << lane) - 1u))] = key[j];
+                if (j < nj) {
+                    cnt += ((key[j] >> sha) == pra ? 1u : 0u) + ((key[j] >> shb) == prb ? 0x10000u : 0u);
                 }
             }
+            uint32_t incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+                if (lane >= d) incl += y;
+            }
+            if (lane == 31) sm.warp_cnt[warp] = incl;
             __syncthreads();
-            const int C = (int)sm.n_cand;   // == pop[t]
-            // finish on the candidates: 8-bit digits, shared-memory histogram (few values)
-            while (shift > 0) {
-                const int ns = shift > 8 ? shift - 8 : 0;
-                const uint32_t mask = (1u << (shift - ns)) - 1u;
-                sm.hist[threadIdx.x] = 0;   // PCT_THREADS == 256
-                __syncthreads();
-                for (int i = threadIdx.x; i < C; i += PCT_THREADS) {
-                    const uint32_t x = sm.cand[i];
-                    if ((x >> shift) == prefix[t]) atomicAdd(&sm.hist[(x >> ns) & mask], 1u);
+            uint32_t base = incl - cnt;
+            uint32_t total = 0;
+#pragma unroll
+            for (int w = 0; w < PCT_THREADS / 32; ++w) {
+                const uint32_t c = sm.warp_cnt[w];
+                if (w < warp) base += c;
+                total += c;
+            }
+            uint32_t posa = base & 0xFFFFu, posb = base >> 16;
+#pragma unroll
+            for (int j = 0; j < PCT_VPT; ++j) {
+                if (j < nj) {
+                    if ((key[j] >> sha) == pra) sm.cand[0][posa++] = key[j];
+                    if ((key[j] >> shb) == prb) sm.cand[1][posb++] = key[j];
+                }
+            }
+            const int Ca = (int)(total & 0xFFFFu), Cb = (int)(total >> 16);   // == pop[t0], pop[t0+1]
+            // finish on the candidates: 8-bit digits, shared-memory histograms (few values);
+            // warp 0 resolves target a, warp 1 target b
+            int s_a = do_a ? sa : 0, s_b = do_b ? sb : 0;
+            uint32_t p_a = pa, p_b = pb, k_a = kk[t0], k_b = two ? kk[t0 + 1] : 0u;
+            while (s_a > 0 || s_b > 0) {
+                const int na = s_a > 8 ? s_a - 8 : 0, nb = s_b > 8 ? s_b - 8 : 0;
+                sm.hist[0][threadIdx.x] = 0;   // PCT_THREADS == 256
+                sm.hist[1][threadIdx.x] = 0;
+                __syncthreads();               // also orders the candidate stores above
+                if (s_a > 0) {
+                    const uint32_t mask = (1u << (s_a - na)) - 1u;
+                    for (int i = threadIdx.x; i < Ca; i += PCT_THREADS) {
+                        const uint32_t x = sm.cand[0][i];
+                        if ((x >> s_a) == p_a) atomicAdd(&sm.hist[0][(x >> na) & mask], 1u);
+                    }
+                }
+                if (s_b > 0) {
+                    const uint32_t mask = (1u << (s_b - nb)) - 1u;
+                    for (int i = threadIdx.x; i < Cb; i += PCT_THREADS) {
+                        const uint32_t x = sm.cand[1][i];
+                        if ((x >> s_b) == p_b) atomicAdd(&sm.hist[1][(x >> nb) & mask], 1u);
+                    }
                 }
                 __syncthreads();
-                if (warp == 0) {
+                if (warp < 2 && (warp == 0 ? s_a > 0 : s_b > 0)) {
+                    const uint32_t *h = sm.hist[warp];
                     uint32_t c[8], tot = 0;
 #pragma unroll
-                    for (int b = 0; b < 8; ++b) {
-                        c[b] = sm.hist[lane * 8 + b];
-                        tot += c[b];
+                    for (int b8 = 0; b8 < 8; ++b8) {
+                        c[b8] = h[lane * 8 + b8];
+                        tot += c[b8];
                     }
-                    uint32_t incl = tot;
+                    uint32_t inc = tot;
 #pragma unroll
                     for (int d = 1; d < 32; d <<= 1) {
-                        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
-                        if (lane >= d) incl += y;
+                        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, inc, d);
+                        if (lane >= d) inc += y;
                     }
-                    const uint32_t excl = incl - tot, k = kk[t];
-                    if (excl < k && k <= incl) {
+                    const uint32_t excl = inc - tot, k = warp == 0 ? k_a : k_b;
+                    if (excl < k && k <= inc) {
                         uint32_t run = excl;
 #pragma unroll
-                        for (int b = 0; b < 8; ++b) {
-                            if (run < k && k <= run + c[b]) {
-                                sm.sel_digit[t] = (uint32_t)(lane * 8 + b);
-                                sm.sel_below[t] = run;
+                        for (int b8 = 0; b8 < 8; ++b8) {
+                            if (run < k && k <= run + c[b8]) {
+                                sm.sel_digit[t0 + warp] = (uint32_t)(lane * 8 + b8);
+                                sm.sel_below[t0 + warp] = run;
                             }
-                            run += c[b];
+                            run += c[b8];
                         }
                     }
                 }
                 __syncthreads();
-                prefix[t] = (prefix[t] << (shift - ns)) | sm.sel_digit[t];
-                kk[t] -= sm.sel_below[t];
-                shift = ns;
+                if (s_a > 0) {
+                    p_a = (p_a << (s_a - na)) | sm.sel_digit[t0];
+                    k_a -= sm.sel_below[t0];
+                    s_a = na;
+                }
+                if (s_b > 0) {
+                    p_b = (p_b << (s_b - nb)) | sm.sel_digit[t0 + 1];
+                    k_b -= sm.sel_below[t0 + 1];
+                    s_b = nb;
+                }
                 __syncthreads();
             }
+            if (do_a) prefix[t0] = p_a;
+            if (do_b) prefix[t0 + 1] = p_b;
         }
     }
     for (int t = 0; t < pl.n_pct; ++t) results[t] = (int64_t)(((uint64_t)hi0 << 32) | prefix[t]);

@@ -319,27 +319,22 @@ __device__ __forceinline__ uint32_t lane_tokens(int64_t tok_base, int64_t tok_pe
     return (uint32_t)tok;
 }
 
-// insert (it + tokens, idx) into the sorted ring of nR entries starting at `head`
-__device__ __forceinline__ void lane_insert(uint32_t *fin, int32_t *sidx, int head, int nR, uint32_t it,
-                                            uint32_t tokens, int32_t idx) {
+// insert (it + tokens, idx) into the sorted ring of nR entries starting at `head`;
+// an entry is one 64-bit word (finish iteration, request index)
+__device__ __forceinline__ void lane_insert(uint2 *ring, int head, int nR, uint32_t it, uint32_t tokens,
+                                            int32_t idx) {
     int h = nR;
     while (h > 0) {
-        const int prev = ((head + h - 1) & (LANE_CAP - 1)) * LANE_THREADS;
-        const uint32_t f = fin[prev];
-        if (f - it <= tokens) break;
-        const int cur = ((head + h) & (LANE_CAP - 1)) * LANE_THREADS;
-        fin[cur] = f;
-        sidx[cur] = sidx[prev];
+        const uint2 e = ring[((head + h - 1) & (LANE_CAP - 1)) * LANE_THREADS];
+        if (e.x - it <= tokens) break;
+        ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = e;
         --h;
     }
-    const int cur = ((head + h) & (LANE_CAP - 1)) * LANE_THREADS;
-    fin[cur] = it + tokens;
-    sidx[cur] = idx;
+    ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = make_uint2(it + tokens, (uint32_t)idx);
 }
 
 __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
-    __shared__ uint32_t s_fin[LANE_CAP * LANE_THREADS];
-    __shared__ int32_t s_idx[LANE_CAP * LANE_THREADS];
+    __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
     const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
     // every lane of a warp stays in the loop below until the whole warp is done (the loop
     // re-converges the warp once per admission step); `live` marks the lanes with work
@@ -359,8 +354,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             rep.n = 0;
         }
     }
-    uint32_t *fin = s_fin + threadIdx.x;
-    int32_t *sidx = s_idx + threadIdx.x;
+    uint2 *ring = s_ring + threadIdx.x;
     const int n = rep.n, slots = rep.slots, policy = rep.policy;
     const asr_cost_model_t *cmp = a.cms + rep.cm_id;
     const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
@@ -386,10 +380,10 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
     int head = 0;      // running set = ring positions head .. head+nR-1, sorted by finish iteration
     uint32_t it = 0;   // engine iterations so far, mod 2^32
-    // look-ahead window over the trace: record p and record p+1 are in registers, so
-    // the load of a record is issued two ingests before its arrival stamp is tested
-    int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, last_arr = 0;
-    int32_t dur0 = 0, dur1 = 0, last_dur = 0;
+    // look-ahead window over the trace: records p .. p+3 are in registers, so the load of
+    // a record is issued four ingests before its arrival stamp is tested
+    int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, arr2 = INT64_MAX, arr3 = INT64_MAX, last_arr = 0;
+    int32_t dur0 = 0, dur1 = 0, dur2 = 0, dur3 = 0, last_dur = 0;
     // (two loads per record on purpose: a 128-bit load would leave the unused est word
     // as a dead destination register that the allocator reuses while the load is in flight)
     if (live && n > 0) {
@@ -399,6 +393,14 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     if (live && n > 1) {
         arr1 = ld_arrival(trace + 1);
         dur1 = __ldg(&trace[1].dur_ms);
+    }
+    if (live && n > 2) {
+        arr2 = ld_arrival(trace + 2);
+        dur2 = __ldg(&trace[2].dur_ms);
+    }
+    if (live && n > 3) {
+        arr3 = ld_arrival(trace + 3);
+        dur3 = __ldg(&trace[3].dur_ms);
     }
     const int64_t first_arrival = n > 0 ? arr0 : 0;
     if (n == 0) live = false;
@@ -414,7 +416,8 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             // t + (m-1)*c, the admission step comes first.
             bool more = nR > 0;
             while (more) {
-                const uint32_t f = fin[head * LANE_THREADS];   // sorted: the head finishes first
+                const uint2 e = ring[head * LANE_THREADS];   // sorted: the head finishes first
+                const uint32_t f = e.x;
                 const uint32_t m = f - it;
                 const uint32_t c = ib + ip * (uint32_t)nR;
                 const int64_t lim = t + (int64_t)((uint64_t)(m - 1u) * c);
@@ -427,8 +430,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     }
                     // lat[i] holds -arrival since admission; a fire-and-forget reduction adds the
                     // completion time, so no load sits on the critical path
-                    const int32_t i = sidx[head * LANE_THREADS];
-                    atomicAdd(reinterpret_cast<unsigned long long *>(lat + i), (unsigned long long)t);
+                    atomicAdd(reinterpret_cast<unsigned long long *>(lat + (int32_t)e.y), (unsigned long long)t);
                     head = (head + 1) & (LANE_CAP - 1);
                     --nR;
                     ++done;
@@ -458,10 +460,14 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 ++nW;
                 arr0 = arr1;
                 dur0 = dur1;
-                arr1 = INT64_MAX;
-                if (p + 1 < n) {
-                    arr1 = ld_arrival(trace + p + 1);
-                    dur1 = __ldg(&trace[p + 1].dur_ms);
+                arr1 = arr2;
+                dur1 = dur2;
+                arr2 = arr3;
+                dur2 = dur3;
+                arr3 = INT64_MAX;
+                if (p + 3 < n) {
+                    arr3 = ld_arrival(trace + p + 3);
+                    dur3 = __ldg(&trace[p + 3].dur_ms);
                 }
             }
             // D. admit k >= 1 requests (a slot is free and somebody waits)
@@ -474,7 +480,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 int64_t t1 = t + (int64_t)(ib + ip * (uint32_t)(nR + k));
                 if (k == 1 && lo == p - 1) {
                     // the request ingested last: everything needed is in registers
-                    lane_insert(fin, sidx, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
+                    lane_insert(ring, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
                     t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
                     ttft[lo] = t1 - last_arr;   // first token (S9)
                     lat[lo] = -last_arr;        // E2E = completion time - arrival: the completion adds its time
@@ -482,7 +488,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     int64_t dur_sum = 0;
                     for (int q = 0; q < k; ++q) {
                         const int32_t dur = __ldg(&trace[lo + q].dur_ms);
-                        lane_insert(fin, sidx, head, nR + q, it, lane_tokens(tok_base, tok_per_s, dur), lo + q);
+                        lane_insert(ring, head, nR + q, it, lane_tokens(tok_base, tok_per_s, dur), lo + q);
                         dur_sum += (int64_t)dur;
                     }
                     t1 += (int64_t)enc_base * (int64_t)k + (int64_t)enc_per * dur_sum;
