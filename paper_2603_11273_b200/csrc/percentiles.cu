@@ -226,7 +226,8 @@ __device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], i
 }
 
 // Returns false (nothing written) when the segment does not qualify.
-__device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N64, const PctList &pl,
+template <int MAXT>
+__device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N64, const PctList &pl,
                                         int64_t *results, PctRegSmem &sm) {
     if (N64 <= 0 || N64 > PCT_REG_MAX) return false;
     const int N = (int)N64;
@@ -252,29 +253,31 @@ __device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N
     for (int w = 0; w < PCT_THREADS / 32; ++w) or_all |= sm.warp_or[w];
     const int bits = or_all == 0u ? 0 : 32 - __clz((int)or_all);
 
-    uint32_t kk[PCT_MAX], prefix[PCT_MAX];
+    uint32_t kk[MAXT], prefix[MAXT];
 #pragma unroll
-    for (int t = 0; t < PCT_MAX; ++t) {
-        kk[t] = t < pl.n_pct ? (uint32_t)(((uint64_t)pl.pct[t] * (uint64_t)N + 99) / 100) : 0u;   // 1-based rank
+    for (int t = 0; t < MAXT; ++t) {
+        kk[t] = t < pl.n_pct ? ((uint32_t)pl.pct[t] * (uint32_t)N + 99u) / 100u : 0u;   // 1-based rank; pct <= 100, N <= 10,240
         prefix[t] = 0;
     }
     if (bits > 0) {
         // first pass: all targets at once, no filter (every key >> bits is 0)
         const int sh1 = bits > PCT_DIG ? bits - PCT_DIG : 0;
         reg_count_pass(key, N, 32, sh1, 0u, kk, 0, pl.n_pct, sm);
-        uint32_t pop[PCT_MAX];
+        uint32_t pop[MAXT];
 #pragma unroll
-        for (int t = 0; t < PCT_MAX; ++t)
+        for (int t = 0; t < MAXT; ++t)
             if (t < pl.n_pct) {
                 prefix[t] = sm.sel_digit[t];
                 kk[t] -= sm.sel_below[t];
                 pop[t] = sm.sel_pop[t];
             }
         __syncthreads();
-        int shiftv[PCT_MAX];
+        int shiftv[MAXT];
 #pragma unroll
-        for (int t = 0; t < PCT_MAX; ++t) shiftv[t] = sh1;
-        for (int t = 0; t < pl.n_pct; ++t) {
+        for (int t = 0; t < MAXT; ++t) shiftv[t] = sh1;
+#pragma unroll
+        for (int t = 0; t < MAXT; ++t) {
+            if (t >= pl.n_pct) break;
             int shift = sh1;
             // more counting passes while the bin is too crowded for the candidate buffer
             while (shift > 0 && pop[t] > (uint32_t)PCT_CAND) {
@@ -292,22 +295,40 @@ __device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N
         const int nj = N > (int)threadIdx.x ? (N - (int)threadIdx.x + PCT_THREADS - 1) / PCT_THREADS : 0;
         // targets two at a time: compact the keys of both selected bins into shared memory
         // (private counts, one block scan, no ballots), then finish both on the candidates
-        for (int t0 = 0; t0 < pl.n_pct; t0 += 2) {
-            const bool two = t0 + 1 < pl.n_pct;
-            const int sa = shiftv[t0], sb = two ? shiftv[t0 + 1] : 0;
-            const uint32_t pa = prefix[t0], pb = two ? prefix[t0 + 1] : 0u;
+#pragma unroll
+        for (int t0 = 0; t0 < MAXT; t0 += 2) {
+            if (t0 >= pl.n_pct) break;
+            const bool two = t0 + 1 < MAXT && t0 + 1 < pl.n_pct;
+            const int sa = shiftv[t0], sb = two ? shiftv[t0 + 1 < MAXT ? t0 + 1 : t0] : 0;
+            const uint32_t pa = prefix[t0], pb = two ? prefix[t0 + 1 < MAXT ? t0 + 1 : t0] : 0u;
             const bool do_a = sa > 0, do_b = two && sb > 0;
             if (!do_a && !do_b) continue;
             // an inactive target matches nothing: shift 31 against an impossible prefix (keys < 2^32)
             const int sha = do_a ? sa : 31, shb = do_b ? sb : 31;
             const uint32_t pra = do_a ? pa : 2u, prb = do_b ? pb : 2u;
-            uint32_t cnt = 0;   // matches of target a in the low half, of target b in the high half
+            // match masks of this thread's values (bit j of word j/32), per target
+            uint32_t ma0 = 0, ma1 = 0, mb0 = 0, mb1 = 0;
 #pragma unroll
             for (int j = 0; j < PCT_VPT; ++j) {
-                if (j < nj) {
-                    cnt += ((key[j] >> sha) == pra ? 1u : 0u) + ((key[j] >> shb) == prb ? 0x10000u : 0u);
+                const bool ia = (key[j] >> sha) == pra, ibb = (key[j] >> shb) == prb;
+                if (j < 32) {
+                    ma0 |= ia ? (1u << j) : 0u;
+                    mb0 |= ibb ? (1u << j) : 0u;
+                } else {
+                    ma1 |= ia ? (1u << (j - 32)) : 0u;
+                    mb1 |= ibb ? (1u << (j - 32)) : 0u;
                 }
             }
+            {   // drop the slots past the end of the segment
+                const uint32_t v0 = nj >= 32 ? 0xFFFFFFFFu : ((1u << nj) - 1u);
+                const uint32_t v1 = nj > 32 ? ((1u << (nj - 32)) - 1u) : 0u;
+                ma0 &= v0;
+                mb0 &= v0;
+                ma1 &= v1;
+                mb1 &= v1;
+            }
+            // matches of target a in the low half, of target b in the high half
+            const uint32_t cnt = (uint32_t)(__popc(ma0) + __popc(ma1)) + ((uint32_t)(__popc(mb0) + __popc(mb1)) << 16);
             uint32_t incl = cnt;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
@@ -324,19 +345,18 @@ __device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N
                 if (w < warp) base += c;
                 total += c;
             }
-            uint32_t posa = base & 0xFFFFu, posb = base >> 16;
+            uint32_t *wa = &sm.cand[0][base & 0xFFFFu], *wb = &sm.cand[1][base >> 16];
 #pragma unroll
             for (int j = 0; j < PCT_VPT; ++j) {
-                if (j < nj) {
-                    if ((key[j] >> sha) == pra) sm.cand[0][posa++] = key[j];
-                    if ((key[j] >> shb) == prb) sm.cand[1][posb++] = key[j];
-                }
+                const uint32_t bit = 1u << (j & 31);
+                if ((j < 32 ? ma0 : ma1) & bit) *wa++ = key[j];
+                if ((j < 32 ? mb0 : mb1) & bit) *wb++ = key[j];
             }
             const int Ca = (int)(total & 0xFFFFu), Cb = (int)(total >> 16);   // == pop[t0], pop[t0+1]
             // finish on the candidates: 8-bit digits, shared-memory histograms (few values);
             // warp 0 resolves target a, warp 1 target b
             int s_a = do_a ? sa : 0, s_b = do_b ? sb : 0;
-            uint32_t p_a = pa, p_b = pb, k_a = kk[t0], k_b = two ? kk[t0 + 1] : 0u;
+            uint32_t p_a = pa, p_b = pb, k_a = kk[t0], k_b = two ? kk[t0 + 1 < MAXT ? t0 + 1 : t0] : 0u;
             while (s_a > 0 || s_b > 0) {
                 const int na = s_a > 8 ? s_a - 8 : 0, nb = s_b > 8 ? s_b - 8 : 0;
                 sm.hist[0][threadIdx.x] = 0;   // PCT_THREADS == 256
@@ -398,10 +418,12 @@ __device__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N
                 __syncthreads();
             }
             if (do_a) prefix[t0] = p_a;
-            if (do_b) prefix[t0 + 1] = p_b;
+            if (do_b) prefix[t0 + 1 < MAXT ? t0 + 1 : t0] = p_b;
         }
     }
-    for (int t = 0; t < pl.n_pct; ++t) results[t] = (int64_t)(((uint64_t)hi0 << 32) | prefix[t]);
+#pragma unroll
+    for (int t = 0; t < MAXT; ++t)
+        if (t < pl.n_pct) results[t] = (int64_t)(((uint64_t)hi0 << 32) | prefix[t]);
     __syncthreads();
     return true;
 }
@@ -413,7 +435,7 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) percentiles_kernel(const int64
     for (int s = blockIdx.x; s < n_seg; s += gridDim.x) {
         const int64_t b = seg_off[s], e = seg_off[s + 1];
         int64_t res[PCT_MAX];
-        if (!segment_percentiles_reg(values + b, e - b, pl, res, sm))
+        if (!segment_percentiles_reg<PCT_MAX>(values + b, e - b, pl, res, sm))
             segment_percentiles(values + b, e - b, pl, res, nullptr);
         if (threadIdx.x == 0)
             for (int j = 0; j < pl.n_pct; ++j) out[(int64_t)s * pl.n_pct + j] = res[j];
@@ -436,7 +458,7 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(con
         if (out_summary[r].n_done < 0) continue;   // invalid descriptor, flagged by the simulator
         const asr_replica_t rep = replicas[r];
         int64_t res[PCT_MAX];
-        if (!segment_percentiles_reg(vals + rep.out_off, rep.n, pl, res, sm))
+        if (!segment_percentiles_reg<2>(vals + rep.out_off, rep.n, pl, res, sm))
             segment_percentiles(vals + rep.out_off, rep.n, pl, res, nullptr);
         if (threadIdx.x == 0) {
             if (blockIdx.y == 0) {
