@@ -455,6 +455,17 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(con
     pl.pct[1] = 90;
     const int64_t *vals = blockIdx.y == 0 ? lat : ttft;
     for (int r = blockIdx.x; r < n_replicas; r += gridDim.x) {
+        if (threadIdx.x == 0 && r + (int)gridDim.x < n_replicas) {
+            // pull the CTA's next segment into L2 while this one is being processed
+            const asr_replica_t nx = replicas[r + gridDim.x];
+            const int64_t bytes = (int64_t)nx.n * 8;
+            if (nx.n > 0 && nx.out_off >= 0 && bytes <= (int64_t)PCT_REG_MAX * 8) {
+                const char *src = reinterpret_cast<const char *>(vals + nx.out_off);
+                const uint32_t sz = (uint32_t)(bytes & ~15ll);
+                if (sz > 0 && (reinterpret_cast<uintptr_t>(src) & 15u) == 0)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(sz) : "memory");
+            }
+        }
         if (out_summary[r].n_done < 0) continue;   // invalid descriptor, flagged by the simulator
         const asr_replica_t rep = replicas[r];
         int64_t res[PCT_MAX];

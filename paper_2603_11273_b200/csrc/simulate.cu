@@ -333,6 +333,24 @@ __device__ __forceinline__ void lane_insert(uint2 *ring, int head, int nR, uint3
     ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = make_uint2(it + tokens, (uint32_t)idx);
 }
 
+// TTFT of request idx (requests are admitted in index order here)
+__device__ __forceinline__ void lane_push_ttft(int64_t *ttft, int idx, int64_t v, bool staged, int64_t &s0,
+                                               int64_t &s1, int64_t &s2, int64_t &s3) {
+    if (!staged) {
+        ttft[idx] = v;
+        return;
+    }
+    s0 = s1;
+    s1 = s2;
+    s2 = s3;
+    s3 = v;
+    if ((idx & 3) == 3) {
+        longlong2 *dst = reinterpret_cast<longlong2 *>(ttft + idx - 3);
+        dst[0] = make_longlong2(s0, s1);
+        dst[1] = make_longlong2(s2, s3);
+    }
+}
+
 __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
     __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
     const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
@@ -380,28 +398,24 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
     int head = 0;      // running set = ring positions head .. head+nR-1, sorted by finish iteration
     uint32_t it = 0;   // engine iterations so far, mod 2^32
-    // look-ahead window over the trace: records p .. p+3 are in registers, so the load of
-    // a record is issued four ingests before its arrival stamp is tested
-    int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, arr2 = INT64_MAX, arr3 = INT64_MAX, last_arr = 0;
-    int32_t dur0 = 0, dur1 = 0, dur2 = 0, dur3 = 0, last_dur = 0;
-    // (two loads per record on purpose: a 128-bit load would leave the unused est word
-    // as a dead destination register that the allocator reuses while the load is in flight)
+    // look-ahead window over the trace: records p and p+1 are in registers (one 128-bit
+    // load each: the memory pipeline is paid per lane and access, not per byte)
+    int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, last_arr = 0;
+    int32_t dur0 = 0, dur1 = 0, last_dur = 0;
     if (live && n > 0) {
-        arr0 = ld_arrival(trace);
-        dur0 = __ldg(&trace[0].dur_ms);
+        const Rec q = ld_cached(trace);
+        arr0 = q.arrival_us;
+        dur0 = q.dur_ms;
     }
     if (live && n > 1) {
-        arr1 = ld_arrival(trace + 1);
-        dur1 = __ldg(&trace[1].dur_ms);
+        const Rec q = ld_cached(trace + 1);
+        arr1 = q.arrival_us;
+        dur1 = q.dur_ms;
     }
-    if (live && n > 2) {
-        arr2 = ld_arrival(trace + 2);
-        dur2 = __ldg(&trace[2].dur_ms);
-    }
-    if (live && n > 3) {
-        arr3 = ld_arrival(trace + 3);
-        dur3 = __ldg(&trace[3].dur_ms);
-    }
+    // TTFT values are staged in registers and stored four at a time (requests 4g .. 4g+3
+    // as two 16-byte stores) when the output is 16-byte aligned
+    int64_t st0 = 0, st1 = 0, st2 = 0, st3 = 0;
+    const bool staged = (reinterpret_cast<uintptr_t>(ttft) & 15u) == 0;
     const int64_t first_arrival = n > 0 ? arr0 : 0;
     if (n == 0) live = false;
 
@@ -460,14 +474,11 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 ++nW;
                 arr0 = arr1;
                 dur0 = dur1;
-                arr1 = arr2;
-                dur1 = dur2;
-                arr2 = arr3;
-                dur2 = dur3;
-                arr3 = INT64_MAX;
-                if (p + 3 < n) {
-                    arr3 = ld_arrival(trace + p + 3);
-                    dur3 = __ldg(&trace[p + 3].dur_ms);
+                arr1 = INT64_MAX;
+                if (p + 1 < n) {
+                    const Rec q = ld_cached(trace + p + 1);
+                    arr1 = q.arrival_us;
+                    dur1 = q.dur_ms;
                 }
             }
             // D. admit k >= 1 requests (a slot is free and somebody waits)
@@ -482,8 +493,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     // the request ingested last: everything needed is in registers
                     lane_insert(ring, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
                     t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
-                    ttft[lo] = t1 - last_arr;   // first token (S9)
-                    lat[lo] = -last_arr;        // E2E = completion time - arrival: the completion adds its time
+                    lane_push_ttft(ttft, lo, t1 - last_arr, staged, st0, st1, st2, st3);   // first token (S9)
                 } else {
                     int64_t dur_sum = 0;
                     for (int q = 0; q < k; ++q) {
@@ -492,11 +502,8 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                         dur_sum += (int64_t)dur;
                     }
                     t1 += (int64_t)enc_base * (int64_t)k + (int64_t)enc_per * dur_sum;
-                    for (int q = 0; q < k; ++q) {
-                        const int64_t arr = ld_arrival(trace + lo + q);
-                        ttft[lo + q] = t1 - arr;
-                        lat[lo + q] = -arr;
-                    }
+                    for (int q = 0; q < k; ++q)
+                        lane_push_ttft(ttft, lo + q, t1 - ld_arrival(trace + lo + q), staged, st0, st1, st2, st3);
                 }
                 lo += k;
                 nW -= k;
@@ -511,11 +518,30 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         a.defer_list[pos] = r;
         return;
     }
+    if (valid && staged) {   // requests n - (n & 3) .. n-1 are still in st(4 - tail) .. st3
+        const int tail = n & 3;
+        if (tail >= 3) ttft[n - 3] = st1;
+        if (tail >= 2) ttft[n - 2] = st2;
+        if (tail >= 1) ttft[n - 1] = st3;
+    }
     if (valid && a.out_summary) {
         asr_summary_t *s = a.out_summary + r;
         s->first_arrival_us = first_arrival;
         s->last_done_us = t;
         s->n_done = done;
+    }
+}
+
+// out_lat[i] = -arrival_us[i] for every request of every replica the lane kernel will
+// simulate: a coalesced stream, so that the lane kernel's only per-completion memory
+// operation is the reduction that adds the completion time
+__global__ void __launch_bounds__(256) sim_init_lat_kernel(SimArgs a) {
+    for (int r = blockIdx.x; r < a.n_replicas; r += gridDim.x) {
+        const asr_replica_t rep = a.replicas[r];
+        if (!replica_ok(a, rep, LANE_CAP)) continue;
+        const asr_req_t *trace = a.traces + rep.trace_off;
+        int64_t *lat = a.out_lat + rep.out_off;
+        for (int i = threadIdx.x; i < rep.n; i += 256) __stcs(lat + i, -ld_arrival(trace + i));
     }
 }
 
@@ -584,6 +610,13 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
     if (a_in.n_replicas <= 0) return ASR_OK;
     SimArgs a = a_in;
     if (use_lane && max_slots <= LANE_CAP) {
+        {
+            KernelTimer kt(KID_SIM_INIT_LAT, st);
+            const int grid = a.n_replicas < 148 * 8 ? a.n_replicas : 148 * 8;
+            sim_init_lat_kernel<<<grid, 256, 0, st>>>(a);
+        }
+        int rc0 = check_launch("sim_init_lat_kernel");
+        if (rc0) return rc0;
         {
             KernelTimer kt(KID_SIM_LANE, st);
             sim_lane_kernel<<<(a.n_replicas + LANE_THREADS - 1) / LANE_THREADS, LANE_THREADS, 0, st>>>(a);
