@@ -222,7 +222,7 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
     if (rc) return rc;
     SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
-              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, g_opt_escalate.load()};
+              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, summary_only ? 1 : 0, g_opt_escalate.load()};
     // many small replicas: one thread each; few or wide ones: one warp each
     const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
     rc = launch_simulate(a, max_slots, use_lane, st);

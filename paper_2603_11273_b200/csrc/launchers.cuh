@@ -20,6 +20,7 @@ struct SimArgs {
     int64_t total_requests;
     int32_t n_replicas;
     int32_t n_cms;
+    int32_t order_free;       // 1: summary-only call, out_lat/out_ttft are workspace arrays whose order is free
     int32_t escalate_window;  // waiting window (requests) beyond which a warp hands its replica to the CTA kernel
 };
 

@@ -322,7 +322,7 @@ __device__ __forceinline__ uint32_t lane_tokens(int64_t tok_base, int64_t tok_pe
 // insert (it + tokens, idx) into the sorted ring of nR entries starting at `head`;
 // an entry is one 64-bit word (finish iteration, request index)
 __device__ __forceinline__ void lane_insert(uint2 *ring, int head, int nR, uint32_t it, uint32_t tokens,
-                                            int32_t idx) {
+                                            uint32_t payload) {
     int h = nR;
     while (h > 0) {
         const uint2 e = ring[((head + h - 1) & (LANE_CAP - 1)) * LANE_THREADS];
@@ -330,7 +330,7 @@ __device__ __forceinline__ void lane_insert(uint2 *ring, int head, int nR, uint3
         ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = e;
         --h;
     }
-    ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = make_uint2(it + tokens, (uint32_t)idx);
+    ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = make_uint2(it + tokens, payload);
 }
 
 // TTFT of request idx (requests are admitted in index order here)
@@ -351,6 +351,46 @@ __device__ __forceinline__ void lane_push_ttft(int64_t *ttft, int idx, int64_t v
     }
 }
 
+// Order-free outputs (summary-only calls: the per-request arrays live in the workspace and
+// only feed the percentile reduction, which does not care about their order).  Values
+// known to be below 2^32 are staged in four registers and written as one aligned 32-byte
+// sector of zero-extended int64; `ph` is the element phase of base[0] within its sector.
+struct Stage32 {
+    uint32_t v0, v1, v2, v3;
+};
+
+__device__ __forceinline__ void stage_push(int64_t *base, int ph, int pos, uint32_t v, Stage32 &s) {
+    s.v0 = s.v1;
+    s.v1 = s.v2;
+    s.v2 = s.v3;
+    s.v3 = v;
+    if (((ph + pos) & 3) == 3) {
+        if (pos >= 3) {
+            ulonglong2 *dst = reinterpret_cast<ulonglong2 *>(base + pos - 3);
+            dst[0] = make_ulonglong2(s.v0, s.v1);
+            dst[1] = make_ulonglong2(s.v2, s.v3);
+        } else {   // short head before the first sector boundary
+            if (pos >= 2) base[pos - 2] = (int64_t)s.v1;
+            if (pos >= 1) base[pos - 1] = (int64_t)s.v2;
+            base[pos] = (int64_t)s.v3;
+        }
+    }
+}
+
+__device__ __forceinline__ void stage_tail(int64_t *base, int ph, int n, const Stage32 &s) {
+    int cnt = (ph + n) & 3;
+    cnt = cnt < n ? cnt : n;
+    if (cnt >= 3) base[n - 3] = (int64_t)s.v1;
+    if (cnt >= 2) base[n - 2] = (int64_t)s.v2;
+    if (cnt >= 1) base[n - 1] = (int64_t)s.v3;
+}
+
+// FREE = order-free outputs: the ring carries the low word of the arrival time instead of
+// the request index, E2E latency is formed at completion and both outputs are emitted in
+// event order through Stage32.  Exact as long as every value is below 2^32 us, which the
+// kernel proves with the start of the current busy period (every request in the system
+// arrived at or after it); a busy period of 2^32 us sends the replica to the warp kernel.
+template <bool FREE>
 __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
     __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
     const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
@@ -395,6 +435,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     int64_t *ttft = a.out_ttft + rep.out_off;
 
     int64_t t = 0;     // the current iteration boundary
+    int64_t tb = 0;    // FREE: start of the current busy period (arrival of its first request)
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
     int head = 0;      // running set = ring positions head .. head+nR-1, sorted by finish iteration
     uint32_t it = 0;   // engine iterations so far, mod 2^32
@@ -412,10 +453,14 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         arr1 = q.arrival_us;
         dur1 = q.dur_ms;
     }
-    // TTFT values are staged in registers and stored four at a time (requests 4g .. 4g+3
-    // as two 16-byte stores) when the output is 16-byte aligned
+    // !FREE: TTFT values are staged in registers and stored four at a time (requests
+    // 4g .. 4g+3 as two 16-byte stores) when the output is 16-byte aligned
     int64_t st0 = 0, st1 = 0, st2 = 0, st3 = 0;
     const bool staged = (reinterpret_cast<uintptr_t>(ttft) & 15u) == 0;
+    // FREE: both outputs through Stage32
+    Stage32 sq_t = {0, 0, 0, 0}, sq_l = {0, 0, 0, 0};
+    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft) >> 3) & 3u);
+    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat) >> 3) & 3u);
     const int64_t first_arrival = n > 0 ? arr0 : 0;
     if (n == 0) live = false;
 
@@ -442,13 +487,24 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                         t = lim + c;
                         it = f;
                     }
-                    // lat[i] holds -arrival since admission; a fire-and-forget reduction adds the
-                    // completion time, so no load sits on the critical path
-                    atomicAdd(reinterpret_cast<unsigned long long *>(lat + (int32_t)e.y), (unsigned long long)t);
+                    if (FREE) {
+                        if (((uint64_t)(t - tb) >> 32) != 0) {   // cannot prove the value fits 32 bits
+                            deferred = true;
+                            live = false;
+                            more = false;
+                        } else {
+                            stage_push(lat, ph_l, done, (uint32_t)t - e.y, sq_l);   // E2E = t - arrival
+                        }
+                    } else {
+                        // lat[i] holds -arrival (sim_init_lat_kernel); a fire-and-forget reduction
+                        // adds the completion time, so no load sits on the critical path
+                        atomicAdd(reinterpret_cast<unsigned long long *>(lat + (int32_t)e.y),
+                                  (unsigned long long)t);
+                    }
                     head = (head + 1) & (LANE_CAP - 1);
                     --nR;
                     ++done;
-                    more = nR > 0;
+                    more = more && nR > 0;
                 }
             }
             if (done >= n) live = false;
@@ -456,6 +512,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
         if (live) {
             // B. the boundary of the admission step
+            if (nW == 0 && nR == 0) tb = arr0;   // a new busy period starts with the next arrival
             if (nW == 0 && arr0 > t) {
                 if (nR == 0) {
                     t = arr0;   // idle server: the clock jumps to the next arrival (S14)
@@ -491,19 +548,30 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 int64_t t1 = t + (int64_t)(ib + ip * (uint32_t)(nR + k));
                 if (k == 1 && lo == p - 1) {
                     // the request ingested last: everything needed is in registers
-                    lane_insert(ring, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur), lo);
+                    lane_insert(ring, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur),
+                                FREE ? (uint32_t)last_arr : (uint32_t)lo);
                     t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
-                    lane_push_ttft(ttft, lo, t1 - last_arr, staged, st0, st1, st2, st3);   // first token (S9)
+                    // first token (S9)
+                    if (FREE) stage_push(ttft, ph_t, lo, (uint32_t)t1 - (uint32_t)last_arr, sq_t);
+                    else lane_push_ttft(ttft, lo, t1 - last_arr, staged, st0, st1, st2, st3);
                 } else {
                     int64_t dur_sum = 0;
                     for (int q = 0; q < k; ++q) {
-                        const int32_t dur = __ldg(&trace[lo + q].dur_ms);
-                        lane_insert(ring, head, nR + q, it, lane_tokens(tok_base, tok_per_s, dur), lo + q);
-                        dur_sum += (int64_t)dur;
+                        const Rec rq = ld_cached(trace + lo + q);
+                        lane_insert(ring, head, nR + q, it, lane_tokens(tok_base, tok_per_s, rq.dur_ms),
+                                    FREE ? (uint32_t)rq.arrival_us : (uint32_t)(lo + q));
+                        dur_sum += (int64_t)rq.dur_ms;
                     }
                     t1 += (int64_t)enc_base * (int64_t)k + (int64_t)enc_per * dur_sum;
-                    for (int q = 0; q < k; ++q)
-                        lane_push_ttft(ttft, lo + q, t1 - ld_arrival(trace + lo + q), staged, st0, st1, st2, st3);
+                    for (int q = 0; q < k; ++q) {
+                        const int64_t arr = ld_arrival(trace + lo + q);
+                        if (FREE) stage_push(ttft, ph_t, lo + q, (uint32_t)t1 - (uint32_t)arr, sq_t);
+                        else lane_push_ttft(ttft, lo + q, t1 - arr, staged, st0, st1, st2, st3);
+                    }
+                }
+                if (FREE && ((uint64_t)(t1 - tb) >> 32) != 0) {   // a TTFT of this step may not fit 32 bits
+                    deferred = true;
+                    live = false;
                 }
                 lo += k;
                 nW -= k;
@@ -518,7 +586,11 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         a.defer_list[pos] = r;
         return;
     }
-    if (valid && staged) {   // requests n - (n & 3) .. n-1 are still in st(4 - tail) .. st3
+    if (valid && FREE) {
+        stage_tail(ttft, ph_t, n, sq_t);
+        stage_tail(lat, ph_l, n, sq_l);
+    }
+    if (valid && !FREE && staged) {   // requests n - (n & 3) .. n-1 are still in st(4 - tail) .. st3
         const int tail = n & 3;
         if (tail >= 3) ttft[n - 3] = st1;
         if (tail >= 2) ttft[n - 2] = st2;
@@ -610,16 +682,20 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
     if (a_in.n_replicas <= 0) return ASR_OK;
     SimArgs a = a_in;
     if (use_lane && max_slots <= LANE_CAP) {
-        {
-            KernelTimer kt(KID_SIM_INIT_LAT, st);
-            const int grid = a.n_replicas < 148 * 8 ? a.n_replicas : 148 * 8;
-            sim_init_lat_kernel<<<grid, 256, 0, st>>>(a);
-        }
-        int rc0 = check_launch("sim_init_lat_kernel");
-        if (rc0) return rc0;
-        {
+        const int lane_grid = (a.n_replicas + LANE_THREADS - 1) / LANE_THREADS;
+        if (a.order_free) {
             KernelTimer kt(KID_SIM_LANE, st);
-            sim_lane_kernel<<<(a.n_replicas + LANE_THREADS - 1) / LANE_THREADS, LANE_THREADS, 0, st>>>(a);
+            sim_lane_kernel<true><<<lane_grid, LANE_THREADS, 0, st>>>(a);
+        } else {
+            {
+                KernelTimer kt(KID_SIM_INIT_LAT, st);
+                const int grid = a.n_replicas < 148 * 8 ? a.n_replicas : 148 * 8;
+                sim_init_lat_kernel<<<grid, 256, 0, st>>>(a);
+            }
+            int rc0 = check_launch("sim_init_lat_kernel");
+            if (rc0) return rc0;
+            KernelTimer kt(KID_SIM_LANE, st);
+            sim_lane_kernel<false><<<lane_grid, LANE_THREADS, 0, st>>>(a);
         }
         int rc = check_launch("sim_lane_kernel");
         if (rc) return rc;

@@ -117,3 +117,18 @@ def test_other_cost_models(asr):
         L, T, S = run_batched([tr], reps, cost, 32)
         for i, (_, p, s) in enumerate(reps):
             check_replica(tr, p, s, cost, L[i], T[i], S[i], "cost=%r" % (cost,))
+
+
+def test_lane_kernel_hand_overs(asr):
+    """cases the thread-per-replica kernel must pass on: a busy period longer than 2^32 us (its
+    32-bit proof for order-free outputs fails) and iteration costs beyond 31 bits"""
+    toy = (1000000, 0, 100000, 0, 0, 5)           # Fig. 1 cost model: seconds per request
+    br = wl.stress_trace("burst", 1500, 21)        # one slot -> ~6000 s of continuous service
+    sp = wl.stress_trace("lognormal", 300, 22, rate_per_s=0.5)
+    for cost, traces in ((toy, [br]), ((20000, 2, 3_000_000_000, 50, 1, 4), [sp])):
+        reps = [(0, p, s) for p in POL for s in (1, 4)]
+        L, T, S = run_batched(traces, reps, cost, 32)
+        _, _, S2 = run_batched(traces, reps, cost, 32, summary_only=True)
+        for i, (t, p, s) in enumerate(reps):
+            check_replica(traces[t], p, s, cost, L[i], T[i], S[i], "cost=%r rep %d" % (cost, i))
+        assert np.array_equal(S.view(np.uint8), S2.view(np.uint8))
