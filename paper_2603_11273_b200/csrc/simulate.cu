@@ -319,6 +319,17 @@ __device__ __forceinline__ uint32_t lane_tokens(int64_t tok_base, int64_t tok_pe
     return (uint32_t)tok;
 }
 
+// the same for 0 <= tok_per_s < 2^31 and |tok_base| < 2^30: 32-bit arithmetic whenever the
+// product fits (quotient < 4.3e6, so neither the sum nor the upper clamp can overflow)
+__device__ __forceinline__ uint32_t lane_tokens_small(int32_t tok_base, uint32_t tok_per_s, int32_t dur_ms) {
+    const uint64_t prod = (uint64_t)tok_per_s * (uint32_t)dur_ms;
+    if (dur_ms >= 0 && (prod >> 32) == 0) {
+        const int32_t tok = tok_base + (int32_t)((uint32_t)prod / 1000u);
+        return (uint32_t)(tok < 1 ? 1 : tok);
+    }
+    return lane_tokens((int64_t)tok_base, (int64_t)tok_per_s, dur_ms);
+}
+
 // insert (it + tokens, idx) into the sorted ring of nR entries starting at `head`;
 // an entry is one 64-bit word (finish iteration, request index)
 __device__ __forceinline__ void lane_insert(uint2 *ring, int head, int nR, uint32_t it, uint32_t tokens,
@@ -417,11 +428,13 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     const asr_cost_model_t *cmp = a.cms + rep.cm_id;
     const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
     const int64_t iter_base64 = __ldg(&cmp->iter_base_us), iter_per64 = __ldg(&cmp->iter_per_running_us);
-    const int64_t tok_base = __ldg(&cmp->tok_base), tok_per_s = __ldg(&cmp->tok_per_s);
+    const int32_t tok_base = __ldg(&cmp->tok_base), tok_per_s_i = __ldg(&cmp->tok_per_s);
+    const uint32_t tok_per_s = (uint32_t)tok_per_s_i;
     // this kernel computes iteration costs in 32 bits; any other cost model goes to the warp kernel
     const int64_t lim31 = (int64_t)1 << 31;
     const bool small = enc_base64 >= 0 && enc_base64 < lim31 && enc_per64 >= 0 && enc_per64 < lim31 &&
-                       iter_base64 >= 0 && iter_per64 >= 0 && iter_base64 + iter_per64 * LANE_CAP < lim31;
+                       iter_base64 >= 0 && iter_per64 >= 0 && iter_base64 + iter_per64 * LANE_CAP < lim31 &&
+                       tok_per_s_i >= 0 && tok_base > -(1 << 30) && tok_base < (1 << 30);
     bool deferred = false;
     if (live && !small) {
         deferred = true;
@@ -443,6 +456,9 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     // load each: the memory pipeline is paid per lane and access, not per byte)
     int64_t arr0 = INT64_MAX, arr1 = INT64_MAX, last_arr = 0;
     int32_t dur0 = 0, dur1 = 0, last_dur = 0;
+    // the est word of the load is kept live until the record is consumed: a dead destination
+    // register would be reused, and its next writer would wait for the load in flight
+    int32_t est1 = 0;
     if (live && n > 0) {
         const Rec q = ld_cached(trace);
         arr0 = q.arrival_us;
@@ -452,6 +468,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         const Rec q = ld_cached(trace + 1);
         arr1 = q.arrival_us;
         dur1 = q.dur_ms;
+        est1 = q.est;
     }
     // !FREE: TTFT values are staged in registers and stored four at a time (requests
     // 4g .. 4g+3 as two 16-byte stores) when the output is 16-byte aligned
@@ -474,13 +491,14 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             // slot is free and somebody is waiting, or the next arrival falls at or before
             // t + (m-1)*c, the admission step comes first.
             bool more = nR > 0;
+            const int64_t a_eff = nW > 0 ? INT64_MIN : arr0;   // somebody waiting: admit at the first free slot
             while (more) {
                 const uint2 e = ring[head * LANE_THREADS];   // sorted: the head finishes first
                 const uint32_t f = e.x;
                 const uint32_t m = f - it;
                 const uint32_t c = ib + ip * (uint32_t)nR;
                 const int64_t lim = t + (int64_t)((uint64_t)(m - 1u) * c);
-                if (m > 0u && nR < slots && (nW > 0 || arr0 <= lim)) {
+                if (m > 0u && nR < slots && a_eff <= lim) {
                     more = false;
                 } else {
                     if (m > 0u) {
@@ -488,13 +506,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                         it = f;
                     }
                     if (FREE) {
-                        if (((uint64_t)(t - tb) >> 32) != 0) {   // cannot prove the value fits 32 bits
-                            deferred = true;
-                            live = false;
-                            more = false;
-                        } else {
-                            stage_push(lat, ph_l, done, (uint32_t)t - e.y, sq_l);   // E2E = t - arrival
-                        }
+                        stage_push(lat, ph_l, done, (uint32_t)t - e.y, sq_l);   // E2E = t - arrival
                     } else {
                         // lat[i] holds -arrival (sim_init_lat_kernel); a fire-and-forget reduction
                         // adds the completion time, so no load sits on the critical path
@@ -504,10 +516,16 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     head = (head + 1) & (LANE_CAP - 1);
                     --nR;
                     ++done;
-                    more = more && nR > 0;
+                    more = nR > 0;
                 }
             }
             if (done >= n) live = false;
+            // every value emitted so far (TTFT of the previous step, the latencies above) is at
+            // most t - tb; beyond 32 bits the proof fails and the warp kernel redoes the replica
+            if (FREE && ((uint64_t)(t - tb) >> 32) != 0) {
+                deferred = true;
+                live = false;
+            }
         }
         if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
         if (live) {
@@ -531,11 +549,13 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 ++nW;
                 arr0 = arr1;
                 dur0 = dur1;
+                asm volatile("" ::"r"(est1));
                 arr1 = INT64_MAX;
                 if (p + 1 < n) {
                     const Rec q = ld_cached(trace + p + 1);
                     arr1 = q.arrival_us;
                     dur1 = q.dur_ms;
+                    est1 = q.est;
                 }
             }
             // D. admit k >= 1 requests (a slot is free and somebody waits)
@@ -548,7 +568,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 int64_t t1 = t + (int64_t)(ib + ip * (uint32_t)(nR + k));
                 if (k == 1 && lo == p - 1) {
                     // the request ingested last: everything needed is in registers
-                    lane_insert(ring, head, nR, it, lane_tokens(tok_base, tok_per_s, last_dur),
+                    lane_insert(ring, head, nR, it, lane_tokens_small(tok_base, tok_per_s, last_dur),
                                 FREE ? (uint32_t)last_arr : (uint32_t)lo);
                     t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
                     // first token (S9)
@@ -558,7 +578,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     int64_t dur_sum = 0;
                     for (int q = 0; q < k; ++q) {
                         const Rec rq = ld_cached(trace + lo + q);
-                        lane_insert(ring, head, nR + q, it, lane_tokens(tok_base, tok_per_s, rq.dur_ms),
+                        lane_insert(ring, head, nR + q, it, lane_tokens_small(tok_base, tok_per_s, rq.dur_ms),
                                     FREE ? (uint32_t)rq.arrival_us : (uint32_t)(lo + q));
                         dur_sum += (int64_t)rq.dur_ms;
                     }
@@ -568,10 +588,6 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                         if (FREE) stage_push(ttft, ph_t, lo + q, (uint32_t)t1 - (uint32_t)arr, sq_t);
                         else lane_push_ttft(ttft, lo + q, t1 - arr, staged, st0, st1, st2, st3);
                     }
-                }
-                if (FREE && ((uint64_t)(t1 - tb) >> 32) != 0) {   // a TTFT of this step may not fit 32 bits
-                    deferred = true;
-                    live = false;
                 }
                 lo += k;
                 nW -= k;
