@@ -549,7 +549,9 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 ++nW;
                 arr0 = arr1;
                 dur0 = dur1;
-                asm volatile("" ::"r"(est1));
+                // (a real, harmless use: a prefetch that is never issued; ptxas drops anything less)
+                asm volatile("{ .reg .pred p; setp.eq.s32 p, %0, -2147483647; @p prefetch.global.L2 [%1]; }" ::"r"(est1),
+                             "l"(trace));
                 arr1 = INT64_MAX;
                 if (p + 1 < n) {
                     const Rec q = ld_cached(trace + p + 1);
