@@ -323,7 +323,7 @@ def run_ours(args):
         stage_ms[kname] = k_tot
         # ALU/issue-bound: achieved = warp instructions issued per second; the per-request
         # instruction count is the ncu figure committed in profiles/roofline_constants.json
-        wi = consts.get(kname + "_warp_instr_per_request")
+        wi = consts.get(kname + "_warp_instr_per_request") if n == 10000 and cfg3["slots"] == 32 else None
         a = (wi * total / (k_avg / 1e3)) if wi else None
         rooflines[kname] = {
             "bound": "alu", "achieved": a, "peak": ALU_PEAK_WARP_INSTR_PER_S, "unit": "warp-instr/s",
