@@ -167,18 +167,20 @@ def oracle_select_sample(n_queues: int, q_len: int, threads: int):
     return n_queues * q_len * 16 * len(cfg["policies"]) / dt / 1e9, dt
 
 
-def cpu_baseline(n: int, target_s: float = 12.0):
+def cpu_baseline(n: int, target_s: float = 25.0):
     cores = os.cpu_count() or 1
     req, dt = oracle_sweep_sample(cores, n, 0, cores)          # pilot: one replica per core
     per_replica = dt / max(1, req // n) * cores
-    count = int(max(cores, min(4096, target_s * cores / max(per_replica, 1e-6))))
+    count = int(max(cores, min(98304, target_s * cores / max(per_replica, 1e-6))))
     req, dt = oracle_sweep_sample(count, n, 0, cores)
-    sel_gbs, sel_dt = oracle_select_sample(max(cores * 8, 64), 4096, cores)
+    _, pilot_dt = oracle_select_sample(cores * 4, 4096, cores)
+    n_sel = int(max(cores * 4, min(65536, 4.0 * cores * 4 / max(pilot_dt, 1e-6))))   # about 4 s
+    sel_gbs, sel_dt = oracle_select_sample(n_sel, 4096, cores)
     return {"value": req / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "%d of the 98,304 config-3 replicas (evenly spaced over seeds x rates x policies, "
                       "n=%d each; generate+simulate+p50/p90), %.1f s wall on %d threads" % (req // n, n, dt, cores),
             "select_gbs": sel_gbs,
-            "select_sample": "%d config-5 queues x 4096, HRRN+SJF full sort, %.1f s" % (max(cores * 8, 64), sel_dt)}
+            "select_sample": "%d config-5 queues x 4096, HRRN+SJF full sort, %.1f s" % (n_sel, sel_dt)}
 
 
 def run_reference(args):
@@ -212,6 +214,65 @@ def run_reference(args):
 # ---------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------
+
+def side_configs(asr, dev, d_tables, reps=5):
+    """BASELINE.json configs[0], [1] and [3] (the small and the deep-backlog cases): generate ->
+    simulate with per-request outputs and summary, CUDA events, median of `reps` runs.  Not part of
+    `value`; parity of all three is in tests/ (-m gpu)."""
+    import torch
+    out = {}
+
+    def timed(fn, reps=reps, warm=True):
+        ms = []
+        if warm:
+            fn()
+        torch.cuda.synchronize()
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return statistics.median(ms)
+
+    for cfg, rates in ((wl.config1(), None), (wl.config2(), wl.config2()["rates_mhz"])):
+        rates = rates or (cfg["rate_mhz"],)
+        n, pols = cfg["n"], cfg["policies"]
+        specs = np.zeros(len(rates), dtype=asr.SPEC_DTYPE)
+        specs["seed"], specs["rate_mhz"], specs["dist"] = cfg["seed"], rates, cfg["dist"]
+        n_rep = len(rates) * len(pols)
+        rep = asr.make_replicas(np.repeat(np.arange(len(rates), dtype=np.int64) * n, len(pols)),
+                                np.arange(n_rep, dtype=np.int64) * n, n,
+                                np.tile(np.asarray(pols, dtype=np.int32), len(rates)), cfg["slots"], 0)
+        d_specs, d_rep, d_cost = (asr.to_device(x, dev) for x in (specs, rep, asr.make_cost(*cfg["cost"])))
+        d_tr = torch.empty(len(rates) * n * 16, dtype=torch.uint8, device=dev)
+        d_lat = torch.empty(n_rep * n, dtype=torch.int64, device=dev)
+        d_ttft = torch.empty(n_rep * n, dtype=torch.int64, device=dev)
+        d_sum = torch.zeros(n_rep * asr.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+
+        def step():
+            asr.gen_trace_batched(d_specs, len(rates), n, d_tables, out=d_tr)
+            asr.simulate_batched(d_tr, d_rep, n_rep, d_cost, 1, n_rep * n, cfg["slots"], d_lat, d_ttft, d_sum)
+        ms = timed(step)
+        out[cfg["name"]] = {"replicas": n_rep, "requests_per_replica": n, "ms": ms,
+                            "requests_per_s": n_rep * n / (ms / 1e3)}
+    cfg = wl.config4()
+    n = cfg["n"]
+    cost = asr.make_cost(*cfg["cost"])
+    d_tr = torch.empty(n * 16, dtype=torch.uint8, device=dev)
+    res = {}
+
+    def step4():
+        asr.gen_trace(cfg["seed"], cfg["rate_mhz"], cfg["dist"], n, d_tables, out=d_tr)
+        for pol in cfg["policies"]:
+            res[pol] = asr.simulate(d_tr, n, pol, cost, cfg["slots"])
+    ms = timed(step4, reps=2, warm=False)   # seconds per run: kept short
+    out[cfg["name"]] = {"replicas": len(cfg["policies"]), "requests_per_replica": n, "ms": ms,
+                        "requests_per_s": len(cfg["policies"]) * n / (ms / 1e3),
+                        "note": "one sequential replica per policy (HRRN, SJF), backlog ~2.3e5 waiting"}
+    return out
+
 
 def run_ours(args):
     import torch
@@ -383,6 +444,10 @@ def run_ours(args):
         except Exception as exc:  # pinned allocation can fail on a small host
             e2e["select_error"] = str(exc)[:200]
 
+    side = None
+    if rank == 0 and not args.no_side_configs:
+        side = side_configs(asr, dev, d_tables)
+
     base = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         base = cpu_baseline(n)
@@ -406,7 +471,7 @@ def run_ours(args):
                        "frac_of_measured_peak": select_gbs / world / hbm_peak,
                        "frac_of_nominal_8TBs": select_gbs / world / 8000.0},
             "roofline": roofline, "rooflines": rooflines, "clocks": clocks, "e2e": e2e,
-            "gpu_launches": int(launches), "cpu_baseline": base,
+            "gpu_launches": int(launches), "cpu_baseline": base, "configs": side,
             "kernel_ms_total": {k_: v[0] for k_, v in ktimes.items() if v[1]},
         }
         print(json.dumps(line), flush=True)
@@ -426,6 +491,7 @@ def main():
     ap.add_argument("--ref-replicas", type=int, default=256, help="--impl reference: replicas per step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-side-configs", action="store_true", help="skip the config 1/2/4 timings")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
