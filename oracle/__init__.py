@@ -21,7 +21,7 @@ _SRC = os.path.join(_HERE, "asr_oracle.c")
 _HDR = os.path.join(_HERE, "asr_oracle.h")
 _LIB = os.path.join(_HERE, "libasr_oracle.so")
 
-FCFS, SJF, HRRN = 0, 1, 2
+FCFS, SJF, HRRN, ADAPTIVE = 0, 1, 2, 3
 DIST_LOGNORMAL, DIST_UNIFORM = 0, 1
 
 REQ = np.dtype([("arrival_us", "<i8"), ("dur_ms", "<i4"), ("est", "<i4")])
@@ -36,6 +36,23 @@ class Cost(C.Structure):
         ("tok_base", C.c_int32),
         ("tok_per_s", C.c_int32),
     ]
+
+
+class Ext(C.Structure):
+    """orc_ext_t: KV-memory model (f1) and policy switching (f3)"""
+    _fields_ = [
+        ("kv_budget", C.c_int64),
+        ("kv_base", C.c_int64),
+        ("kv_per_s", C.c_int64),
+        ("depth1", C.c_int32),
+        ("depth2", C.c_int32),
+        ("pol", C.c_int32 * 3),
+        ("pad", C.c_int32),
+    ]
+
+
+def ext(kv_budget=0, kv_base=0, kv_per_s=0, depth1=0, depth2=0, pol=(0, 0, 0)) -> Ext:
+    return Ext(kv_budget, kv_base, kv_per_s, depth1, depth2, (C.c_int32 * 3)(*pol), 0)
 
 
 def build(force: bool = False) -> str:
@@ -72,6 +89,13 @@ def lib():
                                    C.POINTER(i64), C.POINTER(i64)]
         L.orc_percentile.restype = i64
         L.orc_percentile.argtypes = [vp, i64, i32]
+        L.orc_simulate_ex.restype = C.c_int
+        L.orc_simulate_ex.argtypes = [vp, i64, C.c_int, C.POINTER(Cost), C.POINTER(Ext), i32, vp, vp,
+                                      C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
+        L.orc_tpot.restype = C.c_int
+        L.orc_tpot.argtypes = [vp, i64, C.POINTER(Cost), vp, vp, vp]
+        L.orc_estimate.restype = C.c_int
+        L.orc_estimate.argtypes = [vp, i64, vp, i32, vp, vp]
         L.orc_tokens.restype = i64
         L.orc_tokens.argtypes = [C.POINTER(Cost), i32]
         L.orc_enc_cost.restype = i64
@@ -133,6 +157,45 @@ def simulate(trace, policy: int, cm: Cost, slots: int):
     if rc != 0:
         raise ValueError("orc_simulate rc=%d" % rc)
     return lat, ttft, fa.value, ld.value
+
+
+def simulate_ex(trace, policy: int, cm: Cost, ex, slots: int):
+    """orc_simulate_ex -> (lat[n], ttft[n], first_arrival_us, last_done_us, n_preempt)"""
+    trace = _req(trace)
+    n = trace.shape[0]
+    lat = np.full(n, -1, dtype=np.int64)
+    ttft = np.full(n, -1, dtype=np.int64)
+    fa, ld, npre = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+    rc = lib().orc_simulate_ex(trace.ctypes.data, n, policy, C.byref(cm), C.byref(ex) if ex is not None else None,
+                               slots, lat.ctypes.data, ttft.ctypes.data, C.byref(fa), C.byref(ld), C.byref(npre))
+    if rc != 0:
+        raise ValueError("orc_simulate_ex rc=%d" % rc)
+    return lat, ttft, fa.value, ld.value, npre.value
+
+
+def tpot(trace, cm: Cost, lat, ttft) -> np.ndarray:
+    trace = _req(trace)
+    lat = np.ascontiguousarray(lat, dtype=np.int64)
+    ttft = np.ascontiguousarray(ttft, dtype=np.int64)
+    out = np.empty(trace.shape[0], dtype=np.int64)
+    rc = lib().orc_tpot(trace.ctypes.data, trace.shape[0], C.byref(cm), lat.ctypes.data, ttft.ctypes.data,
+                        out.ctypes.data)
+    if rc != 0:
+        raise ValueError("orc_tpot rc=%d" % rc)
+    return out
+
+
+def estimate(recs, kappa_milli_by_lang, lang=None, speech_ms=None) -> np.ndarray:
+    """returns a copy of recs with est = max(1, floor(d_ms * kappa_milli / 1e6))"""
+    out = _req(recs).copy()
+    kap = np.ascontiguousarray(kappa_milli_by_lang, dtype=np.int32)
+    lg = None if lang is None else np.ascontiguousarray(lang, dtype=np.uint8)
+    sp = None if speech_ms is None else np.ascontiguousarray(speech_ms, dtype=np.int32)
+    rc = lib().orc_estimate(out.ctypes.data, out.shape[0], kap.ctypes.data, kap.shape[0],
+                            None if lg is None else lg.ctypes.data, None if sp is None else sp.ctypes.data)
+    if rc != 0:
+        raise ValueError("orc_estimate rc=%d" % rc)
+    return out
 
 
 def percentile(v, p: int) -> int:

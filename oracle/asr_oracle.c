@@ -187,6 +187,182 @@ int orc_simulate(const orc_req_t *trace, int64_t n, int policy,
 }
 
 /* ------------------------------------------------------------------ */
+/* 8(f) extensions: preemption, policy switching           */
+/* (PAPER.md:156), TPOT, estimator          */
+/* ------------------------------------------------------------------ */
+
+static int eff_policy(int policy, const orc_ext_t *ext, int64_t n_waiting) {
+    if (policy != ORC_ADAPTIVE) return policy;
+    if (n_waiting < ext->depth1) return ext->pol[0];
+    if (n_waiting < ext->depth2) return ext->pol[1];
+    return ext->pol[2];
+}
+
+static int64_t kv_enc(const orc_ext_t *ext, int32_t dur_ms) {
+    return ext->kv_base + (ext->kv_per_s * (int64_t)dur_ms) / 1000;
+}
+
+int orc_simulate_ex(const orc_req_t *trace, int64_t n, int policy,
+                    const orc_cost_t *cm, const orc_ext_t *ext, int32_t slots,
+                    int64_t *lat, int64_t *ttft, int64_t *first_arrival_us,
+                    int64_t *last_done_us, int64_t *n_preempt) {
+    if (n_preempt) *n_preempt = 0;
+    if (!ext) {
+        if (policy == ORC_ADAPTIVE) return -1;
+        return orc_simulate(trace, n, policy, cm, slots, lat, ttft,
+                            first_arrival_us, last_done_us);
+    }
+    if (n < 0 || slots < 1 || policy < 0 || policy > 3 || !cm) return -1;
+    if (policy == ORC_ADAPTIVE) {
+        if (ext->depth1 > ext->depth2) return -1;
+        for (int j = 0; j < 3; j++)
+            if (ext->pol[j] < 0 || ext->pol[j] > 2) return -1;
+    }
+    const int64_t B = ext->kv_budget;
+    if (B > 0) /* E8: every request must fit alone, or it could never finish */
+        for (int64_t i = 0; i < n; i++)
+            if (kv_enc(ext, trace[i].dur_ms) + orc_tokens(cm, trace[i].dur_ms) > B)
+                return -3;
+    if (first_arrival_us) *first_arrival_us = n > 0 ? trace[0].arrival_us : 0;
+    if (last_done_us) *last_done_us = 0;
+    if (n == 0) return 0;
+
+    int64_t *W = (int64_t *)malloc(sizeof(int64_t) * (size_t)n);
+    int64_t *R = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots);
+    int64_t *rem = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots);
+    int64_t *mem = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots);
+    char *fresh = (char *)malloc((size_t)slots);      /* admitted in this step */
+    char *ever = (char *)calloc((size_t)n, 1);        /* had a first token */
+    if (!W || !R || !rem || !mem || !fresh || !ever) {
+        free(W); free(R); free(rem); free(mem); free(fresh); free(ever);
+        return -2;
+    }
+    int64_t nW = 0, nR = 0, p = 0, done = 0, t = 0;
+    int blocked = 0; /* E6: admission cut short by memory; retried only
+                        after the waiting or the running set has changed */
+
+    while (done < n) {
+        /* 1. ingest (S13) */
+        while (p < n && trace[p].arrival_us <= t) {
+            W[nW++] = p++;
+            blocked = 0;
+        }
+        /* 2. idle server (S14) */
+        if (nR == 0 && nW == 0) {
+            t = trace[p].arrival_us;
+            continue;
+        }
+        const int pol = eff_policy(policy, ext, nW); /* E7: depth after ingest */
+        /* 3a. memory pressure (E1-E4): one more token for everyone must fit */
+        int64_t preempted = 0;
+        if (B > 0) {
+            int64_t M = 0;
+            for (int64_t s = 0; s < nR; s++) M += mem[s];
+            while (M + nR > B) { /* nR >= 2 here by E8 */
+                int64_t v = 0;   /* the WORST running request at now = t */
+                for (int64_t s = 1; s < nR; s++)
+                    if (orc_better(&trace[R[v]], R[v], &trace[R[s]], R[s], pol, t))
+                        v = s;
+                W[nW++] = R[v]; /* waits again, keeps its arrival time */
+                M -= mem[v];
+                for (int64_t s = v + 1; s < nR; s++) {
+                    R[s - 1] = R[s];
+                    rem[s - 1] = rem[s];
+                    mem[s - 1] = mem[s];
+                }
+                nR--;
+                preempted++;
+                blocked = 0;
+            }
+        }
+        if (n_preempt) *n_preempt += preempted;
+        /* 3b. admission: only in a step without preemption (E5) */
+        int64_t enc_sum = 0;
+        for (int64_t s = 0; s < nR; s++) fresh[s] = 0;
+        if (preempted == 0 && !blocked && nW > 0 && nR < slots) {
+            wait_ctx_t c = {trace, pol, t};
+            qsort_r(W, (size_t)nW, sizeof(int64_t), cmp_wait, &c);
+            int64_t M = 0;
+            for (int64_t s = 0; s < nR; s++) M += mem[s];
+            int64_t k = 0;
+            while (k < nW && nR < slots) {
+                int64_t i = W[k];
+                int64_t kv = B > 0 ? kv_enc(ext, trace[i].dur_ms) : 0;
+                if (B > 0 && M + kv + nR + 1 > B) { /* head of line does not fit */
+                    blocked = 1;
+                    break;
+                }
+                R[nR] = i;
+                rem[nR] = orc_tokens(cm, trace[i].dur_ms);
+                mem[nR] = kv;
+                fresh[nR] = 1;
+                M += kv;
+                nR++;
+                k++;
+                enc_sum += orc_enc_cost(cm, trace[i].dur_ms); /* recompute pays again */
+            }
+            memmove(W, W + k, sizeof(int64_t) * (size_t)(nW - k));
+            nW -= k;
+        }
+        /* 4. one engine iteration */
+        t += enc_sum + cm->iter_base_us + cm->iter_per_running_us * nR;
+        for (int64_t s = 0; s < nR; s++) {
+            rem[s] -= 1;
+            mem[s] += 1;
+        }
+        /* 5. record */
+        for (int64_t s = 0; s < nR; s++)
+            if (fresh[s] && !ever[R[s]]) {
+                ttft[R[s]] = t - trace[R[s]].arrival_us; /* first admission only */
+                ever[R[s]] = 1;
+            }
+        int64_t keep = 0;
+        for (int64_t s = 0; s < nR; s++) {
+            if (rem[s] == 0) {
+                lat[R[s]] = t - trace[R[s]].arrival_us;
+                done++;
+                blocked = 0;
+            } else {
+                R[keep] = R[s];
+                rem[keep] = rem[s];
+                mem[keep] = mem[s];
+                keep++;
+            }
+        }
+        nR = keep;
+    }
+    if (last_done_us) *last_done_us = t;
+    free(W); free(R); free(rem); free(mem); free(fresh); free(ever);
+    return 0;
+}
+
+int orc_tpot(const orc_req_t *trace, int64_t n, const orc_cost_t *cm,
+             const int64_t *lat, const int64_t *ttft, int64_t *out) {
+    if (n < 0 || !cm) return -1;
+    for (int64_t i = 0; i < n; i++) {
+        int64_t tok = orc_tokens(cm, trace[i].dur_ms);
+        out[i] = tok > 1 ? (lat[i] - ttft[i]) / (tok - 1) : -1;
+    }
+    return 0;
+}
+
+int orc_estimate(orc_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang,
+                 int32_t n_lang, const uint8_t *lang, const int32_t *speech_ms) {
+    if (n < 0 || n_lang < 1 || !kappa_milli_by_lang) return -1;
+    for (int64_t i = 0; i < n; i++) {
+        int32_t l = lang ? (int32_t)lang[i] : 0;
+        if (l >= n_lang) return -1;
+        int64_t d = speech_ms ? speech_ms[i] : recs[i].dur_ms;
+        if (d < 0) d = 0;
+        int64_t e = (d * (int64_t)kappa_milli_by_lang[l]) / 1000000;
+        if (e < 1) e = 1;
+        if (e > 0x7FFFFFFF) e = 0x7FFFFFFF;
+        recs[i].est = (int32_t)e;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
 /* c3. nearest-rank percentile (S8)            */
 /* ------------------------------------------------------------------ */
 

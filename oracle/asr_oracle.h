@@ -20,6 +20,13 @@
  *                               bit stream is a recipe of this repo
  *                                -- the paper fixes
  *                               only "Poisson, burstiness 1.0".
+ *   orc_tpot / orc_estimate   : pinned (closed forms; Fig. 1 caption's 40/20/10
+ *                               tokens)
+ *   orc_simulate_ex           : reduces to orc_simulate (pinned) with the memory
+ *                               model off; the preemption model itself is this
+ *                               repo's reading of one sentence:
+ *                               pinned by a hand-worked example and invariants,
+ *                               PARITY UNPINNED against the paper's system.
  *   The paper's Table 1/2 trends: PARITY UNPINNED (real-system measurements).
  */
 #ifndef ASR_ORACLE_H
@@ -64,6 +71,50 @@ int orc_simulate(const orc_req_t *trace, int64_t n, int policy,
                  const orc_cost_t *cm, int32_t slots, int64_t *lat,
                  int64_t *ttft, int64_t *first_arrival_us,
                  int64_t *last_done_us);
+
+/* ---- SURVEY.md 8(f) extensions ------------------ */
+
+/* f1 preemption under memory pressure (A.4 "Preemption logic") and
+ * f3 dynamic policy switching on queue depth.  One KV unit = the
+ * cache of one decoded token.  A running request holds
+ *   kv_base + kv_per_s*dur_ms/1000 (encoder / cross-attention cache, floor)
+ *   + the tokens it has generated so far.
+ * kv_budget <= 0 switches the memory model off. */
+typedef struct {
+    int64_t kv_budget;
+    int64_t kv_base;
+    int64_t kv_per_s;
+    int32_t depth1, depth2; /* ORC_ADAPTIVE: waiting < depth1 -> pol[0],   */
+    int32_t pol[3];         /*   < depth2 -> pol[1], else pol[2]            */
+    int32_t pad;
+} orc_ext_t;                /* 48 bytes */
+
+enum { ORC_ADAPTIVE = 3 };
+
+/* orc_simulate with the extensions; ext == NULL is orc_simulate.  Step order
+ * (readings E1-E8): ingest; while the running set would not fit after
+ * one more token each, preempt the WORST running request under the policy's total
+ * order at now = t (SJF: largest est; HRRN: lowest ratio; FCFS: latest arrival),
+ * which loses its progress and waits again; only a step without preemption
+ * admits, best first, stopping at the first request that does not fit; iterate.
+ * TTFT is that of the first admission.  n_preempt (nullable) counts evictions.
+ * Returns -3 if a request alone cannot fit the budget. */
+int orc_simulate_ex(const orc_req_t *trace, int64_t n, int policy,
+                    const orc_cost_t *cm, const orc_ext_t *ext, int32_t slots,
+                    int64_t *lat, int64_t *ttft, int64_t *first_arrival_us,
+                    int64_t *last_done_us, int64_t *n_preempt);
+
+/* f2 time per output token (A.2): (E2E - TTFT) / (tokens - 1),
+ * floor, for requests with more than one token; -1 otherwise */
+int orc_tpot(const orc_req_t *trace, int64_t n, const orc_cost_t *cm,
+             const int64_t *lat, const int64_t *ttft, int64_t *out);
+
+/* f3 duration-based estimator (Eq. 1, Listing 1):
+ * est = max(1, floor(d_ms * kappa_milli / 10^6)) with d = speech_ms[i] when given
+ * (VAD speech-active duration) else dur_ms, and kappa_milli =
+ * kappa_milli_by_lang[lang[i]] (lang == NULL: entry 0) */
+int orc_estimate(orc_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang,
+                 int32_t n_lang, const uint8_t *lang, const int32_t *speech_ms);
 
 /* nearest-rank percentile, p in [1,100]; n == 0 -> -1 */
 int64_t orc_percentile(const int64_t *v, int64_t n, int32_t p);
