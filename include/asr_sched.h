@@ -55,6 +55,7 @@ extern "C" {
 #define ASR_SCHED_VERSION 100
 
 enum { ASR_FCFS = 0, ASR_SJF = 1, ASR_HRRN = 2 };          /* PAPER.md:287 */
+enum { ASR_ADAPTIVE = 3 };  /* policy switching on queue depth, asr_sched_simulate_batched_ex only */
 enum { ASR_DIST_LOGNORMAL = 0, ASR_DIST_UNIFORM = 1 };
 enum { ASR_OK = 0, ASR_EINVAL = -1, ASR_ECUDA = -2, ASR_EUNSUPPORTED = -3 };
 
@@ -170,6 +171,65 @@ int asr_sched_simulate_batched(const asr_req_t *traces, const asr_replica_t *rep
                                asr_summary_t *out_summary, void *workspace,
                                size_t workspace_bytes, void *stream);
 
+/* ------------------------------------------------------------------ */
+/* extensions: preemption, policy switching, TPOT, estimator */
+/* ------------------------------------------------------------------ */
+
+/* Per cost model, 48 bytes.  f1, "Preemption logic": one KV unit is
+ * the cache of one decoded token; a running request holds
+ * kv_base + kv_per_s*dur_ms/1000 (floor) + the tokens it has generated;
+ * kv_budget <= 0 switches the memory model off.  f3, "Dynamic policy
+ * switching": a replica with policy ASR_ADAPTIVE uses, at every scheduling step
+ * with w requests waiting (after ingest), pol[0] if w < depth1, pol[1] if
+ * w < depth2, else pol[2] (each ASR_FCFS/SJF/HRRN; depth1 <= depth2). */
+typedef struct {
+    int64_t kv_budget;
+    int64_t kv_base;
+    int64_t kv_per_s;
+    int32_t depth1, depth2;
+    int32_t pol[3];
+    int32_t pad;
+} asr_sim_ext_t;
+
+/* asr_sched_simulate_batched with exts[cm_id] applied to every replica (one WARP
+ * per replica).  Scheduling step (readings E1-E8): ingest; while one more
+ * token for every running request would exceed kv_budget, the WORST running request
+ * under the step's policy at now = t is preempted (SJF: largest est; HRRN: lowest
+ * ratio; FCFS: latest arrival), loses its progress and waits again with its
+ * original arrival time; only a step without preemption admits, best first, and
+ * stops at the first request whose cache plus one token does not fit (it is not
+ * retried until the waiting or the running set changes); one engine iteration.
+ * A re-admitted request pays its encoder again; its TTFT stays that of its first
+ * admission.  A request that cannot fit the budget alone marks its replica invalid
+ * (n_done = -1).
+ *   exts DEVICE [n_cms]; out_preempt DEVICE [n_replicas] or NULL (evictions per
+ *   replica); everything else as asr_sched_simulate_batched; workspace sized with
+ *   ASR_OP_SIMULATE_EX. */
+int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_replica_t *replicas,
+                                  int32_t n_replicas, const asr_cost_model_t *cms,
+                                  const asr_sim_ext_t *exts, int32_t n_cms,
+                                  int64_t total_requests, int32_t max_slots, int64_t *out_lat,
+                                  int64_t *out_ttft, asr_summary_t *out_summary,
+                                  int64_t *out_preempt, void *workspace,
+                                  size_t workspace_bytes, void *stream);
+
+/* f2, PAPER.md:214 time per output token: out[i] = (lat[i] - ttft[i]) / (tokens_i - 1)
+ * (floor) for requests with more than one token, else -1.
+ *   trace, lat, ttft, out DEVICE [n]; cm HOST. */
+int asr_sched_tpot(const asr_req_t *trace, int64_t n, const asr_cost_model_t *cm,
+                   const int64_t *lat, const int64_t *ttft, int64_t *out, void *stream);
+
+/* f3, Eq. 1 and Listing 1: rewrites recs[i].est =
+ * max(1, floor(d_ms * kappa_milli / 10^6)), d = speech_ms[i] if given (speech-active
+ * duration from a VAD) else dur_ms, kappa_milli =
+ * kappa_milli_by_lang[lang[i]] (entry 0 if lang is NULL; per-language kappa,
+ * PAPER.md:154).  A lang id >= n_lang reads entry 0.
+ *   recs DEVICE [n] (only est is written); kappa_milli_by_lang HOST [n_lang],
+ *   1 <= n_lang <= 64; lang DEVICE [n] or NULL; speech_ms DEVICE [n] or NULL. */
+int asr_sched_estimate(asr_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang,
+                       int32_t n_lang, const uint8_t *lang, const int32_t *speech_ms,
+                       void *stream);
+
 /* Segmented nearest-rank percentiles: segment s is values[seg_off[s] ..
  * seg_off[s+1]); out[s*n_pct + j] = element of rank ceil(pcts[j]*N/100) of the
  * sorted segment, -1 for an empty segment.  `values` is not modified.
@@ -223,9 +283,9 @@ int asr_sched_select_host(const asr_req_t *keys, int32_t n_queues, int32_t q_len
 /* helpers                                                             */
 /* ------------------------------------------------------------------ */
 
-enum { ASR_OP_SELECT = 0, ASR_OP_SIMULATE = 1, ASR_OP_PERCENTILES = 2 };
+enum { ASR_OP_SELECT = 0, ASR_OP_SIMULATE = 1, ASR_OP_PERCENTILES = 2, ASR_OP_SIMULATE_EX = 3 };
 /* Workspace bytes needed.  SELECT: a = n, b = k.  SIMULATE: a = total_requests,
- * b = n_replicas, c = 1 if summary-only (out_lat/out_ttft NULL) else 0.
+ * b = n_replicas, c = 1 if summary-only (out_lat/out_ttft NULL) else 0 (SIMULATE_EX alike).
  * PERCENTILES: a = total values, b = n_seg.  Returns 0 for an unknown op. */
 size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c);
 

@@ -9,9 +9,9 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libasr_sched.so")
 
-FCFS, SJF, HRRN = 0, 1, 2
+FCFS, SJF, HRRN, ADAPTIVE = 0, 1, 2, 3
 DIST_LOGNORMAL, DIST_UNIFORM = 0, 1
-OP_SELECT, OP_SIMULATE, OP_PERCENTILES = 0, 1, 2
+OP_SELECT, OP_SIMULATE, OP_PERCENTILES, OP_SIMULATE_EX = 0, 1, 2, 3
 
 # numpy views of the ABI structs (include/asr_sched.h)
 REQ_DTYPE = np.dtype([("arrival_us", "<i8"), ("dur_ms", "<i4"), ("est", "<i4")])
@@ -24,13 +24,17 @@ SUMMARY_DTYPE = np.dtype([("p50_e2e_us", "<i8"), ("p90_e2e_us", "<i8"), ("p50_tt
                           ("n_done", "<i8")])
 SPEC_DTYPE = np.dtype([("seed", "<u8"), ("rate_mhz", "<i4"), ("dist", "<i4")])
 TABLES_DTYPE = np.dtype([("ln_dur", "<u4", (4097,)), ("exp_t", "<u4", (4097,))])
+EXT_DTYPE = np.dtype([("kv_budget", "<i8"), ("kv_base", "<i8"), ("kv_per_s", "<i8"), ("depth1", "<i4"),
+                      ("depth2", "<i4"), ("pol", "<i4", (3,)), ("pad", "<i4")])
+assert EXT_DTYPE.itemsize == 48
 assert REQ_DTYPE.itemsize == 16 and COST_DTYPE.itemsize == 40 and REPLICA_DTYPE.itemsize == 32
 assert SUMMARY_DTYPE.itemsize == 56 and SPEC_DTYPE.itemsize == 16 and TABLES_DTYPE.itemsize == 2 * 4097 * 4
 
 EXPORTS = (
     "asr_sched_select", "asr_sched_select_batched", "asr_sched_simulate", "asr_sched_simulate_batched",
     "asr_sched_percentiles", "asr_sched_gen_trace", "asr_sched_gen_trace_batched", "asr_sched_gen_queues",
-    "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_workspace_bytes", "asr_sched_last_error",
+    "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_simulate_batched_ex", "asr_sched_tpot",
+    "asr_sched_estimate", "asr_sched_workspace_bytes", "asr_sched_last_error",
     "asr_sched_version", "asr_sched_launch_count", "asr_sched_timing_enable", "asr_sched_timing_reset",
     "asr_sched_timing_read", "asr_sched_kernel_name", "asr_sched_set_option",
 )
@@ -67,7 +71,10 @@ def lib():
         L.asr_sched_gen_queues.argtypes = [u64, i64, i64, i64, vp, vp, vp]
         L.asr_sched_sweep_host.argtypes = [vp, i32, i64, vp, vp, i32, i32, vp, vp]
         L.asr_sched_select_host.argtypes = [vp, i32, i32, i32, i64, i32, vp]
-        for name in EXPORTS[:10]:
+        L.asr_sched_simulate_batched_ex.argtypes = [vp, vp, i32, vp, vp, i32, i64, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.asr_sched_tpot.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+        L.asr_sched_estimate.argtypes = [vp, i64, vp, i32, vp, vp, vp]
+        for name in EXPORTS[:13]:
             getattr(L, name).restype = C.c_int
         L.asr_sched_workspace_bytes.argtypes = [i32, i64, i64, i64]
         L.asr_sched_workspace_bytes.restype = sz
@@ -243,6 +250,49 @@ def simulate_batched(traces, replicas, n_replicas: int, cms, n_cms: int, total_r
                                             _ptr(out_summary), _ptr(workspace), workspace.numel(), _stream()),
            "asr_sched_simulate_batched")
     return out_lat, out_ttft, out_summary
+
+
+def make_ext(kv_budget=0, kv_base=0, kv_per_s=0, depth1=0, depth2=0, pol=(0, 0, 0)) -> np.ndarray:
+    e = np.zeros(1, dtype=EXT_DTYPE)
+    e["kv_budget"], e["kv_base"], e["kv_per_s"] = kv_budget, kv_base, kv_per_s
+    e["depth1"], e["depth2"] = depth1, depth2
+    e["pol"][0] = pol
+    return e
+
+
+def simulate_batched_ex(traces, replicas, n_replicas: int, cms, exts, n_cms: int, total_requests: int,
+                        max_slots: int, out_lat=None, out_ttft=None, out_summary=None, out_preempt=None,
+                        workspace=None):
+    """asr_sched_simulate_batched_ex: KV-budget preemption and policy switching (exts[cm_id])."""
+    summary_only = out_lat is None
+    if workspace is None:
+        workspace = _workspace(workspace_bytes(OP_SIMULATE_EX, total_requests, n_replicas, 1 if summary_only else 0),
+                               traces.device)
+    _check(lib().asr_sched_simulate_batched_ex(_ptr(traces), _ptr(replicas), n_replicas, _ptr(cms), _ptr(exts), n_cms,
+                                               total_requests, max_slots, _ptr(out_lat), _ptr(out_ttft),
+                                               _ptr(out_summary), _ptr(out_preempt), _ptr(workspace),
+                                               workspace.numel(), _stream()),
+           "asr_sched_simulate_batched_ex")
+    return out_lat, out_ttft, out_summary, out_preempt
+
+
+def tpot(trace, n: int, cm: np.ndarray, lat, ttft, out=None):
+    """asr_sched_tpot -> int64[n] device tensor, (lat - ttft) / (tokens - 1), -1 for one-token requests"""
+    torch = _torch()
+    if out is None:
+        out = torch.empty(max(n, 1), dtype=torch.int64, device=trace.device)[:n]
+    cm = np.ascontiguousarray(cm, dtype=COST_DTYPE)
+    _check(lib().asr_sched_tpot(_ptr(trace), n, cm.ctypes.data, _ptr(lat), _ptr(ttft), _ptr(out), _stream()),
+           "asr_sched_tpot")
+    return out
+
+
+def estimate(recs, n: int, kappa_milli_by_lang, lang=None, speech_ms=None):
+    """asr_sched_estimate: rewrites est of the device records in place"""
+    kap = np.ascontiguousarray(kappa_milli_by_lang, dtype=np.int32)
+    _check(lib().asr_sched_estimate(_ptr(recs), n, kap.ctypes.data, kap.shape[0], _ptr(lang), _ptr(speech_ms),
+                                    _stream()), "asr_sched_estimate")
+    return recs
 
 
 def percentiles(values, seg_off, n_seg: int, pcts, out=None):

@@ -36,7 +36,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
-    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel"};
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel"};
 struct TimedLaunch {
     int kid;
     cudaEvent_t start, stop;
@@ -176,6 +176,7 @@ extern "C" size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, in
     switch (op) {
         case ASR_OP_SELECT: return select_workspace_bytes(a, b);
         case ASR_OP_SIMULATE: return sim_ws(a, b, c != 0).total + 512;   // + descriptors of the single-replica call
+        case ASR_OP_SIMULATE_EX: return sim_ws(a, b, c != 0).total + sim_ws(a, b, c != 0).bitmap_bytes;
         case ASR_OP_PERCENTILES: return 0;
     }
     return 0;
@@ -222,13 +223,101 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
     if (rc) return rc;
     SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
-              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, summary_only ? 1 : 0, g_opt_escalate.load()};
+              out_lat, out_ttft, out_summary, nullptr, nullptr, nullptr, total_requests, n_replicas, n_cms, summary_only ? 1 : 0,
+              g_opt_escalate.load()};
     // many small replicas: one thread each; few or wide ones: one warp each
     const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
     rc = launch_simulate(a, max_slots, use_lane, st);
     if (rc) return rc;
     if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
     return rc;
+}
+
+extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_replica_t *replicas,
+                                             int32_t n_replicas, const asr_cost_model_t *cms,
+                                             const asr_sim_ext_t *exts, int32_t n_cms, int64_t total_requests,
+                                             int32_t max_slots, int64_t *out_lat, int64_t *out_ttft,
+                                             asr_summary_t *out_summary, int64_t *out_preempt, void *workspace,
+                                             size_t workspace_bytes, void *stream) {
+    if (n_replicas < 0 || n_cms < 1 || total_requests < 0 || max_slots < 1) {
+        set_error("simulate_batched_ex: bad argument (n_replicas=%d n_cms=%d total=%lld max_slots=%d)", n_replicas,
+                  n_cms, (long long)total_requests, max_slots);
+        return ASR_EINVAL;
+    }
+    if (max_slots > 256) {
+        set_error("simulate_batched_ex: max_slots=%d exceeds the limit 256", max_slots);
+        return ASR_EUNSUPPORTED;
+    }
+    if (n_replicas == 0) return ASR_OK;
+    if (!replicas || !cms || !exts || (!traces && total_requests > 0) ||
+        ((out_lat == nullptr) != (out_ttft == nullptr))) {
+        set_error("simulate_batched_ex: null pointer (out_lat and out_ttft must both be given or both be NULL)");
+        return ASR_EINVAL;
+    }
+    const bool summary_only = out_lat == nullptr;
+    if (summary_only && !out_summary) {
+        set_error("simulate_batched_ex: nothing to output");
+        return ASR_EINVAL;
+    }
+    const SimWorkspace w = sim_ws(total_requests, n_replicas, summary_only);
+    if (!workspace || workspace_bytes < w.total + w.bitmap_bytes) {
+        set_error("simulate_batched_ex: workspace too small (%zu < %zu)", workspace_bytes, w.total + w.bitmap_bytes);
+        return ASR_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    int64_t *bm_off = (int64_t *)ws;
+    uint32_t *bitmap = (uint32_t *)(ws + w.bm_off_bytes);
+    int32_t *defer = (int32_t *)(ws + w.bm_off_bytes + w.bitmap_bytes);
+    if (summary_only) {
+        out_lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes);
+        out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + w.lat_bytes);
+    }
+    uint32_t *bitmap2 = (uint32_t *)(ws + w.total);
+    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
+    if (rc) return rc;
+    SimArgs a{traces,  replicas, cms,         bm_off, bitmap,  defer + 64,  defer,          defer + 64 + n_replicas, defer + 1,
+              out_lat, out_ttft, out_summary, exts,   bitmap2, out_preempt, total_requests, n_replicas, n_cms, 0,
+              g_opt_escalate.load()};
+    rc = launch_simulate_ex(a, max_slots, st);
+    if (rc) return rc;
+    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
+    return rc;
+}
+
+extern "C" int asr_sched_tpot(const asr_req_t *trace, int64_t n, const asr_cost_model_t *cm, const int64_t *lat,
+                              const int64_t *ttft, int64_t *out, void *stream) {
+    if (n < 0 || !cm) {
+        set_error("tpot: bad argument (n=%lld)", (long long)n);
+        return ASR_EINVAL;
+    }
+    if (n == 0) return ASR_OK;
+    if (!trace || !lat || !ttft || !out) {
+        set_error("tpot: null pointer");
+        return ASR_EINVAL;
+    }
+    return launch_tpot(trace, n, *cm, lat, ttft, out, (cudaStream_t)stream);
+}
+
+extern "C" int asr_sched_estimate(asr_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang, int32_t n_lang,
+                                  const uint8_t *lang, const int32_t *speech_ms, void *stream) {
+    if (n < 0 || !kappa_milli_by_lang || n_lang < 1) {
+        set_error("estimate: bad argument (n=%lld n_lang=%d)", (long long)n, n_lang);
+        return ASR_EINVAL;
+    }
+    if (n_lang > 64) {
+        set_error("estimate: n_lang=%d exceeds the limit 64", n_lang);
+        return ASR_EUNSUPPORTED;
+    }
+    if (n == 0) return ASR_OK;
+    if (!recs) {
+        set_error("estimate: null pointer");
+        return ASR_EINVAL;
+    }
+    KappaTable kt;
+    kt.n_lang = n_lang;
+    for (int j = 0; j < 64; ++j) kt.kappa_milli[j] = j < n_lang ? kappa_milli_by_lang[j] : 0;
+    return launch_estimate(recs, n, kt, lang, speech_ms, (cudaStream_t)stream);
 }
 
 extern "C" int asr_sched_simulate(const asr_req_t *trace, int64_t n, int32_t policy, const asr_cost_model_t *cm,

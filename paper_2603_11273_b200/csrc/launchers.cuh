@@ -17,6 +17,9 @@ struct SimArgs {
     int64_t *out_lat;
     int64_t *out_ttft;
     asr_summary_t *out_summary;  // nullable
+    const asr_sim_ext_t *exts;   // [n_cms], extension calls only
+    uint32_t *bitmap2;           // second bitmap (requests that had a first token), extension calls only
+    int64_t *out_preempt;        // [n_replicas] nullable, extension calls only
     int64_t total_requests;
     int32_t n_replicas;
     int32_t n_cms;
@@ -26,6 +29,15 @@ struct SimArgs {
 
 int launch_simulate(const SimArgs &a, int max_slots, bool use_lane, cudaStream_t st);
 int launch_simulate_cta(const SimArgs &a, cudaStream_t st);
+int launch_simulate_ex(const SimArgs &a, int max_slots, cudaStream_t st);
+int launch_tpot(const asr_req_t *trace, int64_t n, asr_cost_model_t cm, const int64_t *lat, const int64_t *ttft,
+                int64_t *out, cudaStream_t st);
+struct KappaTable {
+    int32_t n_lang;
+    int32_t kappa_milli[64];
+};
+int launch_estimate(asr_req_t *recs, int64_t n, const KappaTable &kt, const uint8_t *lang, const int32_t *speech_ms,
+                    cudaStream_t st);
 int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,
                        cudaStream_t st);
 int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg, const int32_t *pcts,
