@@ -274,6 +274,76 @@ def side_configs(asr, dev, d_tables, reps=5):
     return out
 
 
+def extension_lines(asr, dev, d_tables, hbm_peak, reps=5):
+    """SURVEY.md 8(f) rows, each timed alone (CUDA events through the library's per-kernel timers):
+    the two HBM streams against the measured HBM peak, the extended simulator on an overloaded
+    sweep with a KV budget that binds."""
+    import torch
+    out = {}
+    cost_h = asr.make_cost(*wl.CONFIG_COST)
+    # --- estimate + tpot on 2^26 records
+    n = 1 << 26
+    d_tr = asr.gen_queues(77, 0, n, 10**10, d_tables)
+    d_lat = torch.randint(10**5, 10**7, (n,), dtype=torch.int64, device=dev)
+    d_ttft = torch.randint(10**3, 10**5, (n,), dtype=torch.int64, device=dev)
+    d_out = torch.empty(n, dtype=torch.int64, device=dev)
+    d_lang = torch.randint(0, 4, (n,), dtype=torch.uint8, device=dev)
+    for _ in range(2):
+        asr.estimate(d_tr, n, [5000, 2500, 7300, 4100], d_lang)
+        asr.tpot(d_tr, n, cost_h, d_lat, d_ttft, d_out)
+    torch.cuda.synchronize()
+    asr.timing_enable(True)
+    asr.timing_reset()
+    for _ in range(reps):
+        asr.estimate(d_tr, n, [5000, 2500, 7300, 4100], d_lang)
+        asr.tpot(d_tr, n, cost_h, d_lat, d_ttft, d_out)
+    kt = asr.timing_read()
+    for name, bytes_per in (("estimate_kernel", 16 + 1 + 4), ("tpot_kernel", 16 + 8 + 8 + 8)):
+        ms, cnt = kt.get(name, (0.0, 0))
+        if cnt:
+            a = n * bytes_per / (ms / cnt / 1e3) / 1e9
+            out[name] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak,
+                         "algorithmic_bytes_per_launch": n * bytes_per, "avg_launch_ms": ms / cnt, "records": n}
+    del d_tr, d_lat, d_ttft, d_out, d_lang
+    # --- extended simulator: 256 seeds x 8 overload rates x 3 policies, 3,000 requests, 16 slots, KV budget
+    n_seeds, n_req, slots = 256, 3000, 16
+    rates = [16000, 18000, 20000, 22000, 24000, 26000, 28000, 30000]        # PAPER.md:104 heavy range, mHz
+    seeds = np.repeat(np.arange(n_seeds, dtype=np.uint64) + 5000, len(rates))
+    specs = np.zeros(len(seeds), dtype=asr.SPEC_DTYPE)
+    specs["seed"], specs["rate_mhz"], specs["dist"] = seeds, np.tile(rates, n_seeds), 0
+    n_tr, n_rep = len(seeds), len(seeds) * 3
+    rep = asr.make_replicas(np.repeat(np.arange(n_tr, dtype=np.int64) * n_req, 3),
+                            np.arange(n_rep, dtype=np.int64) * n_req, n_req,
+                            np.tile(np.asarray([0, 1, 2], dtype=np.int32), n_tr), slots, 0)
+    d_specs, d_rep, d_cost = (asr.to_device(x, dev) for x in (specs, rep, cost_h))
+    d_ext = asr.to_device(asr.make_ext(kv_budget=25 * slots, kv_base=20, kv_per_s=2), dev)
+    d_trs = asr.gen_trace_batched(d_specs, n_tr, n_req, d_tables)
+    d_sum = torch.zeros(n_rep * asr.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    d_pre = torch.zeros(n_rep, dtype=torch.int64, device=dev)
+    from paper_2603_11273_b200 import binding as B
+    d_ws = torch.empty(asr.workspace_bytes(B.OP_SIMULATE_EX, n_rep * n_req, n_rep, 1), dtype=torch.uint8, device=dev)
+
+    def step():
+        asr.simulate_batched_ex(d_trs, d_rep, n_rep, d_cost, d_ext, 1, n_rep * n_req, slots, None, None, d_sum, d_pre,
+                                workspace=d_ws)
+    step()
+    torch.cuda.synchronize()
+    asr.timing_reset()
+    for _ in range(reps):
+        step()
+    kt = asr.timing_read()
+    asr.timing_enable(False)
+    ms, cnt = kt.get("sim_ex_kernel", (0.0, 0))
+    summ = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
+    if cnt:
+        out["sim_ex_kernel"] = {"bound": "alu", "workload": "%d replicas x %d requests at 16-30 req/s, %d slots, KV budget %d "
+                                "(base 20 + 2/s of audio + generated tokens)" % (n_rep, n_req, slots, 25 * slots),
+                                "avg_launch_ms": ms / cnt, "requests_per_s": n_rep * n_req / (ms / cnt / 1e3),
+                                "preemptions_per_request": float(d_pre.sum().item()) / (n_rep * n_req),
+                                "replicas_done": int((summ["n_done"] == n_req).sum())}
+    return out
+
+
 def run_ours(args):
     import torch
     import paper_2603_11273_b200 as asr
@@ -444,9 +514,12 @@ def run_ours(args):
         except Exception as exc:  # pinned allocation can fail on a small host
             e2e["select_error"] = str(exc)[:200]
 
-    side = None
+    side = ext_lines = None
     if rank == 0 and not args.no_side_configs:
+        del d_traces, d_ws, d_queues
+        torch.cuda.empty_cache()
         side = side_configs(asr, dev, d_tables)
+        ext_lines = extension_lines(asr, dev, d_tables, hbm_peak)
 
     base = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -471,7 +544,7 @@ def run_ours(args):
                        "frac_of_measured_peak": select_gbs / world / hbm_peak,
                        "frac_of_nominal_8TBs": select_gbs / world / 8000.0},
             "roofline": roofline, "rooflines": rooflines, "clocks": clocks, "e2e": e2e,
-            "gpu_launches": int(launches), "cpu_baseline": base, "configs": side,
+            "gpu_launches": int(launches), "cpu_baseline": base, "configs": side, "extensions": ext_lines,
             "kernel_ms_total": {k_: v[0] for k_, v in ktimes.items() if v[1]},
         }
         print(json.dumps(line), flush=True)
