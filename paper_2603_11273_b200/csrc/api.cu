@@ -223,7 +223,7 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
     if (rc) return rc;
     SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
-              out_lat, out_ttft, out_summary, nullptr, nullptr, nullptr, total_requests, n_replicas, n_cms, summary_only ? 1 : 0,
+              out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, summary_only ? 1 : 0,
               g_opt_escalate.load()};
     // many small replicas: one thread each; few or wide ones: one warp each
     const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
@@ -276,9 +276,14 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
     uint32_t *bitmap2 = (uint32_t *)(ws + w.total);
     int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
     if (rc) return rc;
-    SimArgs a{traces,  replicas, cms,         bm_off, bitmap,  defer + 64,  defer,          defer + 64 + n_replicas, defer + 1,
-              out_lat, out_ttft, out_summary, exts,   bitmap2, out_preempt, total_requests, n_replicas, n_cms, 0,
-              g_opt_escalate.load()};
+    SimExArgs a;
+    static_cast<SimArgs &>(a) = SimArgs{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer,
+                                        defer + 64 + n_replicas, defer + 1,
+                                        out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, 0,
+                                        g_opt_escalate.load()};
+    a.exts = exts;
+    a.bitmap2 = bitmap2;
+    a.out_preempt = out_preempt;
     rc = launch_simulate_ex(a, max_slots, st);
     if (rc) return rc;
     if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);

@@ -17,9 +17,6 @@ struct SimArgs {
     int64_t *out_lat;
     int64_t *out_ttft;
     asr_summary_t *out_summary;  // nullable
-    const asr_sim_ext_t *exts;   // [n_cms], extension calls only
-    uint32_t *bitmap2;           // second bitmap (requests that had a first token), extension calls only
-    int64_t *out_preempt;        // [n_replicas] nullable, extension calls only
     int64_t total_requests;
     int32_t n_replicas;
     int32_t n_cms;
@@ -29,7 +26,13 @@ struct SimArgs {
 
 int launch_simulate(const SimArgs &a, int max_slots, bool use_lane, cudaStream_t st);
 int launch_simulate_cta(const SimArgs &a, cudaStream_t st);
-int launch_simulate_ex(const SimArgs &a, int max_slots, cudaStream_t st);
+// the extension kernel's arguments (kept out of SimArgs: the base kernels' parameter block stays as it was)
+struct SimExArgs : SimArgs {
+    const asr_sim_ext_t *exts;   // [n_cms]
+    uint32_t *bitmap2;           // second bitmap: requests that had a first token
+    int64_t *out_preempt;        // [n_replicas] nullable
+};
+int launch_simulate_ex(const SimExArgs &a, int max_slots, cudaStream_t st);
 int launch_tpot(const asr_req_t *trace, int64_t n, asr_cost_model_t cm, const int64_t *lat, const int64_t *ttft,
                 int64_t *out, cudaStream_t st);
 struct KappaTable {

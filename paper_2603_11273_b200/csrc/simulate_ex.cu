@@ -38,7 +38,7 @@ __device__ __forceinline__ bool ext_ok(const asr_sim_ext_t &ex, int policy) {
 }
 
 template <int SPL>
-__device__ __forceinline__ void sim_ex_replica(const SimArgs &a, const int r) {
+__device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) {
     const int lane = lane_id();
     asr_replica_t rep = a.replicas[r];
     const int n = rep.n, slots = rep.slots, policy = rep.policy;
@@ -323,18 +323,18 @@ __device__ __forceinline__ void sim_ex_replica(const SimArgs &a, const int r) {
 }
 
 template <int SPL>
-__global__ void __launch_bounds__(SIM_WARPS * 32) sim_ex_kernel(SimArgs a) {
+__global__ void __launch_bounds__(SIM_WARPS * 32) sim_ex_kernel(SimExArgs a) {
     const int gw = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
     if (gw < a.n_replicas) sim_ex_replica<SPL>(a, gw);
 }
 
 template <int SPL>
-static void launch_ex(const SimArgs &a, cudaStream_t st) {
+static void launch_ex(const SimExArgs &a, cudaStream_t st) {
     KernelTimer kt(KID_SIM_EX, st);
     sim_ex_kernel<SPL><<<(a.n_replicas + SIM_WARPS - 1) / SIM_WARPS, SIM_WARPS * 32, 0, st>>>(a);
 }
 
-int launch_simulate_ex(const SimArgs &a, int max_slots, cudaStream_t st) {
+int launch_simulate_ex(const SimExArgs &a, int max_slots, cudaStream_t st) {
     if (a.n_replicas <= 0) return ASR_OK;
     if (max_slots <= 32) launch_ex<1>(a, st);
     else if (max_slots <= 64) launch_ex<2>(a, st);
