@@ -92,6 +92,8 @@ def lib():
         L.orc_simulate_ex.restype = C.c_int
         L.orc_simulate_ex.argtypes = [vp, i64, C.c_int, C.POINTER(Cost), C.POINTER(Ext), i32, vp, vp,
                                       C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
+        L.orc_itl.restype = C.c_int
+        L.orc_itl.argtypes = [vp, i64, C.c_int, C.POINTER(Cost), i32, vp, i32, vp, C.POINTER(i64), C.POINTER(i64)]
         L.orc_tpot.restype = C.c_int
         L.orc_tpot.argtypes = [vp, i64, C.POINTER(Cost), vp, vp, vp]
         L.orc_estimate.restype = C.c_int
@@ -171,6 +173,19 @@ def simulate_ex(trace, policy: int, cm: Cost, ex, slots: int):
     if rc != 0:
         raise ValueError("orc_simulate_ex rc=%d" % rc)
     return lat, ttft, fa.value, ld.value, npre.value
+
+
+def itl(trace, policy: int, cm: Cost, slots: int, pcts):
+    """orc_itl -> (percentiles list, count, sum) of the inter-token gaps"""
+    trace = _req(trace)
+    pc = np.ascontiguousarray(pcts, dtype=np.int32)
+    out = np.empty(len(pc), dtype=np.int64)
+    cnt, sm = C.c_int64(0), C.c_int64(0)
+    rc = lib().orc_itl(trace.ctypes.data, trace.shape[0], policy, C.byref(cm), slots, pc.ctypes.data, len(pc),
+                       out.ctypes.data, C.byref(cnt), C.byref(sm))
+    if rc != 0:
+        raise ValueError("orc_itl rc=%d" % rc)
+    return [int(x) for x in out], cnt.value, sm.value
 
 
 def tpot(trace, cm: Cost, lat, ttft) -> np.ndarray:

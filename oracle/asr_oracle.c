@@ -336,6 +336,77 @@ int orc_simulate_ex(const orc_req_t *trace, int64_t n, int policy,
     return 0;
 }
 
+int orc_itl(const orc_req_t *trace, int64_t n, int policy, const orc_cost_t *cm,
+            int32_t slots, const int32_t *pcts, int32_t n_pct, int64_t *out_pcts,
+            int64_t *out_count, int64_t *out_sum) {
+    if (n < 0 || slots < 1 || policy < 0 || policy > 2 || !cm || n_pct < 0) return -1;
+    int64_t cap = 1024, cnt = 0, sum = 0;
+    int64_t *gaps = (int64_t *)malloc(sizeof(int64_t) * (size_t)cap);
+    int64_t *W = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
+    int64_t *R = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots);
+    int64_t *rem = (int64_t *)malloc(sizeof(int64_t) * (size_t)slots);
+    if (!gaps || !W || !R || !rem) {
+        free(gaps); free(W); free(R); free(rem);
+        return -2;
+    }
+    int64_t nW = 0, nR = 0, p = 0, done = 0, t = 0;
+    while (done < n) { /* the loop of orc_simulate, one iteration at a time */
+        while (p < n && trace[p].arrival_us <= t) W[nW++] = p++;
+        if (nR == 0 && nW == 0) {
+            t = trace[p].arrival_us;
+            continue;
+        }
+        int64_t free_slots = (int64_t)slots - nR;
+        int64_t k = free_slots < nW ? free_slots : nW;
+        int64_t enc_sum = 0, already = nR;
+        if (k > 0) {
+            wait_ctx_t c = {trace, policy, t};
+            qsort_r(W, (size_t)nW, sizeof(int64_t), cmp_wait, &c);
+            for (int64_t j = 0; j < k; j++) {
+                int64_t i = W[j];
+                R[nR] = i;
+                rem[nR] = orc_tokens(cm, trace[i].dur_ms);
+                nR++;
+                enc_sum += orc_enc_cost(cm, trace[i].dur_ms);
+            }
+            memmove(W, W + k, sizeof(int64_t) * (size_t)(nW - k));
+            nW -= k;
+        }
+        const int64_t dt = enc_sum + cm->iter_base_us + cm->iter_per_running_us * nR;
+        t += dt;
+        for (int64_t s = 0; s < already; s++) { /* one gap per request that was running */
+            if (cnt == cap) {
+                cap *= 2;
+                int64_t *g2 = (int64_t *)realloc(gaps, sizeof(int64_t) * (size_t)cap);
+                if (!g2) {
+                    free(gaps); free(W); free(R); free(rem);
+                    return -2;
+                }
+                gaps = g2;
+            }
+            gaps[cnt++] = dt;
+            sum += dt;
+        }
+        int64_t keep = 0;
+        for (int64_t s = 0; s < nR; s++) {
+            rem[s] -= 1;
+            if (rem[s] == 0) {
+                done++;
+            } else {
+                R[keep] = R[s];
+                rem[keep] = rem[s];
+                keep++;
+            }
+        }
+        nR = keep;
+    }
+    for (int32_t j = 0; j < n_pct; j++) out_pcts[j] = orc_percentile(gaps, cnt, pcts[j]);
+    if (out_count) *out_count = cnt;
+    if (out_sum) *out_sum = sum;
+    free(gaps); free(W); free(R); free(rem);
+    return 0;
+}
+
 int orc_tpot(const orc_req_t *trace, int64_t n, const orc_cost_t *cm,
              const int64_t *lat, const int64_t *ttft, int64_t *out) {
     if (n < 0 || !cm) return -1;

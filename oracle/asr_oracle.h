@@ -20,6 +20,9 @@
  *                               bit stream is a recipe of this repo
  *                                -- the paper fixes
  *                               only "Poisson, burstiness 1.0".
+ *   orc_itl                   : pinned (closed forms: isolated request, two
+ *                               overlapping requests by hand; sum = sum of
+ *                               (E2E - TTFT) over requests)
  *   orc_tpot / orc_estimate   : pinned (closed forms; Fig. 1 caption's 40/20/10
  *                               tokens)
  *   orc_simulate_ex           : reduces to orc_simulate (pinned) with the memory
@@ -108,6 +111,17 @@ int orc_simulate_ex(const orc_req_t *trace, int64_t n, int policy,
  * floor, for requests with more than one token; -1 otherwise */
 int orc_tpot(const orc_req_t *trace, int64_t n, const orc_cost_t *cm,
              const int64_t *lat, const int64_t *ttft, int64_t *out);
+
+/* f2 inter-token latency (A.2 "P50 ITL"): the multiset of the gaps
+ * between consecutive output tokens of every request.  A token appears at the end
+ * of every engine iteration its request is running in, so each iteration adds one
+ * sample of its own duration (iteration cost plus the encoders admitted in it) for
+ * every request that was ALREADY running (a request's first token belongs to TTFT).
+ * out_pcts[j] = nearest-rank percentile pcts[j] of the multiset (-1 if empty),
+ * out_count = its size, out_sum = the sum of its samples (mean = sum / count). */
+int orc_itl(const orc_req_t *trace, int64_t n, int policy, const orc_cost_t *cm,
+            int32_t slots, const int32_t *pcts, int32_t n_pct, int64_t *out_pcts,
+            int64_t *out_count, int64_t *out_sum);
 
 /* f3 duration-based estimator (Eq. 1, Listing 1):
  * est = max(1, floor(d_ms * kappa_milli / 10^6)) with d = speech_ms[i] when given

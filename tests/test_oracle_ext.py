@@ -117,3 +117,31 @@ def test_estimator_fig1_tokens_and_floor():
     assert list(out["est"]) == [40, 10, 5, 1, 1]
     out = orc.estimate(tr, [5000], speech_ms=[4000, 4000, 0, 100, 1000])  # VAD: speech-active duration
     assert list(out["est"]) == [20, 20, 1, 1, 5]
+
+
+def test_itl_isolated_and_two_overlapping_requests():
+    """PAPER.md:214.  Alone, every gap is 8,000 + 50 us: a 6 s request (25 tokens) has 24 of them.
+    Unit model (1 ms iterations, no encoder), two slots: A (3 tokens) at t=0, B (2 tokens) arrives at
+    500 us and is admitted at 1000: iterations [0,1000) A first token; [1000,2000) A gap, B first
+    token; [2000,3000) A gap + B gap.  Three gaps of 1000."""
+    cm = orc.cost(*wl.CONFIG_COST)
+    p, cnt, sm = orc.itl(orc.make_trace([0], [6000]), orc.FCFS, cm, 4, [1, 50, 100])
+    assert (p, cnt, sm) == ([8050, 8050, 8050], 24, 24 * 8050)
+    p, cnt, sm = orc.itl(orc.make_trace([0, 500], [3000, 2000]), orc.FCFS, UNIT, 2, [50])
+    assert (p, cnt, sm) == ([1000], 3, 3000)
+    # an encoder stall is felt by the requests already running: A (3 tokens) alone, then B admitted
+    enc = orc.cost(700, 0, 1000, 0, 0, 1)
+    p, cnt, sm = orc.itl(orc.make_trace([0, 500], [3000, 2000]), orc.FCFS, enc, 2, [1, 100])
+    assert (p, cnt, sm) == ([1000, 1700], 3, 1000 + 1700 + 1000)
+    assert orc.itl(orc.make_trace([0], [0]), orc.FCFS, cm, 1, [50]) == ([-1], 0, 0)       # one token: no gap
+
+
+def test_itl_sum_is_the_decode_time_of_all_requests():
+    tr = wl.stress_trace("lognormal", 400, 11, rate_per_s=24.0)
+    cm = orc.cost(*wl.CONFIG_COST)
+    for pol in POL:
+        lat, ttft, _, _ = orc.simulate(tr, pol, cm, 8)
+        p, cnt, sm = orc.itl(tr, pol, cm, 8, [25, 50, 90])
+        assert sm == int((lat - ttft).sum())
+        assert cnt == sum(orc.tokens(cm, int(d)) - 1 for d in tr["dur_ms"])
+        assert p[0] <= p[1] <= p[2] and p[0] >= 8000 + 50
