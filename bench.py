@@ -335,6 +335,21 @@ def extension_lines(asr, dev, d_tables, hbm_peak, reps=5):
     asr.timing_enable(False)
     ms, cnt = kt.get("sim_ex_kernel", (0.0, 0))
     summ = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
+    # --- inter-token latency of the same replicas (simulate with gap capture + weighted percentiles)
+    asr.timing_enable(True)
+    asr.timing_reset()
+    d_ws_itl = torch.empty(asr.workspace_bytes(B.OP_ITL, n_rep * n_req, n_rep, 0), dtype=torch.uint8, device=dev)
+    for _ in range(reps):
+        d_itl = asr.itl_batched(d_trs, d_rep, n_rep, d_cost, 1, n_rep * n_req, slots, [50, 90], workspace=d_ws_itl)
+    kt_itl = asr.timing_read()
+    asr.timing_enable(False)
+    ms_p, cnt_p = kt_itl.get("itl_percentiles_kernel", (0.0, 0))
+    ms_s, cnt_s = kt_itl.get("sim_ex_kernel", (0.0, 0))
+    if cnt_p and cnt_s:
+        gaps = int(d_itl[:, 2].sum().item())
+        out["itl"] = {"workload": "the same %d replicas, no KV budget; P50/P90 of %d inter-token gaps per pass" % (n_rep, gaps),
+                      "sim_ex_kernel_ms": ms_s / cnt_s, "itl_percentiles_kernel_ms": ms_p / cnt_p,
+                      "requests_per_s": n_rep * n_req / ((ms_s / cnt_s + ms_p / cnt_p) / 1e3)}
     if cnt:
         out["sim_ex_kernel"] = {"bound": "alu", "workload": "%d replicas x %d requests at 16-30 req/s, %d slots, KV budget %d "
                                 "(base 20 + 2/s of audio + generated tokens)" % (n_rep, n_req, slots, 25 * slots),

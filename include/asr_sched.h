@@ -219,6 +219,23 @@ int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_replica_t *
 int asr_sched_tpot(const asr_req_t *trace, int64_t n, const asr_cost_model_t *cm,
                    const int64_t *lat, const int64_t *ttft, int64_t *out, void *stream);
 
+/* f2, PAPER.md:214 inter-token latency: the multiset of the gaps between consecutive
+ * output tokens of every request of a replica.  A token appears at the end of every
+ * engine iteration its request runs in, so an iteration contributes one sample of its
+ * own duration (iteration cost plus the encoders admitted in it) for every request
+ * that was already running; first tokens belong to TTFT.  Simulates the replicas
+ * (policies ASR_FCFS/SJF/HRRN, no memory model) and writes, per replica,
+ * out[r*(n_pct+2) ..] = the n_pct nearest-rank percentiles (-1 if there is no gap),
+ * the number of gaps, their sum (mean = sum / count); all -1 for an invalid replica.
+ *   pcts HOST [n_pct], 1..100, n_pct <= 8; out DEVICE [n_replicas*(n_pct+2)];
+ *   workspace sized with ASR_OP_ITL (a = total_requests, b = n_replicas);
+ *   everything else as asr_sched_simulate_batched. */
+int asr_sched_itl_batched(const asr_req_t *traces, const asr_replica_t *replicas,
+                          int32_t n_replicas, const asr_cost_model_t *cms, int32_t n_cms,
+                          int64_t total_requests, int32_t max_slots, const int32_t *pcts,
+                          int32_t n_pct, int64_t *out, void *workspace,
+                          size_t workspace_bytes, void *stream);
+
 /* f3, Eq. 1 and Listing 1: rewrites recs[i].est =
  * max(1, floor(d_ms * kappa_milli / 10^6)), d = speech_ms[i] if given (speech-active
  * duration from a VAD) else dur_ms, kappa_milli =
@@ -283,7 +300,7 @@ int asr_sched_select_host(const asr_req_t *keys, int32_t n_queues, int32_t q_len
 /* helpers                                                             */
 /* ------------------------------------------------------------------ */
 
-enum { ASR_OP_SELECT = 0, ASR_OP_SIMULATE = 1, ASR_OP_PERCENTILES = 2, ASR_OP_SIMULATE_EX = 3 };
+enum { ASR_OP_SELECT = 0, ASR_OP_SIMULATE = 1, ASR_OP_PERCENTILES = 2, ASR_OP_SIMULATE_EX = 3, ASR_OP_ITL = 4 };
 /* Workspace bytes needed.  SELECT: a = n, b = k.  SIMULATE: a = total_requests,
  * b = n_replicas, c = 1 if summary-only (out_lat/out_ttft NULL) else 0 (SIMULATE_EX alike).
  * PERCENTILES: a = total values, b = n_seg.  Returns 0 for an unknown op. */

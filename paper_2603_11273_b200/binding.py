@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_PKG, "libasr_sched.so")
 
 FCFS, SJF, HRRN, ADAPTIVE = 0, 1, 2, 3
 DIST_LOGNORMAL, DIST_UNIFORM = 0, 1
-OP_SELECT, OP_SIMULATE, OP_PERCENTILES, OP_SIMULATE_EX = 0, 1, 2, 3
+OP_SELECT, OP_SIMULATE, OP_PERCENTILES, OP_SIMULATE_EX, OP_ITL = 0, 1, 2, 3, 4
 
 # numpy views of the ABI structs (include/asr_sched.h)
 REQ_DTYPE = np.dtype([("arrival_us", "<i8"), ("dur_ms", "<i4"), ("est", "<i4")])
@@ -34,7 +34,7 @@ EXPORTS = (
     "asr_sched_select", "asr_sched_select_batched", "asr_sched_simulate", "asr_sched_simulate_batched",
     "asr_sched_percentiles", "asr_sched_gen_trace", "asr_sched_gen_trace_batched", "asr_sched_gen_queues",
     "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_simulate_batched_ex", "asr_sched_tpot",
-    "asr_sched_estimate", "asr_sched_workspace_bytes", "asr_sched_last_error",
+    "asr_sched_estimate", "asr_sched_itl_batched", "asr_sched_workspace_bytes", "asr_sched_last_error",
     "asr_sched_version", "asr_sched_launch_count", "asr_sched_timing_enable", "asr_sched_timing_reset",
     "asr_sched_timing_read", "asr_sched_kernel_name", "asr_sched_set_option",
 )
@@ -74,7 +74,8 @@ def lib():
         L.asr_sched_simulate_batched_ex.argtypes = [vp, vp, i32, vp, vp, i32, i64, i32, vp, vp, vp, vp, vp, sz, vp]
         L.asr_sched_tpot.argtypes = [vp, i64, vp, vp, vp, vp, vp]
         L.asr_sched_estimate.argtypes = [vp, i64, vp, i32, vp, vp, vp]
-        for name in EXPORTS[:13]:
+        L.asr_sched_itl_batched.argtypes = [vp, vp, i32, vp, i32, i64, i32, vp, i32, vp, vp, sz, vp]
+        for name in EXPORTS[:14]:
             getattr(L, name).restype = C.c_int
         L.asr_sched_workspace_bytes.argtypes = [i32, i64, i64, i64]
         L.asr_sched_workspace_bytes.restype = sz
@@ -274,6 +275,21 @@ def simulate_batched_ex(traces, replicas, n_replicas: int, cms, exts, n_cms: int
                                                workspace.numel(), _stream()),
            "asr_sched_simulate_batched_ex")
     return out_lat, out_ttft, out_summary, out_preempt
+
+
+def itl_batched(traces, replicas, n_replicas: int, cms, n_cms: int, total_requests: int, max_slots: int, pcts,
+                out=None, workspace=None):
+    """asr_sched_itl_batched -> int64 [n_replicas, n_pct + 2] device tensor: percentiles, gap count, gap sum"""
+    torch = _torch()
+    pcts = np.ascontiguousarray(pcts, dtype=np.int32)
+    if out is None:
+        out = torch.empty((max(n_replicas, 1), len(pcts) + 2), dtype=torch.int64, device=traces.device)[:n_replicas]
+    if workspace is None:
+        workspace = _workspace(workspace_bytes(OP_ITL, total_requests, n_replicas, 0), traces.device)
+    _check(lib().asr_sched_itl_batched(_ptr(traces), _ptr(replicas), n_replicas, _ptr(cms), n_cms, total_requests,
+                                       max_slots, pcts.ctypes.data, len(pcts), _ptr(out), _ptr(workspace),
+                                       workspace.numel(), _stream()), "asr_sched_itl_batched")
+    return out
 
 
 def tpot(trace, n: int, cm: np.ndarray, lat, ttft, out=None):

@@ -36,7 +36,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
-    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel"};
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel"};
 struct TimedLaunch {
     int kid;
     cudaEvent_t start, stop;
@@ -91,6 +91,23 @@ static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summ
     w.defer_bytes = align_up(sizeof(int32_t) * (size_t)(2 * n_replicas + 64));   // [0], [1]: counters, [64..]: the two lists
     w.lat_bytes = summary_only ? align_up(sizeof(int64_t) * (size_t)total_requests) : 0;
     w.total = w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + 2 * w.lat_bytes;
+    return w;
+}
+
+// asr_sched_itl_batched: the summary-only simulate workspace + second bitmap + zeroed extension
+// descriptors + gap histogram + (duration, weight) pairs + pair counts
+struct ItlWorkspace {
+    size_t sim_bytes, ext_bytes, hist_bytes, pairs_bytes, np_bytes, total;
+};
+static ItlWorkspace itl_ws(int64_t total_requests, int64_t n_replicas) {
+    ItlWorkspace w;
+    const SimWorkspace s = sim_ws(total_requests, n_replicas, true);
+    w.sim_bytes = s.total + s.bitmap_bytes;
+    w.ext_bytes = align_up(sizeof(asr_sim_ext_t) * 4096);   // n_cms <= 4096 for this call
+    w.hist_bytes = align_up(sizeof(unsigned long long) * (size_t)ITL_BINS * (size_t)n_replicas);
+    w.pairs_bytes = align_up(sizeof(int64_t) * 2 * (size_t)(total_requests + 1));
+    w.np_bytes = align_up(sizeof(int32_t) * (size_t)(n_replicas + 1));
+    w.total = w.sim_bytes + w.ext_bytes + w.hist_bytes + w.pairs_bytes + w.np_bytes;
     return w;
 }
 
@@ -178,6 +195,7 @@ extern "C" size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, in
         case ASR_OP_SIMULATE: return sim_ws(a, b, c != 0).total + 512;   // + descriptors of the single-replica call
         case ASR_OP_SIMULATE_EX: return sim_ws(a, b, c != 0).total + sim_ws(a, b, c != 0).bitmap_bytes;
         case ASR_OP_PERCENTILES: return 0;
+        case ASR_OP_ITL: return itl_ws(a, b).total;
     }
     return 0;
 }
@@ -284,10 +302,78 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
     a.exts = exts;
     a.bitmap2 = bitmap2;
     a.out_preempt = out_preempt;
+    a.itl_hist = nullptr;
+    a.itl_pairs = nullptr;
+    a.itl_npairs = nullptr;
     rc = launch_simulate_ex(a, max_slots, st);
     if (rc) return rc;
     if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
     return rc;
+}
+
+extern "C" int asr_sched_itl_batched(const asr_req_t *traces, const asr_replica_t *replicas, int32_t n_replicas,
+                                     const asr_cost_model_t *cms, int32_t n_cms, int64_t total_requests,
+                                     int32_t max_slots, const int32_t *pcts, int32_t n_pct, int64_t *out,
+                                     void *workspace, size_t workspace_bytes, void *stream) {
+    if (n_replicas < 0 || n_cms < 1 || total_requests < 0 || max_slots < 1 || n_pct < 0 || (n_pct > 0 && !pcts)) {
+        set_error("itl_batched: bad argument (n_replicas=%d n_cms=%d total=%lld max_slots=%d n_pct=%d)", n_replicas,
+                  n_cms, (long long)total_requests, max_slots, n_pct);
+        return ASR_EINVAL;
+    }
+    if (max_slots > 256 || n_pct > 8 || n_cms > 4096) {
+        set_error("itl_batched: limit exceeded (max_slots=%d n_pct=%d n_cms=%d)", max_slots, n_pct, n_cms);
+        return ASR_EUNSUPPORTED;
+    }
+    ItlPcts pl;
+    pl.n_pct = n_pct;
+    for (int j = 0; j < 8; ++j) {
+        pl.pct[j] = j < n_pct ? pcts[j] : 0;
+        if (j < n_pct && (pcts[j] < 1 || pcts[j] > 100)) {
+            set_error("itl_batched: percentile %d out of 1..100", pcts[j]);
+            return ASR_EINVAL;
+        }
+    }
+    if (n_replicas == 0) return ASR_OK;
+    if (!replicas || !cms || !out || (!traces && total_requests > 0)) {
+        set_error("itl_batched: null pointer");
+        return ASR_EINVAL;
+    }
+    const ItlWorkspace iw = itl_ws(total_requests, n_replicas);
+    if (!workspace || workspace_bytes < iw.total) {
+        set_error("itl_batched: workspace too small (%zu < %zu)", workspace_bytes, iw.total);
+        return ASR_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const SimWorkspace w = sim_ws(total_requests, n_replicas, true);
+    char *ws = (char *)workspace;
+    int64_t *bm_off = (int64_t *)ws;
+    uint32_t *bitmap = (uint32_t *)(ws + w.bm_off_bytes);
+    int32_t *defer = (int32_t *)(ws + w.bm_off_bytes + w.bitmap_bytes);
+    int64_t *lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes);
+    int64_t *ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + w.lat_bytes);
+    uint32_t *bitmap2 = (uint32_t *)(ws + w.total);
+    char *extra = ws + iw.sim_bytes;
+    asr_sim_ext_t *exts = (asr_sim_ext_t *)extra;
+    unsigned long long *hist = (unsigned long long *)(extra + iw.ext_bytes);
+    int64_t *pairs = (int64_t *)(extra + iw.ext_bytes + iw.hist_bytes);
+    int32_t *npairs = (int32_t *)(extra + iw.ext_bytes + iw.hist_bytes + iw.pairs_bytes);
+    CUDA_TRY(cudaMemsetAsync(extra, 0, iw.ext_bytes + iw.hist_bytes, st), "itl_batched: memset");
+    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
+    if (rc) return rc;
+    SimExArgs a;
+    static_cast<SimArgs &>(a) = SimArgs{traces, replicas, cms,     bm_off,         bitmap,     defer + 64, defer,
+                                        defer + 64 + n_replicas, defer + 1,
+                                        lat,    ttft,     nullptr, total_requests, n_replicas, n_cms, 0,
+                                        g_opt_escalate.load()};
+    a.exts = exts;
+    a.bitmap2 = bitmap2;
+    a.out_preempt = nullptr;
+    a.itl_hist = hist;
+    a.itl_pairs = pairs;
+    a.itl_npairs = npairs;
+    rc = launch_simulate_ex(a, max_slots, st);
+    if (rc) return rc;
+    return launch_itl_percentiles(a, pl, out, st);
 }
 
 extern "C" int asr_sched_tpot(const asr_req_t *trace, int64_t n, const asr_cost_model_t *cm, const int64_t *lat,

@@ -31,7 +31,18 @@ struct SimExArgs : SimArgs {
     const asr_sim_ext_t *exts;   // [n_cms]
     uint32_t *bitmap2;           // second bitmap: requests that had a first token
     int64_t *out_preempt;        // [n_replicas] nullable
+    // inter-token latency capture (nullable): per replica ITL_BINS weights of the plain iterations, indexed by
+    // |running|, and (duration, weight) pairs of the iterations that admitted somebody, at 2*out_off
+    unsigned long long *itl_hist;
+    int64_t *itl_pairs;
+    int32_t *itl_npairs;
 };
+constexpr int ITL_BINS = 257;
+struct ItlPcts {
+    int32_t n_pct;
+    int32_t pct[8];
+};
+int launch_itl_percentiles(const SimExArgs &a, const ItlPcts &pl, int64_t *out, cudaStream_t st);
 int launch_simulate_ex(const SimExArgs &a, int max_slots, cudaStream_t st);
 int launch_tpot(const asr_req_t *trace, int64_t n, asr_cost_model_t cm, const int64_t *lat, const int64_t *ttft,
                 int64_t *out, cudaStream_t st);

@@ -49,6 +49,7 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
             if (lane == 0) {
                 flag_invalid(a, r);
                 if (a.out_preempt) a.out_preempt[r] = 0;
+                if (a.itl_npairs) a.itl_npairs[r] = -1;
             }
             return;
         }
@@ -73,7 +74,7 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
         rmem[s] = 0;
     }
     int64_t t = 0, M = 0, n_pre = 0;
-    int p = 0, lo = 0, nW = 0, nR = 0, done = 0, bm_hi = 0;
+    int p = 0, lo = 0, nW = 0, nR = 0, done = 0, bm_hi = 0, n_pairs = 0;
     bool blocked = false, bad = false;
     const int64_t first_arrival = n > 0 ? trace[0].arrival_us : 0;
 
@@ -249,6 +250,7 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
         if (bad) break;
         // ---- 4. one engine iteration with the encoders of the admitted ...
         const int64_t c = cm.iter_base_us + cm.iter_per_running_us * (int64_t)nR;
+        const int64_t t0 = t;
         int64_t t1 = t + c;
         if (k > 0) {
             const int64_t dur_sum = warp_sum_u32(dur_sum_part);
@@ -280,6 +282,24 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
             }
         }
         t = t1 + (j - 1) * c;
+        if (a.itl_hist) {
+            // inter-token gaps: this step's first iteration lasted t1 - t0 for the
+            // requests that were already running; the j-1 fast-forwarded ones cost c for everybody
+            const int already = nR - k;
+            if (k > 0) {
+                if (already > 0) {
+                    if (lane == 0) {
+                        a.itl_pairs[2 * (rep.out_off + n_pairs)] = t1 - t0;
+                        a.itl_pairs[2 * (rep.out_off + n_pairs) + 1] = already;
+                    }
+                    ++n_pairs;
+                }
+            } else if (lane == 0) {
+                a.itl_hist[(int64_t)r * ITL_BINS + nR] += (unsigned long long)nR;
+            }
+            if (j > 1 && lane == 0)
+                a.itl_hist[(int64_t)r * ITL_BINS + nR] += (unsigned long long)(j - 1) * (unsigned long long)nR;
+        }
         // ---- 5. tokens, memory, completions
         M += j * (int64_t)nR;
         int fin = 0;
@@ -319,6 +339,7 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
             s->n_done = done;
         }
         if (a.out_preempt) a.out_preempt[r] = n_pre;
+        if (a.itl_npairs) a.itl_npairs[r] = bad ? -1 : n_pairs;
     }
 }
 

@@ -167,3 +167,26 @@ def test_estimator(asr):
     asr.estimate(d, 3, [5000])
     torch.cuda.synchronize()
     assert list(d.cpu().numpy().view(asr.REQ_DTYPE)["est"]) == [40, 20, 10]
+
+
+def test_inter_token_latency(asr):
+    """weighted nearest-rank percentiles, count and sum of the gap multiset"""
+    import torch
+    traces = [wl.stress_trace("lognormal", 900, 41, rate_per_s=24.0), wl.burst_trace(),
+              wl.stress_trace("uniform", 700, 42, rate_per_s=3.0), orc.make_trace([0], [0]),
+              orc.make_trace([0, 500], [3000, 2000])]
+    reps = [(t, p, s) for t in range(5) for p in POL for s in (2, 16)] + [(0, orc.SJF, 100), (1, orc.HRRN, 256)]
+    offs = np.concatenate([[0], np.cumsum([len(t) for t in traces])]).astype(np.int64)
+    ns = np.array([len(traces[t]) for t, _, _ in reps], dtype=np.int64)
+    out_off = np.concatenate([[0], np.cumsum(ns)]).astype(np.int64)
+    rep = asr.make_replicas([offs[t] for t, _, _ in reps], out_off[:-1], ns, [p for _, p, _ in reps],
+                            [s for _, _, s in reps], 0)
+    for cost in (wl.CONFIG_COST, (700, 0, 1000, 0, 0, 1), wl.MEDIUM_COST):
+        pcts = [1, 25, 50, 90, 99, 100]
+        got = asr.itl_batched(dev_trace(np.concatenate(traces)), asr.to_device(rep), len(reps),
+                              asr.to_device(asr.make_cost(*cost)), 1, int(out_off[-1]), 256, pcts)
+        torch.cuda.synchronize()
+        got = got.cpu().numpy()
+        for i, (t, pol, slots) in enumerate(reps):
+            p, cnt, sm = orc.itl(traces[t], pol, orc.cost(*cost), slots, pcts)
+            assert list(got[i]) == p + [cnt, sm], "ITL mismatch rep %d cost %r: %r != %r" % (i, cost, list(got[i]), p + [cnt, sm])
