@@ -330,18 +330,35 @@ __device__ __forceinline__ uint32_t lane_tokens_small(int32_t tok_base, uint32_t
     return lane_tokens((int64_t)tok_base, (int64_t)tok_per_s, dur_ms);
 }
 
-// insert (it + tokens, idx) into the sorted ring of nR entries starting at `head`;
-// an entry is one 64-bit word (finish iteration, request index)
-__device__ __forceinline__ void lane_insert(uint2 *ring, int head, int nR, uint32_t it, uint32_t tokens,
+// The ring is addressed with 32-bit shared-memory byte addresses: `sbase` is the thread's
+// column, `hoff` the byte offset of the head entry (a multiple of RING_STEP below RING_BYTES).
+constexpr uint32_t RING_STEP = LANE_THREADS * 8;            // one ring position, all threads
+constexpr uint32_t RING_MASK = LANE_CAP * RING_STEP - 1;    // 16 KB ring per CTA
+
+__device__ __forceinline__ uint2 ring_ld(uint32_t addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void ring_st(uint32_t addr, uint2 v) {
+    asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(addr), "r"(v.x), "r"(v.y));
+}
+
+// insert (it + tokens, payload) into the sorted ring of nR entries starting at the head;
+// an entry is one 64-bit word (finish iteration, payload)
+__device__ __forceinline__ void lane_insert(uint32_t sbase, uint32_t hoff, int nR, uint32_t it, uint32_t tokens,
                                             uint32_t payload) {
+    uint32_t off = (hoff + (uint32_t)nR * RING_STEP) & RING_MASK;   // first free position
     int h = nR;
     while (h > 0) {
-        const uint2 e = ring[((head + h - 1) & (LANE_CAP - 1)) * LANE_THREADS];
+        const uint32_t prev = (off - RING_STEP) & RING_MASK;
+        const uint2 e = ring_ld(sbase + prev);
         if (e.x - it <= tokens) break;
-        ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = e;
+        ring_st(sbase + off, e);
+        off = prev;
         --h;
     }
-    ring[((head + h) & (LANE_CAP - 1)) * LANE_THREADS] = make_uint2(it + tokens, payload);
+    ring_st(sbase + off, make_uint2(it + tokens, payload));
 }
 
 // TTFT of request idx (requests are admitted in index order here)
@@ -423,7 +440,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             rep.n = 0;
         }
     }
-    uint2 *ring = s_ring + threadIdx.x;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_ring) + threadIdx.x * 8u;
     const int n = rep.n, slots = rep.slots, policy = rep.policy;
     const asr_cost_model_t *cmp = a.cms + rep.cm_id;
     const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
@@ -450,7 +467,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     int64_t t = 0;     // the current iteration boundary
     int64_t tb = 0;    // FREE: start of the current busy period (arrival of its first request)
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
-    int head = 0;      // running set = ring positions head .. head+nR-1, sorted by finish iteration
+    uint32_t hoff = 0;   // running set = nR ring positions from byte offset hoff, sorted by finish iteration
     uint32_t it = 0;   // engine iterations so far, mod 2^32
     // look-ahead window over the trace: records p and p+1 are in registers (one 128-bit
     // load each: the memory pipeline is paid per lane and access, not per byte)
@@ -493,7 +510,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             bool more = nR > 0;
             const int64_t a_eff = nW > 0 ? INT64_MIN : arr0;   // somebody waiting: admit at the first free slot
             while (more) {
-                const uint2 e = ring[head * LANE_THREADS];   // sorted: the head finishes first
+                const uint2 e = ring_ld(sbase + hoff);   // sorted: the head finishes first
                 const uint32_t f = e.x;
                 const uint32_t m = f - it;
                 const uint32_t c = ib + ip * (uint32_t)nR;
@@ -513,7 +530,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                         atomicAdd(reinterpret_cast<unsigned long long *>(lat + (int32_t)e.y),
                                   (unsigned long long)t);
                     }
-                    head = (head + 1) & (LANE_CAP - 1);
+                    hoff = (hoff + RING_STEP) & RING_MASK;
                     --nR;
                     ++done;
                     more = nR > 0;
@@ -570,7 +587,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 int64_t t1 = t + (int64_t)(ib + ip * (uint32_t)(nR + k));
                 if (k == 1 && lo == p - 1) {
                     // the request ingested last: everything needed is in registers
-                    lane_insert(ring, head, nR, it, lane_tokens_small(tok_base, tok_per_s, last_dur),
+                    lane_insert(sbase, hoff, nR, it, lane_tokens_small(tok_base, tok_per_s, last_dur),
                                 FREE ? (uint32_t)last_arr : (uint32_t)lo);
                     t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
                     // first token (S9)
@@ -580,7 +597,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     int64_t dur_sum = 0;
                     for (int q = 0; q < k; ++q) {
                         const Rec rq = ld_cached(trace + lo + q);
-                        lane_insert(ring, head, nR + q, it, lane_tokens_small(tok_base, tok_per_s, rq.dur_ms),
+                        lane_insert(sbase, hoff, nR + q, it, lane_tokens_small(tok_base, tok_per_s, rq.dur_ms),
                                     FREE ? (uint32_t)rq.arrival_us : (uint32_t)(lo + q));
                         dur_sum += (int64_t)rq.dur_ms;
                     }
