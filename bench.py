@@ -509,8 +509,8 @@ def run_ours(args):
         h2d = specs.nbytes + tables_h.nbytes + cost_h.nbytes + pol_h.nbytes
         e2e = {"value": world * total * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(out_h.nbytes), "steps": e2e_steps,
-               "call": "asr_sched_sweep_host (host specs/tables in, host summaries out; device scratch "
-                       "allocated inside the call)"}
+               "call": "asr_sched_sweep_host (host specs/tables in, host summaries out; device scratch from the "
+                       "stream-ordered pool inside the call, cached between calls)"}
         # select with host records: pinned host keys in, host indices out
         try:
             h_keys = torch.empty(nq * ql * 16, dtype=torch.uint8, pin_memory=True)

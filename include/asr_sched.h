@@ -291,6 +291,11 @@ int asr_sched_sweep_host(const asr_trace_spec_t *specs, int32_t n_traces,
                          const int32_t *policies, int32_t n_policies, int32_t slots,
                          const asr_cost_model_t *cm, asr_summary_t *out_summary);
 
+/* The two *_host calls take their device scratch from the device's default
+ * stream-ordered memory pool and leave it cached there for the next call;
+ * asr_sched_trim_scratch synchronises the device and returns it to the driver. */
+int asr_sched_trim_scratch(void);
+
 /* asr_sched_select_batched with HOST keys / out_idx (q_count, now_per_queue
  * not supported: pass full queues). */
 int asr_sched_select_host(const asr_req_t *keys, int32_t n_queues, int32_t q_len,

@@ -34,7 +34,7 @@ EXPORTS = (
     "asr_sched_select", "asr_sched_select_batched", "asr_sched_simulate", "asr_sched_simulate_batched",
     "asr_sched_percentiles", "asr_sched_gen_trace", "asr_sched_gen_trace_batched", "asr_sched_gen_queues",
     "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_simulate_batched_ex", "asr_sched_tpot",
-    "asr_sched_estimate", "asr_sched_itl_batched", "asr_sched_workspace_bytes", "asr_sched_last_error",
+    "asr_sched_estimate", "asr_sched_itl_batched", "asr_sched_trim_scratch", "asr_sched_workspace_bytes", "asr_sched_last_error",
     "asr_sched_version", "asr_sched_launch_count", "asr_sched_timing_enable", "asr_sched_timing_reset",
     "asr_sched_timing_read", "asr_sched_kernel_name", "asr_sched_set_option",
 )
@@ -75,7 +75,7 @@ def lib():
         L.asr_sched_tpot.argtypes = [vp, i64, vp, vp, vp, vp, vp]
         L.asr_sched_estimate.argtypes = [vp, i64, vp, i32, vp, vp, vp]
         L.asr_sched_itl_batched.argtypes = [vp, vp, i32, vp, i32, i64, i32, vp, i32, vp, vp, sz, vp]
-        for name in EXPORTS[:14]:
+        for name in EXPORTS[:15]:
             getattr(L, name).restype = C.c_int
         L.asr_sched_workspace_bytes.argtypes = [i32, i64, i64, i64]
         L.asr_sched_workspace_bytes.restype = sz
@@ -374,6 +374,10 @@ def sweep_host(specs, n_per_trace: int, tables, policies, slots: int, cm, out_su
                                       policies.ctypes.data, policies.shape[0], slots, cm.ctypes.data,
                                       _host_ptr(out_summary)), "asr_sched_sweep_host")
     return out_summary
+
+
+def trim_scratch():
+    _check(lib().asr_sched_trim_scratch(), "asr_sched_trim_scratch")
 
 
 def select_host(keys, n_queues: int, q_len: int, policy: int, now: int, k: int, out_idx=None):

@@ -507,12 +507,33 @@ extern "C" int asr_sched_gen_queues(uint64_t seed, int64_t first, int64_t n, int
 // synchronous HOST-buffer entry points
 // ---------------------------------------------------------------------------
 namespace {
+// Device scratch of the synchronous host-buffer calls: stream-ordered allocations from the
+// device's default memory pool, whose release threshold is raised once so that the pool keeps
+// the memory between calls (a sweep needs ~26 GB of scratch; cudaMalloc/cudaFree of that much
+// cost more than the kernels).  asr_sched_trim_scratch() gives it back.
+static void keep_pool_memory() {
+    static std::atomic<bool> done{false};
+    if (done.exchange(true)) return;
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        uint64_t thr = UINT64_MAX;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    cudaGetLastError();
+}
+
 struct DevBuf {
     void *p = nullptr;
+    cudaStream_t st = nullptr;
     ~DevBuf() {
-        if (p) cudaFree(p);
+        if (p) cudaFreeAsync(p, st);
     }
-    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 1); }
+    cudaError_t alloc(size_t bytes, cudaStream_t stream = nullptr) {
+        keep_pool_memory();
+        st = stream;
+        return cudaMallocAsync(&p, bytes ? bytes : 1, st);
+    }
 };
 
 __global__ void build_sweep_replicas_kernel(asr_replica_t *rep, int32_t n_traces, int64_t n_per_trace,
@@ -584,6 +605,16 @@ extern "C" int asr_sched_sweep_host(const asr_trace_spec_t *specs, int32_t n_tra
     CUDA_TRY(cudaMemcpyAsync(out_summary, d_sum.p, sizeof(asr_summary_t) * (size_t)n_rep, cudaMemcpyDeviceToHost, st),
              "sweep_host: D2H summaries");
     CUDA_TRY(cudaStreamSynchronize(st), "sweep_host: synchronize");
+    return ASR_OK;
+}
+
+extern "C" int asr_sched_trim_scratch(void) {
+    int dev = 0;
+    cudaMemPool_t pool;
+    CUDA_TRY(cudaGetDevice(&dev), "trim_scratch: cudaGetDevice");
+    CUDA_TRY(cudaDeviceSynchronize(), "trim_scratch: synchronize");
+    CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, dev), "trim_scratch: default pool");
+    CUDA_TRY(cudaMemPoolTrimTo(pool, 0), "trim_scratch: trim");
     return ASR_OK;
 }
 
