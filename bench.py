@@ -483,11 +483,13 @@ def run_ours(args):
                                          "frac": a / hbm_peak, "traffic": consts.get("gen_trace_dram_bytes_per_launch"),
                                          "algorithmic_bytes_per_launch": n_traces * n * 16, "avg_launch_ms": gen_avg}
     if pct_avg:
-        a = 2 * total * 8 / (pct_avg / 1e3) / 1e9
+        # summary-only sweeps hand the reduction uint32 values (the lane kernel proves < 2^32 us): 4 B per value
+        pct_bytes = 2 * total * 4
+        a = pct_bytes / (pct_avg / 1e3) / 1e9
         rooflines["summary_percentiles_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
                                                    "frac": a / hbm_peak,
                                                    "traffic": consts.get("summary_percentiles_dram_bytes_per_launch"),
-                                                   "algorithmic_bytes_per_launch": 2 * total * 8,
+                                                   "algorithmic_bytes_per_launch": pct_bytes,
                                                    "avg_launch_ms": pct_avg}
     dominant = max(stage_ms, key=lambda k_: stage_ms[k_] or 0.0)
     roofline = dict(rooflines.get(dominant, {}), kernel=dominant,

@@ -247,7 +247,8 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
     rc = launch_simulate(a, max_slots, use_lane, st);
     if (rc) return rc;
-    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
+    if (out_summary)
+        rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, use_lane && summary_only, st);
     return rc;
 }
 
@@ -307,7 +308,7 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
     a.itl_npairs = nullptr;
     rc = launch_simulate_ex(a, max_slots, st);
     if (rc) return rc;
-    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, st);
+    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, false, st);
     return rc;
 }
 

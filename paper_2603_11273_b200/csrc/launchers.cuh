@@ -56,8 +56,11 @@ int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_
                        cudaStream_t st);
 int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg, const int32_t *pcts,
                        int32_t n_pct, int64_t *out, cudaStream_t st);
+// fmt_flags: the lane kernel ran in order-free mode and left ASR_FMT32 / 0 in p50_e2e_us and p50_ttft_us of
+// every valid replica (ASR_FMT32: the replica's values are uint32 in the first half of its region)
+constexpr int64_t ASR_FMT32 = INT64_MIN + 32;
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
-                               const int64_t *ttft, asr_summary_t *out_summary, cudaStream_t st);
+                               const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, cudaStream_t st);
 int launch_gen_trace(const asr_trace_spec_t *specs, asr_trace_spec_t one, int32_t n_traces, int64_t n_per_trace,
                      const asr_tables_t *tables, asr_req_t *out, cudaStream_t st);
 int launch_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now, const asr_tables_t *tables,

@@ -51,7 +51,8 @@ __device__ __forceinline__ int64_t block_reduce_minmax(int64_t v, bool is_min, i
 
 // All threads of the CTA call this; results[j] valid on every thread afterwards.
 __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, const PctList &pl,
-                                    int64_t *results, int64_t *smem_vals) {
+                                    int64_t *results, int64_t *smem_vals, bool is32 = false) {
+    const uint32_t *v32 = reinterpret_cast<const uint32_t *>(v);   // is32: N uint32 values at the same address
     __shared__ uint32_t hist[256];
     __shared__ int64_t scratch[PCT_THREADS / 32];
     __shared__ uint32_t sel_digit, sel_below;
@@ -63,7 +64,7 @@ __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, co
     const bool staged = smem_vals != nullptr && N <= PCT_SMEM_VALUES;
     int64_t mn = INT64_MAX, mx = INT64_MIN;
     for (int64_t i = threadIdx.x; i < N; i += PCT_THREADS) {
-        int64_t x = v[i];
+        int64_t x = is32 ? (int64_t)v32[i] : v[i];
         if (staged) smem_vals[i] = x;
         mn = x < mn ? x : mn;
         mx = x > mx ? x : mx;
@@ -85,7 +86,7 @@ __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, co
                 hist[threadIdx.x] = 0;   // PCT_THREADS == 256
                 __syncthreads();
                 for (int64_t i = threadIdx.x; i < N; i += PCT_THREADS) {
-                    uint64_t key = (uint64_t)src[i] - (uint64_t)mn;
+                    uint64_t key = (uint64_t)((is32 && !staged) ? (int64_t)v32[i] : src[i]) - (uint64_t)mn;
                     if (shift + 8 >= 64 || (key >> (shift + 8)) == prefix)
                         atomicAdd(&hist[(key >> shift) & 255u], 1u);
                 }
@@ -226,23 +227,33 @@ __device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], i
 }
 
 // Returns false (nothing written) when the segment does not qualify.
-template <int MAXT>
+template <int MAXT, bool IS32>
 __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restrict__ v, int64_t N64, const PctList &pl,
                                         int64_t *results, PctRegSmem &sm) {
     if (N64 <= 0 || N64 > PCT_REG_MAX) return false;
     const int N = (int)N64;
     const int lane = lane_id(), warp = threadIdx.x >> 5;
     uint32_t key[PCT_VPT];
-    const uint32_t hi0 = (uint32_t)((uint64_t)__ldg(reinterpret_cast<const long long *>(v)) >> 32);
-    uint32_t hi_diff = 0, or_all = 0;
+    uint32_t hi0 = 0, hi_diff = 0, or_all = 0;
+    if (IS32) {   // N uint32 values (the lane kernel's order-free format): no high words to compare
+        const uint32_t *v32 = reinterpret_cast<const uint32_t *>(v);
 #pragma unroll
-    for (int j = 0; j < PCT_VPT; ++j) {
-        const int i = j * PCT_THREADS + threadIdx.x;
-        uint64_t x = (uint64_t)hi0 << 32;
-        if (i < N) x = (uint64_t)__ldcs(reinterpret_cast<const long long *>(v + i));   // read once: streaming
-        key[j] = (uint32_t)x;
-        hi_diff |= (uint32_t)(x >> 32) ^ hi0;
-        or_all |= (uint32_t)x;
+        for (int j = 0; j < PCT_VPT; ++j) {
+            const int i = j * PCT_THREADS + threadIdx.x;
+            key[j] = i < N ? __ldcs(v32 + i) : 0u;
+            or_all |= key[j];
+        }
+    } else {
+        hi0 = (uint32_t)((uint64_t)__ldg(reinterpret_cast<const long long *>(v)) >> 32);
+#pragma unroll
+        for (int j = 0; j < PCT_VPT; ++j) {
+            const int i = j * PCT_THREADS + threadIdx.x;
+            uint64_t x = (uint64_t)hi0 << 32;
+            if (i < N) x = (uint64_t)__ldcs(reinterpret_cast<const long long *>(v + i));   // read once: streaming
+            key[j] = (uint32_t)x;
+            hi_diff |= (uint32_t)(x >> 32) ^ hi0;
+            or_all |= (uint32_t)x;
+        }
     }
     if (__syncthreads_or(hi_diff != 0u)) return false;
     or_all = __reduce_or_sync(ASR_FULL_MASK, or_all);
@@ -435,7 +446,7 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) percentiles_kernel(const int64
     for (int s = blockIdx.x; s < n_seg; s += gridDim.x) {
         const int64_t b = seg_off[s], e = seg_off[s + 1];
         int64_t res[PCT_MAX];
-        if (!segment_percentiles_reg<PCT_MAX>(values + b, e - b, pl, res, sm))
+        if (!segment_percentiles_reg<PCT_MAX, false>(values + b, e - b, pl, res, sm))
             segment_percentiles(values + b, e - b, pl, res, nullptr);
         if (threadIdx.x == 0)
             for (int j = 0; j < pl.n_pct; ++j) out[(int64_t)s * pl.n_pct + j] = res[j];
@@ -446,7 +457,7 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) percentiles_kernel(const int64
 __global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(const asr_replica_t *replicas,
                                                                           int32_t n_replicas, const int64_t *lat,
                                                                           const int64_t *ttft,
-                                                                          asr_summary_t *out_summary) {
+                                                                          asr_summary_t *out_summary, bool fmt_flags) {
     extern __shared__ __align__(16) unsigned char dyn_smem[];
     PctRegSmem &sm = *reinterpret_cast<PctRegSmem *>(dyn_smem);
     PctList pl;
@@ -457,8 +468,10 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(con
     for (int r = blockIdx.x; r < n_replicas; r += gridDim.x) {
         if (threadIdx.x == 0 && r + (int)gridDim.x < n_replicas) {
             // pull the CTA's next segment into L2 while this one is being processed
-            const asr_replica_t nx = replicas[r + gridDim.x];
-            const int64_t bytes = (int64_t)nx.n * 8;
+            const int rn = r + gridDim.x;
+            const asr_replica_t nx = replicas[rn];
+            const int64_t flag = blockIdx.y == 0 ? out_summary[rn].p50_e2e_us : out_summary[rn].p50_ttft_us;
+            const int64_t bytes = (int64_t)nx.n * ((fmt_flags && flag == ASR_FMT32) ? 4 : 8);
             if (nx.n > 0 && nx.out_off >= 0 && bytes <= (int64_t)PCT_REG_MAX * 8) {
                 const char *src = reinterpret_cast<const char *>(vals + nx.out_off);
                 const uint32_t sz = (uint32_t)(bytes & ~15ll);
@@ -467,10 +480,15 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(con
             }
         }
         if (out_summary[r].n_done < 0) continue;   // invalid descriptor, flagged by the simulator
+        // order-free runs of the lane kernel leave the element format in the field this CTA fills in
+        const int64_t flag = blockIdx.y == 0 ? out_summary[r].p50_e2e_us : out_summary[r].p50_ttft_us;
+        const bool is32 = fmt_flags && flag == ASR_FMT32;
         const asr_replica_t rep = replicas[r];
         int64_t res[PCT_MAX];
-        if (!segment_percentiles_reg<2>(vals + rep.out_off, rep.n, pl, res, sm))
-            segment_percentiles(vals + rep.out_off, rep.n, pl, res, nullptr);
+        bool ok;
+        if (is32) ok = segment_percentiles_reg<2, true>(vals + rep.out_off, rep.n, pl, res, sm);
+        else ok = segment_percentiles_reg<2, false>(vals + rep.out_off, rep.n, pl, res, sm);
+        if (!ok) segment_percentiles(vals + rep.out_off, rep.n, pl, res, nullptr, is32);
         if (threadIdx.x == 0) {
             if (blockIdx.y == 0) {
                 out_summary[r].p50_e2e_us = res[0];
@@ -520,7 +538,7 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
 }
 
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
-                               const int64_t *ttft, asr_summary_t *out_summary, cudaStream_t st) {
+                               const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, cudaStream_t st) {
     if (n_replicas <= 0) return ASR_OK;
     static bool attr = false;
     if (!attr) {
@@ -533,7 +551,8 @@ int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas
     dim3 grid(gx, 2);
     {
         KernelTimer kt(KID_SUMMARY_PCT, st);
-        summary_percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary);
+        summary_percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary,
+                                                                            fmt_flags);
     }
     return check_launch("summary_percentiles_kernel");
 }

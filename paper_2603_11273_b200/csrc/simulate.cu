@@ -381,36 +381,36 @@ __device__ __forceinline__ void lane_push_ttft(int64_t *ttft, int idx, int64_t v
 
 // Order-free outputs (summary-only calls: the per-request arrays live in the workspace and
 // only feed the percentile reduction, which does not care about their order).  Values
-// known to be below 2^32 are staged in four registers and written as one aligned 32-byte
-// sector of zero-extended int64; `ph` is the element phase of base[0] within its sector.
+// known to be below 2^32 are staged in four registers and written as one aligned 16-byte
+// store of four uint32 into the FIRST HALF of the replica's int64 region; the replica's
+// summary carries ASR_FMT32 in its percentile fields so that the reduction reads that
+// format.  `ph` is the element phase of base[0] within its 16-byte line.
 struct Stage32 {
     uint32_t v0, v1, v2, v3;
 };
 
-__device__ __forceinline__ void stage_push(int64_t *base, int ph, int pos, uint32_t v, Stage32 &s) {
+__device__ __forceinline__ void stage_push(uint32_t *base, int ph, int pos, uint32_t v, Stage32 &s) {
     s.v0 = s.v1;
     s.v1 = s.v2;
     s.v2 = s.v3;
     s.v3 = v;
     if (((ph + pos) & 3) == 3) {
         if (pos >= 3) {
-            ulonglong2 *dst = reinterpret_cast<ulonglong2 *>(base + pos - 3);
-            dst[0] = make_ulonglong2(s.v0, s.v1);
-            dst[1] = make_ulonglong2(s.v2, s.v3);
-        } else {   // short head before the first sector boundary
-            if (pos >= 2) base[pos - 2] = (int64_t)s.v1;
-            if (pos >= 1) base[pos - 1] = (int64_t)s.v2;
-            base[pos] = (int64_t)s.v3;
+            *reinterpret_cast<uint4 *>(base + pos - 3) = make_uint4(s.v0, s.v1, s.v2, s.v3);
+        } else {   // short head before the first 16-byte boundary
+            if (pos >= 2) base[pos - 2] = s.v1;
+            if (pos >= 1) base[pos - 1] = s.v2;
+            base[pos] = s.v3;
         }
     }
 }
 
-__device__ __forceinline__ void stage_tail(int64_t *base, int ph, int n, const Stage32 &s) {
+__device__ __forceinline__ void stage_tail(uint32_t *base, int ph, int n, const Stage32 &s) {
     int cnt = (ph + n) & 3;
     cnt = cnt < n ? cnt : n;
-    if (cnt >= 3) base[n - 3] = (int64_t)s.v1;
-    if (cnt >= 2) base[n - 2] = (int64_t)s.v2;
-    if (cnt >= 1) base[n - 1] = (int64_t)s.v3;
+    if (cnt >= 3) base[n - 3] = s.v1;
+    if (cnt >= 2) base[n - 2] = s.v2;
+    if (cnt >= 1) base[n - 1] = s.v3;
 }
 
 // FREE = order-free outputs: the ring carries the low word of the arrival time instead of
@@ -493,8 +493,9 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     const bool staged = (reinterpret_cast<uintptr_t>(ttft) & 15u) == 0;
     // FREE: both outputs through Stage32
     Stage32 sq_t = {0, 0, 0, 0}, sq_l = {0, 0, 0, 0};
-    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft) >> 3) & 3u);
-    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat) >> 3) & 3u);
+    uint32_t *ttft32 = reinterpret_cast<uint32_t *>(ttft), *lat32 = reinterpret_cast<uint32_t *>(lat);
+    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft) >> 2) & 3u);
+    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat) >> 2) & 3u);
     const int64_t first_arrival = n > 0 ? arr0 : 0;
     if (n == 0) live = false;
 
@@ -523,7 +524,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                         it = f;
                     }
                     if (FREE) {
-                        stage_push(lat, ph_l, done, (uint32_t)t - e.y, sq_l);   // E2E = t - arrival
+                        stage_push(lat32, ph_l, done, (uint32_t)t - e.y, sq_l);   // E2E = t - arrival
                     } else {
                         // lat[i] holds -arrival (sim_init_lat_kernel); a fire-and-forget reduction
                         // adds the completion time, so no load sits on the critical path
@@ -591,7 +592,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                                 FREE ? (uint32_t)last_arr : (uint32_t)lo);
                     t1 += (int64_t)enc_per * (int64_t)last_dur + (int64_t)enc_base;
                     // first token (S9)
-                    if (FREE) stage_push(ttft, ph_t, lo, (uint32_t)t1 - (uint32_t)last_arr, sq_t);
+                    if (FREE) stage_push(ttft32, ph_t, lo, (uint32_t)t1 - (uint32_t)last_arr, sq_t);
                     else lane_push_ttft(ttft, lo, t1 - last_arr, staged, st0, st1, st2, st3);
                 } else {
                     int64_t dur_sum = 0;
@@ -604,7 +605,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                     t1 += (int64_t)enc_base * (int64_t)k + (int64_t)enc_per * dur_sum;
                     for (int q = 0; q < k; ++q) {
                         const int64_t arr = ld_arrival(trace + lo + q);
-                        if (FREE) stage_push(ttft, ph_t, lo + q, (uint32_t)t1 - (uint32_t)arr, sq_t);
+                        if (FREE) stage_push(ttft32, ph_t, lo + q, (uint32_t)t1 - (uint32_t)arr, sq_t);
                         else lane_push_ttft(ttft, lo + q, t1 - arr, staged, st0, st1, st2, st3);
                     }
                 }
@@ -619,11 +620,19 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     if (deferred) {
         const int pos = atomicAdd(a.defer_count, 1);
         a.defer_list[pos] = r;
+        if (FREE && a.out_summary) {   // the warp kernel will write int64 values
+            a.out_summary[r].p50_e2e_us = 0;
+            a.out_summary[r].p50_ttft_us = 0;
+        }
         return;
     }
     if (valid && FREE) {
-        stage_tail(ttft, ph_t, n, sq_t);
-        stage_tail(lat, ph_l, n, sq_l);
+        stage_tail(ttft32, ph_t, n, sq_t);
+        stage_tail(lat32, ph_l, n, sq_l);
+        if (a.out_summary) {
+            a.out_summary[r].p50_e2e_us = ASR_FMT32;
+            a.out_summary[r].p50_ttft_us = ASR_FMT32;
+        }
     }
     if (valid && !FREE && staged) {   // requests n - (n & 3) .. n-1 are still in st(4 - tail) .. st3
         const int tail = n & 3;
