@@ -132,3 +132,16 @@ def test_lane_kernel_hand_overs(asr):
         for i, (t, p, s) in enumerate(reps):
             check_replica(traces[t], p, s, cost, L[i], T[i], S[i], "cost=%r rep %d" % (cost, i))
         assert np.array_equal(S.view(np.uint8), S2.view(np.uint8))
+
+
+def test_summary_only_long_segments_and_odd_offsets(asr):
+    """summary-only calls keep the per-request values in the workspace (uint32, any order, on the
+    thread-per-replica path): segments beyond the register-resident percentile path (> 10,240
+    values), odd lengths and offsets, light and heavy load, every policy"""
+    traces = [wl.stress_trace("lognormal", 12345, 51, rate_per_s=3.0), wl.stress_trace("uniform", 10241, 52, rate_per_s=1.0),
+              wl.stress_trace("lognormal", 4099, 53, rate_per_s=21.0), wl.stress_trace("six", 3, 54, rate_per_s=1.0),
+              wl.stress_trace("lognormal", 10239, 55, rate_per_s=0.5)]
+    reps = [(t, p, s) for t in range(5) for p in POL for s in (7, 32)]
+    _, _, S = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    for i, (t, p, s) in enumerate(reps):
+        check_replica(traces[t], p, s, wl.CONFIG_COST, None, None, S[i], "rep %d" % i)
