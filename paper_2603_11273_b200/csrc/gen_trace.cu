@@ -50,52 +50,125 @@ __device__ __forceinline__ void st_rec(asr_req_t *p, int64_t arr, int32_t dur) {
     *reinterpret_cast<int4 *>(p) = v;
 }
 
-// one CTA per trace; 256 records per step, running int64 carry
+// One CTA per aligned block of GEN_GROUP consecutive specs, cut into runs of equal (seed, dist).  The draws of
+// record i depend on (seed, i) only (common random numbers: the traces of one seed at different rates are
+// time-scaled copies), so a run hashes and interpolates each record ONCE and every trace of the run only
+// scales the unit exponential by its own mean gap, scans and stores.  A thread owns GEN_RPT consecutive
+// records of a GEN_CHUNK-record step: local prefix in registers, one warp scan of the thread totals per
+// trace, one pass of warp 0 over the [trace][warp] totals that also carries the running sum.
+constexpr int GEN_RPT = 4;
+constexpr int GEN_CHUNK = GEN_THREADS * GEN_RPT;
+constexpr int GEN_GROUP = 8;
+constexpr int GEN_WARPS = GEN_THREADS / 32;
+static_assert(GEN_GROUP * GEN_WARPS == 64, "warp 0 folds the [trace][warp] totals two per lane");
+
+// (e * mean_gap) >> 32 for e < 2^38 (clz <= 63 times a 32-bit ln 2, plus a 32-bit table value), mean_gap < 2^30
+__device__ __forceinline__ uint64_t scale_gap(uint64_t e, uint32_t mean_gap) {
+    return (uint64_t)(uint32_t)(e >> 32) * mean_gap + __umulhi((uint32_t)e, mean_gap);
+}
+
 __global__ void __launch_bounds__(GEN_THREADS) gen_trace_kernel(const asr_trace_spec_t *specs, asr_trace_spec_t one,
                                                                 int32_t n_traces, int64_t n_per_trace,
                                                                 const asr_tables_t *tables, asr_req_t *out) {
-    __shared__ int64_t warp_tot[GEN_THREADS / 32];
+    __shared__ int64_t warp_tot[GEN_GROUP][GEN_WARPS];   // per trace: the warps' gap sums of this step
+    __shared__ int64_t warp_off[GEN_GROUP][GEN_WARPS];   // per trace: arrival before the warp's first record
+    __shared__ uint64_t s_seed[GEN_GROUP];
+    __shared__ int32_t s_dist[GEN_GROUP];
+    __shared__ uint32_t s_gap[GEN_GROUP];                // mean gap in us, 0: trace skipped (rate_mhz < 1)
     const int lane = lane_id(), warp = threadIdx.x >> 5;
-    for (int tr = blockIdx.x; tr < n_traces; tr += gridDim.x) {
-        const asr_trace_spec_t sp = specs ? specs[tr] : one;
-        asr_req_t *dst = out + (int64_t)tr * n_per_trace;
-        if (sp.rate_mhz < 1) continue;
-        const uint64_t mean_gap = 1000000000ull / (uint64_t)sp.rate_mhz;
-        const uint64_t ln2_q32 = tables->exp_t[4096];
-        const uint64_t b0 = stream_base(sp.seed, 0), b1 = stream_base(sp.seed, 1), b2 = stream_base(sp.seed, 2);
-        int64_t carry = 0;
-        for (int64_t base = 0; base < n_per_trace; base += GEN_THREADS) {
-            const int64_t i = base + threadIdx.x;
-            int64_t gap = 0;
-            int32_t dur = 0;
-            if (i < n_per_trace) {
-                const uint64_t u0 = draw(b0, (uint64_t)i), u1 = draw(b1, (uint64_t)i), u2 = draw(b2, (uint64_t)i);
-                const uint64_t e = (uint64_t)__clzll((long long)(u0 | 1ull)) * ln2_q32 +
-                                   table_interp(tables->exp_t, u1);
-                gap = (int64_t)((__umul64hi(e, mean_gap) << 32) | ((e * mean_gap) >> 32));
-                dur = draw_dur(u2, sp.dist, tables->ln_dur);
-            }
-            // inclusive block scan of the gaps
-            int64_t x = gap;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                int64_t y = shfl64(x, lane >= d ? lane - d : lane);
-                if (lane >= d) x += y;
-            }
-            __syncthreads();
-            if (lane == 31) warp_tot[warp] = x;
-            __syncthreads();
-            int64_t before = 0, total = 0;
-#pragma unroll
-            for (int w = 0; w < GEN_THREADS / 32; ++w) {
-                const int64_t wt = warp_tot[w];
-                if (w < warp) before += wt;
-                total += wt;
-            }
-            if (i < n_per_trace) st_rec(dst + i, carry + before + x, dur);
-            carry += total;
+    const uint64_t ln2_q32 = tables->exp_t[4096];
+    const int n_units = (n_traces + GEN_GROUP - 1) / GEN_GROUP;
+    for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+        const int t_first = unit * GEN_GROUP;
+        const int cnt = n_traces - t_first < GEN_GROUP ? n_traces - t_first : GEN_GROUP;
+        __syncthreads();
+        if ((int)threadIdx.x < cnt) {
+            const asr_trace_spec_t sp = specs ? specs[t_first + threadIdx.x] : one;
+            s_seed[threadIdx.x] = sp.seed;
+            s_dist[threadIdx.x] = sp.dist;
+            s_gap[threadIdx.x] = sp.rate_mhz < 1 ? 0u : (uint32_t)(1000000000u / (uint32_t)sp.rate_mhz);
         }
         __syncthreads();
+        for (int r0 = 0; r0 < cnt;) {
+            const uint64_t seed = s_seed[r0];
+            const int dist = s_dist[r0];
+            int m = 1;
+            while (r0 + m < cnt && s_seed[r0 + m] == seed && s_dist[r0 + m] == dist) ++m;
+            const uint64_t b0 = stream_base(seed, 0), b1 = stream_base(seed, 1), b2 = stream_base(seed, 2);
+            asr_req_t *dst = out + (int64_t)(t_first + r0) * n_per_trace;
+            // warp 0, lanes 0-7 of each 8-lane segment: running arrival of traces (lane>>3) and (lane>>3)+4
+            int64_t carry_a = 0, carry_b = 0;
+            for (int64_t base = 0; base < n_per_trace; base += GEN_CHUNK) {
+                const int64_t i0 = base + (int64_t)threadIdx.x * GEN_RPT;
+                uint64_t e[GEN_RPT];
+                int32_t dur[GEN_RPT];
+#pragma unroll
+                for (int j = 0; j < GEN_RPT; ++j) {
+                    const uint64_t i = (uint64_t)(i0 + j);
+                    e[j] = 0;
+                    dur[j] = 0;
+                    if (i0 + j < n_per_trace) {
+                        const uint64_t u0 = draw(b0, i), u1 = draw(b1, i), u2 = draw(b2, i);
+                        e[j] = (uint64_t)__clzll((long long)(u0 | 1ull)) * ln2_q32 + table_interp(tables->exp_t, u1);
+                        dur[j] = draw_dur(u2, dist, tables->ln_dur);
+                    }
+                }
+                int64_t excl[GEN_GROUP];   // per trace: gap sum of the warp's lower lanes
+#pragma unroll
+                for (int g = 0; g < GEN_GROUP; ++g) {
+                    excl[g] = 0;
+                    if (g < m) {
+                        const uint32_t mg = s_gap[r0 + g];
+                        int64_t tot = 0;
+#pragma unroll
+                        for (int j = 0; j < GEN_RPT; ++j) tot += (int64_t)scale_gap(e[j], mg);
+                        int64_t x = tot;
+#pragma unroll
+                        for (int d = 1; d < 32; d <<= 1) {
+                            const int64_t y = shfl64(x, lane >= d ? lane - d : lane);
+                            if (lane >= d) x += y;
+                        }
+                        excl[g] = x - tot;
+                        if (lane == 31) warp_tot[g][warp] = x;
+                    }
+                }
+                __syncthreads();
+                if (warp == 0) {
+                    const int ga = lane >> 3, w = lane & 7;
+                    int64_t ta = ga < m ? warp_tot[ga][w] : 0, tb = ga + 4 < m ? warp_tot[ga + 4][w] : 0;
+                    int64_t xa = ta, xb = tb;
+#pragma unroll
+                    for (int d = 1; d < 8; d <<= 1) {
+                        const int64_t ya = shfl64(xa, w >= d ? lane - d : lane), yb = shfl64(xb, w >= d ? lane - d : lane);
+                        if (w >= d) {
+                            xa += ya;
+                            xb += yb;
+                        }
+                    }
+                    if (ga < m) warp_off[ga][w] = carry_a + xa - ta;
+                    if (ga + 4 < m) warp_off[ga + 4][w] = carry_b + xb - tb;
+                    carry_a += shfl64(xa, lane | 7);
+                    carry_b += shfl64(xb, lane | 7);
+                }
+                __syncthreads();
+#pragma unroll
+                for (int g = 0; g < GEN_GROUP; ++g) {
+                    if (g < m) {
+                        const uint32_t mg = s_gap[r0 + g];
+                        if (mg != 0u) {
+                            asr_req_t *d = dst + (int64_t)g * n_per_trace + i0;
+                            int64_t arr = warp_off[g][warp] + excl[g];
+#pragma unroll
+                            for (int j = 0; j < GEN_RPT; ++j) {
+                                arr += (int64_t)scale_gap(e[j], mg);
+                                if (i0 + j < n_per_trace) st_rec(d + j, arr, dur[j]);
+                            }
+                        }
+                    }
+                }
+            }
+            r0 += m;
+        }
     }
 }
 
@@ -114,7 +187,8 @@ __global__ void __launch_bounds__(GEN_THREADS) gen_queues_kernel(uint64_t seed, 
 int launch_gen_trace(const asr_trace_spec_t *specs, asr_trace_spec_t one, int32_t n_traces, int64_t n_per_trace,
                      const asr_tables_t *tables, asr_req_t *out, cudaStream_t st) {
     if (n_traces <= 0 || n_per_trace <= 0) return ASR_OK;
-    int grid = n_traces < 148 * 64 ? n_traces : 148 * 64;
+    const int n_units = (n_traces + GEN_GROUP - 1) / GEN_GROUP;
+    int grid = n_units < 148 * 64 ? n_units : 148 * 64;
     {
         KernelTimer kt(KID_GEN_TRACE, st);
         gen_trace_kernel<<<grid, GEN_THREADS, 0, st>>>(specs, one, n_traces, n_per_trace, tables, out);

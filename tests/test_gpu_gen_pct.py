@@ -45,6 +45,31 @@ def test_gen_trace_batched_matches_oracle(asr, tables):
         assert np.array_equal(got[t].view(np.uint8), ref.view(np.uint8)), t
 
 
+def test_gen_trace_batched_irregular_runs(asr, tables):
+    """specs that do not fall into aligned blocks of eight rates per seed: runs of equal (seed, dist) of
+    every length, the same seed under both distributions, repeated rates, a partial last block, and record
+    counts around the generator's 1,024-record step"""
+    import torch
+    d_tab = asr.tables_to_device(*tables)
+    rng = np.random.default_rng(11)
+    seeds, rates, dist = [], [], []
+    for run_len in (1, 3, 2, 8, 5, 9, 1, 1, 7, 4, 2):
+        sd, ds = int(rng.integers(0, 2**63)), int(rng.integers(0, 2))
+        for _ in range(run_len):
+            seeds.append(sd); dist.append(ds); rates.append(int(rng.integers(1, 40000)))
+    seeds += [5, 5, 5, 5]; dist += [0, 1, 0, 1]; rates += [777, 777, 777, 1000000]
+    assert len(seeds) % 8 != 0
+    for n in (1, 1023, 1024, 1025, 2500):
+        specs = np.zeros(len(seeds), dtype=asr.SPEC_DTYPE)
+        specs["seed"], specs["rate_mhz"], specs["dist"] = seeds, rates, dist
+        out = asr.gen_trace_batched(asr.to_device(specs), len(specs), n, d_tab)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().view(asr.REQ_DTYPE).reshape(len(specs), n)
+        for t in range(len(specs)):
+            ref = orc.gen_trace(seeds[t], rates[t], dist[t], n, *tables)
+            assert np.array_equal(got[t].view(np.uint8), ref.view(np.uint8)), (n, t)
+
+
 def test_percentiles_match_oracle(asr):
     import torch
     rng = np.random.default_rng(2)
