@@ -38,6 +38,7 @@ constexpr int POOL_CAP = 2048;
 constexpr int POOL_EPT = POOL_CAP / CTA_T;
 constexpr int POOL_TARGET = 1024;      // strong members wanted from a rebuild
 constexpr int HIST_BINS = 2048;
+constexpr int KSEL_SMALL = 32;         // up to this many admissions the k-th scalar is found by extraction
 constexpr int64_t H_MAX = 1ll << 36;   // (2^38 + 2^36) * 2^24 < 2^63
 
 struct CtaSmem {
@@ -47,6 +48,7 @@ struct CtaSmem {
     int4 wbest[CTA_T / 32];    // per-warp winners of the fallback scan
     uint32_t hist[HIST_BINS];
     int32_t rep[HIST_BINS];    // one trace position per histogram bin
+    uint64_t wsel[CTA_T / 32][KSEL_SMALL];   // small k: every warp's k smallest order scalars, ascending
     uint16_t tie[POOL_CAP];
     uint16_t hole[CTA_T], surv[CTA_T];
     int64_t red64[CTA_T / 32];
@@ -115,6 +117,30 @@ __device__ __forceinline__ int4 cand_of(const asr_req_t *trace, int pos) {
 // the bitmap is updated with atomics (performed in L2): read it past L1
 __device__ __forceinline__ bool is_admitted(const uint32_t *bm, int pos) { return (__ldcg(bm + (pos >> 5)) >> (pos & 31)) & 1u; }
 
+// Visit every waiting request of the window [lo, p): f(candidate record).  One CTA walks a window of up to
+// 10^6 positions out of L2, so the loop is bound by load latency: SCAN_U bitmap words and SCAN_U records per
+// thread are requested before the first one is looked at (the record load does not wait for its bitmap word).
+constexpr int SCAN_U = 8;
+template <class F>
+__device__ __forceinline__ void scan_waiting(const asr_req_t *trace, const uint32_t *bm, int lo, int p, F &&f) {
+    for (int base = lo + (int)threadIdx.x; base < p; base += CTA_T * SCAN_U) {
+        int4 v[SCAN_U];
+        uint32_t w[SCAN_U];
+#pragma unroll
+        for (int u = 0; u < SCAN_U; ++u) {
+            const int pos = base + u * CTA_T;
+            const bool in = pos < p;
+            w[u] = in ? __ldcg(bm + (pos >> 5)) : 0xFFFFFFFFu;
+            v[u] = in ? __ldg(reinterpret_cast<const int4 *>(trace + pos)) : make_int4(0, 0, 0, 0);
+        }
+#pragma unroll
+        for (int u = 0; u < SCAN_U; ++u) {
+            const int pos = base + u * CTA_T;
+            if (!((w[u] >> (pos & 31)) & 1u)) f(make_int4(v[u].x, v[u].y, v[u].w < 1 ? 1 : v[u].w, pos));
+        }
+    }
+}
+
 // approximate 32-bit key of a waiting request, smaller = better; only used to pick a threshold
 __device__ __forceinline__ int32_t approx_key(int policy, const int4 &e, int64_t t0) {
     if (policy == ASR_SJF) return e.z;
@@ -173,8 +199,7 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
     if (tid == 0) sm.pool_n = 0;
     __syncthreads();
     if (nW <= POOL_CAP) {
-        for (int pos = lo + tid; pos < p; pos += CTA_T)
-            if (!is_admitted(bm, pos)) sm.pool[atomicAdd(&sm.pool_n, 1)] = cand_of(trace, pos);
+        scan_waiting(trace, bm, lo, p, [&](const int4 &e) { sm.pool[atomicAdd(&sm.pool_n, 1)] = e; });
         __syncthreads();
         ps.P = sm.pool_n;
         ps.complete = true;
@@ -182,12 +207,11 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
     }
     // --- threshold mode: pick theta with a histogram over the approximate key
     int kmin = 0x7FFFFFFF, kmax = 0;
-    for (int pos = lo + tid; pos < p; pos += CTA_T)
-        if (!is_admitted(bm, pos)) {
-            const int key = approx_key(policy, cand_of(trace, pos), t);
-            kmin = key < kmin ? key : kmin;
-            kmax = key > kmax ? key : kmax;
-        }
+    scan_waiting(trace, bm, lo, p, [&](const int4 &e) {
+        const int key = approx_key(policy, e, t);
+        kmin = key < kmin ? key : kmin;
+        kmax = key > kmax ? key : kmax;
+    });
     const int64_t lo_k0 = block_min(kmin, sm), hi_k0 = block_max(kmax, sm);
     int target = POOL_TARGET;
   for (int attempt = 0; attempt < 4; ++attempt) {
@@ -201,15 +225,14 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
             sm.rep[b] = -1;
         }
         __syncthreads();
-        for (int pos = lo + tid; pos < p; pos += CTA_T)
-            if (!is_admitted(bm, pos)) {
-                const int64_t key = approx_key(policy, cand_of(trace, pos), t);
-                if (key >= lo_k && key <= hi_k) {
-                    const int b = (int)((key - lo_k) / width);
-                    atomicAdd(&sm.hist[b], 1u);
-                    sm.rep[b] = pos;
-                }
+        scan_waiting(trace, bm, lo, p, [&](const int4 &e) {
+            const int64_t key = approx_key(policy, e, t);
+            if (key >= lo_k && key <= hi_k) {
+                const int b = (int)((uint32_t)(key - lo_k) / (uint32_t)width);   // keys are 32-bit: so is the range
+                atomicAdd(&sm.hist[b], 1u);
+                sm.rep[b] = e.w;
             }
+        });
         __syncthreads();
         if (tid == 0) {
             // smallest bin b with base_above + cum(b) >= target
@@ -251,17 +274,15 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
         if (tid == 0) sm.pool_n = 0;
         __syncthreads();
         int strong = 0;
-        for (int pos = lo + tid; pos < p; pos += CTA_T)
-            if (!is_admitted(bm, pos)) {
-                const int4 e = cand_of(trace, pos);
-                if (pool_pass(policy, ps, e)) {
-                    const int at = atomicAdd(&sm.pool_n, 1);
-                    if (at < POOL_CAP) sm.pool[at] = e;
-                    if (policy == ASR_HRRN &&
-                        mul64x32(t - rec_arr(e), (uint32_t)ps.thrE) >= mul64x32(ps.thrW, (uint32_t)e.z))
-                        strong++;
-                }
+        scan_waiting(trace, bm, lo, p, [&](const int4 &e) {
+            if (pool_pass(policy, ps, e)) {
+                const int at = atomicAdd(&sm.pool_n, 1);
+                if (at < POOL_CAP) sm.pool[at] = e;
+                if (policy == ASR_HRRN &&
+                    mul64x32(t - rec_arr(e), (uint32_t)ps.thrE) >= mul64x32(ps.thrW, (uint32_t)e.z))
+                    strong++;
             }
+        });
         strong = block_sum(strong, sm);
         const int cnt = sm.pool_n;
         if (cnt <= POOL_CAP) {
@@ -283,6 +304,64 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
     }
     if (target < 1) return;
   }
+}
+
+// minimum of a 64-bit unsigned value over the warp: two 32-bit REDUX steps
+__device__ __forceinline__ uint64_t warp_min_u64(uint64_t x) {
+    const uint32_t hi = (uint32_t)(x >> 32);
+    const uint32_t mh = __reduce_min_sync(ASR_FULL_MASK, hi);
+    const uint32_t ml = __reduce_min_sync(ASR_FULL_MASK, hi == mh ? (uint32_t)x : 0xFFFFFFFFu);
+    return ((uint64_t)mh << 32) | ml;
+}
+
+// The k-th smallest order scalar (with multiplicity) of the pool for k <= KSEL_SMALL < P, without a single
+// pivot: a steady-state step admits a handful of requests out of a pool of one or two thousand, where a
+// random-pivot quickselect spends ~2 ln P block-wide rounds.  Every warp extracts the k smallest of its 256
+// scalars (k rounds of a warp minimum; only the lane that held it looks for its next one), then warp 0 merges
+// the eight ascending lists k steps deep.  Scalars are >= 0, so they compare as unsigned; empty slots hold
+// INT64_MAX, which no valid scalar exceeds, and the pool has more than k members.
+__device__ __forceinline__ int64_t kth_scalar_small(CtaSmem &sm, const int64_t (&Kr)[POOL_EPT], int k) {
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    uint32_t taken = 0;
+    uint64_t mine = ~0ull;
+#pragma unroll
+    for (int e = 0; e < POOL_EPT; ++e) mine = (uint64_t)Kr[e] < mine ? (uint64_t)Kr[e] : mine;
+    for (int r = 0; r < k; ++r) {
+        const uint64_t wm = warp_min_u64(mine);
+        if (lane == 0) sm.wsel[warp][r] = wm;
+        const int who = __ffs(__ballot_sync(ASR_FULL_MASK, mine == wm)) - 1;
+        if (lane == who) {
+            bool found = false;
+            mine = ~0ull;
+#pragma unroll
+            for (int e = 0; e < POOL_EPT; ++e) {
+                const bool free_e = !((taken >> e) & 1u);
+                if (free_e && !found && (uint64_t)Kr[e] == wm) {
+                    taken |= 1u << e;
+                    found = true;
+                } else if (free_e) {
+                    mine = (uint64_t)Kr[e] < mine ? (uint64_t)Kr[e] : mine;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    if (warp == 0) {
+        int h = 0;
+        uint64_t cur = lane < CTA_T / 32 ? sm.wsel[lane][0] : ~0ull;
+        uint64_t wm = 0;
+        for (int r = 0; r < k; ++r) {
+            wm = warp_min_u64(cur);
+            const int who = __ffs(__ballot_sync(ASR_FULL_MASK, cur == wm)) - 1;
+            if (lane == who) {
+                ++h;
+                cur = h < k ? sm.wsel[lane][h] : ~0ull;
+            }
+        }
+        if (lane == 0) sm.bc64 = (int64_t)wm;
+    }
+    __syncthreads();
+    return sm.bc64;
 }
 
 // ---- exact k-set of the pool -> sm.adm[0..k), members removed from the pool ----------------
@@ -311,6 +390,16 @@ __device__ __forceinline__ void pool_select(CtaSmem &sm, PoolState &ps, int poli
         int64_t Klo = 0, Khi = 0, v = 0;
         bool lo_inf = true, hi_inf = true;
         int cl = 0, ce = 0;
+        if (k <= KSEL_SMALL) {
+            v = kth_scalar_small(sm, Kr, k);
+            int c = 0;
+#pragma unroll
+            for (int e = 0; e < POOL_EPT; ++e)
+                if (e * CTA_T + tid < P) c += (Kr[e] < v ? 1 : 0) + (Kr[e] <= v ? 0x10000 : 0);
+            c = block_sum(c, sm);
+            cl = c & 0xFFFF;
+            ce = c >> 16;
+        } else
         for (;;) {
             int64_t pv = 0;
             bool ok = false;
