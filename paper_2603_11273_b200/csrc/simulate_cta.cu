@@ -320,30 +320,38 @@ __device__ __forceinline__ uint64_t warp_min_u64(uint64_t x) {
 // scalars (k rounds of a warp minimum; only the lane that held it looks for its next one), then warp 0 merges
 // the eight ascending lists k steps deep.  Scalars are >= 0, so they compare as unsigned; empty slots hold
 // INT64_MAX, which no valid scalar exceeds, and the pool has more than k members.
+__device__ __forceinline__ void cmp_swap_u64(uint64_t &a, uint64_t &b) {
+    const bool sw = b < a;
+    const uint64_t lo = sw ? b : a, hi = sw ? a : b;
+    a = lo;
+    b = hi;
+}
+
 __device__ __forceinline__ int64_t kth_scalar_small(CtaSmem &sm, const int64_t (&Kr)[POOL_EPT], int k) {
+    static_assert(POOL_EPT == 8, "the sorting network below is the 19-exchange network for 8 keys");
     const int lane = lane_id(), warp = threadIdx.x >> 5;
-    uint32_t taken = 0;
-    uint64_t mine = ~0ull;
-#pragma unroll
-    for (int e = 0; e < POOL_EPT; ++e) mine = (uint64_t)Kr[e] < mine ? (uint64_t)Kr[e] : mine;
+    // the lane's 8 scalars ascending, so that the lane a minimum came from only shifts its list
+    uint64_t s0 = (uint64_t)Kr[0], s1 = (uint64_t)Kr[1], s2 = (uint64_t)Kr[2], s3 = (uint64_t)Kr[3],
+             s4 = (uint64_t)Kr[4], s5 = (uint64_t)Kr[5], s6 = (uint64_t)Kr[6], s7 = (uint64_t)Kr[7];
+    cmp_swap_u64(s0, s1); cmp_swap_u64(s2, s3); cmp_swap_u64(s4, s5); cmp_swap_u64(s6, s7);
+    cmp_swap_u64(s0, s2); cmp_swap_u64(s1, s3); cmp_swap_u64(s4, s6); cmp_swap_u64(s5, s7);
+    cmp_swap_u64(s1, s2); cmp_swap_u64(s5, s6); cmp_swap_u64(s0, s4); cmp_swap_u64(s3, s7);
+    cmp_swap_u64(s1, s5); cmp_swap_u64(s2, s6);
+    cmp_swap_u64(s1, s4); cmp_swap_u64(s3, s6);
+    cmp_swap_u64(s2, s4); cmp_swap_u64(s3, s5);
+    cmp_swap_u64(s3, s4);
     for (int r = 0; r < k; ++r) {
-        const uint64_t wm = warp_min_u64(mine);
+        const uint64_t wm = warp_min_u64(s0);
         if (lane == 0) sm.wsel[warp][r] = wm;
-        const int who = __ffs(__ballot_sync(ASR_FULL_MASK, mine == wm)) - 1;
-        if (lane == who) {
-            bool found = false;
-            mine = ~0ull;
-#pragma unroll
-            for (int e = 0; e < POOL_EPT; ++e) {
-                const bool free_e = !((taken >> e) & 1u);
-                if (free_e && !found && (uint64_t)Kr[e] == wm) {
-                    taken |= 1u << e;
-                    found = true;
-                } else if (free_e) {
-                    mine = (uint64_t)Kr[e] < mine ? (uint64_t)Kr[e] : mine;
-                }
-            }
-        }
+        const bool me = lane == __ffs(__ballot_sync(ASR_FULL_MASK, s0 == wm)) - 1;
+        s0 = me ? s1 : s0;
+        s1 = me ? s2 : s1;
+        s2 = me ? s3 : s2;
+        s3 = me ? s4 : s3;
+        s4 = me ? s5 : s4;
+        s5 = me ? s6 : s5;
+        s6 = me ? s7 : s6;
+        s7 = me ? ~0ull : s7;
     }
     __syncthreads();
     if (warp == 0) {
