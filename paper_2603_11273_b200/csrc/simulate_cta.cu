@@ -30,13 +30,16 @@
 // filled by the exact integer tests).  If no pool can be built (massive ties)
 // the step falls back to an exact block-wide arg-best scan of the window.
 #include "sim_common.cuh"
+#ifdef CTA_STATS
+#include <cstdio>
+#endif
 
 namespace asr {
 
 constexpr int CTA_T = 256;
 constexpr int POOL_CAP = 2048;
 constexpr int POOL_EPT = POOL_CAP / CTA_T;
-constexpr int POOL_TARGET = 1024;      // strong members wanted from a rebuild
+constexpr int POOL_TARGET = 768;       // strong members wanted from a rebuild
 constexpr int HIST_BINS = 2048;
 constexpr int KSEL_SMALL = 32;         // up to this many admissions the k-th scalar is found by extraction
 constexpr int64_t H_MAX = 1ll << 36;   // (2^38 + 2^36) * 2^24 < 2^63
@@ -121,8 +124,16 @@ __device__ __forceinline__ bool is_admitted(const uint32_t *bm, int pos) { retur
 // 10^6 positions out of L2, so the loop is bound by load latency: SCAN_U bitmap words and SCAN_U records per
 // thread are requested before the first one is looked at (the record load does not wait for its bitmap word).
 constexpr int SCAN_U = 8;
+#ifdef CTA_STATS
+__device__ unsigned long long g_stat[8];
+#define STAT(i, v) do { if (threadIdx.x == 0) g_stat[i] += (v); } while (0)
+#else
+#define STAT(i, v) do { } while (0)
+#endif
 template <class F>
 __device__ __forceinline__ void scan_waiting(const asr_req_t *trace, const uint32_t *bm, int lo, int p, F &&f) {
+    STAT(1, 1);
+    STAT(2, p - lo);
     for (int base = lo + (int)threadIdx.x; base < p; base += CTA_T * SCAN_U) {
         int4 v[SCAN_U];
         uint32_t w[SCAN_U];
@@ -158,6 +169,9 @@ struct PoolState {
     int64_t t0H;       // HRRN: the guarantee holds up to this time
     int64_t t0;
     int64_t H;
+    int G0, P0;        // HRRN: strong members and members right after the build
+    int32_t prev_key;  // approximate key of the last threshold: centre of the next histogram
+    bool prev_valid;
 };
 
 // membership test of the current threshold for a request (threshold mode)
@@ -190,7 +204,22 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
             break;
         }
     }
-    if (policy == ASR_HRRN && ps.thr_valid && t > ps.t0H && ps.G >= k && ps.H < H_MAX) ps.H *= 2;   // horizon ran out first
+    if (policy == ASR_HRRN && ps.thr_valid) {
+        // Horizon from the life of the pool that just lapsed.  Requests cross the threshold at the rate they
+        // are served, so the strong members last  elapsed * target / used  and the weak members a horizon H
+        // lets in grow like  weak0 * H / H0 : cover 1.25 lives, within 0.8 of the room the pool has for them.
+        const float elapsed = (float)(t - ps.t0), used = (float)(ps.G0 - ps.G);
+        const float h0 = (float)(ps.t0H - ps.t0), weak0 = (float)(ps.P0 - ps.G0);
+        float h = (float)ps.H;
+        if (used >= 1.f && elapsed >= 1.f) h = 1.25f * elapsed * (float)POOL_TARGET / used;
+        else if (t > ps.t0H && ps.G >= k) h *= 2.f;   // horizon ran out before anything was learnt
+        if (weak0 >= 1.f && h0 >= 1.f) h = fminf(h, 0.8f * (float)(POOL_CAP - POOL_TARGET) * h0 / weak0);
+        const int64_t hi = (int64_t)fminf(h, (float)H_MAX);
+        ps.H = hi < 1000 ? 1000 : (hi > H_MAX ? H_MAX : hi);
+    }
+    STAT(0, 1);
+    if (policy == ASR_HRRN && ps.thr_valid && t > ps.t0H) STAT(3, 1);
+    if (ps.thr_valid && ps.G < k) STAT(4, 1);
     ps.thr_valid = false;
     ps.complete = false;
     ps.P = 0;
@@ -206,19 +235,31 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
         return;
     }
     // --- threshold mode: pick theta with a histogram over the approximate key
-    int kmin = 0x7FFFFFFF, kmax = 0;
-    scan_waiting(trace, bm, lo, p, [&](const int4 &e) {
-        const int key = approx_key(policy, e, t);
-        kmin = key < kmin ? key : kmin;
-        kmax = key > kmax ? key : kmax;
-    });
-    const int64_t lo_k0 = block_min(kmin, sm), hi_k0 = block_max(kmax, sm);
+    // The threshold moves slowly between rebuilds: the first histogram is centred on the last threshold's key
+    // and also counts what lies above its window; only if the target rank falls outside it does the full
+    // procedure (key range by a scan of its own, then refinement levels) run.
+    int64_t lo_k0 = 0, hi_k0 = -1;
+    bool guess = ps.prev_valid;
     int target = POOL_TARGET;
   for (int attempt = 0; attempt < 4; ++attempt) {
-    int64_t lo_k = lo_k0, hi_k = hi_k0;
+    if (!guess && hi_k0 < lo_k0) {
+        int kmin = 0x7FFFFFFF, kmax = 0;
+        scan_waiting(trace, bm, lo, p, [&](const int4 &e) {
+            const int key = approx_key(policy, e, t);
+            kmin = key < kmin ? key : kmin;
+            kmax = key > kmax ? key : kmax;
+        });
+        lo_k0 = block_min(kmin, sm);
+        hi_k0 = block_max(kmax, sm);
+    }
+    const int64_t guess_w = policy == ASR_SJF ? 1023 : (1 << 18);   // est in ms; 3% of a ratio in float bits
+    int64_t lo_k = guess ? (int64_t)ps.prev_key - guess_w : lo_k0, hi_k = guess ? (int64_t)ps.prev_key + guess_w : hi_k0;
     int base_above = 0;
     int theta_pos = -1;
+    bool guess_failed = false;
     for (int level = 0; level < 4 && theta_pos < 0; ++level) {
+        const bool guess_level = guess && level == 0;
+        int above = 0;
         const int64_t width = (hi_k - lo_k + HIST_BINS) / HIST_BINS;   // >= 1
         for (int b = tid; b < HIST_BINS; b += CTA_T) {
             sm.hist[b] = 0;
@@ -231,8 +272,11 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
                 const int b = (int)((uint32_t)(key - lo_k) / (uint32_t)width);   // keys are 32-bit: so is the range
                 atomicAdd(&sm.hist[b], 1u);
                 sm.rep[b] = e.w;
+            } else if (guess_level && key < lo_k) {
+                above++;
             }
         });
+        if (guess_level) base_above = block_sum(above, sm);
         __syncthreads();
         if (tid == 0) {
             // smallest bin b with base_above + cum(b) >= target
@@ -247,6 +291,7 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
             else if (cum + (int)sm.hist[b] <= POOL_CAP / 2 + POOL_CAP / 4) verdict = sm.rep[b];
             else if (cum >= target / 8 && prev >= 0) verdict = sm.rep[prev];
             else verdict = width > 1 ? -1 : -2;
+            if (guess_level && (base_above >= target || b == HIST_BINS)) verdict = -3;   // outside the window
             sm.bc32[0] = verdict;
             sm.bc32[1] = b;
             sm.bc32[2] = cum;
@@ -258,16 +303,27 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
             base_above = sm.bc32[2];
             lo_k = lo_k + (int64_t)sm.bc32[1] * width;
             hi_k = lo_k + width - 1;
+        } else if (verdict == -3) {
+            guess_failed = true;
+            __syncthreads();
+            break;
         } else {
             __syncthreads();
             return;   // no usable threshold (massive ties): the caller scans the window directly
         }
         __syncthreads();
     }
+    if (guess_failed) {
+        guess = false;
+        --attempt;
+        continue;
+    }
     if (theta_pos < 0) return;
     const int4 th = cand_of(trace, theta_pos);
     ps.thrE = th.z;
     ps.thrW = wait_of(rec_arr(th), t);
+    ps.prev_key = approx_key(policy, th, t);
+    ps.prev_valid = true;
     // --- fill the pool with the exact tests; shrink the horizon until it fits
     for (;;) {
         ps.t0H = t + (policy == ASR_HRRN ? ps.H : 0);
@@ -286,13 +342,21 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
         strong = block_sum(strong, sm);
         const int cnt = sm.pool_n;
         if (cnt <= POOL_CAP) {
-            ps.P = cnt;
-            ps.G = strong;
+            ps.P = ps.P0 = cnt;
+            ps.G = ps.G0 = strong;
             ps.thr_valid = true;
             return;
         }
         if (policy == ASR_HRRN && ps.H > 0) {
-            ps.H = ps.H >= 4096 ? ps.H / 4 : 0;
+            // too many weak members: they grow like the horizon, so aim at 0.8 of the room left by the strong
+            STAT(5, 1);
+            const int weak = cnt - strong;
+            int64_t h = ps.H / 2;
+            if (strong <= POOL_CAP * 3 / 4 && weak > 0) {
+                const int64_t fit = (int64_t)((float)ps.H * 0.8f * (float)(POOL_CAP - strong) / (float)weak);
+                h = fit < h ? fit : h;
+            }
+            ps.H = h >= 1024 ? h : 0;
             continue;
         }
         // theta lets too many through (ties, or a crowded histogram bin): aim lower and pick again
@@ -558,6 +622,9 @@ __device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
     ps.t0H = 0;
     ps.t0 = 0;
     ps.H = 1000000;
+    ps.G0 = ps.P0 = 0;
+    ps.prev_key = 0;
+    ps.prev_valid = false;
     uint32_t seed = 0x9E3779B9u * (uint32_t)(r + 1);
     int cbase = 0;
     int64_t carr = tid < n ? __ldg(reinterpret_cast<const long long *>(trace + tid)) : INT64_MAX;
@@ -694,6 +761,13 @@ __device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
         nR -= nfin;
         done += nfin;
     }
+#ifdef CTA_STATS
+    if (tid == 0) {
+        printf("cta stats: policy %d rebuilds %llu scans %llu positions %llu horizon-out %llu strong-out %llu shrinks %llu H %lld\n",
+               policy, g_stat[0], g_stat[1], g_stat[2], g_stat[3], g_stat[4], g_stat[5], (long long)ps.H);
+        for (int i = 0; i < 8; ++i) g_stat[i] = 0;
+    }
+#endif
     if (a.out_summary && tid == 0) {
         asr_summary_t *s = a.out_summary + r;
         s->first_arrival_us = first_arrival;
