@@ -67,16 +67,129 @@ __device__ __forceinline__ uint64_t scale_gap(uint64_t e, uint32_t mean_gap) {
     return (uint64_t)(uint32_t)(e >> 32) * mean_gap + __umulhi((uint32_t)e, mean_gap);
 }
 
-__global__ void __launch_bounds__(GEN_THREADS) gen_trace_kernel(const asr_trace_spec_t *specs, asr_trace_spec_t one,
-                                                                int32_t n_traces, int64_t n_per_trace,
-                                                                const asr_tables_t *tables, asr_req_t *out) {
-    __shared__ int64_t warp_tot[GEN_GROUP][GEN_WARPS];   // per trace: the warps' gap sums of this step
-    __shared__ int64_t warp_off[GEN_GROUP][GEN_WARPS];   // per trace: arrival before the warp's first record
-    __shared__ uint64_t s_seed[GEN_GROUP];
-    __shared__ int32_t s_dist[GEN_GROUP];
-    __shared__ uint32_t s_gap[GEN_GROUP];                // mean gap in us, 0: trace skipped (rate_mhz < 1)
+// four consecutive records of one thread: two 256-bit stores when the address allows it (sm_100 has them; a
+// 16-byte store per lane at a 64-byte stride would fill every 32-byte sector in two separate requests)
+__device__ __forceinline__ void st_rec4(asr_req_t *p, const int64_t (&arr)[GEN_RPT], const int32_t (&dur)[GEN_RPT],
+                                        bool wide, int n_valid) {
+    static_assert(GEN_RPT == 4, "two 32-byte stores");
+    if (wide && n_valid == GEN_RPT) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint64_t d0 = ((uint64_t)(uint32_t)dur[2 * h] << 32) | (uint32_t)dur[2 * h];   // dur_ms, est = dur_ms
+            const uint64_t d1 = ((uint64_t)(uint32_t)dur[2 * h + 1] << 32) | (uint32_t)dur[2 * h + 1];
+            asm volatile("st.global.v4.b64 [%0], {%1, %2, %3, %4};" ::"l"(p + 2 * h), "l"(arr[2 * h]), "l"(d0),
+                         "l"(arr[2 * h + 1]), "l"(d1)
+                         : "memory");
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < GEN_RPT; ++j)
+            if (j < n_valid) st_rec(p + j, arr[j], dur[j]);
+    }
+}
+
+struct GenSmem {
+    int64_t warp_tot[GEN_GROUP][GEN_WARPS];   // per trace: the warps' gap sums of this step
+    int64_t warp_off[GEN_GROUP][GEN_WARPS];   // per trace: arrival before the warp's first record
+    uint64_t seed[GEN_GROUP];
+    int32_t dist[GEN_GROUP];
+    uint32_t gap[GEN_GROUP];                  // mean gap in us, 0: trace skipped (rate_mhz < 1)
+};
+
+// one run of m traces with equal (seed, dist), first trace r0 of the unit; FULL: m == GEN_GROUP, so that the
+// per-trace blocks carry no branch and the compiler interleaves the eight independent scans
+template <bool FULL>
+__device__ __forceinline__ void gen_run(GenSmem &sm, int r0, int m, int64_t n_per_trace, const asr_tables_t *tables,
+                                        asr_req_t *dst) {
     const int lane = lane_id(), warp = threadIdx.x >> 5;
     const uint64_t ln2_q32 = tables->exp_t[4096];
+    const uint64_t seed = sm.seed[r0];
+    const int dist = sm.dist[r0];
+    const uint64_t b0 = stream_base(seed, 0), b1 = stream_base(seed, 1), b2 = stream_base(seed, 2);
+    const bool wide = (n_per_trace & 1) == 0 && (reinterpret_cast<uintptr_t>(dst) & 31u) == 0;
+    // warp 0, every 8-lane segment: running arrival of traces (lane>>3) and (lane>>3)+4
+    int64_t carry_a = 0, carry_b = 0;
+    for (int64_t base = 0; base < n_per_trace; base += GEN_CHUNK) {
+        const int64_t i0 = base + (int64_t)threadIdx.x * GEN_RPT;
+        const int64_t left = n_per_trace - i0;
+        const int n_valid = left >= GEN_RPT ? GEN_RPT : (left > 0 ? (int)left : 0);
+        uint64_t e[GEN_RPT];
+        int32_t dur[GEN_RPT];
+#pragma unroll
+        for (int j = 0; j < GEN_RPT; ++j) {
+            const uint64_t i = (uint64_t)(i0 + j);
+            e[j] = 0;
+            dur[j] = 0;
+            if (j < n_valid) {
+                const uint64_t u0 = draw(b0, i), u1 = draw(b1, i), u2 = draw(b2, i);
+                e[j] = (uint64_t)__clzll((long long)(u0 | 1ull)) * ln2_q32 + table_interp(tables->exp_t, u1);
+                dur[j] = draw_dur(u2, dist, tables->ln_dur);
+            }
+        }
+        int64_t excl[GEN_GROUP];   // per trace: gap sum of the warp's lower lanes
+#pragma unroll
+        for (int g = 0; g < GEN_GROUP; ++g) {
+            excl[g] = 0;
+            if (FULL || g < m) {
+                const uint32_t mg = sm.gap[r0 + g];
+                int64_t tot = 0;
+#pragma unroll
+                for (int j = 0; j < GEN_RPT; ++j) tot += (int64_t)scale_gap(e[j], mg);
+                int64_t x = tot;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int64_t y = shfl64(x, lane >= d ? lane - d : lane);
+                    if (lane >= d) x += y;
+                }
+                excl[g] = x - tot;
+                if (lane == 31) sm.warp_tot[g][warp] = x;
+            }
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const int ga = lane >> 3, w = lane & 7;
+            int64_t ta = ga < m ? sm.warp_tot[ga][w] : 0, tb = ga + 4 < m ? sm.warp_tot[ga + 4][w] : 0;
+            int64_t xa = ta, xb = tb;
+#pragma unroll
+            for (int d = 1; d < 8; d <<= 1) {
+                const int64_t ya = shfl64(xa, w >= d ? lane - d : lane), yb = shfl64(xb, w >= d ? lane - d : lane);
+                if (w >= d) {
+                    xa += ya;
+                    xb += yb;
+                }
+            }
+            if (ga < m) sm.warp_off[ga][w] = carry_a + xa - ta;
+            if (ga + 4 < m) sm.warp_off[ga + 4][w] = carry_b + xb - tb;
+            carry_a += shfl64(xa, lane | 7);
+            carry_b += shfl64(xb, lane | 7);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int g = 0; g < GEN_GROUP; ++g) {
+            if (FULL || g < m) {
+                const uint32_t mg = sm.gap[r0 + g];
+                if (mg != 0u && n_valid > 0) {
+                    int64_t arr[GEN_RPT];
+                    int64_t run = sm.warp_off[g][warp] + excl[g];
+#pragma unroll
+                    for (int j = 0; j < GEN_RPT; ++j) {
+                        run += (int64_t)scale_gap(e[j], mg);
+                        arr[j] = run;
+                    }
+                    st_rec4(dst + (int64_t)g * n_per_trace + i0, arr, dur, wide, n_valid);
+                }
+            }
+        }
+    }
+}
+
+#ifndef GEN_MIN_CTAS
+#define GEN_MIN_CTAS 4
+#endif
+__global__ void __launch_bounds__(GEN_THREADS, GEN_MIN_CTAS) gen_trace_kernel(const asr_trace_spec_t *specs, asr_trace_spec_t one,
+                                                                int32_t n_traces, int64_t n_per_trace,
+                                                                const asr_tables_t *tables, asr_req_t *out) {
+    __shared__ GenSmem sm;
     const int n_units = (n_traces + GEN_GROUP - 1) / GEN_GROUP;
     for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
         const int t_first = unit * GEN_GROUP;
@@ -84,89 +197,17 @@ __global__ void __launch_bounds__(GEN_THREADS) gen_trace_kernel(const asr_trace_
         __syncthreads();
         if ((int)threadIdx.x < cnt) {
             const asr_trace_spec_t sp = specs ? specs[t_first + threadIdx.x] : one;
-            s_seed[threadIdx.x] = sp.seed;
-            s_dist[threadIdx.x] = sp.dist;
-            s_gap[threadIdx.x] = sp.rate_mhz < 1 ? 0u : (uint32_t)(1000000000u / (uint32_t)sp.rate_mhz);
+            sm.seed[threadIdx.x] = sp.seed;
+            sm.dist[threadIdx.x] = sp.dist;
+            sm.gap[threadIdx.x] = sp.rate_mhz < 1 ? 0u : (uint32_t)(1000000000u / (uint32_t)sp.rate_mhz);
         }
         __syncthreads();
         for (int r0 = 0; r0 < cnt;) {
-            const uint64_t seed = s_seed[r0];
-            const int dist = s_dist[r0];
             int m = 1;
-            while (r0 + m < cnt && s_seed[r0 + m] == seed && s_dist[r0 + m] == dist) ++m;
-            const uint64_t b0 = stream_base(seed, 0), b1 = stream_base(seed, 1), b2 = stream_base(seed, 2);
+            while (r0 + m < cnt && sm.seed[r0 + m] == sm.seed[r0] && sm.dist[r0 + m] == sm.dist[r0]) ++m;
             asr_req_t *dst = out + (int64_t)(t_first + r0) * n_per_trace;
-            // warp 0, lanes 0-7 of each 8-lane segment: running arrival of traces (lane>>3) and (lane>>3)+4
-            int64_t carry_a = 0, carry_b = 0;
-            for (int64_t base = 0; base < n_per_trace; base += GEN_CHUNK) {
-                const int64_t i0 = base + (int64_t)threadIdx.x * GEN_RPT;
-                uint64_t e[GEN_RPT];
-                int32_t dur[GEN_RPT];
-#pragma unroll
-                for (int j = 0; j < GEN_RPT; ++j) {
-                    const uint64_t i = (uint64_t)(i0 + j);
-                    e[j] = 0;
-                    dur[j] = 0;
-                    if (i0 + j < n_per_trace) {
-                        const uint64_t u0 = draw(b0, i), u1 = draw(b1, i), u2 = draw(b2, i);
-                        e[j] = (uint64_t)__clzll((long long)(u0 | 1ull)) * ln2_q32 + table_interp(tables->exp_t, u1);
-                        dur[j] = draw_dur(u2, dist, tables->ln_dur);
-                    }
-                }
-                int64_t excl[GEN_GROUP];   // per trace: gap sum of the warp's lower lanes
-#pragma unroll
-                for (int g = 0; g < GEN_GROUP; ++g) {
-                    excl[g] = 0;
-                    if (g < m) {
-                        const uint32_t mg = s_gap[r0 + g];
-                        int64_t tot = 0;
-#pragma unroll
-                        for (int j = 0; j < GEN_RPT; ++j) tot += (int64_t)scale_gap(e[j], mg);
-                        int64_t x = tot;
-#pragma unroll
-                        for (int d = 1; d < 32; d <<= 1) {
-                            const int64_t y = shfl64(x, lane >= d ? lane - d : lane);
-                            if (lane >= d) x += y;
-                        }
-                        excl[g] = x - tot;
-                        if (lane == 31) warp_tot[g][warp] = x;
-                    }
-                }
-                __syncthreads();
-                if (warp == 0) {
-                    const int ga = lane >> 3, w = lane & 7;
-                    int64_t ta = ga < m ? warp_tot[ga][w] : 0, tb = ga + 4 < m ? warp_tot[ga + 4][w] : 0;
-                    int64_t xa = ta, xb = tb;
-#pragma unroll
-                    for (int d = 1; d < 8; d <<= 1) {
-                        const int64_t ya = shfl64(xa, w >= d ? lane - d : lane), yb = shfl64(xb, w >= d ? lane - d : lane);
-                        if (w >= d) {
-                            xa += ya;
-                            xb += yb;
-                        }
-                    }
-                    if (ga < m) warp_off[ga][w] = carry_a + xa - ta;
-                    if (ga + 4 < m) warp_off[ga + 4][w] = carry_b + xb - tb;
-                    carry_a += shfl64(xa, lane | 7);
-                    carry_b += shfl64(xb, lane | 7);
-                }
-                __syncthreads();
-#pragma unroll
-                for (int g = 0; g < GEN_GROUP; ++g) {
-                    if (g < m) {
-                        const uint32_t mg = s_gap[r0 + g];
-                        if (mg != 0u) {
-                            asr_req_t *d = dst + (int64_t)g * n_per_trace + i0;
-                            int64_t arr = warp_off[g][warp] + excl[g];
-#pragma unroll
-                            for (int j = 0; j < GEN_RPT; ++j) {
-                                arr += (int64_t)scale_gap(e[j], mg);
-                                if (i0 + j < n_per_trace) st_rec(d + j, arr, dur[j]);
-                            }
-                        }
-                    }
-                }
-            }
+            if (m == GEN_GROUP) gen_run<true>(sm, r0, m, n_per_trace, tables, dst);
+            else gen_run<false>(sm, r0, m, n_per_trace, tables, dst);
             r0 += m;
         }
     }
