@@ -153,10 +153,10 @@ struct PctRegSmem {
 };
 
 // One counting pass over the register-resident keys.  Counts digit
-// (key >> new_shift) & (2^width - 1) of every valid key with key >> shift ==
-// prefix (no filter when shift >= 32), then resolves every rank kk[t] of the
-// targets [t0, t1): sel_digit/sel_below/sel_pop.
-__device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], int N, int shift, int new_shift,
+// (key >> new_shift) & (2^width - 1) of every key with key >> shift == prefix
+// (no filter when shift >= 32) among the thread's first nvalid slots, then
+// resolves every rank kk[t] of the targets [t0, t1): sel_digit/sel_below/sel_pop.
+__device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], int nvalid, int shift, int new_shift,
                                                uint32_t prefix, const uint32_t *kk, int t0, int t1,
                                                PctRegSmem &sm) {
     const int lane = lane_id(), warp = threadIdx.x >> 5;
@@ -171,8 +171,7 @@ __device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], i
     unsigned char *mine = &sm.tab[warp][lane];
 #pragma unroll
     for (int j = 0; j < PCT_VPT; ++j) {
-        const int i = j * PCT_THREADS + threadIdx.x;
-        const bool in = i < N && (shift >= 32 || (key[j] >> shift) == prefix);
+        const bool in = j < nvalid && (shift >= 32 || (key[j] >> shift) == prefix);
         if (in) {
             unsigned char *c = mine + ((key[j] >> new_shift) & mask) * PCT_BIN_STRIDE;
             *c = (unsigned char)(*c + 1);
@@ -236,12 +235,21 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
     uint32_t key[PCT_VPT];
     uint32_t hi0 = 0, hi_diff = 0, or_all = 0;
     if (IS32) {   // N uint32 values (the lane kernel's order-free format): no high words to compare
-        const uint32_t *v32 = reinterpret_cast<const uint32_t *>(v);
+        // which slot holds which value is irrelevant to a rank: four consecutive values per 128-bit load;
+        // a segment that is not made of whole aligned quads takes the general path
+        if ((N & 3) != 0 || (reinterpret_cast<uintptr_t>(v) & 15u) != 0) return false;
+        const uint4 *v128 = reinterpret_cast<const uint4 *>(v);
+        const int n4 = N >> 2;
 #pragma unroll
-        for (int j = 0; j < PCT_VPT; ++j) {
-            const int i = j * PCT_THREADS + threadIdx.x;
-            key[j] = i < N ? __ldcs(v32 + i) : 0u;
-            or_all |= key[j];
+        for (int q = 0; q < PCT_VPT / 4; ++q) {
+            const int i = q * PCT_THREADS + threadIdx.x;
+            uint4 x = make_uint4(0u, 0u, 0u, 0u);
+            if (i < n4) x = __ldcs(v128 + i);
+            key[4 * q] = x.x;
+            key[4 * q + 1] = x.y;
+            key[4 * q + 2] = x.z;
+            key[4 * q + 3] = x.w;
+            or_all |= (x.x | x.y) | (x.z | x.w);
         }
     } else {
         hi0 = (uint32_t)((uint64_t)__ldg(reinterpret_cast<const long long *>(v)) >> 32);
@@ -254,6 +262,14 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
             hi_diff |= (uint32_t)(x >> 32) ^ hi0;
             or_all |= (uint32_t)x;
         }
+    }
+    // the thread's valid slots are a prefix of its PCT_VPT slots under both layouts
+    int nvalid;
+    if (IS32) {
+        const int n4 = N >> 2;
+        nvalid = n4 > (int)threadIdx.x ? 4 * ((n4 - (int)threadIdx.x + PCT_THREADS - 1) / PCT_THREADS) : 0;
+    } else {
+        nvalid = N > (int)threadIdx.x ? (N - (int)threadIdx.x + PCT_THREADS - 1) / PCT_THREADS : 0;
     }
     if (__syncthreads_or(hi_diff != 0u)) return false;
     or_all = __reduce_or_sync(ASR_FULL_MASK, or_all);
@@ -273,7 +289,7 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
     if (bits > 0) {
         // first pass: all targets at once, no filter (every key >> bits is 0)
         const int sh1 = bits > PCT_DIG ? bits - PCT_DIG : 0;
-        reg_count_pass(key, N, 32, sh1, 0u, kk, 0, pl.n_pct, sm);
+        reg_count_pass(key, nvalid, 32, sh1, 0u, kk, 0, pl.n_pct, sm);
         uint32_t pop[MAXT];
 #pragma unroll
         for (int t = 0; t < MAXT; ++t)
@@ -293,7 +309,7 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
             // more counting passes while the bin is too crowded for the candidate buffer
             while (shift > 0 && pop[t] > (uint32_t)PCT_CAND) {
                 const int ns = shift > PCT_DIG ? shift - PCT_DIG : 0;
-                reg_count_pass(key, N, shift, ns, prefix[t], kk, t, t + 1, sm);
+                reg_count_pass(key, nvalid, shift, ns, prefix[t], kk, t, t + 1, sm);
                 prefix[t] = (prefix[t] << (shift - ns)) | sm.sel_digit[t];
                 kk[t] -= sm.sel_below[t];
                 pop[t] = sm.sel_pop[t];
@@ -302,8 +318,6 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
             }
             shiftv[t] = shift;
         }
-        // number of valid values of this thread (value j of a thread is element j*PCT_THREADS + tid)
-        const int nj = N > (int)threadIdx.x ? (N - (int)threadIdx.x + PCT_THREADS - 1) / PCT_THREADS : 0;
         // targets two at a time: compact the keys of both selected bins into shared memory
         // (private counts, one block scan, no ballots), then finish both on the candidates
 #pragma unroll
@@ -331,8 +345,8 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
                 }
             }
             {   // drop the slots past the end of the segment
-                const uint32_t v0 = nj >= 32 ? 0xFFFFFFFFu : ((1u << nj) - 1u);
-                const uint32_t v1 = nj > 32 ? ((1u << (nj - 32)) - 1u) : 0u;
+                const uint32_t v0 = nvalid >= 32 ? 0xFFFFFFFFu : ((1u << nvalid) - 1u);
+                const uint32_t v1 = nvalid > 32 ? ((1u << (nvalid - 32)) - 1u) : 0u;
                 ma0 &= v0;
                 mb0 &= v0;
                 ma1 &= v1;
