@@ -123,32 +123,49 @@ __device__ __forceinline__ bool is_admitted(const uint32_t *bm, int pos) { retur
 // Visit every waiting request of the window [lo, p): f(candidate record).  One CTA walks a window of up to
 // 10^6 positions out of L2, so the loop is bound by load latency: SCAN_U bitmap words and SCAN_U records per
 // thread are requested before the first one is looked at (the record load does not wait for its bitmap word).
-constexpr int SCAN_U = 8;
+#ifndef SCAN_U_N
+#define SCAN_U_N 4
+#endif
+constexpr int SCAN_U = SCAN_U_N;
 #ifdef CTA_STATS
 __device__ unsigned long long g_stat[8];
 #define STAT(i, v) do { if (threadIdx.x == 0) g_stat[i] += (v); } while (0)
 #else
 #define STAT(i, v) do { } while (0)
 #endif
+struct ScanBatch {
+    int4 v[SCAN_U];
+    uint32_t w[SCAN_U];
+};
+__device__ __forceinline__ void scan_load(ScanBatch &b, const asr_req_t *trace, const uint32_t *bm, int base, int p) {
+#pragma unroll
+    for (int u = 0; u < SCAN_U; ++u) {
+        const int pos = base + u * CTA_T;
+        const bool in = pos < p;
+        b.w[u] = in ? __ldcg(bm + (pos >> 5)) : 0xFFFFFFFFu;   // past the window: reads as admitted
+        b.v[u] = in ? __ldg(reinterpret_cast<const int4 *>(trace + pos)) : make_int4(0, 0, 0, 0);
+    }
+}
 template <class F>
 __device__ __forceinline__ void scan_waiting(const asr_req_t *trace, const uint32_t *bm, int lo, int p, F &&f) {
     STAT(1, 1);
     STAT(2, p - lo);
-    for (int base = lo + (int)threadIdx.x; base < p; base += CTA_T * SCAN_U) {
-        int4 v[SCAN_U];
-        uint32_t w[SCAN_U];
+    // the next batch is requested before the current one is looked at: its latency hides behind f
+    ScanBatch cur;
+    int base = lo + (int)threadIdx.x;
+    if (base < p) scan_load(cur, trace, bm, base, p);
+    while (base < p) {
+        const int nbase = base + CTA_T * SCAN_U;
+        ScanBatch nxt;
+        if (nbase < p) scan_load(nxt, trace, bm, nbase, p);
 #pragma unroll
         for (int u = 0; u < SCAN_U; ++u) {
             const int pos = base + u * CTA_T;
-            const bool in = pos < p;
-            w[u] = in ? __ldcg(bm + (pos >> 5)) : 0xFFFFFFFFu;
-            v[u] = in ? __ldg(reinterpret_cast<const int4 *>(trace + pos)) : make_int4(0, 0, 0, 0);
+            if (!((cur.w[u] >> (pos & 31)) & 1u))
+                f(make_int4(cur.v[u].x, cur.v[u].y, cur.v[u].w < 1 ? 1 : cur.v[u].w, pos));
         }
-#pragma unroll
-        for (int u = 0; u < SCAN_U; ++u) {
-            const int pos = base + u * CTA_T;
-            if (!((w[u] >> (pos & 31)) & 1u)) f(make_int4(v[u].x, v[u].y, v[u].w < 1 ? 1 : v[u].w, pos));
-        }
+        if (nbase < p) cur = nxt;
+        base = nbase;
     }
 }
 
