@@ -380,6 +380,15 @@ def run_ours(args):
     hbm_peak, peak_src = load_peaks()
     consts = load_profile_constants()
 
+    if args.side_configs_only:
+        # configs 1, 2 and 4 alone (the warp- and CTA-per-replica tiers): the command the ncu captures of those
+        # kernels are taken with; prints its own line, not the bench line
+        d_tables = asr.to_device(asr.make_tables(wl.ln_dur_table(), wl.exp_table()), dev)
+        if rank == 0:
+            print(json.dumps({"configs": side_configs(asr, dev, d_tables, reps=args.steps)}))
+        D.finalize()
+        return
+
     # ---- inputs, resident in HBM before any timed region ------------------
     cfg3 = wl.config3(n_seeds=args.seeds, n=args.n, seed0=D.seed_block(rank, args.seeds))
     seeds, rates, dist = wl.config3_traces(cfg3)
@@ -590,6 +599,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side-configs", action="store_true", help="skip the config 1/2/4 timings")
+    ap.add_argument("--side-configs-only", action="store_true", help="time configs 1, 2 and 4 and nothing else")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

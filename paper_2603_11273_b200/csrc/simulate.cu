@@ -304,8 +304,11 @@ __global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
 // and stops; the warp kernel then simulates that replica from the start with
 // its coalesced window scan.  Results are identical either way.
 // ---------------------------------------------------------------------------
-constexpr int LANE_THREADS = 64;
-constexpr int LANE_BLOCKS_PER_SM = 12;
+#ifndef LANE_THREADS_N
+#define LANE_THREADS_N 64
+#endif
+constexpr int LANE_THREADS = LANE_THREADS_N;
+constexpr int LANE_BLOCKS_PER_SM = 768 / LANE_THREADS;
 constexpr int LANE_CAP = 32;   // slots per replica handled by the lane kernel
 
 __device__ __forceinline__ int64_t ld_arrival(const asr_req_t *p) {

@@ -54,6 +54,7 @@ struct CtaSmem {
     uint64_t wsel[CTA_T / 32][KSEL_SMALL];   // small k: every warp's k smallest order scalars, ascending
     uint16_t tie[POOL_CAP];
     uint16_t hole[CTA_T], surv[CTA_T];
+    int64_t carr_win[CTA_T];   // arrival stamps of the trace window [cbase, cbase + CTA_T)
     int64_t red64[CTA_T / 32];
     int32_t red32[CTA_T / 32];
     int64_t bc64;
@@ -92,6 +93,27 @@ __device__ __forceinline__ int64_t block_sum64(int64_t v, CtaSmem &sm) {
 #pragma unroll
     for (int w = 0; w < CTA_T / 32; ++w) s += sm.red64[w];
     return s;
+}
+// sum of the admitted durations and minimum of the remaining tokens in one pair of barriers
+__device__ __forceinline__ void block_sum_min(int32_t dur, int32_t rem, int64_t &dur_sum, int32_t &rem_min, CtaSmem &sm) {
+    // dur = hi * 65536 + lo with 0 <= lo < 65536 (any sign of dur): two 32-bit REDUX instead of ten shuffles
+    const int lo = __reduce_add_sync(ASR_FULL_MASK, dur & 0xFFFF), hi = __reduce_add_sync(ASR_FULL_MASK, dur >> 16);
+    const int mn = __reduce_min_sync(ASR_FULL_MASK, rem);
+    __syncthreads();
+    if (lane_id() == 0) {
+        sm.red64[threadIdx.x >> 5] = (int64_t)hi * 65536 + (int64_t)lo;
+        sm.red32[threadIdx.x >> 5] = mn;
+    }
+    __syncthreads();
+    int64_t s = 0;
+    int m = sm.red32[0];
+#pragma unroll
+    for (int w = 0; w < CTA_T / 32; ++w) {
+        s += sm.red64[w];
+        m = sm.red32[w] < m ? sm.red32[w] : m;
+    }
+    dur_sum = s;
+    rem_min = m;
 }
 // exclusive rank of this thread among the threads with flag set
 __device__ __forceinline__ int block_rank(bool flag, CtaSmem &sm) {
@@ -458,17 +480,18 @@ __device__ __forceinline__ void pool_select(CtaSmem &sm, PoolState &ps, int poli
     const int tid = threadIdx.x;
     const int P = ps.P;
     int64_t Kr[POOL_EPT];
+    const bool small_k = k < P && k <= KSEL_SMALL;   // kth_scalar_small: no probes into sm.K, barriers of its own
 #pragma unroll
     for (int e = 0; e < POOL_EPT; ++e) {
         const int i = e * CTA_T + tid;
         Kr[e] = INT64_MAX;
         if (i < P) {
             Kr[e] = order_scalar_rt(policy, sm.pool[i], t);
-            sm.K[i] = Kr[e];
+            if (!small_k) sm.K[i] = Kr[e];
         }
     }
     if (tid == 0) sm.adm_n = sm.hole_n = sm.surv_n = sm.tie_n = 0;
-    __syncthreads();
+    if (!small_k) __syncthreads();
     uint32_t admmask = 0;
     if (k >= P) {
 #pragma unroll
@@ -479,7 +502,7 @@ __device__ __forceinline__ void pool_select(CtaSmem &sm, PoolState &ps, int poli
         int64_t Klo = 0, Khi = 0, v = 0;
         bool lo_inf = true, hi_inf = true;
         int cl = 0, ce = 0;
-        if (k <= KSEL_SMALL) {
+        if (small_k) {
             v = kth_scalar_small(sm, Kr, k);
             int c = 0;
 #pragma unroll
@@ -645,6 +668,7 @@ __device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
     uint32_t seed = 0x9E3779B9u * (uint32_t)(r + 1);
     int cbase = 0;
     int64_t carr = tid < n ? __ldg(reinterpret_cast<const long long *>(trace + tid)) : INT64_MAX;
+    sm.carr_win[tid] = carr;   // read after the ingest loop's first barrier
     const int64_t first_arrival = n > 0 ? __ldg(reinterpret_cast<const long long *>(trace)) : 0;
 
     while (done < n) {
@@ -680,15 +704,10 @@ __device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
             if (cnt == 0 || p < cbase + CTA_T) break;
             cbase += CTA_T;
             carr = cbase + tid < n ? __ldg(reinterpret_cast<const long long *>(trace + cbase + tid)) : INT64_MAX;
+            sm.carr_win[tid] = carr;   // the loop's next barrier orders it before any read
         }
         // arrival stamp of the next request (p < cbase + CTA_T here)
-        int64_t next_arr = INT64_MAX;
-        if (p < n) {
-            __syncthreads();
-            if (tid == p - cbase) sm.bc64 = carr;
-            __syncthreads();
-            next_arr = sm.bc64;
-        }
+        const int64_t next_arr = p < n ? sm.carr_win[p - cbase] : INT64_MAX;
         // ---- 2. idle server
         if (nR == 0 && nW == 0) {
             t = next_arr;
@@ -746,12 +765,13 @@ __device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
         // ---- 4. one engine iteration with the encoders of the admitted, then the exact fast-forward
         const int64_t c = cm.iter_base_us + cm.iter_per_running_us * (int64_t)nR;
         int64_t t1 = t + c;
+        int64_t dur_sum;
+        int32_t m;   // >= 1: nR >= 1 here
+        block_sum_min(my_dur, rem, dur_sum, m, sm);
         if (k > 0) {
-            const int64_t dur_sum = block_sum64((int64_t)my_dur, sm);
             t1 += cm.enc_base_us * (int64_t)k + cm.enc_per_ms_us * dur_sum;
             if (newly) ttft[ridx] = t1 - rarr;   // first token (S9)
         }
-        const int32_t m = block_min(rem, sm);   // >= 1: nR >= 1 here
         int64_t j = 1;
         if (m > 1) {
             if (nR == slots || p >= n || c <= 0) {
