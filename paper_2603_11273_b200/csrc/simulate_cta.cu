@@ -155,39 +155,43 @@ __device__ unsigned long long g_stat[8];
 #else
 #define STAT(i, v) do { } while (0)
 #endif
-struct ScanBatch {
-    int4 v[SCAN_U];
-    uint32_t w[SCAN_U];
-};
-__device__ __forceinline__ void scan_load(ScanBatch &b, const asr_req_t *trace, const uint32_t *bm, int base, int p) {
-#pragma unroll
-    for (int u = 0; u < SCAN_U; ++u) {
-        const int pos = base + u * CTA_T;
-        const bool in = pos < p;
-        b.w[u] = in ? __ldcg(bm + (pos >> 5)) : 0xFFFFFFFFu;   // past the window: reads as admitted
-        b.v[u] = in ? __ldg(reinterpret_cast<const int4 *>(trace + pos)) : make_int4(0, 0, 0, 0);
-    }
-}
 template <class F>
 __device__ __forceinline__ void scan_waiting(const asr_req_t *trace, const uint32_t *bm, int lo, int p, F &&f) {
     STAT(1, 1);
     STAT(2, p - lo);
-    // the next batch is requested before the current one is looked at: its latency hides behind f
-    ScanBatch cur;
-    int base = lo + (int)threadIdx.x;
-    if (base < p) scan_load(cur, trace, bm, base, p);
-    while (base < p) {
-        const int nbase = base + CTA_T * SCAN_U;
-        ScanBatch nxt;
-        if (nbase < p) scan_load(nxt, trace, bm, nbase, p);
+    if (lo >= p) return;
+    // A thread takes one bitmap word (32 positions) at a time and walks its zero bits, so the admitted
+    // positions -- most of a deep window -- cost nothing; up to SCAN_U records are requested before the first
+    // one is looked at, and the thread's next word is requested before the current one is walked.
+    const int w0 = lo >> 5, w1 = (p - 1) >> 5;
+    const uint32_t head = ~((1u << (lo & 31)) - 1u);                                   // positions >= lo of word w0
+    const uint32_t tail = ((p - 1) & 31) == 31 ? 0xFFFFFFFFu : (2u << ((p - 1) & 31)) - 1u;   // positions < p of word w1
+    int w = w0 + (int)threadIdx.x;
+    uint32_t word = w <= w1 ? __ldcg(bm + w) : 0xFFFFFFFFu;
+    while (w <= w1) {
+        const int wn = w + CTA_T;
+        const uint32_t word_n = wn <= w1 ? __ldcg(bm + wn) : 0xFFFFFFFFu;
+        uint32_t inv = ~word;
+        if (w == w0) inv &= head;
+        if (w == w1) inv &= tail;
+        while (inv) {
+            int4 v[SCAN_U];
+            int pos[SCAN_U];
 #pragma unroll
-        for (int u = 0; u < SCAN_U; ++u) {
-            const int pos = base + u * CTA_T;
-            if (!((cur.w[u] >> (pos & 31)) & 1u))
-                f(make_int4(cur.v[u].x, cur.v[u].y, cur.v[u].w < 1 ? 1 : cur.v[u].w, pos));
+            for (int u = 0; u < SCAN_U; ++u) {
+                pos[u] = -1;
+                if (inv) {
+                    pos[u] = w * 32 + __ffs((int)inv) - 1;
+                    inv &= inv - 1u;
+                    v[u] = __ldg(reinterpret_cast<const int4 *>(trace + pos[u]));
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < SCAN_U; ++u)
+                if (pos[u] >= 0) f(make_int4(v[u].x, v[u].y, v[u].w < 1 ? 1 : v[u].w, pos[u]));
         }
-        if (nbase < p) cur = nxt;
-        base = nbase;
+        w = wn;
+        word = word_n;
     }
 }
 
