@@ -146,7 +146,7 @@ __device__ __forceinline__ bool is_admitted(const uint32_t *bm, int pos) { retur
 // 10^6 positions out of L2, so the loop is bound by load latency: SCAN_U bitmap words and SCAN_U records per
 // thread are requested before the first one is looked at (the record load does not wait for its bitmap word).
 #ifndef SCAN_U_N
-#define SCAN_U_N 4
+#define SCAN_U_N 8
 #endif
 constexpr int SCAN_U = SCAN_U_N;
 #ifdef CTA_STATS
