@@ -34,9 +34,18 @@
 
 namespace asr {
 
-constexpr int SEL_WARPS = 20;                   // warps (= queues in flight) per CTA, one CTA per SM
-constexpr int SEL_CHUNK = 256;                  // records per staged chunk (4 KB)
-constexpr int SEL_STAGES = 2;                   // TMA ring depth per warp
+#ifndef SEL_WARPS_N
+#define SEL_WARPS_N 20
+#endif
+#ifndef SEL_CHUNK_N
+#define SEL_CHUNK_N 256
+#endif
+#ifndef SEL_STAGES_N
+#define SEL_STAGES_N 2
+#endif
+constexpr int SEL_WARPS = SEL_WARPS_N;          // warps (= queues in flight) per CTA, one CTA per SM
+constexpr int SEL_CHUNK = SEL_CHUNK_N;          // records per staged chunk (4 KB)
+constexpr int SEL_STAGES = SEL_STAGES_N;        // TMA ring depth per warp
 constexpr int SEL_UNROLL = 2;                   // records per lane loaded and tested together
 constexpr int SEL_ROWS = 6;                     // candidate buffer: rows of 32
 constexpr int SEL_BUFCAP = SEL_ROWS * 32;       // 192 candidates
