@@ -22,7 +22,14 @@
 
 namespace asr {
 
-constexpr int PCT_THREADS = 256;
+#ifndef PCT_MIN_CTAS
+#define PCT_MIN_CTAS 3
+#endif
+#ifndef PCT_THREADS_N
+#define PCT_THREADS_N 256
+#endif
+constexpr int PCT_THREADS = PCT_THREADS_N;   // 256 (40 values per thread) or 320 (32 values per thread)
+static_assert(PCT_THREADS >= 256 && PCT_THREADS % 64 == 0 && 10240 % PCT_THREADS == 0, "see PCT_VPT");
 constexpr int PCT_SMEM_VALUES = 12288;   // 96 KB of int64 staged per CTA
 constexpr int PCT_MAX = 8;
 
@@ -83,7 +90,7 @@ __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, co
         if (bits > 0) {
             for (int shift = top_shift;; shift -= 8) {
                 __syncthreads();
-                hist[threadIdx.x] = 0;   // PCT_THREADS == 256
+                if (PCT_THREADS == 256 || threadIdx.x < 256) hist[threadIdx.x] = 0;
                 __syncthreads();
                 for (int64_t i = threadIdx.x; i < N; i += PCT_THREADS) {
                     uint64_t key = (uint64_t)((is32 && !staged) ? (int64_t)v32[i] : src[i]) - (uint64_t)mn;
@@ -133,9 +140,13 @@ __device__ void segment_percentiles(const int64_t *__restrict__ v, int64_t N, co
 // ---------------------------------------------------------------------------
 // register path
 // ---------------------------------------------------------------------------
-constexpr int PCT_VPT = 40;                                  // values per thread
+constexpr int PCT_VPT = 10240 / PCT_THREADS;                 // values per thread
+static_assert(PCT_VPT % 4 == 0 && PCT_VPT <= 64, "quads of values per 128-bit load, two 32-bit match masks");
 constexpr int PCT_REG_MAX = PCT_THREADS * PCT_VPT;           // 10,240 values
-constexpr int PCT_DIG = 7;                                   // digit width of a counting pass
+#ifndef PCT_DIG_N
+#define PCT_DIG_N 7
+#endif
+constexpr int PCT_DIG = PCT_DIG_N;                                   // digit width of a counting pass
 constexpr int PCT_BINS = 1 << PCT_DIG;
 constexpr int PCT_BIN_STRIDE = 36;                           // bytes: 32 lane counters + 4 padding
 constexpr int PCT_TAB_BYTES = PCT_BINS * PCT_BIN_STRIDE;     // per warp
@@ -178,13 +189,14 @@ __device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], i
         }
     }
     __syncthreads();
-    // column sums: thread (half, bin) adds the 32 lane counters of 4 warps
-    {
+    // column sums: thread (half, bin) adds the 32 lane counters of its half of the warps
+    if (PCT_THREADS == 2 * PCT_BINS || threadIdx.x < 2 * PCT_BINS) {
+        constexpr int HW = PCT_THREADS / 64;   // warps per half
         const int bin = threadIdx.x & (PCT_BINS - 1), half = threadIdx.x >> PCT_DIG;
         uint32_t tot = 0;
 #pragma unroll
-        for (int w = 0; w < 4; ++w) {
-            const uint32_t *row = reinterpret_cast<const uint32_t *>(&sm.tab[half * 4 + w][bin * PCT_BIN_STRIDE]);
+        for (int w = 0; w < HW; ++w) {
+            const uint32_t *row = reinterpret_cast<const uint32_t *>(&sm.tab[half * HW + w][bin * PCT_BIN_STRIDE]);
 #pragma unroll
             for (int q = 0; q < 8; ++q) tot = __dp4a(row[q], 0x01010101u, tot);
         }
@@ -192,11 +204,12 @@ __device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], i
     }
     __syncthreads();
     if (warp == 0) {
-        // lane L owns bins 4L .. 4L+3
-        uint32_t c[4], tot = 0;
+        // lane L owns bins BPL*L .. BPL*L + BPL-1
+        constexpr int BPL = PCT_BINS / 32;
+        uint32_t c[BPL], tot = 0;
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            c[b] = sm.part[0][lane * 4 + b] + sm.part[1][lane * 4 + b];
+        for (int b = 0; b < BPL; ++b) {
+            c[b] = sm.part[0][lane * BPL + b] + sm.part[1][lane * BPL + b];
             tot += c[b];
         }
         uint32_t incl = tot;
@@ -211,9 +224,9 @@ __device__ __forceinline__ void reg_count_pass(const uint32_t (&key)[PCT_VPT], i
             if (excl < k && k <= incl) {
                 uint32_t run = excl;
 #pragma unroll
-                for (int b = 0; b < 4; ++b) {
+                for (int b = 0; b < BPL; ++b) {
                     if (run < k && k <= run + c[b]) {
-                        sm.sel_digit[t] = (uint32_t)(lane * 4 + b);
+                        sm.sel_digit[t] = (uint32_t)(lane * BPL + b);
                         sm.sel_below[t] = run;
                         sm.sel_pop[t] = c[b];
                     }
@@ -384,8 +397,10 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
             uint32_t p_a = pa, p_b = pb, k_a = kk[t0], k_b = two ? kk[t0 + 1 < MAXT ? t0 + 1 : t0] : 0u;
             while (s_a > 0 || s_b > 0) {
                 const int na = s_a > 8 ? s_a - 8 : 0, nb = s_b > 8 ? s_b - 8 : 0;
-                sm.hist[0][threadIdx.x] = 0;   // PCT_THREADS == 256
-                sm.hist[1][threadIdx.x] = 0;
+                if (PCT_THREADS == 256 || threadIdx.x < 256) {
+                    sm.hist[0][threadIdx.x] = 0;
+                    sm.hist[1][threadIdx.x] = 0;
+                }
                 __syncthreads();               // also orders the candidate stores above
                 if (s_a > 0) {
                     const uint32_t mask = (1u << (s_a - na)) - 1u;
@@ -453,7 +468,7 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
     return true;
 }
 
-__global__ void __launch_bounds__(PCT_THREADS, 3) percentiles_kernel(const int64_t *values, const int64_t *seg_off,
+__global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) percentiles_kernel(const int64_t *values, const int64_t *seg_off,
                                                                   int32_t n_seg, PctList pl, int64_t *out) {
     extern __shared__ __align__(16) unsigned char dyn_smem[];
     PctRegSmem &sm = *reinterpret_cast<PctRegSmem *>(dyn_smem);
@@ -468,7 +483,7 @@ __global__ void __launch_bounds__(PCT_THREADS, 3) percentiles_kernel(const int64
 }
 
 // p50/p90 of E2E latency (blockIdx.y = 0) and TTFT (blockIdx.y = 1) of every replica
-__global__ void __launch_bounds__(PCT_THREADS, 3) summary_percentiles_kernel(const asr_replica_t *replicas,
+__global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles_kernel(const asr_replica_t *replicas,
                                                                           int32_t n_replicas, const int64_t *lat,
                                                                           const int64_t *ttft,
                                                                           asr_summary_t *out_summary, bool fmt_flags) {
