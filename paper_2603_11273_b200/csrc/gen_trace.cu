@@ -88,12 +88,13 @@ __device__ __forceinline__ void st_rec4(asr_req_t *p, const int64_t (&arr)[GEN_R
     }
 }
 
+constexpr uint32_t GEN_SKIP = 0xFFFFFFFFu;
 struct GenSmem {
     int64_t warp_tot[GEN_GROUP][GEN_WARPS];   // per trace: the warps' gap sums of this step
     int64_t warp_off[GEN_GROUP][GEN_WARPS];   // per trace: arrival before the warp's first record
     uint64_t seed[GEN_GROUP];
     int32_t dist[GEN_GROUP];
-    uint32_t gap[GEN_GROUP];                  // mean gap in us, 0: trace skipped (rate_mhz < 1)
+    uint32_t gap[GEN_GROUP];                  // mean gap in us (<= 10^9; 0 above 10^9 mHz), GEN_SKIP: rate_mhz < 1
 };
 
 // one run of m traces with equal (seed, dist), first trace r0 of the unit; FULL: m == GEN_GROUP, so that the
@@ -168,7 +169,7 @@ __device__ __forceinline__ void gen_run(GenSmem &sm, int r0, int m, int64_t n_pe
         for (int g = 0; g < GEN_GROUP; ++g) {
             if (FULL || g < m) {
                 const uint32_t mg = sm.gap[r0 + g];
-                if (mg != 0u && n_valid > 0) {
+                if (mg != GEN_SKIP && n_valid > 0) {
                     int64_t arr[GEN_RPT];
                     int64_t run = sm.warp_off[g][warp] + excl[g];
 #pragma unroll
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(GEN_THREADS, GEN_MIN_CTAS) gen_trace_kernel(co
             const asr_trace_spec_t sp = specs ? specs[t_first + threadIdx.x] : one;
             sm.seed[threadIdx.x] = sp.seed;
             sm.dist[threadIdx.x] = sp.dist;
-            sm.gap[threadIdx.x] = sp.rate_mhz < 1 ? 0u : (uint32_t)(1000000000u / (uint32_t)sp.rate_mhz);
+            sm.gap[threadIdx.x] = sp.rate_mhz < 1 ? GEN_SKIP : (uint32_t)(1000000000u / (uint32_t)sp.rate_mhz);
         }
         __syncthreads();
         for (int r0 = 0; r0 < cnt;) {

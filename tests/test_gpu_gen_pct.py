@@ -21,7 +21,7 @@ def test_gen_trace_matches_oracle(asr, tables):
     d_tab = asr.tables_to_device(*tables)
     for seed, rate, dist, n in [(0, 2000, 0, 1000), (1, 500, 1, 3000), (1, 4000, 1, 3000), (4, 35408, 0, 70000),
                                 (9, 1, 0, 5), (2**40 + 3, 123457, 1, 257), (7, 1000, 0, 1), (7, 1000, 0, 255),
-                                (7, 1000, 0, 256), (7, 1000, 0, 0)]:
+                                (7, 1000, 0, 256), (7, 1000, 0, 0), (3, 2_000_000_000, 0, 300)]:
         out = asr.gen_trace(seed, rate, dist, n, d_tab)
         torch.cuda.synchronize()
         got = out.cpu().numpy().view(asr.REQ_DTYPE)
@@ -57,7 +57,7 @@ def test_gen_trace_batched_irregular_runs(asr, tables):
         sd, ds = int(rng.integers(0, 2**63)), int(rng.integers(0, 2))
         for _ in range(run_len):
             seeds.append(sd); dist.append(ds); rates.append(int(rng.integers(1, 40000)))
-    seeds += [5, 5, 5, 5]; dist += [0, 1, 0, 1]; rates += [777, 777, 777, 1000000]
+    seeds += [5, 5, 5, 5]; dist += [0, 1, 0, 1]; rates += [777, 777, 2_000_000_000, 1000000]   # mean gap 0 us: a burst
     assert len(seeds) % 8 != 0
     for n in (1, 1023, 1024, 1025, 2500):
         specs = np.zeros(len(seeds), dtype=asr.SPEC_DTYPE)
