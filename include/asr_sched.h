@@ -267,7 +267,12 @@ int asr_sched_gen_trace(uint64_t seed, int32_t rate_mhz, int32_t dist, int64_t n
                         const asr_tables_t *tables, asr_req_t *out, void *stream);
 
 /* n_traces traces of n_per_trace records each; trace t is written at
- * out[t*n_per_trace ..).  specs DEVICE [n_traces]. */
+ * out[t*n_per_trace ..).  specs DEVICE [n_traces] (not validated: a spec with
+ * rate_mhz < 1 leaves its trace untouched; above 10^9 mHz the mean gap is 0 us
+ * and every arrival is 0).  The draws of record i depend on (seed, i) only
+ * (identical request sequences across runs), so consecutive specs
+ * with equal (seed, dist) -- the rates of one seed -- are generated together;
+ * the result does not depend on the order of the specs. */
 int asr_sched_gen_trace_batched(const asr_trace_spec_t *specs, int32_t n_traces,
                                 int64_t n_per_trace, const asr_tables_t *tables,
                                 asr_req_t *out, void *stream);
