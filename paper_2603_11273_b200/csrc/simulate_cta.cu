@@ -357,6 +357,7 @@ __device__ __noinline__ void pool_rebuild(CtaSmem &sm, PoolState &ps, const asr_
         __syncthreads();
     }
     if (guess_failed) {
+        STAT(6, 1);
         guess = false;
         --attempt;
         continue;
@@ -804,8 +805,8 @@ __device__ void cta_replica(const SimArgs &a, const int r, CtaSmem &sm) {
     }
 #ifdef CTA_STATS
     if (tid == 0) {
-        printf("cta stats: policy %d rebuilds %llu scans %llu positions %llu horizon-out %llu strong-out %llu shrinks %llu H %lld\n",
-               policy, g_stat[0], g_stat[1], g_stat[2], g_stat[3], g_stat[4], g_stat[5], (long long)ps.H);
+        printf("cta stats: policy %d rebuilds %llu scans %llu positions %llu horizon-out %llu strong-out %llu shrinks %llu guess-fail %llu H %lld\n",
+               policy, g_stat[0], g_stat[1], g_stat[2], g_stat[3], g_stat[4], g_stat[5], g_stat[6], (long long)ps.H);
         for (int i = 0; i < 8; ++i) g_stat[i] = 0;
     }
 #endif

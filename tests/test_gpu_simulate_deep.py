@@ -112,6 +112,23 @@ def test_tie_heavy_deep_backlog(asr_mod):
     assert ms > 0.5, "the CTA tier did not run"
 
 
+def test_hrrn_pool_overflow_shrinks_the_horizon(asr_cta):
+    """one early request, then thousands arriving within a few milliseconds: at the first threshold build every
+    wait is a few tens of milliseconds, so the default one-second horizon lets nearly the whole backlog reach the
+    threshold ratio; the pool overflows and the horizon has to shrink until it fits (the branch the Poisson traces
+    never reach).  Later, with waits of many seconds, the same horizon fits again."""
+    rng = np.random.Generator(np.random.PCG64(33))
+    n = 5000
+    arr = np.concatenate([[0], 1000 + np.arange(n, dtype=np.int64) * 3])
+    dur = np.concatenate([[1000], np.clip(np.rint(np.exp(rng.normal(np.log(6000.0), 0.6, size=n))), 1000, 35000)])
+    tr = np.zeros(n + 1, dtype=wl.REQ)
+    tr["arrival_us"], tr["dur_ms"], tr["est"] = arr, dur.astype(np.int32), dur.astype(np.int32)
+    reps = [(0, orc.HRRN, 64), (0, orc.SJF, 64), (0, orc.HRRN, 8)]
+    L, T, S = run_batched([tr], reps, wl.CONFIG_COST, 64)
+    for i, (_, p, s) in enumerate(reps):
+        check_replica(tr, p, s, wl.CONFIG_COST, L[i], T[i], S[i], "overflow rep=%d" % i)
+
+
 def _digests(v):
     u = v.astype(np.uint64)
     i = np.arange(len(u), dtype=np.uint64)
