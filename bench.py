@@ -51,15 +51,30 @@ def load_peaks():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def csrc_sha16():
+    """hash of the kernel sources the committed ncu constants were captured from"""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2603_11273_b200", "csrc", "*.cu*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
 def load_profile_constants():
-    """per-launch DRAM traffic and warp instructions per request, from the committed ncu summaries"""
+    """per-launch DRAM traffic and instructions per request, from the committed ncu summaries.  They are
+    counters of a capture under ncu (never of this run): the file carries the hash of the kernel sources it
+    was taken from, and a run on other sources marks every figure derived from it as stale."""
     p = os.path.join(ROOT, "profiles", "roofline_constants.json")
     if os.path.exists(p):
         try:
-            return json.load(open(p))
+            c = json.load(open(p))
+            c["stale"] = c.get("csrc_sha16") != csrc_sha16()
+            return c
         except Exception:
             pass
-    return {}
+    return {"stale": True}
 
 
 class ClockSampler:
@@ -123,15 +138,16 @@ class ClockSampler:
 # CPU oracle legs (cpu_baseline of the default run, and --impl reference)
 # ---------------------------------------------------------------------------
 
-def oracle_sweep_sample(n_replicas: int, n: int, seed0: int, threads: int):
+def oracle_sweep_sample(n_replicas: int, n: int, seed0: int, threads: int, keep=None, n_seeds: int = 4096):
     """Run the oracle on `n_replicas` replicas spread evenly over the sweep
-    (generate -> simulate -> p50/p90).  -> (requests, seconds)"""
+    (generate -> simulate -> p50/p90).  -> (requests, seconds).  `keep` (a dict) receives
+    replica index -> the oracle's summary tuple, for the parity check after the timed legs."""
     import concurrent.futures as cf
     import oracle as orc
-    cfg = wl.config3(n=n, seed0=seed0)
+    cfg = wl.config3(n_seeds=n_seeds, n=n, seed0=seed0)
     ln_dur, exp_t = wl.ln_dur_table(), wl.exp_table()
     total = cfg["n_seeds"] * len(cfg["rates_mhz"]) * len(cfg["policies"])
-    picks = np.unique(np.linspace(0, total - 1, n_replicas).astype(np.int64))
+    picks = np.unique(np.linspace(0, total - 1, min(n_replicas, total)).astype(np.int64))
     cm = orc.cost(*cfg["cost"])
     orc.lib()
 
@@ -140,16 +156,22 @@ def oracle_sweep_sample(n_replicas: int, n: int, seed0: int, threads: int):
         s, ri = divmod(t, 8)
         dist = 1 if s >= cfg["n_seeds"] // 2 else 0
         tr = orc.gen_trace(seed0 + s, cfg["rates_mhz"][ri], dist, n, ln_dur, exp_t)
-        lat, ttft, _, _ = orc.simulate(tr, cfg["policies"][pol], cm, cfg["slots"])
-        return (orc.percentile(lat, 50), orc.percentile(lat, 90), orc.percentile(ttft, 50), orc.percentile(ttft, 90))
+        lat, ttft, first, end = orc.simulate(tr, cfg["policies"][pol], cm, cfg["slots"])
+        return (orc.percentile(lat, 50), orc.percentile(lat, 90), orc.percentile(ttft, 50), orc.percentile(ttft, 90),
+                first, end, n)
 
     t0 = time.perf_counter()
     with cf.ThreadPoolExecutor(max_workers=threads) as ex:   # ctypes releases the GIL
-        list(ex.map(one, picks))
-    return len(picks) * n, time.perf_counter() - t0
+        res = list(ex.map(one, picks))
+    dt = time.perf_counter() - t0
+    if keep is not None:
+        keep.update((int(r), v) for r, v in zip(picks, res))
+    return len(picks) * n, dt
 
 
-def oracle_select_sample(n_queues: int, q_len: int, threads: int):
+def oracle_select_sample(n_queues: int, q_len: int, threads: int, keep=None):
+    """the first n_queues queues of the config-5 stream, HRRN + SJF, sort everything and take k.
+    `keep` (a dict) receives policy -> int32[n_queues, k] of the oracle's indices."""
     import concurrent.futures as cf
     import oracle as orc
     cfg = wl.config5(q_len=q_len)
@@ -157,30 +179,61 @@ def oracle_select_sample(n_queues: int, q_len: int, threads: int):
     qs = orc.gen_queue(cfg["seed"], 0, n_queues * q_len, cfg["now"], ln_dur).reshape(n_queues, q_len)
 
     def one(i):
-        for pol in cfg["policies"]:
-            orc.select(qs[i], pol, cfg["now"], cfg["k"])
+        return [orc.select(qs[i], pol, cfg["now"], cfg["k"]) for pol in cfg["policies"]]
 
     t0 = time.perf_counter()
     with cf.ThreadPoolExecutor(max_workers=threads) as ex:
-        list(ex.map(one, range(n_queues)))
+        res = list(ex.map(one, range(n_queues)))
     dt = time.perf_counter() - t0
+    if keep is not None:
+        for j, pol in enumerate(cfg["policies"]):
+            keep[pol] = np.stack([r[j] for r in res]) if res else np.zeros((0, cfg["k"]), dtype=np.int32)
     return n_queues * q_len * 16 * len(cfg["policies"]) / dt / 1e9, dt
 
 
-def cpu_baseline(n: int, target_s: float = 25.0):
+SUMMARY_FIELDS = ("p50_e2e_us", "p90_e2e_us", "p50_ttft_us", "p90_ttft_us", "first_arrival_us", "last_done_us",
+                  "n_done")
+
+
+def cpu_baseline(n: int, n_seeds: int, q_len: int, summ, idx_by_policy, target_s: float = 25.0):
+    """The oracle as it stands, timed on the host cores over a bounded sample of the workload -- and, because
+    those results are the oracle's answers for the very replicas and queues the timed launches processed,
+    compared (after the clock has stopped) with the GPU's full-size outputs: `summ` = the per-replica summaries
+    of the timed sweep, `idx_by_policy` = the index rows of the timed select launches.
+    -> (cpu_baseline dict, parity_checked dict)"""
     cores = os.cpu_count() or 1
-    req, dt = oracle_sweep_sample(cores, n, 0, cores)          # pilot: one replica per core
+    total_rep = n_seeds * 8 * 3
+    req, dt = oracle_sweep_sample(cores, n, 0, cores, n_seeds=n_seeds)          # pilot: one replica per core
     per_replica = dt / max(1, req // n) * cores
-    count = int(max(cores, min(98304, target_s * cores / max(per_replica, 1e-6))))
-    req, dt = oracle_sweep_sample(count, n, 0, cores)
-    _, pilot_dt = oracle_select_sample(cores * 4, 4096, cores)
+    count = int(max(cores, min(total_rep, target_s * cores / max(per_replica, 1e-6))))
+    kept = {}
+    req, dt = oracle_sweep_sample(count, n, 0, cores, keep=kept, n_seeds=n_seeds)
+    _, pilot_dt = oracle_select_sample(cores * 4, q_len, cores)
+    n_have = min(len(v) for v in idx_by_policy.values()) if idx_by_policy else 0
     n_sel = int(max(cores * 4, min(65536, 4.0 * cores * 4 / max(pilot_dt, 1e-6))))   # about 4 s
-    sel_gbs, sel_dt = oracle_select_sample(n_sel, 4096, cores)
-    return {"value": req / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "%d of the 98,304 config-3 replicas (evenly spaced over seeds x rates x policies, "
-                      "n=%d each; generate+simulate+p50/p90), %.1f s wall on %d threads" % (req // n, n, dt, cores),
+    kept_sel = {}
+    sel_gbs, sel_dt = oracle_select_sample(n_sel, q_len, cores, keep=kept_sel)
+    # ---- parity of the full-size launches against what the oracle just computed (untimed)
+    bad_rep = [r for r, want in kept.items()
+               if r < len(summ) and tuple(int(summ[r][f]) for f in SUMMARY_FIELDS) != tuple(int(x) for x in want)]
+    n_q = min(n_sel, n_have)
+    bad_q = {pol: int((np.asarray(idx_by_policy[pol][:n_q]) != kept_sel[pol][:n_q]).any(axis=1).sum())
+             for pol in kept_sel if pol in idx_by_policy}
+    parity = {"replicas": len([r for r in kept if r < len(summ)]), "replicas_total": int(len(summ)),
+              "queues": int(n_q), "queues_total": int(n_have), "queue_policies": sorted(bad_q),
+              "mismatches": len(bad_rep) + sum(bad_q.values()),
+              "what": "oracle summaries (p50/p90 E2E, p50/p90 TTFT, first arrival, last completion, n_done) of the "
+                      "sampled config-3 replicas vs the timed sweep's output; oracle top-k index rows of the first "
+                      "queues of config 5 vs the timed select launches' output, per policy; tolerance 0"}
+    if bad_rep:
+        parity["first_bad_replicas"] = bad_rep[:8]
+    base = {"value": req / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%d of the %d config-3 replicas (evenly spaced over seeds x rates x policies, "
+                      "n=%d each; generate+simulate+p50/p90), %.1f s wall on %d threads"
+                      % (req // n, total_rep, n, dt, cores),
             "select_gbs": sel_gbs,
-            "select_sample": "%d config-5 queues x 4096, HRRN+SJF full sort, %.1f s" % (n_sel, sel_dt)}
+            "select_sample": "%d config-5 queues x %d, HRRN+SJF full sort, %.1f s" % (n_sel, q_len, sel_dt)}
+    return base, parity
 
 
 def run_reference(args):
@@ -456,6 +509,13 @@ def run_ours(args):
     ktimes = asr.timing_read()
     asr.timing_enable(False)
     clocks = sampler.stop()
+    # the index rows of the same launches once more, per policy, for the parity check of the cpu_baseline leg
+    idx_by_policy = {}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        for pol in cfg5["policies"]:
+            asr.select_batched(d_queues, nq, ql, pol, now5, k5, out_idx=d_idx)
+            torch.cuda.synchronize()
+            idx_by_policy[pol] = d_idx.cpu().numpy().copy()
 
     summ = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
     assert int((summ["n_done"] == n).sum()) == n_rep, "replicas did not finish"
@@ -484,15 +544,25 @@ def run_ours(args):
         if not k_avg:
             continue
         stage_ms[kname] = k_tot
-        # ALU/issue-bound: achieved = warp instructions issued per second; the per-request
-        # instruction count is the ncu figure committed in profiles/roofline_constants.json
-        wi = consts.get(kname + "_warp_instr_per_request") if n == 10000 and cfg3["slots"] == 32 else None
+        # ALU/issue-bound: achieved = warp instructions issued per second; the per-request instruction counts
+        # are ncu counters committed in profiles/roofline_constants.json (stale = captured from other sources).
+        # A kernel that executed MORE instructions per request would score higher on `frac`, so the line also
+        # carries the thread-level figure: thread instructions (warp instructions x active threads) per second
+        # against 32 threads per issue slot.
+        full = n == 10000 and cfg3["slots"] == 32
+        wi = consts.get(kname + "_warp_instr_per_request") if full else None
+        ti = consts.get(kname + "_thread_instr_per_request") if full else None
         a = (wi * total / (k_avg / 1e3)) if wi else None
+        at = (ti * total / (k_avg / 1e3)) if ti else None
         rooflines[kname] = {
             "bound": "alu", "achieved": a, "peak": ALU_PEAK_WARP_INSTR_PER_S, "unit": "warp-instr/s",
             "frac": (a / ALU_PEAK_WARP_INSTR_PER_S) if a else None,
             "traffic": consts.get(kname + "_dram_bytes_per_launch"),
-            "warp_instr_per_request": wi, "avg_launch_ms": k_avg,
+            "warp_instr_per_request": wi, "thread_instr_per_request": ti,
+            "threads_per_warp_instr": (ti / wi) if (wi and ti) else None,
+            "frac_thread_level": (at / (32 * ALU_PEAK_WARP_INSTR_PER_S)) if at else None,
+            "algorithmic_bytes_per_launch": (n_traces * n * 16 + 2 * total * 4) if kname == "sim_lane_kernel" else None,
+            "avg_launch_ms": k_avg, "constants_stale": bool(consts.get("stale")),
             "peak_source": "148 SMs x 4 schedulers x 1.965 GHz (DESIGN.md)"}
     if gen_avg:
         a = n_traces * n * 16 / (gen_avg / 1e3) / 1e9
@@ -555,9 +625,9 @@ def run_ours(args):
         side = side_configs(asr, dev, d_tables)
         ext_lines = extension_lines(asr, dev, d_tables, hbm_peak)
 
-    base = None
+    base = parity = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        base = cpu_baseline(n)
+        base, parity = cpu_baseline(n, args.seeds, ql, summ, idx_by_policy)
 
     if rank == 0:
         line = {
@@ -578,11 +648,15 @@ def run_ours(args):
                        "frac_of_measured_peak": select_gbs / world / hbm_peak,
                        "frac_of_nominal_8TBs": select_gbs / world / 8000.0},
             "roofline": roofline, "rooflines": rooflines, "clocks": clocks, "e2e": e2e,
-            "gpu_launches": int(launches), "cpu_baseline": base, "configs": side, "extensions": ext_lines,
+            "gpu_launches": int(launches), "cpu_baseline": base, "parity_checked": parity, "configs": side,
+            "extensions": ext_lines,
             "kernel_ms_total": {k_: v[0] for k_, v in ktimes.items() if v[1]},
         }
         print(json.dumps(line), flush=True)
     D.finalize()
+    if parity is not None and parity["mismatches"] != 0:
+        print("bench.py: the timed launches disagree with the oracle: %r" % parity, file=sys.stderr)
+        return 3
     return 0
 
 

@@ -16,13 +16,19 @@
  * CONVENTIONS (apply to every call unless the call says otherwise)
  *  - Pointers marked DEVICE are device addresses allocated and owned by the
  *    caller; pointers marked HOST are ordinary host addresses read during the
- *    call.  The library never allocates or frees caller-visible memory; scratch
- *    comes from the caller-supplied DEVICE `workspace` (size it with
- *    asr_sched_workspace_bytes; its contents need no initialisation).
+ *    call (small descriptors: a single cost model, percentile lists, kappa
+ *    tables; they may be freed as soon as the call returns).  The stream-ordered
+ *    calls never allocate or free memory: scratch comes from the caller-supplied
+ *    DEVICE `workspace` (size it with asr_sched_workspace_bytes; its contents
+ *    need no initialisation).
  *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *    Calls only enqueue work on it and return without synchronising; outputs
- *    are valid once the caller has synchronised the stream.  The *_host entry
- *    points are the exception: they are synchronous and take HOST buffers.
+ *    are valid once the caller has synchronised the stream.
+ *  - EXCEPTION: the two *_host entry points (asr_sched_sweep_host,
+ *    asr_sched_select_host) are synchronous, take HOST buffers only, and DO
+ *    allocate: their device scratch comes from the device's default
+ *    stream-ordered memory pool and stays cached there between calls until
+ *    asr_sched_trim_scratch.
  *  - Return value: 0 success; -1 invalid argument (null pointer, negative size,
  *    unknown policy, slots < 1, workspace too small); -2 CUDA runtime error
  *    (text via asr_sched_last_error); -3 unsupported shape (exceeds a limit
@@ -140,8 +146,11 @@ int asr_sched_select_batched(const asr_req_t *keys, int32_t n_queues, int32_t q_
 /* ------------------------------------------------------------------ */
 
 /* One replica.  trace DEVICE [n] sorted by arrival_us non-decreasing
- * (precondition); cm HOST; out_lat/out_ttft DEVICE [n] or NULL; out_summary
- * DEVICE [1] or NULL; workspace DEVICE.  slots in 1..256 (else -3). */
+ * (precondition); out_lat/out_ttft DEVICE [n] or NULL; out_summary DEVICE [1]
+ * or NULL; workspace DEVICE.  slots in 1..256 (else -3).
+ * cm is a HOST pointer here (one 40-byte struct, copied into the workspace
+ * during the call), whereas the batched calls below take `cms` as a DEVICE
+ * array that the kernels index by replica.cm_id. */
 int asr_sched_simulate(const asr_req_t *trace, int64_t n, int32_t policy,
                        const asr_cost_model_t *cm, int32_t slots, int64_t *out_lat,
                        int64_t *out_ttft, asr_summary_t *out_summary, void *workspace,
@@ -240,7 +249,8 @@ int asr_sched_itl_batched(const asr_req_t *traces, const asr_replica_t *replicas
  * max(1, floor(d_ms * kappa_milli / 10^6)), d = speech_ms[i] if given (speech-active
  * duration from a VAD) else dur_ms, kappa_milli =
  * kappa_milli_by_lang[lang[i]] (entry 0 if lang is NULL; per-language kappa,
- * PAPER.md:154).  A lang id >= n_lang reads entry 0.
+ * PAPER.md:154).  A lang id >= n_lang reads entry 0.  est is clamped to
+ * [1, 2^24], the range the comparator is exact on (CONVENTIONS above).
  *   recs DEVICE [n] (only est is written); kappa_milli_by_lang HOST [n_lang],
  *   1 <= n_lang <= 64; lang DEVICE [n] or NULL; speech_ms DEVICE [n] or NULL. */
 int asr_sched_estimate(asr_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang,

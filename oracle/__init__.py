@@ -19,7 +19,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "asr_oracle.c")
 _HDR = os.path.join(_HERE, "asr_oracle.h")
-_LIB = os.path.join(_HERE, "libasr_oracle.so")
+# ASR_ORACLE_SANITIZE=1 (set by tests/test_oracle_sanitized.py for a child pytest run): the same source built
+# with -fsanitize=address,undefined into a library of its own
+_SANITIZE = os.environ.get("ASR_ORACLE_SANITIZE", "") == "1"
+_LIB = os.path.join(_HERE, "libasr_oracle_san.so" if _SANITIZE else "libasr_oracle.so")
 
 FCFS, SJF, HRRN, ADAPTIVE = 0, 1, 2, 3
 DIST_LOGNORMAL, DIST_UNIFORM = 0, 1
@@ -64,9 +67,9 @@ def build(force: bool = False) -> str:
     )
     if stale:
         tmp = _LIB + ".tmp.%d" % os.getpid()
+        san = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-g", "-O1"] if _SANITIZE else ["-O2"]
         subprocess.check_call(
-            ["gcc", "-O2", "-std=gnu11", "-fPIC", "-shared", "-Wall", "-Wextra",
-             "-o", tmp, _SRC]
+            ["gcc"] + san + ["-std=gnu11", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC]
         )
         os.replace(tmp, _LIB)
     return _LIB
@@ -82,6 +85,10 @@ def lib():
         vp, i64, i32, u64, u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_uint32
         L.orc_better.restype = C.c_int
         L.orc_better.argtypes = [vp, i64, vp, i64, C.c_int, i64]
+        L.orc_bound_violations.restype = i64
+        L.orc_bound_violations.argtypes = []
+        L.orc_bound_violations_reset.restype = None
+        L.orc_bound_violations_reset.argtypes = []
         L.orc_select.restype = C.c_int
         L.orc_select.argtypes = [vp, i64, C.c_int, i64, i32, vp]
         L.orc_simulate.restype = C.c_int
@@ -136,6 +143,11 @@ def better(q, ia: int, ib: int, policy: int, now: int) -> bool:
     q = _req(q)
     base = q.ctypes.data
     return bool(lib().orc_better(base + 16 * ia, ia, base + 16 * ib, ib, policy, now))
+
+
+def bound_violations() -> int:
+    """HRRN cross-products >= 2^62 seen by this thread's orc_better calls (outside the boundary's bounds)"""
+    return int(lib().orc_bound_violations())
 
 
 def select(q, policy: int, now: int, k: int) -> np.ndarray:

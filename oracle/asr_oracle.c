@@ -36,6 +36,19 @@ static int earlier(const orc_req_t *a, int64_t ia, const orc_req_t *b,
     return ia < ib;
 }
 
+/* "The oracle multiplies in __int128 and asserts the products
+ * fit int64".  The boundary's documented bound is wait * est < 2^62
+ * (wait < 2^38, est <= 2^24).  A product at or beyond it is counted here and
+ * turned into error -4 by orc_select / orc_simulate* / orc_itl, so an input
+ * outside the boundary's contract is caught by the checker instead of being
+ * compared against an int64 path that may have wrapped.  The ordering itself
+ * stays exact in 128 bits. */
+static __thread int64_t g_bound_violations = 0;
+static const i128 HRRN_PRODUCT_BOUND = (i128)1 << 62;
+
+int64_t orc_bound_violations(void) { return g_bound_violations; }
+void orc_bound_violations_reset(void) { g_bound_violations = 0; }
+
 int orc_better(const orc_req_t *a, int64_t ia, const orc_req_t *b, int64_t ib,
                int policy, int64_t now) {
     if (policy == ORC_FCFS) return earlier(a, ia, b, ib);
@@ -51,6 +64,7 @@ int orc_better(const orc_req_t *a, int64_t ia, const orc_req_t *b, int64_t ib,
      * evaluated exactly in 128-bit integers. */
     i128 lhs = (i128)wait_of(a, now) * (i128)est_of(b);
     i128 rhs = (i128)wait_of(b, now) * (i128)est_of(a);
+    if (lhs >= HRRN_PRODUCT_BOUND || rhs >= HRRN_PRODUCT_BOUND) g_bound_violations++;
     if (lhs != rhs) return lhs > rhs;
     return earlier(a, ia, b, ib);
 }
@@ -76,10 +90,11 @@ int orc_select(const orc_req_t *q, int64_t n, int policy, int64_t now,
     if (!pos) return -2;
     for (int64_t i = 0; i < n; i++) pos[i] = i;
     sort_ctx_t c = {q, policy, now};
+    const int64_t v0 = g_bound_violations;
     qsort_r(pos, (size_t)n, sizeof(int64_t), cmp_pos, &c);
     for (int32_t j = 0; j < k; j++) out_idx[j] = j < n ? (int32_t)pos[j] : -1;
     free(pos);
-    return 0;
+    return g_bound_violations != v0 ? -4 : 0;
 }
 
 /* ------------------------------------------------------------------ */
@@ -133,6 +148,7 @@ int orc_simulate(const orc_req_t *trace, int64_t n, int policy,
         return -2;
     }
     int64_t nW = 0, nR = 0, p = 0, done = 0, t = 0;
+    const int64_t v0 = g_bound_violations;
 
     while (done < n) {
         /* 1. ingest: arrivals at or before the iteration boundary (S13) */
@@ -183,7 +199,7 @@ int orc_simulate(const orc_req_t *trace, int64_t n, int policy,
     }
     if (last_done_us) *last_done_us = t;
     free(W); free(R); free(rem);
-    return 0;
+    return g_bound_violations != v0 ? -4 : 0;
 }
 
 /* ------------------------------------------------------------------ */
@@ -240,6 +256,7 @@ int orc_simulate_ex(const orc_req_t *trace, int64_t n, int policy,
     int64_t nW = 0, nR = 0, p = 0, done = 0, t = 0;
     int blocked = 0; /* E6: admission cut short by memory; retried only
                         after the waiting or the running set has changed */
+    const int64_t v0 = g_bound_violations;
 
     while (done < n) {
         /* 1. ingest (S13) */
@@ -333,7 +350,7 @@ int orc_simulate_ex(const orc_req_t *trace, int64_t n, int policy,
     }
     if (last_done_us) *last_done_us = t;
     free(W); free(R); free(rem); free(mem); free(fresh); free(ever);
-    return 0;
+    return g_bound_violations != v0 ? -4 : 0;
 }
 
 int orc_itl(const orc_req_t *trace, int64_t n, int policy, const orc_cost_t *cm,
@@ -350,6 +367,7 @@ int orc_itl(const orc_req_t *trace, int64_t n, int policy, const orc_cost_t *cm,
         return -2;
     }
     int64_t nW = 0, nR = 0, p = 0, done = 0, t = 0;
+    const int64_t v0 = g_bound_violations;
     while (done < n) { /* the loop of orc_simulate, one iteration at a time */
         while (p < n && trace[p].arrival_us <= t) W[nW++] = p++;
         if (nR == 0 && nW == 0) {
@@ -404,7 +422,7 @@ int orc_itl(const orc_req_t *trace, int64_t n, int policy, const orc_cost_t *cm,
     if (out_count) *out_count = cnt;
     if (out_sum) *out_sum = sum;
     free(gaps); free(W); free(R); free(rem);
-    return 0;
+    return g_bound_violations != v0 ? -4 : 0;
 }
 
 int orc_tpot(const orc_req_t *trace, int64_t n, const orc_cost_t *cm,
@@ -422,12 +440,13 @@ int orc_estimate(orc_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang,
     if (n < 0 || n_lang < 1 || !kappa_milli_by_lang) return -1;
     for (int64_t i = 0; i < n; i++) {
         int32_t l = lang ? (int32_t)lang[i] : 0;
-        if (l >= n_lang) return -1;
+        if (l >= n_lang) l = 0; /* DESIGN.md reading E12: an unknown language id uses entry 0 */
         int64_t d = speech_ms ? speech_ms[i] : recs[i].dur_ms;
         if (d < 0) d = 0;
         int64_t e = (d * (int64_t)kappa_milli_by_lang[l]) / 1000000;
         if (e < 1) e = 1;
-        if (e > 0x7FFFFFFF) e = 0x7FFFFFFF;
+        if (e > ((int64_t)1 << 24)) e = (int64_t)1 << 24; /* DESIGN.md reading E10: the
+                                        comparator's documented bound est <= 2^24 */
         recs[i].est = (int32_t)e;
     }
     return 0;

@@ -61,7 +61,13 @@ typedef struct {
 enum { ORC_FCFS = 0, ORC_SJF = 1, ORC_HRRN = 2 };
 enum { ORC_DIST_LOGNORMAL = 0, ORC_DIST_UNIFORM = 1 };
 
-/* 1 if request a (at position ia) is strictly better than b (at ib). */
+/* 1 if request a (at position ia) is strictly better than b (at ib).
+ * HRRN multiplies in 128 bits; a cross-product >= 2^62 (outside the boundary's
+ * documented bounds wait < 2^38, est <= 2^24) is counted in a
+ * thread-local counter, and orc_select / orc_simulate / orc_simulate_ex /
+ * orc_itl return -4 when a comparison of theirs tripped it. */
+int64_t orc_bound_violations(void);
+void orc_bound_violations_reset(void);
 int orc_better(const orc_req_t *a, int64_t ia, const orc_req_t *b, int64_t ib,
                int policy, int64_t now);
 
@@ -126,7 +132,8 @@ int orc_itl(const orc_req_t *trace, int64_t n, int policy, const orc_cost_t *cm,
 /* f3 duration-based estimator (Eq. 1, Listing 1):
  * est = max(1, floor(d_ms * kappa_milli / 10^6)) with d = speech_ms[i] when given
  * (VAD speech-active duration) else dur_ms, and kappa_milli =
- * kappa_milli_by_lang[lang[i]] (lang == NULL: entry 0) */
+ * kappa_milli_by_lang[lang[i]] (lang == NULL or lang[i] >= n_lang: entry 0;
+ * PAPER.md:154); est is clamped to the comparator's bound 2^24 */
 int orc_estimate(orc_req_t *recs, int64_t n, const int32_t *kappa_milli_by_lang,
                  int32_t n_lang, const uint8_t *lang, const int32_t *speech_ms);
 

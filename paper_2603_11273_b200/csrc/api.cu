@@ -33,6 +33,27 @@ int check_launch(const char *what) {
 
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+// grids are sized from the SM count of the device the call runs on
+int sm_count() {
+    static std::atomic<int> cache[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return 148;
+    }
+    if (dev >= 0 && dev < 64) {
+        const int c = cache[dev].load(std::memory_order_relaxed);
+        if (c > 0) return c;
+    }
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+        cudaGetLastError();
+        n = 148;
+    }
+    if (dev >= 0 && dev < 64) cache[dev].store(n, std::memory_order_relaxed);
+    return n;
+}
+
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
@@ -238,7 +259,7 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
         out_lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes);
         out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + w.lat_bytes);
     }
-    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
+    int rc = launch_sim_prepare(replicas, n_replicas, total_requests, bm_off, defer, st);
     if (rc) return rc;
     SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
               out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, summary_only ? 1 : 0,
@@ -293,7 +314,7 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
         out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + w.lat_bytes);
     }
     uint32_t *bitmap2 = (uint32_t *)(ws + w.total);
-    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
+    int rc = launch_sim_prepare(replicas, n_replicas, total_requests, bm_off, defer, st);
     if (rc) return rc;
     SimExArgs a;
     static_cast<SimArgs &>(a) = SimArgs{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer,
@@ -359,7 +380,7 @@ extern "C" int asr_sched_itl_batched(const asr_req_t *traces, const asr_replica_
     int64_t *pairs = (int64_t *)(extra + iw.ext_bytes + iw.hist_bytes);
     int32_t *npairs = (int32_t *)(extra + iw.ext_bytes + iw.hist_bytes + iw.pairs_bytes);
     CUDA_TRY(cudaMemsetAsync(extra, 0, iw.ext_bytes + iw.hist_bytes, st), "itl_batched: memset");
-    int rc = launch_sim_prepare(replicas, n_replicas, bm_off, defer, st);
+    int rc = launch_sim_prepare(replicas, n_replicas, total_requests, bm_off, defer, st);
     if (rc) return rc;
     SimExArgs a;
     static_cast<SimArgs &>(a) = SimArgs{traces, replicas, cms,     bm_off,         bitmap,     defer + 64, defer,
@@ -594,7 +615,8 @@ extern "C" int asr_sched_sweep_host(const asr_trace_spec_t *specs, int32_t n_tra
     if (rc) return rc;
     {
         KernelTimer kt(KID_SWEEP_REPLICAS, st);
-        build_sweep_replicas_kernel<<<(int)((n_rep + 255) / 256 < 1184 ? (n_rep + 255) / 256 : 1184), 256, 0, st>>>(
+        const int64_t cap = (int64_t)sm_count() * 8;
+        build_sweep_replicas_kernel<<<(int)((n_rep + 255) / 256 < cap ? (n_rep + 255) / 256 : cap), 256, 0, st>>>(
             (asr_replica_t *)d_rep.p, n_traces, n_per_trace, n_policies, slots, (const int32_t *)d_pol.p);
     }
     rc = check_launch("build_sweep_replicas_kernel");

@@ -15,6 +15,7 @@ namespace asr {
 void set_error(const char *fmt, ...);
 int check_launch(const char *what);   // cudaGetLastError -> ASR_OK / ASR_ECUDA
 void count_launch(int n = 1);
+int sm_count();                       // SMs of the current device (queried, cached per device)
 
 // kernel ids of the per-kernel CUDA-event timing facility (asr_sched_timing_*)
 enum KernelId {

@@ -230,7 +230,7 @@ int launch_gen_trace(const asr_trace_spec_t *specs, asr_trace_spec_t one, int32_
                      const asr_tables_t *tables, asr_req_t *out, cudaStream_t st) {
     if (n_traces <= 0 || n_per_trace <= 0) return ASR_OK;
     const int n_units = (n_traces + GEN_GROUP - 1) / GEN_GROUP;
-    int grid = n_units < 148 * 64 ? n_units : 148 * 64;
+    int grid = n_units < sm_count() * 64 ? n_units : sm_count() * 64;
     {
         KernelTimer kt(KID_GEN_TRACE, st);
         gen_trace_kernel<<<grid, GEN_THREADS, 0, st>>>(specs, one, n_traces, n_per_trace, tables, out);
@@ -242,7 +242,7 @@ int launch_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now, cons
                       asr_req_t *out, cudaStream_t st) {
     if (n <= 0) return ASR_OK;
     int64_t want = (n + GEN_THREADS - 1) / GEN_THREADS;
-    int grid = (int)(want < 148 * 16 ? want : 148 * 16);
+    int grid = (int)(want < (int64_t)sm_count() * 16 ? want : (int64_t)sm_count() * 16);
     {
         KernelTimer kt(KID_GEN_QUEUES, st);
         gen_queues_kernel<<<grid, GEN_THREADS, 0, st>>>(seed, first, n, now, tables, out);

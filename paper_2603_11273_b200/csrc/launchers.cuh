@@ -52,8 +52,8 @@ struct KappaTable {
 };
 int launch_estimate(asr_req_t *recs, int64_t n, const KappaTable &kt, const uint8_t *lang, const int32_t *speech_ms,
                     cudaStream_t st);
-int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,
-                       cudaStream_t st);
+int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t total_requests, int64_t *bm_off,
+                       int32_t *defer_count, cudaStream_t st);
 int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_seg, const int32_t *pcts,
                        int32_t n_pct, int64_t *out, cudaStream_t st);
 // fmt_flags: the lane kernel ran in order-free mode and left ASR_FMT32 / 0 in p50_e2e_us and p50_ttft_us of

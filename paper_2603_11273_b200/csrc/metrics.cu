@@ -19,6 +19,8 @@ __global__ void __launch_bounds__(256) tpot_kernel(const asr_req_t *__restrict__
     }
 }
 
+constexpr int64_t EST_MAX = (int64_t)1 << 24;
+
 __global__ void __launch_bounds__(256) estimate_kernel(asr_req_t *recs, int64_t n, KappaTable kt,
                                                        const uint8_t *__restrict__ lang,
                                                        const int32_t *__restrict__ speech_ms) {
@@ -29,7 +31,7 @@ __global__ void __launch_bounds__(256) estimate_kernel(asr_req_t *recs, int64_t 
         int64_t d = speech_ms ? (int64_t)speech_ms[i] : (int64_t)recs[i].dur_ms;
         d = d < 0 ? 0 : d;
         int64_t e = (d * (int64_t)kt.kappa_milli[l]) / 1000000;
-        e = e < 1 ? 1 : (e > 0x7FFFFFFF ? 0x7FFFFFFF : e);
+        e = e < 1 ? 1 : (e > EST_MAX ? EST_MAX : e);   // the comparator's documented bound (asr_sched.h: est <= 2^24)
         recs[i].est = (int32_t)e;
     }
 }
@@ -172,7 +174,7 @@ __global__ void __launch_bounds__(ITL_THREADS) itl_percentiles_kernel(SimExArgs 
 }
 
 int launch_itl_percentiles(const SimExArgs &a, const ItlPcts &pl, int64_t *out, cudaStream_t st) {
-    const int grid = a.n_replicas < 148 * 8 ? a.n_replicas : 148 * 8;
+    const int grid = a.n_replicas < sm_count() * 8 ? a.n_replicas : sm_count() * 8;
     {
         KernelTimer kt(KID_ITL_PCT, st);
         itl_percentiles_kernel<<<grid, ITL_THREADS, 0, st>>>(a, pl, out);
@@ -182,7 +184,7 @@ int launch_itl_percentiles(const SimExArgs &a, const ItlPcts &pl, int64_t *out, 
 
 static int stream_grid(int64_t n) {
     const int64_t want = (n + 255) / 256;
-    return (int)(want < 148 * 16 ? want : 148 * 16);
+    return (int)(want < (int64_t)sm_count() * 16 ? want : (int64_t)sm_count() * 16);
 }
 
 int launch_tpot(const asr_req_t *trace, int64_t n, asr_cost_model_t cm, const int64_t *lat, const int64_t *ttft,

@@ -501,7 +501,8 @@ __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles
             const asr_replica_t nx = replicas[rn];
             const int64_t flag = blockIdx.y == 0 ? out_summary[rn].p50_e2e_us : out_summary[rn].p50_ttft_us;
             const int64_t bytes = (int64_t)nx.n * ((fmt_flags && flag == ASR_FMT32) ? 4 : 8);
-            if (nx.n > 0 && nx.out_off >= 0 && bytes <= (int64_t)PCT_REG_MAX * 8) {
+            // only a descriptor the simulator accepted (n_done >= 0) is dereferenced
+            if (out_summary[rn].n_done >= 0 && nx.n > 0 && bytes <= (int64_t)PCT_REG_MAX * 8) {
                 const char *src = reinterpret_cast<const char *>(vals + nx.out_off);
                 const uint32_t sz = (uint32_t)(bytes & ~15ll);
                 if (sz > 0 && (reinterpret_cast<uintptr_t>(src) & 15u) == 0)
@@ -533,14 +534,8 @@ __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles
 static constexpr size_t PCT_DYN_SMEM = sizeof(PctRegSmem);
 
 static int pct_grid(int n_units, const void *fn) {
-    static int n_sm = 0;
+    const int n_sm = sm_count();
     int per_sm = 0;
-    if (n_sm == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (n_sm < 1) n_sm = 148;
-    }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, PCT_THREADS, PCT_DYN_SMEM);
     if (per_sm < 1) per_sm = 1;
     int cap = n_sm * per_sm;
@@ -553,11 +548,8 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
     PctList pl;
     pl.n_pct = n_pct;
     for (int j = 0; j < PCT_MAX; ++j) pl.pct[j] = j < n_pct ? pcts[j] : 0;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(percentiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PCT_DYN_SMEM);
-        attr = true;
-    }
+    // per-device opt-in, set on every launch
+    cudaFuncSetAttribute(percentiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PCT_DYN_SMEM);
     const int grid = pct_grid(n_seg, (const void *)percentiles_kernel);
     {
         KernelTimer kt(KID_PERCENTILES, st);
@@ -569,12 +561,7 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
                                const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, cudaStream_t st) {
     if (n_replicas <= 0) return ASR_OK;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(summary_percentiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)PCT_DYN_SMEM);
-        attr = true;
-    }
+    cudaFuncSetAttribute(summary_percentiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PCT_DYN_SMEM);
     int gx = pct_grid(n_replicas, (const void *)summary_percentiles_kernel);
     gx = gx > 1 ? (gx + 1) / 2 : 1;
     dim3 grid(gx, 2);

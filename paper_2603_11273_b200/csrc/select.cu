@@ -515,15 +515,8 @@ __global__ void __launch_bounds__(SEL_WARPS * 32, 1) select_topk_kernel(SelArgs 
 template <int POLICY, bool INDIRECT>
 static int launch_one(const SelArgs &a, cudaStream_t st) {
     if (a.n_queues <= 0 || a.k <= 0) return ASR_OK;
-    static int n_sm = 0;
-    static bool attr_set = false;
-    if (n_sm == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (n_sm < 1) n_sm = 148;
-    }
-    if (!attr_set) {
+    // the opt-in to > 48 KB of dynamic shared memory is per device: set it on every launch (cheap)
+    {
         cudaError_t e = cudaFuncSetAttribute(select_topk_kernel<POLICY, INDIRECT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM_BYTES);
         if (e != cudaSuccess) {
@@ -531,8 +524,8 @@ static int launch_one(const SelArgs &a, cudaStream_t st) {
             cudaGetLastError();
             return ASR_ECUDA;
         }
-        attr_set = true;
     }
+    const int n_sm = sm_count();
     // persistent: one CTA of SEL_WARPS queue-streams per SM
     const int64_t want = ((int64_t)a.n_queues + SEL_WARPS - 1) / SEL_WARPS;
     const int grid = (int)(want < (int64_t)n_sm ? want : (int64_t)n_sm);

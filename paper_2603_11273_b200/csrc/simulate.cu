@@ -665,8 +665,12 @@ __global__ void __launch_bounds__(256) sim_init_lat_kernel(SimArgs a) {
 }
 
 // exclusive prefix sum of the per-replica bitmap sizes (words), one CTA
+// A descriptor that replica_ok() will reject (n or out_off out of range) gets the two slack
+// words only, so that one bad descriptor cannot push the bitmaps of the valid replicas past
+// the workspace (which is sized from total_requests: the valid regions are disjoint).
 __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *replicas, int32_t n_replicas,
-                                                           int64_t *bm_off, int32_t *defer_count) {
+                                                           int64_t total_requests, int64_t *bm_off,
+                                                           int32_t *defer_count) {
     __shared__ int64_t warp_tot[32];
     __shared__ int64_t carry_s;
     if (threadIdx.x == 0) {
@@ -680,8 +684,10 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
         const int r = base + threadIdx.x;
         int64_t v = 0;
         if (r < n_replicas) {
-            int n = replicas[r].n;
-            v = (int64_t)((n < 0 ? 0 : n) >> 5) + 2;   // ceil(n/32) + slack word
+            const int n = replicas[r].n;
+            const int64_t off = replicas[r].out_off;
+            const bool sane = n >= 0 && off >= 0 && off + (int64_t)n <= total_requests;
+            v = (int64_t)((sane ? n : 0) >> 5) + 2;   // ceil(n/32) + slack word
         }
         int64_t x = v;
 #pragma unroll
@@ -736,7 +742,7 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
         } else {
             {
                 KernelTimer kt(KID_SIM_INIT_LAT, st);
-                const int grid = a.n_replicas < 148 * 8 ? a.n_replicas : 148 * 8;
+                const int grid = a.n_replicas < sm_count() * 8 ? a.n_replicas : sm_count() * 8;
                 sim_init_lat_kernel<<<grid, 256, 0, st>>>(a);
             }
             int rc0 = check_launch("sim_init_lat_kernel");
@@ -748,7 +754,7 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
         if (rc) return rc;
         // worklist pass: empty (and a few microseconds) when nothing was handed over
         const int want = (a.n_replicas + SIM_WARPS - 1) / SIM_WARPS;
-        launch_warp_any(a, max_slots, want < 148 * 8 ? want : 148 * 8, st);
+        launch_warp_any(a, max_slots, want < sm_count() * 8 ? want : sm_count() * 8, st);
         rc = check_launch("sim_warp_kernel");
         if (rc) return rc;
         return launch_simulate_cta(a, st);   // worklist of the warp kernel; empty unless a backlog ran deep
@@ -761,11 +767,11 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
     return launch_simulate_cta(a, st);
 }
 
-int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t *bm_off, int32_t *defer_count,
-                       cudaStream_t st) {
+int launch_sim_prepare(const asr_replica_t *replicas, int32_t n_replicas, int64_t total_requests, int64_t *bm_off,
+                       int32_t *defer_count, cudaStream_t st) {
     {
         KernelTimer kt(KID_SIM_PREPARE, st);
-        sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, bm_off, defer_count);
+        sim_prepare_kernel<<<1, 1024, 0, st>>>(replicas, n_replicas, total_requests, bm_off, defer_count);
     }
     return check_launch("sim_prepare_kernel");
 }

@@ -827,8 +827,7 @@ __global__ void __launch_bounds__(CTA_T) sim_cta_kernel(SimArgs a) {
 }
 
 int launch_simulate_cta(const SimArgs &a, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
+    {   // per-device opt-in, set on every launch
         cudaError_t e = cudaFuncSetAttribute(sim_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)sizeof(CtaSmem));
         if (e != cudaSuccess) {
@@ -836,9 +835,8 @@ int launch_simulate_cta(const SimArgs &a, cudaStream_t st) {
             cudaGetLastError();
             return ASR_ECUDA;
         }
-        attr = true;
     }
-    const int grid = a.n_replicas < 148 * 2 ? a.n_replicas : 148 * 2;
+    const int grid = a.n_replicas < sm_count() * 2 ? a.n_replicas : sm_count() * 2;
     {
         KernelTimer kt(KID_SIM_CTA, st);
         sim_cta_kernel<<<grid, CTA_T, sizeof(CtaSmem), st>>>(a);

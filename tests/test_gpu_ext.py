@@ -15,8 +15,7 @@ POL = (orc.FCFS, orc.SJF, orc.HRRN)
 @pytest.fixture(scope="module")
 def asr():
     import torch
-    if not torch.cuda.is_available():
-        pytest.skip("no CUDA device")
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device (there is no CPU fallback)"
     import paper_2603_11273_b200 as m
     return m
 
@@ -162,6 +161,17 @@ def test_estimator(asr):
         got = d.cpu().numpy().view(asr.REQ_DTYPE)
         want = orc.estimate(tr, kap if lg is not None else kap[:1], lang=lg, speech_ms=sp)
         assert np.array_equal(got.view(np.uint8), want.view(np.uint8))
+    # DESIGN.md E10/E12: est is clamped to the comparator's bound 2^24; an unknown language id reads entry 0
+    big = orc.make_trace(np.zeros(6), [2_000_000_000, 1 << 24, (1 << 24) + 1, 8000, 8000, 8000])
+    lg6 = np.array([0, 0, 0, 1, 2, 255], dtype=np.uint8)
+    for kap2 in ([1_000_000, 2500], [999_999, 5000]):
+        d = dev_trace(big)
+        asr.estimate(d, 6, kap2, asr.to_device(lg6))
+        torch.cuda.synchronize()
+        got = d.cpu().numpy().view(asr.REQ_DTYPE)
+        want = orc.estimate(big, kap2, lang=lg6)
+        assert np.array_equal(got.view(np.uint8), want.view(np.uint8))
+        assert got["est"].max() == 1 << 24
     # 8 / 4 / 2 s at kappa = 5 -> 40, 20, 10 tokens
     d = dev_trace(orc.make_trace([0, 0, 0], [8000, 4000, 2000]))
     asr.estimate(d, 3, [5000])

@@ -108,6 +108,40 @@ def test_mixed_batch_summary_only_and_invalid_descriptors(asr):
     assert list(s["n_done"]) == [700, -1, -1, -1]
 
 
+def test_invalid_descriptor_with_huge_n_does_not_displace_the_others(asr):
+    """a descriptor whose n / out_off is out of range sits BEFORE contended SJF/HRRN replicas: it gets
+    n_done = -1 and the bitmaps of the replicas behind it stay inside the workspace (they are sized from
+    total_requests; the kernels must not trust the n of a descriptor they are going to reject)"""
+    import torch
+    tr = wl.stress_trace("lognormal", 1500, 31, rate_per_s=26.0)       # overloaded at 8 slots: real choices
+    n = len(tr)
+    rep = asr.make_replicas([0] * 6, [0, 0, n, 2 * n, 0, 3 * n], [n, 2**31 - 1, n, n, n, n],
+                            [orc.FCFS, orc.SJF, orc.SJF, orc.HRRN, orc.HRRN, orc.FCFS], 8, 0)
+    rep["out_off"][1] = 2**40                 # out of range as well
+    rep["n"][4] = -5                          # negative n
+    rep["out_off"][4] = -1
+    total = 4 * n
+    for summary_only in (False, True):
+        d_sum = torch.zeros(6 * asr.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device="cuda")
+        lat = ttft = None
+        if not summary_only:
+            lat = torch.full((total,), -7, dtype=torch.int64, device="cuda")
+            ttft = torch.full((total,), -7, dtype=torch.int64, device="cuda")
+        ws_bytes = asr.workspace_bytes(1, total, 6, 1 if summary_only else 0)
+        ws = torch.zeros(ws_bytes + 4096, dtype=torch.uint8, device="cuda")
+        ws[ws_bytes:] = 0xA5                  # canary behind the workspace the library was promised
+        asr.simulate_batched(dev_trace(tr), asr.to_device(rep), 6, asr.to_device(asr.make_cost(*wl.CONFIG_COST)), 1,
+                             total, 8, lat, ttft, d_sum, workspace=ws[:ws_bytes])
+        torch.cuda.synchronize()
+        assert bool((ws[ws_bytes:] == 0xA5).all()), "wrote past the workspace"
+        s = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
+        assert list(s["n_done"]) == [n, -1, n, n, -1, n]
+        for i, pol in ((0, orc.FCFS), (2, orc.SJF), (3, orc.HRRN), (5, orc.FCFS)):
+            off = int(rep["out_off"][i])
+            check_replica(tr, pol, 8, wl.CONFIG_COST, None if summary_only else lat[off:off + n].cpu().numpy(),
+                          None if summary_only else ttft[off:off + n].cpu().numpy(), s[i], "rep %d" % i)
+
+
 def test_other_cost_models(asr):
     """zero per-running cost, zero encoder, big encoder, token floor"""
     tr = wl.stress_trace("lognormal", 800, 12, rate_per_s=9.0)

@@ -119,6 +119,19 @@ def test_estimator_fig1_tokens_and_floor():
     assert list(out["est"]) == [20, 20, 1, 1, 5]
 
 
+def test_estimator_clamp_and_unknown_language():
+    """DESIGN.md readings E10/E12: est never leaves the comparator's documented range [1, 2^24]
+    (asr_sched.h: wait * est < 2^62), and a language id without a table entry uses entry 0."""
+    tr = orc.make_trace([0, 0, 0], [2_000_000_000, 16_777_216, 16_777_217])
+    out = orc.estimate(tr, [1_000_000])                  # kappa = 1000 tokens/s: est = d_ms
+    assert list(out["est"]) == [1 << 24, 1 << 24, 1 << 24]
+    out = orc.estimate(tr, [999_999])
+    assert list(out["est"]) == [1 << 24, 16_777_199, 16_777_200]
+    tr = orc.make_trace([0, 0, 0], [8000, 8000, 8000])
+    out = orc.estimate(tr, [5000, 2500], lang=[1, 2, 255])
+    assert list(out["est"]) == [20, 40, 40]
+
+
 def test_itl_isolated_and_two_overlapping_requests():
     """PAPER.md:214.  Alone, every gap is 8,000 + 50 us: a 6 s request (25 tokens) has 24 of them.
     Unit model (1 ms iterations, no encoder), two slots: A (3 tokens) at t=0, B (2 tokens) arrives at

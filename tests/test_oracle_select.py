@@ -139,6 +139,30 @@ def test_hrrn_needs_exact_arithmetic():
     assert list(orc.select(q, orc.HRRN, now, 2)) == [1, 0]
 
 
+def test_products_beyond_the_documented_bounds_are_reported():
+    """the oracle multiplies in 128 bits and reports a cross-product that would not fit the
+    boundary's int64 contract (wait < 2^38, est <= 2^24 => wait * est < 2^62) instead of silently ordering it."""
+    e_max, now = 1 << 24, (1 << 38) - 1
+    inside = orc.make_trace([0, 1, now - 5], [e_max, e_max - 1, 7])        # largest legal products
+    assert orc.bound_violations() == orc.bound_violations()
+    before = orc.bound_violations()
+    assert list(orc.select(inside, orc.HRRN, now, 3)) == ref_order(inside, orc.HRRN, now)
+    assert orc.bound_violations() == before
+    outside = orc.make_trace([0, 1], [e_max, e_max])                        # wait 2^38: product 2^62
+    with pytest.raises(ValueError, match="rc=-4"):
+        orc.select(outside, orc.HRRN, 1 << 38, 2)
+    assert orc.bound_violations() > before
+    # the other policies never multiply: no report
+    assert list(orc.select(outside, orc.SJF, 1 << 38, 2)) == [0, 1]
+    assert list(orc.select(outside, orc.FCFS, 1 << 38, 2)) == [0, 1]
+    # and the simulator passes the report on: one slot, two requests wait 2^38 us behind a long first one
+    cm = orc.cost(1 << 38, 0, 10, 0, 1, 0)
+    tr = orc.make_trace([0, 0, 0], [1, 1, 1], est=[1, e_max, e_max])
+    with pytest.raises(ValueError, match="rc=-4"):
+        orc.simulate(tr, orc.HRRN, cm, 1)
+    orc.simulate(tr, orc.FCFS, cm, 1)
+
+
 def test_six_duration_ties_stress():
     # PAPER.md:96 synthetic split {5,...,30} s -> massive SJF ties
     q = wl.stress_queue("six", 500, 3, 10**8)
