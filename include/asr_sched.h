@@ -332,8 +332,12 @@ size_t asr_sched_workspace_bytes(int32_t op, int64_t a, int64_t b, int64_t c);
  * INT32_MAX = never).
  * ASR_OPT_SIM_ESCALATE_WINDOW: waiting-window length (requests) beyond which the
  * warp kernel hands a SJF/HRRN replica to the CTA kernel (default 4096; 0 = as
- * soon as the policy has to choose; INT32_MAX = never). */
-enum { ASR_OPT_SIM_LANE_MIN_REPLICAS = 0, ASR_OPT_SIM_ESCALATE_WINDOW = 1 };
+ * soon as the policy has to choose; INT32_MAX = never).
+ * ASR_OPT_SIM_LANE_SPLIT: 1 (default) lets a summary-only thread-per-replica
+ * call cut lightly loaded replicas into time segments that are simulated side
+ * by side and stitched at regeneration points (server idle at an arrival);
+ * 0 simulates every replica in one piece. */
+enum { ASR_OPT_SIM_LANE_MIN_REPLICAS = 0, ASR_OPT_SIM_ESCALATE_WINDOW = 1, ASR_OPT_SIM_LANE_SPLIT = 2 };
 int asr_sched_set_option(int32_t option, int64_t value);
 
 const char *asr_sched_last_error(void); /* thread-local, never NULL */

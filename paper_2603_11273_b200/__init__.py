@@ -12,6 +12,6 @@ from .binding import (  # noqa: F401
     workspace_bytes, to_device, tables_to_device, select, select_batched, simulate,
     simulate_batched, percentiles, gen_trace, gen_trace_batched, gen_queues, sweep_host,
     select_host, make_tables, make_replicas, make_cost, timing_enable, timing_reset, timing_read,
-    set_option, OPT_SIM_LANE_MIN_REPLICAS, OPT_SIM_ESCALATE_WINDOW, ADAPTIVE, EXT_DTYPE, make_ext,
+    set_option, OPT_SIM_LANE_MIN_REPLICAS, OPT_SIM_ESCALATE_WINDOW, OPT_SIM_LANE_SPLIT, ADAPTIVE, EXT_DTYPE, make_ext,
     simulate_batched_ex, tpot, estimate, itl_batched, trim_scratch,
 )

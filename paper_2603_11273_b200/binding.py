@@ -106,6 +106,7 @@ def launch_count() -> int:
 
 OPT_SIM_LANE_MIN_REPLICAS = 0
 OPT_SIM_ESCALATE_WINDOW = 1
+OPT_SIM_LANE_SPLIT = 2
 
 
 def set_option(option: int, value: int):

@@ -57,7 +57,7 @@ int sm_count() {
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
-    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel"};
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel", "summary_fast_kernel", "lane_plan_kernels", "sim_lane_kernel(repair)", "sim_lane_kernel(redo)"};
 struct TimedLaunch {
     int kid;
     cudaEvent_t start, stop;
@@ -99,11 +99,14 @@ static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a
 
 struct SimWorkspace {
     size_t bm_off_bytes, bitmap_bytes, defer_bytes, lat_bytes, total;
+    // summary-only calls: the time-split plan of the thread-per-replica tier, behind everything else
+    size_t plan_off, order_bytes, seg_bytes, unit_q_bytes;
 };
 
 // asr_sched_set_option values
 static std::atomic<int> g_opt_lane_min{1024};
 static std::atomic<int> g_opt_escalate{4096};
+static std::atomic<int> g_opt_lane_split{1};
 
 static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summary_only) {
     SimWorkspace w;
@@ -112,6 +115,11 @@ static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summ
     w.defer_bytes = align_up(sizeof(int32_t) * (size_t)(2 * n_replicas + 64));   // [0], [1]: counters, [64..]: the two lists
     w.lat_bytes = summary_only ? align_up(sizeof(int64_t) * (size_t)total_requests) : 0;
     w.total = w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + 2 * w.lat_bytes;
+    w.plan_off = w.total;
+    w.order_bytes = summary_only ? align_up(sizeof(int32_t) * (size_t)n_replicas) : 0;   // also: failed
+    w.seg_bytes = summary_only ? align_up((size_t)n_replicas) : 0;                        // load class; segments
+    w.unit_q_bytes = summary_only ? align_up(sizeof(int32_t) * (size_t)n_replicas * LANE_MAX_SEG + 64) : 0;   // + counters
+    w.total += 2 * w.order_bytes + 2 * w.seg_bytes + w.unit_q_bytes;
     return w;
 }
 
@@ -158,6 +166,10 @@ extern "C" int asr_sched_set_option(int32_t option, int64_t value) {
         case ASR_OPT_SIM_ESCALATE_WINDOW:
             if (value < 0 || value > INT32_MAX) break;
             g_opt_escalate.store((int)value);
+            return ASR_OK;
+        case ASR_OPT_SIM_LANE_SPLIT:
+            if (value < 0 || value > 1) break;
+            g_opt_lane_split.store((int)value);
             return ASR_OK;
     }
     set_error("set_option: bad option %d or value %lld", option, (long long)value);
@@ -263,13 +275,25 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     if (rc) return rc;
     SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
               out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, summary_only ? 1 : 0,
-              g_opt_escalate.load()};
+              g_opt_escalate.load(), LanePlan{}};
     // many small replicas: one thread each; few or wide ones: one warp each
     const bool use_lane = max_slots <= 32 && n_replicas >= g_opt_lane_min.load();
+    if (use_lane && summary_only && g_opt_lane_split.load() && (int64_t)n_replicas * LANE_MAX_SEG < INT32_MAX) {
+        char *pl = ws + w.plan_off;
+        a.plan.order = (int32_t *)pl;
+        a.plan.failed = (int32_t *)(pl + w.order_bytes);
+        pl += 2 * w.order_bytes;
+        a.plan.bucket = (uint8_t *)pl;
+        a.plan.nseg = (uint8_t *)(pl + w.seg_bytes);
+        pl += 2 * w.seg_bytes;
+        a.plan.unit_q = (int32_t *)pl;
+        a.plan.counters = a.plan.unit_q + (size_t)n_replicas * LANE_MAX_SEG;
+    }
     rc = launch_simulate(a, max_slots, use_lane, st);
     if (rc) return rc;
     if (out_summary)
-        rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, use_lane && summary_only, st);
+        rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, use_lane && summary_only,
+                                        a.plan.order, defer + 64, defer + 2, st);   // the hand-over lists are spent: miss lists
     return rc;
 }
 
@@ -320,7 +344,7 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
     static_cast<SimArgs &>(a) = SimArgs{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer,
                                         defer + 64 + n_replicas, defer + 1,
                                         out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, 0,
-                                        g_opt_escalate.load()};
+                                        g_opt_escalate.load(), LanePlan{}};
     a.exts = exts;
     a.bitmap2 = bitmap2;
     a.out_preempt = out_preempt;
@@ -329,7 +353,7 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
     a.itl_npairs = nullptr;
     rc = launch_simulate_ex(a, max_slots, st);
     if (rc) return rc;
-    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, false, st);
+    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, false, nullptr, nullptr, nullptr, st);
     return rc;
 }
 
@@ -386,7 +410,7 @@ extern "C" int asr_sched_itl_batched(const asr_req_t *traces, const asr_replica_
     static_cast<SimArgs &>(a) = SimArgs{traces, replicas, cms,     bm_off,         bitmap,     defer + 64, defer,
                                         defer + 64 + n_replicas, defer + 1,
                                         lat,    ttft,     nullptr, total_requests, n_replicas, n_cms, 0,
-                                        g_opt_escalate.load()};
+                                        g_opt_escalate.load(), LanePlan{}};
     a.exts = exts;
     a.bitmap2 = bitmap2;
     a.out_preempt = nullptr;

@@ -19,6 +19,9 @@
 // Nearest rank (asr_sched.h): element of 1-based rank
 // ceil(p*N/100) of the sorted segment; an empty segment gives -1.
 #include "launchers.cuh"
+#ifdef PCT_STATS
+#include <cstdio>
+#endif
 
 namespace asr {
 
@@ -468,6 +471,404 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
     return true;
 }
 
+
+// ---------------------------------------------------------------------------
+// carried-window kernel (order-free uint32 segments of a sweep: p50/p90)
+//
+// A CTA walks a run of consecutive segments.  Consecutive segments of a sweep
+// are alike (the same trace under another policy, the neighbouring seed or
+// rate), so the two ranks of segment i are looked for in windows of values
+// around the answers of segment i-1: ONE pass over the register-resident keys
+// counts, per rank, the keys below the window's end and appends the keys
+// inside the window to per-thread private slots (no atomics, no tables to
+// clear); the window is then resolved exactly by a two-level 10-bit histogram
+// over the few hundred collected keys.  Every count is exact and the window is
+// only a guess: a rank that falls outside moves the window that way and
+// doubles it, a thread that runs out of slots halves it, and the pass is
+// repeated on the keys still in registers.  A CTA's first segment finds its
+// windows by bisection on the key bits (count-only passes).  A segment in
+// another format, or one that is not settled after PF_TRIES passes, goes to
+// the miss list, which summary_percentiles_kernel (radix path) works off.
+// No result depends on a guess.
+// ---------------------------------------------------------------------------
+#ifndef PF_SLOTS_N
+#define PF_SLOTS_N 24
+#endif
+#ifndef PF_MIN_CTAS
+#define PF_MIN_CTAS 3
+#endif
+#ifdef PCT_STATS
+__device__ unsigned long long g_pct_stats[8];   // segments, settled, passes, bootstraps, misses, in-window keys, -, -
+#endif
+constexpr int PF_SLOTS = PF_SLOTS_N;   // private slots per thread and rank
+constexpr int PF_GROUP = 8;            // slots are checked once per group of keys
+constexpr int PF_BINS = 1024;          // bins per histogram level
+constexpr int PF_MAX_SHIFT = 10;       // window = PF_BINS << shift values; the second level resolves 2^shift
+constexpr int PF_HALF = PCT_THREADS / 2;
+constexpr int PF_TRIES = 6;
+constexpr uint32_t PF_IN_MANY = 64u * (PF_SLOTS - PF_GROUP), PF_IN_FEW = PF_IN_MANY / 4;   // keys wanted inside a window
+static_assert(PCT_VPT % PF_GROUP == 0 && PF_SLOTS > PF_GROUP, "slot check granularity");
+
+struct PctFastSmem {
+    uint32_t slot[2][PF_SLOTS][PCT_THREADS];
+    uint32_t hist[2][2][PF_BINS];            // [level][rank][bin]
+    uint32_t wtot[2][2][PCT_THREADS / 32];   // [parity][rank][warp]: keys below the window's end | keys inside << 16
+    uint32_t wovf[2][PCT_THREADS / 32];      // [parity][warp]: bit t = a thread closed its window of rank t
+    uint32_t wsum[2][PCT_THREADS / 64];
+    uint32_t sel_bin[2][2], sel_rem[2][2];   // [level][rank]
+};
+
+__device__ __forceinline__ uint32_t pf_end(uint32_t lo, int sh) {   // saturated: a key 2^32-1 is never inside
+    const uint32_t hi = lo + ((uint32_t)PF_BINS << sh);
+    return hi < lo ? 0xFFFFFFFFu : hi;
+}
+
+// inclusive scan of the PF_BINS bins of histogram h by the PF_HALF threads of one rank: thread j owns
+// bins 8j .. 8j+7.  Part A leaves the per-warp totals in wsum; after a barrier part B locates rank k.
+__device__ __forceinline__ void pf_scan_a(const uint32_t *h, int j, uint32_t (&c)[8], uint32_t &tot, uint32_t &incl,
+                                          uint32_t *wsum) {
+    static_assert(PF_BINS == PF_HALF * 8, "eight bins per thread");
+    const uint4 a = *reinterpret_cast<const uint4 *>(h + 8 * j), b = *reinterpret_cast<const uint4 *>(h + 8 * j + 4);
+    c[0] = a.x, c[1] = a.y, c[2] = a.z, c[3] = a.w, c[4] = b.x, c[5] = b.y, c[6] = b.z, c[7] = b.w;
+    tot = ((c[0] + c[1]) + (c[2] + c[3])) + ((c[4] + c[5]) + (c[6] + c[7]));
+    incl = tot;
+    const int lane = lane_id();
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+        if (lane >= d) incl += y;
+    }
+    if (lane == 31) wsum[j >> 5] = incl;
+}
+
+__device__ __forceinline__ void pf_scan_b(const uint32_t (&c)[8], uint32_t tot, uint32_t incl, const uint32_t *wsum, int j,
+                                          uint32_t k, uint32_t *sel_bin, uint32_t *sel_rem) {
+    uint32_t excl = incl - tot;
+#pragma unroll
+    for (int w = 0; w < PF_HALF / 32; ++w)
+        if (w < (j >> 5)) excl += wsum[w];
+    if (excl < k && k <= excl + tot) {
+        uint32_t run = excl;
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+            if (run < k && k <= run + c[b]) {
+                *sel_bin = (uint32_t)(8 * j + b);
+                *sel_rem = k - run;
+            }
+            run += c[b];
+        }
+    }
+}
+
+// One pass over the keys.  Per key and rank: one compare-and-count below the window's end, one compare for
+// "inside", a predicated store and a predicated pointer bump (written out in PTX: the compiler's version of the
+// same loop took nine instructions per key and rank).  Returns, for rank t, T[t] = keys below the end | keys
+// inside << 16 over the whole CTA, and ov = bit t set if some thread closed its window t for lack of slots
+// (then "inside" of rank t is short; "below the end" is always exact).  n[t] = this thread's keys inside.
+__device__ __forceinline__ void pf_pass(const uint32_t (&key)[PCT_VPT], uint32_t lo0, uint32_t hi0, uint32_t lo1,
+                                        uint32_t hi1, PctFastSmem &fs, int par, uint32_t (&T)[2], uint32_t &ov,
+                                        int (&n)[2]) {
+    const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
+    uint32_t c0 = 0, c1 = 0;
+    const uint32_t b0 = (uint32_t)__cvta_generic_to_shared(&fs.slot[0][0][tid]);
+    const uint32_t b1 = (uint32_t)__cvta_generic_to_shared(&fs.slot[1][0][tid]);
+    uint32_t p0 = b0, p1 = b1;
+    constexpr uint32_t ROW = PCT_THREADS * 4;   // bytes between two slots of a thread
+    const uint32_t stop0 = b0 + (PF_SLOTS - PF_GROUP) * ROW, stop1 = b1 + (PF_SLOTS - PF_GROUP) * ROW;
+    uint32_t over = 0;
+#pragma unroll
+    for (int g = 0; g < PCT_VPT / PF_GROUP; ++g) {
+#pragma unroll
+        for (int j = 0; j < PF_GROUP; ++j) {
+            asm volatile(
+                "{\n\t"
+                ".reg .pred a, b;\n\t"
+                "setp.lt.u32 a, %4, %5;\n\t"
+                "@a add.u32 %0, %0, 1;\n\t"
+                "setp.ge.and.u32 b, %4, %6, a;\n\t"
+                "@b st.shared.u32 [%1], %4;\n\t"
+                "@b add.u32 %1, %1, %9;\n\t"
+                "setp.lt.u32 a, %4, %7;\n\t"
+                "@a add.u32 %2, %2, 1;\n\t"
+                "setp.ge.and.u32 b, %4, %8, a;\n\t"
+                "@b st.shared.u32 [%3], %4;\n\t"
+                "@b add.u32 %3, %3, %9;\n\t"
+                "}"
+                : "+r"(c0), "+r"(p0), "+r"(c1), "+r"(p1)
+                : "r"(key[g * PF_GROUP + j]), "r"(hi0), "r"(lo0), "r"(hi1), "r"(lo1), "n"(ROW)
+                : "memory");
+        }
+        // a thread that could run out of slots in the next group closes its window
+        if (p0 > stop0) {
+            lo0 = hi0;
+            over |= 1u;
+        }
+        if (p1 > stop1) {
+            lo1 = hi1;
+            over |= 2u;
+        }
+    }
+    n[0] = (int)((p0 - b0) / ROW);
+    n[1] = (int)((p1 - b1) / ROW);
+    const uint32_t t0 = __reduce_add_sync(ASR_FULL_MASK, c0 | ((uint32_t)n[0] << 16));
+    const uint32_t t1 = __reduce_add_sync(ASR_FULL_MASK, c1 | ((uint32_t)n[1] << 16));
+    const uint32_t wo = __reduce_or_sync(ASR_FULL_MASK, over);
+    if (lane == 0) {
+        fs.wtot[par][0][warp] = t0;
+        fs.wtot[par][1][warp] = t1;
+        fs.wovf[par][warp] = wo;
+    }
+    __syncthreads();
+    T[0] = T[1] = ov = 0;
+#pragma unroll
+    for (int w = 0; w < PCT_THREADS / 32; ++w) {
+        T[0] += fs.wtot[par][0][w];
+        T[1] += fs.wtot[par][1][w];
+        ov |= fs.wovf[par][w];
+    }
+}
+
+// count-only pass: keys below t0 / below t1 over the whole CTA
+__device__ __forceinline__ void pf_count(const uint32_t (&key)[PCT_VPT], uint32_t t0, uint32_t t1, PctFastSmem &fs, int par,
+                                         uint32_t (&C)[2]) {
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    uint32_t c0 = 0, c1 = 0;
+#pragma unroll
+    for (int j = 0; j < PCT_VPT; ++j) {
+        c0 += key[j] < t0 ? 1u : 0u;
+        c1 += key[j] < t1 ? 1u : 0u;
+    }
+    c0 = __reduce_add_sync(ASR_FULL_MASK, c0);
+    c1 = __reduce_add_sync(ASR_FULL_MASK, c1);
+    if (lane == 0) {
+        fs.wtot[par][0][warp] = c0;
+        fs.wtot[par][1][warp] = c1;
+    }
+    __syncthreads();
+    C[0] = C[1] = 0;
+#pragma unroll
+    for (int w = 0; w < PCT_THREADS / 32; ++w) {
+        C[0] += fs.wtot[par][0][w];
+        C[1] += fs.wtot[par][1][w];
+    }
+}
+
+__global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(const asr_replica_t *replicas, int32_t n_replicas,
+                                                                                const int64_t *lat, const int64_t *ttft,
+                                                                                asr_summary_t *out_summary,
+                                                                                const int32_t *order, int32_t chunk,
+                                                                                int32_t *miss_list, int32_t *miss_count) {
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    PctFastSmem &fs = *reinterpret_cast<PctFastSmem *>(dyn_smem);
+    const int tid = threadIdx.x;
+    const int64_t *vals = blockIdx.y == 0 ? lat : ttft;
+    int32_t *my_miss = miss_list + (size_t)blockIdx.y * n_replicas;
+    bool have = false;
+    uint32_t wlo[2] = {0, 0};
+    int wsh[2] = {0, 0};
+    int par = 0;
+    const int i0 = blockIdx.x * chunk, i1 = min(n_replicas, i0 + chunk);
+    for (int i = i0; i < i1; ++i) {
+        const int r = order ? order[i] : i;
+        if (tid == 0 && i + 1 < i1) {
+            // pull the CTA's next segment into L2 while this one is being processed
+            const int rn = order ? order[i + 1] : i + 1;
+            const asr_replica_t nx = replicas[rn];
+            const int64_t flag = blockIdx.y == 0 ? out_summary[rn].p50_e2e_us : out_summary[rn].p50_ttft_us;
+            // only a descriptor the simulator accepted (n_done >= 0) is dereferenced
+            if (out_summary[rn].n_done >= 0 && flag == ASR_FMT32 && nx.n > 0 && nx.n <= PCT_REG_MAX) {
+                const char *src = reinterpret_cast<const char *>(vals + nx.out_off);
+                const uint32_t sz = (uint32_t)(((int64_t)nx.n * 4) & ~15ll);
+                if (sz > 0 && (reinterpret_cast<uintptr_t>(src) & 15u) == 0)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(sz) : "memory");
+            }
+        }
+        if (out_summary[r].n_done < 0) continue;   // invalid descriptor, flagged by the simulator
+        const int64_t flag = blockIdx.y == 0 ? out_summary[r].p50_e2e_us : out_summary[r].p50_ttft_us;
+        const asr_replica_t rep = replicas[r];
+        const int64_t *seg = vals + rep.out_off;
+        const int N = rep.n;
+        bool settled = flag == ASR_FMT32 && N > 0 && N <= PCT_REG_MAX && (N & 3) == 0 &&
+                       (reinterpret_cast<uintptr_t>(seg) & 15u) == 0;
+        uint32_t res[2] = {0, 0};
+        if (settled) {
+            const uint32_t k[2] = {(50u * (uint32_t)N + 99u) / 100u, (90u * (uint32_t)N + 99u) / 100u};
+            // keys: four consecutive values per 128-bit load; slots past the end read as 2^32-1 (below no window end)
+            uint32_t key[PCT_VPT];
+            {
+                const uint4 *v128 = reinterpret_cast<const uint4 *>(seg);
+                const int n4 = N >> 2;
+#pragma unroll
+                for (int q = 0; q < PCT_VPT / 4; ++q) {
+                    const int idx = q * PCT_THREADS + tid;
+                    uint4 x = make_uint4(~0u, ~0u, ~0u, ~0u);
+                    if (idx < n4) x = __ldcs(v128 + idx);
+                    key[4 * q] = x.x, key[4 * q + 1] = x.y, key[4 * q + 2] = x.z, key[4 * q + 3] = x.w;
+                }
+            }
+            // clear both histogram levels (their last readers passed the final barrier of the previous segment)
+            {
+                uint4 *z = reinterpret_cast<uint4 *>(&fs.hist[0][0][0]);
+                constexpr int n16 = 2 * 2 * PF_BINS / 4;
+                static_assert(n16 % PCT_THREADS == 0, "whole passes");
+#pragma unroll
+                for (int q = 0; q < n16 / PCT_THREADS; ++q) z[q * PCT_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
+            }
+            if (!have) {
+                // bisection on the key bits, both ranks at once: bracket [a, a + 2^rem) holds `in` keys, `below` lie under it
+                uint32_t a[2] = {0, 0}, below[2] = {0, 0}, in[2] = {(uint32_t)N, (uint32_t)N};
+                int rem[2] = {32, 32};
+                while (true) {
+                    const bool go0 = rem[0] > PF_MAX_SHIFT + 10 || (in[0] > PF_IN_MANY && rem[0] > 0);
+                    const bool go1 = rem[1] > PF_MAX_SHIFT + 10 || (in[1] > PF_IN_MANY && rem[1] > 0);
+                    if (!go0 && !go1) break;
+                    const uint32_t m0 = go0 ? a[0] + (1u << (rem[0] - 1)) : a[0], m1 = go1 ? a[1] + (1u << (rem[1] - 1)) : a[1];
+                    uint32_t C[2];
+                    pf_count(key, m0, m1, fs, par, C);
+                    par ^= 1;
+                    if (go0) {
+                        --rem[0];
+                        if (k[0] <= C[0]) in[0] = C[0] - below[0];
+                        else in[0] -= C[0] - below[0], below[0] = C[0], a[0] = m0;
+                    }
+                    if (go1) {
+                        --rem[1];
+                        if (k[1] <= C[1]) in[1] = C[1] - below[1];
+                        else in[1] -= C[1] - below[1], below[1] = C[1], a[1] = m1;
+                    }
+                }
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    wlo[t] = a[t];
+                    wsh[t] = rem[t] > 10 ? rem[t] - 10 : 0;
+                }
+                have = true;
+#ifdef PCT_STATS
+                if (tid == 0) atomicAdd(&g_pct_stats[3], 1ull);
+#endif
+            }
+            uint32_t T[2], ov;
+            int n[2];
+            for (int attempt = 0;; ++attempt) {
+                pf_pass(key, wlo[0], pf_end(wlo[0], wsh[0]), wlo[1], pf_end(wlo[1], wsh[1]), fs, par, T, ov, n);
+                par ^= 1;
+#ifdef PCT_STATS
+                if (tid == 0) atomicAdd(&g_pct_stats[2], 1ull);
+#endif
+                bool ok = true;
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    const uint32_t c = T[t] & 0xFFFFu, in = T[t] >> 16, hi = pf_end(wlo[t], wsh[t]);
+                    if (k[t] > c) {   // above the window (exact even when a thread ran out of slots)
+                        ok = false;
+                        if (hi == 0xFFFFFFFFu) attempt = PF_TRIES;   // nothing above: keys of 2^32-1, radix path
+                        wlo[t] = hi;
+                        wsh[t] += wsh[t] < PF_MAX_SHIFT ? 1 : 0;
+                    } else if ((ov >> t) & 1u) {   // too dense for the slots: the upper half, then look again
+                        ok = false;
+                        if (wsh[t] == 0) attempt = PF_TRIES;
+                        else {
+                            --wsh[t];
+                            wlo[t] = hi - ((uint32_t)PF_BINS << wsh[t]);
+                        }
+                    } else if (k[t] <= c - in) {   // below the window
+                        ok = false;
+                        wsh[t] += wsh[t] < PF_MAX_SHIFT ? 1 : 0;
+                        const uint32_t W = (uint32_t)PF_BINS << wsh[t];
+                        wlo[t] = wlo[t] > W ? wlo[t] - W : 0u;
+                    }
+                }
+                if (ok) break;
+                if (attempt >= PF_TRIES - 1) {
+                    settled = false;
+                    break;
+                }
+            }
+            if (settled) {
+                const int sh0 = wsh[0], sh1 = wsh[1];
+                const uint32_t lo0 = wlo[0], lo1 = wlo[1];
+                const uint32_t in0 = T[0] >> 16, in1 = T[1] >> 16;
+                const uint32_t below0 = (T[0] & 0xFFFFu) - in0, below1 = (T[1] & 0xFFFFu) - in1;
+                // level 1: bins of 2^sh values over the window
+                const int nm = n[0] > n[1] ? n[0] : n[1];
+                for (int e = 0; e < nm; ++e) {
+                    if (e < n[0]) atomicAdd(&fs.hist[0][0][(fs.slot[0][e][tid] - lo0) >> sh0], 1u);
+                    if (e < n[1]) atomicAdd(&fs.hist[0][1][(fs.slot[1][e][tid] - lo1) >> sh1], 1u);
+                }
+                __syncthreads();
+                const int tg = tid / PF_HALF, j = tid % PF_HALF;
+                const uint32_t kw = tg == 0 ? k[0] - below0 : k[1] - below1;   // rank inside the window
+                uint32_t c[8], tot, incl;
+                pf_scan_a(fs.hist[0][tg], j, c, tot, incl, fs.wsum[tg]);
+                __syncthreads();
+                pf_scan_b(c, tot, incl, fs.wsum[tg], j, kw, &fs.sel_bin[0][tg], &fs.sel_rem[0][tg]);
+                __syncthreads();
+                const uint32_t bin0 = fs.sel_bin[0][0], bin1 = fs.sel_bin[0][1];
+                uint32_t r0 = lo0 + (bin0 << sh0), r1 = lo1 + (bin1 << sh1);
+                if (sh0 > 0 || sh1 > 0) {
+                    // level 2: the selected bin, one value per bin
+                    const int m0 = sh0 > 0 ? n[0] : 0, m1 = sh1 > 0 ? n[1] : 0, mm = m0 > m1 ? m0 : m1;
+                    for (int e = 0; e < mm; ++e) {
+                        if (e < m0) {
+                            const uint32_t d = fs.slot[0][e][tid] - lo0;
+                            if ((d >> sh0) == bin0) atomicAdd(&fs.hist[1][0][d & ((1u << sh0) - 1u)], 1u);
+                        }
+                        if (e < m1) {
+                            const uint32_t d = fs.slot[1][e][tid] - lo1;
+                            if ((d >> sh1) == bin1) atomicAdd(&fs.hist[1][1][d & ((1u << sh1) - 1u)], 1u);
+                        }
+                    }
+                    __syncthreads();
+                    const bool act = tg == 0 ? sh0 > 0 : sh1 > 0;
+                    if (act) pf_scan_a(fs.hist[1][tg], j, c, tot, incl, fs.wsum[tg]);
+                    __syncthreads();
+                    if (act) pf_scan_b(c, tot, incl, fs.wsum[tg], j, fs.sel_rem[0][tg], &fs.sel_bin[1][tg], &fs.sel_rem[1][tg]);
+                    __syncthreads();
+                    if (sh0 > 0) r0 += fs.sel_bin[1][0];
+                    if (sh1 > 0) r1 += fs.sel_bin[1][1];
+                }
+                res[0] = r0;
+                res[1] = r1;
+                // the next segment's windows: centred on these answers, as wide as keeps the slots comfortably filled
+                const uint32_t inw[2] = {in0, in1};
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    if (inw[t] > PF_IN_MANY) wsh[t] -= wsh[t] > 0 ? 1 : 0;
+                    else if (inw[t] < PF_IN_FEW) wsh[t] += wsh[t] < PF_MAX_SHIFT ? 1 : 0;
+                    const uint32_t half = (uint32_t)PF_BINS << wsh[t] >> 1;
+                    wlo[t] = res[t] > half ? res[t] - half : 0u;
+                }
+#ifdef PCT_STATS
+                if (tid == 0) {
+                    atomicAdd(&g_pct_stats[1], 1ull);
+                    atomicAdd(&g_pct_stats[5], (unsigned long long)(in0 + in1));
+                }
+#endif
+            }
+            __syncthreads();   // the next segment rewrites slots, totals and histograms
+        }
+#ifdef PCT_STATS
+        if (tid == 0) atomicAdd(&g_pct_stats[0], 1ull);
+#endif
+        if (tid == 0) {
+            if (settled) {
+                if (blockIdx.y == 0) {
+                    out_summary[r].p50_e2e_us = (int64_t)res[0];
+                    out_summary[r].p90_e2e_us = (int64_t)res[1];
+                } else {
+                    out_summary[r].p50_ttft_us = (int64_t)res[0];
+                    out_summary[r].p90_ttft_us = (int64_t)res[1];
+                }
+            } else {
+                my_miss[atomicAdd(miss_count + blockIdx.y, 1)] = r;
+#ifdef PCT_STATS
+                atomicAdd(&g_pct_stats[4], 1ull);
+#endif
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) percentiles_kernel(const int64_t *values, const int64_t *seg_off,
                                                                   int32_t n_seg, PctList pl, int64_t *out) {
     extern __shared__ __align__(16) unsigned char dyn_smem[];
@@ -482,11 +883,13 @@ __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) percentiles_kernel(
     }
 }
 
-// p50/p90 of E2E latency (blockIdx.y = 0) and TTFT (blockIdx.y = 1) of every replica
+// p50/p90 of E2E latency (blockIdx.y = 0) and TTFT (blockIdx.y = 1) of every replica, or -- with a work list --
+// of the replicas the carried-window kernel left: list[y*n_replicas + 0 .. count[y]).
 __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles_kernel(const asr_replica_t *replicas,
                                                                           int32_t n_replicas, const int64_t *lat,
                                                                           const int64_t *ttft,
-                                                                          asr_summary_t *out_summary, bool fmt_flags) {
+                                                                          asr_summary_t *out_summary, bool fmt_flags,
+                                                                          const int32_t *list, const int32_t *count) {
     extern __shared__ __align__(16) unsigned char dyn_smem[];
     PctRegSmem &sm = *reinterpret_cast<PctRegSmem *>(dyn_smem);
     PctList pl;
@@ -494,10 +897,13 @@ __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles
     pl.pct[0] = 50;
     pl.pct[1] = 90;
     const int64_t *vals = blockIdx.y == 0 ? lat : ttft;
-    for (int r = blockIdx.x; r < n_replicas; r += gridDim.x) {
-        if (threadIdx.x == 0 && r + (int)gridDim.x < n_replicas) {
+    const int total = list ? count[blockIdx.y] : n_replicas;
+    const int32_t *my_list = list ? list + (size_t)blockIdx.y * n_replicas : nullptr;
+    for (int w = blockIdx.x; w < total; w += gridDim.x) {
+        const int r = my_list ? my_list[w] : w;
+        if (threadIdx.x == 0 && w + (int)gridDim.x < total) {
             // pull the CTA's next segment into L2 while this one is being processed
-            const int rn = r + gridDim.x;
+            const int rn = my_list ? my_list[w + gridDim.x] : w + gridDim.x;
             const asr_replica_t nx = replicas[rn];
             const int64_t flag = blockIdx.y == 0 ? out_summary[rn].p50_e2e_us : out_summary[rn].p50_ttft_us;
             const int64_t bytes = (int64_t)nx.n * ((fmt_flags && flag == ASR_FMT32) ? 4 : 8);
@@ -532,11 +938,12 @@ __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles
 }
 
 static constexpr size_t PCT_DYN_SMEM = sizeof(PctRegSmem);
+static constexpr size_t PF_DYN_SMEM = sizeof(PctFastSmem);
 
-static int pct_grid(int n_units, const void *fn) {
+static int pct_grid(int n_units, const void *fn, size_t smem = PCT_DYN_SMEM) {
     const int n_sm = sm_count();
     int per_sm = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, PCT_THREADS, PCT_DYN_SMEM);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, PCT_THREADS, smem);
     if (per_sm < 1) per_sm = 1;
     int cap = n_sm * per_sm;
     return n_units < cap ? n_units : cap;
@@ -558,17 +965,45 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
     return check_launch("percentiles_kernel");
 }
 
+// fmt_flags with a miss list (2*n_replicas entries + 2 zeroed counters): the carried-window kernel first, the
+// radix kernel on what it left.  Otherwise the radix kernel on every replica.
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
-                               const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, cudaStream_t st) {
+                               const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, const int32_t *order,
+                               int32_t *miss_list, int32_t *miss_count, cudaStream_t st) {
     if (n_replicas <= 0) return ASR_OK;
     cudaFuncSetAttribute(summary_percentiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PCT_DYN_SMEM);
     int gx = pct_grid(n_replicas, (const void *)summary_percentiles_kernel);
     gx = gx > 1 ? (gx + 1) / 2 : 1;
-    dim3 grid(gx, 2);
+    const bool fast = fmt_flags && miss_list && miss_count && PCT_THREADS == 256;
+    if (fast) {
+        cudaFuncSetAttribute(summary_fast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PF_DYN_SMEM);
+        int fx = pct_grid(n_replicas, (const void *)summary_fast_kernel, PF_DYN_SMEM);
+        fx = fx > 1 ? (fx + 1) / 2 : 1;
+        // every CTA walks one run of consecutive segments
+        const int chunk = (n_replicas + fx - 1) / fx;
+        fx = (n_replicas + chunk - 1) / chunk;
+        {
+            KernelTimer kt(KID_SUMMARY_FAST, st);
+            summary_fast_kernel<<<dim3(fx, 2), PCT_THREADS, PF_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary,
+                                                                               order, chunk, miss_list, miss_count);
+        }
+        int rc = check_launch("summary_fast_kernel");
+        if (rc) return rc;
+#ifdef PCT_STATS
+        {
+            unsigned long long h[8], z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            cudaStreamSynchronize(st);
+            cudaMemcpyFromSymbol(h, g_pct_stats, sizeof(h));
+            cudaMemcpyToSymbol(g_pct_stats, z, sizeof(z));
+            fprintf(stderr, "pct stats: segments %llu settled %llu passes %llu bootstraps %llu misses %llu in-window/settled %.0f\n",
+                    h[0], h[1], h[2], h[3], h[4], h[1] ? (double)h[5] / (double)h[1] : 0.0);
+        }
+#endif
+    }
     {
         KernelTimer kt(KID_SUMMARY_PCT, st);
-        summary_percentiles_kernel<<<grid, PCT_THREADS, PCT_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary,
-                                                                            fmt_flags);
+        summary_percentiles_kernel<<<dim3(gx, 2), PCT_THREADS, PCT_DYN_SMEM, st>>>(
+            replicas, n_replicas, lat, ttft, out_summary, fmt_flags, fast ? miss_list : nullptr, fast ? miss_count : nullptr);
     }
     return check_launch("summary_percentiles_kernel");
 }

@@ -421,14 +421,40 @@ __device__ __forceinline__ void stage_tail(uint32_t *base, int ph, int n, const 
 // event order through Stage32.  Exact as long as every value is below 2^32 us, which the
 // kernel proves with the start of the current busy period (every request in the system
 // arrived at or after it); a busy period of 2^32 us sends the replica to the warp kernel.
-template <bool FREE>
-__global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
-    __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
-    const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
+// MODE (order-free outputs only):
+//   LANE_SEQ     a thread simulates a whole replica (with a plan: only the replicas flagged `failed`).
+//   LANE_UNIT    a thread simulates one segment [b, b + L) of a replica's trace AS IF it were a trace of its own:
+//                the server is taken to be idle at the segment's first arrival and the trace to end with the
+//                segment.  It records its regeneration points (server empty at an arrival at or after the clock:
+//                the state is then (empty, t = that arrival) whatever came before) in the replica's bitmap, and
+//                the last one in unit_q -- the segment's end itself if everything completed by the next arrival.
+//   LANE_REPAIR  a thread stitches the boundary between segments s-1 and s: unless segment s-1 ended at a
+//                regeneration point, it simulates from the last regeneration point q of segment s-1 (a TRUE state
+//                when the segments before are stitched) across the boundary until it reaches a regeneration point
+//                that segment s recorded too -- from there on segment s's values are the true ones -- and
+//                overwrites the values of the requests [q, that point) in place (positions = request indices for
+//                both streams: at a regeneration point exactly the requests before it have been emitted).
+// Every value that survives comes from a simulation that started in a true state; a boundary that cannot be
+// stitched inside segment s flags the replica, which is then simulated in one piece.
+enum { LANE_SEQ = 0, LANE_UNIT = 1, LANE_REPAIR = 2 };
+
+__host__ __device__ __forceinline__ int lane_seg_len(int n, int nseg) {
+    return (((n + nseg - 1) / nseg) + 31) & ~31;   // whole bitmap words per segment
+}
+
+// one lane's piece; all 32 lanes of a warp call it together (`live` = this lane has a piece).  sbase = the lane's
+// column of the CTA's ring; r = replica; seg / nseg = its segment (units); uq = its unit_q entry
+template <bool FREE, int MODE>
+__device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase, bool live, const int r, const int seg,
+                                         const int nseg, const int uq) {
+    static_assert(FREE || MODE == LANE_SEQ, "units need order-free outputs");
     // every lane of a warp stays in the loop below until the whole warp is done (the loop
     // re-converges the warp once per admission step); `live` marks the lanes with work
-    bool live = r < a.n_replicas;
+    if (MODE == LANE_REPAIR && seg == 0) live = false;
     bool valid = live;
+    int start = 0;        // first request of this thread's piece (index in the replica)
+    int seg_b = 0;        // first request of segment `seg`
+    int piece_n = -1;     // requests in the piece (-1: the whole replica)
     asr_replica_t rep;
     rep.trace_off = rep.out_off = 0;
     rep.n = 0;
@@ -437,14 +463,29 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     if (live) {
         rep = a.replicas[r];
         if (!replica_ok(a, rep, LANE_CAP)) {
-            flag_invalid(a, r);
+            flag_invalid(a, r);   // (an invalid descriptor is one unit)
             live = valid = false;
             rep.cm_id = 0;
             rep.n = 0;
         }
     }
-    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_ring) + threadIdx.x * 8u;
-    const int n = rep.n, slots = rep.slots, policy = rep.policy;
+    if (MODE != LANE_SEQ && live) {
+        const int L = lane_seg_len(rep.n, nseg);
+        seg_b = seg * L;
+        if (MODE == LANE_UNIT) {
+            start = seg_b;
+            piece_n = min(L, rep.n - seg_b);
+        } else {
+            const int q = a.plan.unit_q[uq - 1];   // the entries of a replica are consecutive
+            if (q >= seg_b || a.plan.failed[r] != 0) {
+                live = valid = false;   // segment s-1 ended at a regeneration point (or the replica is flagged already)
+            } else {
+                start = q;
+                piece_n = min(seg_b + L, rep.n) - q;
+            }
+        }
+    }
+    const int n = piece_n >= 0 ? piece_n : rep.n, slots = rep.slots, policy = rep.policy;
     const asr_cost_model_t *cmp = a.cms + rep.cm_id;
     const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
     const int64_t iter_base64 = __ldg(&cmp->iter_base_us), iter_per64 = __ldg(&cmp->iter_per_running_us);
@@ -463,9 +504,16 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     const uint32_t enc_base = (uint32_t)enc_base64;
     const int32_t enc_per = (int32_t)enc_per64;
     const uint32_t ib = (uint32_t)iter_base64, ip = (uint32_t)iter_per64;
-    const asr_req_t *trace = a.traces + rep.trace_off;
+    const asr_req_t *trace = a.traces + rep.trace_off + start;
     int64_t *lat = a.out_lat + rep.out_off;
     int64_t *ttft = a.out_ttft + rep.out_off;
+    // units: the regeneration points of this piece, one bit per request, in the replica's bitmap (whole words per
+    // segment); `ibits` collects the word `wcur`
+    uint32_t *bm = nullptr;
+    if (MODE != LANE_SEQ && live) bm = a.bitmap + a.bm_off[r] + (seg_b >> 5);
+    uint32_t ibits = 0;
+    int wcur = 0, q_last = 0;
+    bool merged = false;
 
     int64_t t = 0;     // the current iteration boundary
     int64_t tb = 0;    // FREE: start of the current busy period (arrival of its first request)
@@ -496,10 +544,12 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     const bool staged = (reinterpret_cast<uintptr_t>(ttft) & 15u) == 0;
     // FREE: both outputs through Stage32
     Stage32 sq_t = {0, 0, 0, 0}, sq_l = {0, 0, 0, 0};
-    uint32_t *ttft32 = reinterpret_cast<uint32_t *>(ttft), *lat32 = reinterpret_cast<uint32_t *>(lat);
-    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft) >> 2) & 3u);
-    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat) >> 2) & 3u);
-    const int64_t first_arrival = n > 0 ? arr0 : 0;
+    uint32_t *ttft32 = reinterpret_cast<uint32_t *>(ttft) + start, *lat32 = reinterpret_cast<uint32_t *>(lat) + start;
+    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft32) >> 2) & 3u);
+    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat32) >> 2) & 3u);
+    // (written now rather than carried through the loop: the kernel sits at its register limit)
+    if (valid && a.out_summary && (MODE == LANE_SEQ || (MODE == LANE_UNIT && seg == 0)))
+        a.out_summary[r].first_arrival_us = n > 0 ? arr0 : 0;
     if (n == 0) live = false;
 
     // One trip of the outer loop = one admission step, so that the lanes of a warp (32
@@ -551,7 +601,29 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
         if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
         if (live) {
             // B. the boundary of the admission step
-            if (nW == 0 && nR == 0) tb = arr0;   // a new busy period starts with the next arrival
+            if (nW == 0 && nR == 0) {
+                tb = arr0;   // a new busy period starts with the next arrival
+#ifndef LANE_NO_REGEN
+                if (MODE != LANE_SEQ && arr0 >= t && p < n) {
+                    // regeneration point: the server is empty when request p arrives, the clock goes to that arrival
+                    if (MODE == LANE_UNIT) {
+                        while (wcur < (p >> 5)) {
+                            bm[wcur] = ibits;
+                            ibits = 0;
+                            ++wcur;
+                        }
+                        ibits |= 1u << (p & 31);
+                        q_last = p;
+                    } else {
+                        const int d = start + p - seg_b;   // position in segment s
+                        if (d >= 0 && ((__ldcg(bm + (d >> 5)) >> (d & 31)) & 1u)) {
+                            merged = true;   // segment s was in this very state: its values are true from here on
+                            live = false;
+                        }
+                    }
+                }
+#endif
+            }
             if (nW == 0 && arr0 > t) {
                 if (nR == 0) {
                     t = arr0;   // idle server: the clock jumps to the next arrival (S14)
@@ -563,7 +635,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
                 }
             }
             // C. ingest arrivals <= t
-            while (arr0 <= t) {
+            while (arr0 <= t && (MODE != LANE_REPAIR || !merged)) {
                 last_arr = arr0;
                 last_dur = dur0;
                 ++p;
@@ -584,7 +656,9 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             // D. admit k >= 1 requests (a slot is free and somebody waits)
             const int free_slots = slots - nR;
             const int k = free_slots < nW ? free_slots : nW;
-            if (policy != ASR_FCFS && k < nW) {   // a real choice: hand over to the warp kernel
+            if (MODE == LANE_REPAIR && merged) {
+                // stitched: nothing more to simulate
+            } else if (policy != ASR_FCFS && k < nW) {   // a real choice: hand over to the warp kernel
                 deferred = true;
                 live = false;
             } else {
@@ -620,6 +694,42 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
             }
         }
     }
+    if (MODE != LANE_SEQ) {
+        if (deferred) {
+            a.plan.failed[r] = 1;   // whatever stopped this piece, the replica is simulated in one piece
+            return;
+        }
+        if (!valid) return;
+        if (MODE == LANE_UNIT) {
+            stage_tail(ttft32, ph_t, n, sq_t);
+            stage_tail(lat32, ph_l, n, sq_l);
+            for (; wcur <= ((n - 1) >> 5); ++wcur) {
+                bm[wcur] = ibits;
+                ibits = 0;
+            }
+            // everything completed by the next segment's first arrival: the segment's end is a regeneration point
+            if (start + n < rep.n && t <= ld_arrival(trace + n)) q_last = n;
+            a.plan.unit_q[uq] = start + q_last;
+            asr_summary_t *s = a.out_summary + r;
+            if (seg == nseg - 1) {
+                s->last_done_us = t;
+                s->n_done = rep.n;
+                s->p50_e2e_us = ASR_FMT32;
+                s->p50_ttft_us = ASR_FMT32;
+            }
+        } else {
+            const bool to_end = done >= n && start + n == rep.n;   // the last boundary, simulated to the end of the trace
+            if (!merged && !to_end) {
+                a.plan.failed[r] = 1;   // no common regeneration point inside segment s
+                return;
+            }
+            const int cnt = merged ? p : n;   // at a regeneration point exactly the requests before it have been emitted
+            stage_tail(ttft32, ph_t, cnt, sq_t);
+            stage_tail(lat32, ph_l, cnt, sq_l);
+            if (to_end && !merged) a.out_summary[r].last_done_us = t;
+        }
+        return;
+    }
     if (deferred) {
         const int pos = atomicAdd(a.defer_count, 1);
         a.defer_list[pos] = r;
@@ -645,10 +755,159 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     }
     if (valid && a.out_summary) {
         asr_summary_t *s = a.out_summary + r;
-        s->first_arrival_us = first_arrival;
         s->last_done_us = t;
         s->n_done = done;
     }
+}
+
+// a thread simulates a whole replica (with a plan: only the replicas flagged `failed`)
+template <bool FREE>
+__global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
+    __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_ring) + threadIdx.x * 8u;
+    const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
+    bool live = r < a.n_replicas;
+    if (live && a.plan.failed && a.plan.failed[r] == 0) live = false;   // stitched: nothing to redo
+    lane_run<FREE, LANE_SEQ>(a, sbase, live, r, 0, 1, 0);
+}
+
+// persistent warps work off the plan's items (heaviest load class first): lane j of item (group, seg) takes
+// segment seg of replica order[32*group + j]
+#ifndef LANE_WORK_BLOCKS
+#define LANE_WORK_BLOCKS 12
+#endif
+constexpr int LANE_WORK_BLOCKS_PER_SM = LANE_WORK_BLOCKS;   // one CTA less than the replica kernel: the unit's extra state
+template <int MODE>
+__global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lane_work_kernel(SimArgs a) {
+    __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_ring) + threadIdx.x * 8u;
+    const int lane = lane_id();
+    const int n_items = ((a.n_replicas + 31) / 32) * LANE_MAX_SEG;
+    int32_t *next = a.plan.counters + (MODE == LANE_UNIT ? 0 : 1);
+    while (true) {
+        int w = 0;
+        if (lane == 0) w = atomicAdd(next, 1);
+        w = __shfl_sync(ASR_FULL_MASK, w, 0);
+        if (w >= n_items) break;
+        const int2 item = make_int2(w / LANE_MAX_SEG, w % LANE_MAX_SEG);
+        if (MODE == LANE_REPAIR && item.y == 0) continue;
+        const int pos = 32 * item.x + lane;
+        bool live = pos < a.n_replicas;
+        int r = 0, nseg = 1;
+        if (live) {
+            r = a.plan.order[pos];
+            nseg = a.plan.nseg[r];
+            live = item.y < nseg;
+        }
+        if (!__any_sync(ASR_FULL_MASK, live)) continue;   // no replica of the group has this many segments
+        const int uq = pos * LANE_MAX_SEG + item.y;
+        lane_run<true, MODE>(a, sbase, live, r, item.y, nseg, uq);
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------
+// the plan of a summary-only thread-per-replica call: load classes, order, units
+// ---------------------------------------------------------------------------
+// Offered load of a replica in Erlangs, estimated from a few records (mean arrival gap, mean solo service time of
+// a few dozen sampled requests).  It only steers the schedule -- which replicas share a warp, which are cut into
+// segments -- and never a result.
+constexpr int PLAN_BUCKETS = 32;
+constexpr float PLAN_SPLIT_MAX_LOAD = 4.f;   // beyond it regeneration points (about exp(-load) of the arrivals) are too rare to stitch at
+constexpr int PLAN_SAMPLES = 32;
+
+__global__ void __launch_bounds__(256) lane_key_kernel(SimArgs a) {
+    const int r = blockIdx.x * 256 + threadIdx.x;
+    if (r >= a.n_replicas) return;
+    const asr_replica_t rep = a.replicas[r];
+    int bucket = PLAN_BUCKETS - 1, nseg = 1;
+    if (replica_ok(a, rep, LANE_CAP) && rep.n >= 2) {
+        const asr_req_t *tr = a.traces + rep.trace_off;
+        const int n = rep.n;
+        const asr_cost_model_t cm = a.cms[rep.cm_id];
+        float svc = 0.f;
+#pragma unroll 8
+        for (int j = 0; j < PLAN_SAMPLES; ++j) {
+            const int idx = (int)(((int64_t)(2 * j + 1) * n) / (2 * PLAN_SAMPLES));
+            const int32_t dur = __ldg(&tr[idx].dur_ms);
+            svc += (float)(cm.enc_base_us + cm.enc_per_ms_us * (int64_t)dur) +
+                   (float)tokens_of(cm, dur) * (float)(cm.iter_base_us + cm.iter_per_running_us);
+        }
+        svc *= 1.f / PLAN_SAMPLES;
+        const float gap = (float)(ld_arrival(tr + n - 1) - ld_arrival(tr)) / (float)(n - 1);
+        const float load = gap > 0.f ? svc / gap : 1e9f;
+        if (load > 0.f) {
+            const int b = 16 - (int)rintf(4.f * log2f(load));   // four classes per octave, heaviest first
+            bucket = b < 0 ? 0 : (b > PLAN_BUCKETS - 2 ? PLAN_BUCKETS - 2 : b);
+        }
+        if (load <= PLAN_SPLIT_MAX_LOAD && n >= 2 * LANE_SEG_TARGET) {
+            nseg = n / LANE_SEG_TARGET;
+            nseg = nseg > LANE_MAX_SEG ? LANE_MAX_SEG : nseg;
+        }
+    }
+#ifdef PLAN_NO_SORT
+    bucket = 0;
+#endif
+    a.plan.bucket[r] = (uint8_t)bucket;
+    a.plan.nseg[r] = (uint8_t)nseg;
+    a.plan.failed[r] = 0;
+    if (r == 0) a.plan.counters[0] = a.plan.counters[1] = 0;
+}
+
+// exclusive scan over the 1,024 threads of the CTA; returns the thread's offset, *total = the sum
+__device__ __forceinline__ uint32_t block_excl_scan_1024(uint32_t v, uint32_t *wsum, uint32_t *total) {
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    uint32_t x = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, x, d);
+        if (lane >= d) x += y;
+    }
+    __syncthreads();   // wsum's readers of the previous call are done
+    if (lane == 31) wsum[warp] = x;
+    __syncthreads();
+    uint32_t w = wsum[lane];
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, w, d);
+        if (lane >= d) w += y;
+    }
+    *total = __shfl_sync(ASR_FULL_MASK, w, 31);
+    const uint32_t wbase = __shfl_sync(ASR_FULL_MASK, w, warp > 0 ? warp - 1 : 0);
+    return (warp > 0 ? wbase : 0u) + x - v;
+}
+
+// one CTA: stable counting sort of the replicas by load class (thread t owns the replicas [tC, tC + C) and one
+// column of the [class][thread] counters)
+__global__ void __launch_bounds__(1024) lane_sort_kernel(SimArgs a) {
+    extern __shared__ uint32_t cnt[];   // [PLAN_BUCKETS][1024]
+    __shared__ uint32_t wsum[32];
+    const int t = threadIdx.x, n = a.n_replicas;
+    const int C = (n + 1023) / 1024;
+    const int r0 = (int)min((int64_t)n, (int64_t)t * C), r1 = min(n, r0 + C);
+    for (int b = 0; b < PLAN_BUCKETS; ++b) cnt[b * 1024 + t] = 0;
+    for (int r = r0; r < r1; ++r) cnt[a.plan.bucket[r] * 1024 + t]++;
+    uint32_t base = 0;
+    for (int b = 0; b < PLAN_BUCKETS; ++b) {
+        uint32_t tot;
+        const uint32_t v = cnt[b * 1024 + t];
+        cnt[b * 1024 + t] = base + block_excl_scan_1024(v, wsum, &tot);
+        base += tot;
+    }
+    for (int r = r0; r < r1; ++r) a.plan.order[cnt[a.plan.bucket[r] * 1024 + t]++] = r;
+}
+
+int launch_lane_plan(const SimArgs &a, cudaStream_t st) {
+    const int grid = (a.n_replicas + 255) / 256;
+    constexpr int SORT_SMEM = PLAN_BUCKETS * 1024 * 4;
+    cudaFuncSetAttribute(lane_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_SMEM);
+    {
+        KernelTimer kt(KID_LANE_PLAN, st);
+        lane_key_kernel<<<grid, 256, 0, st>>>(a);
+        lane_sort_kernel<<<1, 1024, SORT_SMEM, st>>>(a);
+    }
+    count_launch(1);
+    return check_launch("lane plan kernels");
 }
 
 // out_lat[i] = -arrival_us[i] for every request of every replica the lane kernel will
@@ -677,6 +936,8 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
         carry_s = 0;
         defer_count[0] = 0;   // lane kernel -> warp kernel
         defer_count[1] = 0;   // warp kernel -> CTA kernel
+        defer_count[2] = 0;   // carried-window percentile kernel -> radix kernel, E2E latency
+        defer_count[3] = 0;   // the same, TTFT
     }
     __syncthreads();
     const int lane = lane_id(), warp = threadIdx.x >> 5;
@@ -736,7 +997,26 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
     SimArgs a = a_in;
     if (use_lane && max_slots <= LANE_CAP) {
         const int lane_grid = (a.n_replicas + LANE_THREADS - 1) / LANE_THREADS;
-        if (a.order_free) {
+        if (a.order_free && a.plan.order) {
+            // time-split units, stitched at regeneration points; what could not be stitched, in one piece
+            int rc0 = launch_lane_plan(a, st);
+            if (rc0) return rc0;
+            const int work_grid = sm_count() * LANE_WORK_BLOCKS_PER_SM;
+            {
+                KernelTimer kt(KID_SIM_LANE, st);
+                sim_lane_work_kernel<LANE_UNIT><<<work_grid, LANE_THREADS, 0, st>>>(a);
+            }
+            rc0 = check_launch("sim_lane_work_kernel<units>");
+            if (rc0) return rc0;
+            {
+                KernelTimer kt(KID_SIM_REPAIR, st);
+                sim_lane_work_kernel<LANE_REPAIR><<<work_grid, LANE_THREADS, 0, st>>>(a);
+            }
+            rc0 = check_launch("sim_lane_work_kernel<repair>");
+            if (rc0) return rc0;
+            KernelTimer kt(KID_SIM_REDO, st);
+            sim_lane_kernel<true><<<lane_grid, LANE_THREADS, 0, st>>>(a);
+        } else if (a.order_free) {
             KernelTimer kt(KID_SIM_LANE, st);
             sim_lane_kernel<true><<<lane_grid, LANE_THREADS, 0, st>>>(a);
         } else {
