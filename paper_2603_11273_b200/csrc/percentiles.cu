@@ -492,10 +492,10 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
 // No result depends on a guess.
 // ---------------------------------------------------------------------------
 #ifndef PF_SLOTS_N
-#define PF_SLOTS_N 24
+#define PF_SLOTS_N 16
 #endif
 #ifndef PF_MIN_CTAS
-#define PF_MIN_CTAS 3
+#define PF_MIN_CTAS 4
 #endif
 #ifdef PCT_STATS
 __device__ unsigned long long g_pct_stats[8];   // segments, settled, passes, bootstraps, misses, in-window keys, -, -
@@ -506,7 +506,10 @@ constexpr int PF_BINS = 1024;          // bins per histogram level
 constexpr int PF_MAX_SHIFT = 10;       // window = PF_BINS << shift values; the second level resolves 2^shift
 constexpr int PF_HALF = PCT_THREADS / 2;
 constexpr int PF_TRIES = 6;
-constexpr uint32_t PF_IN_MANY = 64u * (PF_SLOTS - PF_GROUP), PF_IN_FEW = PF_IN_MANY / 4;   // keys wanted inside a window
+#ifndef PF_IN_MANY_N
+#define PF_IN_MANY_N 256   // one key per thread: a thread with more than PF_SLOTS - PF_GROUP closes its window
+#endif
+constexpr uint32_t PF_IN_MANY = PF_IN_MANY_N, PF_IN_FEW = PF_IN_MANY / 4;   // keys wanted inside a window
 static_assert(PCT_VPT % PF_GROUP == 0 && PF_SLOTS > PF_GROUP, "slot check granularity");
 
 struct PctFastSmem {

@@ -21,6 +21,9 @@
 // admitted requests and the admit step scans the trace window [lo, p) with
 // coalesced 128-bit loads, applying the exact comparator of asr_sched.h.
 #include "sim_common.cuh"
+#ifdef LANE_STATS
+#include <cstdio>
+#endif
 
 namespace asr {
 
@@ -437,6 +440,11 @@ __device__ __forceinline__ void stage_tail(uint32_t *base, int ph, int n, const 
 // Every value that survives comes from a simulation that started in a true state; a boundary that cannot be
 // stitched inside segment s flags the replica, which is then simulated in one piece.
 enum { LANE_SEQ = 0, LANE_UNIT = 1, LANE_REPAIR = 2 };
+#ifdef LANE_STATS
+// tuning builds: units run, units flagged, repairs run, repairs that found no common point, replicas redone,
+// requests re-simulated by repairs
+__device__ unsigned long long g_lane_stats[8];
+#endif
 
 __host__ __device__ __forceinline__ int lane_seg_len(int n, int nseg) {
     return (((n + nseg - 1) / nseg) + 31) & ~31;   // whole bitmap words per segment
@@ -697,9 +705,16 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
     if (MODE != LANE_SEQ) {
         if (deferred) {
             a.plan.failed[r] = 1;   // whatever stopped this piece, the replica is simulated in one piece
+#ifdef LANE_STATS
+            atomicAdd(&g_lane_stats[1], 1ull);
+#endif
             return;
         }
         if (!valid) return;
+#ifdef LANE_STATS
+        atomicAdd(&g_lane_stats[MODE == LANE_UNIT ? 0 : 2], 1ull);
+        if (MODE == LANE_REPAIR) atomicAdd(&g_lane_stats[5], (unsigned long long)p);
+#endif
         if (MODE == LANE_UNIT) {
             stage_tail(ttft32, ph_t, n, sq_t);
             stage_tail(lat32, ph_l, n, sq_l);
@@ -721,6 +736,9 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
             const bool to_end = done >= n && start + n == rep.n;   // the last boundary, simulated to the end of the trace
             if (!merged && !to_end) {
                 a.plan.failed[r] = 1;   // no common regeneration point inside segment s
+#ifdef LANE_STATS
+                atomicAdd(&g_lane_stats[3], 1ull);
+#endif
                 return;
             }
             const int cnt = merged ? p : n;   // at a regeneration point exactly the requests before it have been emitted
@@ -768,6 +786,9 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
     const int r = blockIdx.x * LANE_THREADS + threadIdx.x;
     bool live = r < a.n_replicas;
     if (live && a.plan.failed && a.plan.failed[r] == 0) live = false;   // stitched: nothing to redo
+#ifdef LANE_STATS
+    if (live && a.plan.failed) atomicAdd(&g_lane_stats[4], 1ull);
+#endif
     lane_run<FREE, LANE_SEQ>(a, sbase, live, r, 0, 1, 0);
 }
 
@@ -784,11 +805,19 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lan
     const int lane = lane_id();
     const int n_items = ((a.n_replicas + 31) / 32) * LANE_MAX_SEG;
     int32_t *next = a.plan.counters + (MODE == LANE_UNIT ? 0 : 1);
+#ifdef LANE_WORK_GRID
+    // tuning build: one item per warp, handed out by the block scheduler
+    for (int once = 0; once < 1; ++once) {
+        const int w = blockIdx.x * (LANE_THREADS / 32) + (threadIdx.x >> 5);
+        (void)next;
+        if (w >= n_items) break;
+#else
     while (true) {
         int w = 0;
         if (lane == 0) w = atomicAdd(next, 1);
         w = __shfl_sync(ASR_FULL_MASK, w, 0);
         if (w >= n_items) break;
+#endif
         const int2 item = make_int2(w / LANE_MAX_SEG, w % LANE_MAX_SEG);
         if (MODE == LANE_REPAIR && item.y == 0) continue;
         const int pos = 32 * item.x + lane;
@@ -1001,7 +1030,11 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
             // time-split units, stitched at regeneration points; what could not be stitched, in one piece
             int rc0 = launch_lane_plan(a, st);
             if (rc0) return rc0;
+#ifdef LANE_WORK_GRID
+            const int work_grid = (((a.n_replicas + 31) / 32) * LANE_MAX_SEG + LANE_THREADS / 32 - 1) / (LANE_THREADS / 32);
+#else
             const int work_grid = sm_count() * LANE_WORK_BLOCKS_PER_SM;
+#endif
             {
                 KernelTimer kt(KID_SIM_LANE, st);
                 sim_lane_work_kernel<LANE_UNIT><<<work_grid, LANE_THREADS, 0, st>>>(a);
@@ -1014,8 +1047,20 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
             }
             rc0 = check_launch("sim_lane_work_kernel<repair>");
             if (rc0) return rc0;
-            KernelTimer kt(KID_SIM_REDO, st);
-            sim_lane_kernel<true><<<lane_grid, LANE_THREADS, 0, st>>>(a);
+            {
+                KernelTimer kt(KID_SIM_REDO, st);
+                sim_lane_kernel<true><<<lane_grid, LANE_THREADS, 0, st>>>(a);
+            }
+#ifdef LANE_STATS
+            {
+                unsigned long long h[8], z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+                cudaStreamSynchronize(st);
+                cudaMemcpyFromSymbol(h, g_lane_stats, sizeof(h));
+                cudaMemcpyToSymbol(g_lane_stats, z, sizeof(z));
+                fprintf(stderr, "lane stats: units %llu flagged-by-units %llu repairs %llu unstitched %llu redone %llu repair-requests %llu\n",
+                        h[0], h[1], h[2], h[3], h[4], h[5]);
+            }
+#endif
         } else if (a.order_free) {
             KernelTimer kt(KID_SIM_LANE, st);
             sim_lane_kernel<true><<<lane_grid, LANE_THREADS, 0, st>>>(a);

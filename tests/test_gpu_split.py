@@ -1,0 +1,128 @@
+"""-m gpu: the time-split thread-per-replica tier (units, repair, redo) and the carried-window percentile
+kernel of summary-only calls, against the oracle and against the same call with the split switched off.
+
+DESIGN.md "time-split units": a lightly loaded replica is cut into segments that are simulated side by side
+as traces of their own; boundaries are stitched at regeneration points (server empty at an arrival).  The
+results must not depend on any of it (tolerance 0, PAPER.md:100 percentiles by nearest rank)."""
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+from gpu_util import check_replica, run_batched
+
+pytestmark = pytest.mark.gpu
+POL = (orc.FCFS, orc.SJF, orc.HRRN)
+
+
+@pytest.fixture()
+def asr():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2603_11273_b200 as asr_mod
+    asr_mod.set_option(asr_mod.OPT_SIM_LANE_MIN_REPLICAS, 1)
+    asr_mod.set_option(asr_mod.OPT_SIM_LANE_SPLIT, 1)
+    yield asr_mod
+    asr_mod.set_option(asr_mod.OPT_SIM_LANE_MIN_REPLICAS, 1024)
+    asr_mod.set_option(asr_mod.OPT_SIM_LANE_SPLIT, 1)
+
+
+def _trace(arr, dur, est=None):
+    t = np.zeros(len(arr), dtype=orc.REQ)
+    t["arrival_us"] = arr
+    t["dur_ms"] = dur
+    t["est"] = dur if est is None else est
+    return t
+
+
+def _oracle_summary(tr, pol, slots, cost):
+    rl, rt, first, end = orc.simulate(tr, pol, orc.cost(*cost), slots)
+    return (orc.percentile(rl, 50), orc.percentile(rl, 90), orc.percentile(rt, 50), orc.percentile(rt, 90),
+            first, end, len(tr))
+
+
+def _check_all(traces, reps, S, cost, tag):
+    cache = {}
+    for i, (t, p, s) in enumerate(reps):
+        key = (t, p, s)
+        if key not in cache:
+            cache[key] = _oracle_summary(traces[t], p, s, cost)
+        got = tuple(int(S[i][f]) for f in ("p50_e2e_us", "p90_e2e_us", "p50_ttft_us", "p90_ttft_us",
+                                           "first_arrival_us", "last_done_us", "n_done"))
+        assert got == cache[key], "%s: replica %d (trace %d policy %d slots %d): %r != %r" % (
+            tag, i, t, p, s, got, cache[key])
+
+
+def test_split_equals_unsplit_and_oracle(asr):
+    """loads from 0.05 to ~8 Erlangs around the split threshold, several lengths (whole and ragged last
+    segments), slots 4/16/32, every policy: split on == split off == oracle"""
+    specs = [("lognormal", 2500, 0.4), ("lognormal", 4099, 2.0), ("lognormal", 6000, 6.0), ("lognormal", 3000, 11.0),
+             ("uniform", 2600, 1.0), ("uniform", 5003, 3.5), ("uniform", 2500, 6.5), ("six", 2777, 4.0),
+             ("lognormal", 2500, 26.0), ("misest", 3100, 8.0), ("equal_est", 2560, 9.0), ("lognormal", 2499, 3.0)]
+    traces = [wl.stress_trace(k, n, 300 + i, rate_per_s=r) for i, (k, n, r) in enumerate(specs)]
+    reps = [(t, p, s) for t in range(len(traces)) for p in POL for s in (4, 16, 32)]
+    _, _, S1 = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    asr.set_option(asr.OPT_SIM_LANE_SPLIT, 0)
+    _, _, S0 = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    assert np.array_equal(S1.view(np.uint8), S0.view(np.uint8)), "split on/off differ"
+    _check_all(traces, reps, S1, wl.CONFIG_COST, "split")
+
+
+def test_bursty_boundaries_and_unstitchable_replicas(asr):
+    """segment boundaries that fall inside busy periods: (a) clustered arrivals at a low average load, so that
+    most boundaries need a repair over many requests; (b) one huge burst in the middle of a light trace: the
+    repair finds no common regeneration point inside the next segment and the replica is redone in one piece
+    (SJF/HRRN then have to choose and go on to the warp kernel)"""
+    rng = np.random.Generator(np.random.PCG64(77))
+    traces = []
+    for j in range(4):   # (a)
+        n = 5200 + 37 * j
+        sizes = rng.geometric(1.0 / (4 + 3 * j), size=n)
+        gaps = rng.exponential(2.5e6 * (1 + j), size=n).astype(np.int64)
+        arr, t = [], 0
+        for sz, g in zip(sizes, gaps):
+            t += int(g)
+            arr.extend(t + np.sort(rng.integers(0, 200000, size=sz)))
+            if len(arr) >= n:
+                break
+        traces.append(_trace(np.sort(np.asarray(arr[:n], dtype=np.int64)), rng.integers(1000, 20001, size=n)))
+    for j in range(2):   # (b)
+        n = 6400
+        arr = np.cumsum(rng.exponential(1.5e6, size=n).astype(np.int64))
+        arr[2000:2000 + 1500 * (j + 1)] = arr[2000]      # 1500 / 3000 requests at one instant
+        arr = np.maximum.accumulate(arr)
+        traces.append(_trace(arr, rng.integers(1000, 9001, size=n)))
+    reps = [(t, p, s) for t in range(len(traces)) for p in POL for s in (8, 32)]
+    _, _, S1 = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    asr.set_option(asr.OPT_SIM_LANE_SPLIT, 0)
+    _, _, S0 = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    assert np.array_equal(S1.view(np.uint8), S0.view(np.uint8)), "split on/off differ"
+    _check_all(traces, reps, S1, wl.CONFIG_COST, "bursty")
+
+
+def test_carried_window_percentiles(asr):
+    """1,500 replicas in runs and alternations of very different traces (the carried window of the percentile
+    kernel hits, misses either way, overflows its slots and re-seeds), all values equal, lengths that are
+    not whole quads (radix path through the miss list)"""
+    rng = np.random.Generator(np.random.PCG64(5))
+    n = 2560
+    spaced = np.arange(n, dtype=np.int64) * 40_000_000          # one request every 40 s: isolated requests
+    traces = [
+        _trace(spaced, np.full(n, 6000)),                                     # every latency identical
+        _trace(spaced, rng.integers(1000, 1100, size=n)),                     # a few hundred distinct values
+        _trace(spaced, rng.integers(1000, 35001, size=n)),                    # wide
+        wl.stress_trace("lognormal", n, 401, rate_per_s=1.0),
+        wl.stress_trace("lognormal", n, 402, rate_per_s=1.0),                 # a neighbour of the one before
+        wl.stress_trace("uniform", n, 403, rate_per_s=3.0),
+        wl.stress_trace("lognormal", 2558, 404, rate_per_s=2.0),              # not whole quads
+        wl.stress_trace("six", n, 405, rate_per_s=0.3),                       # six durations: massive ties
+        _trace(spaced[:2500], np.where(np.arange(2500) % 2 == 0, 1000, 35000)),   # two values, p50 on the edge
+    ]
+    order = []
+    for rep_len in (40, 1, 7, 2):           # runs of a trace, then strict alternation, ...
+        for t in range(len(traces)):
+            order += [t] * rep_len
+    order = (order * 4)[:1500]
+    reps = [(t, POL[i % 3], 32) for i, t in enumerate(order)]
+    _, _, S = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    _check_all(traces, reps, S, wl.CONFIG_COST, "windows")
