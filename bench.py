@@ -335,6 +335,75 @@ def side_configs(asr, dev, d_tables, reps=5):
     return out
 
 
+def overload_sweep(asr, dev, d_tables, reps=3, n_seeds=512, n=3000):
+    """The contended regime of the BASE simulator (Table 1 rows 20-25 req/s):
+    n_seeds seeds x 8 arrival rates 16..30 req/s x 3 policies x n lognormal requests, at 16 and at 32 slots,
+    through plain asr_sched_simulate_batched (summary-only, default options).  Above ~20 (16 slots) / ~23
+    (32 slots) req/s the queue grows and SJF/HRRN choose at every admission.  Reports requests/s, the split
+    of the time over the thread / warp / CTA tiers and the share of replicas each tier finished; a sample of
+    replicas is compared with the oracle (tolerance 0)."""
+    import torch
+    import oracle as orc
+    rates = np.arange(16000, 31000, 2000, dtype=np.int32)                       # mHz
+    pols = (wl.FCFS, wl.SJF, wl.HRRN)
+    n_tr, n_rep = n_seeds * len(rates), n_seeds * len(rates) * len(pols)
+    specs = np.zeros(n_tr, dtype=asr.SPEC_DTYPE)
+    specs["seed"] = np.repeat(np.arange(n_seeds, dtype=np.uint64) + np.uint64(7000), len(rates))
+    specs["rate_mhz"] = np.tile(rates, n_seeds)
+    specs["dist"] = wl.DIST_LOGNORMAL
+    d_specs, d_cost = asr.to_device(specs, dev), asr.to_device(asr.make_cost(*wl.CONFIG_COST), dev)
+    d_tr = torch.empty(n_tr * n * 16, dtype=torch.uint8, device=dev)
+    asr.gen_trace_batched(d_specs, n_tr, n, d_tables, out=d_tr)
+    d_sum = torch.zeros(n_rep * asr.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    from paper_2603_11273_b200 import binding as B
+    d_ws = torch.empty(asr.workspace_bytes(B.OP_SIMULATE, n_rep * n, n_rep, 1), dtype=torch.uint8, device=dev)
+    out = {"workload": "%d seeds x 8 rates 16-30 req/s x 3 policies = %d replicas x %d lognormal requests, "
+                       "config-1 cost model, summary-only simulate_batched" % (n_seeds, n_rep, n)}
+    ln, ex = wl.ln_dur_table(), wl.exp_table()
+    for slots in (16, 32):
+        rep = asr.make_replicas(np.repeat(np.arange(n_tr, dtype=np.int64) * n, len(pols)),
+                                np.arange(n_rep, dtype=np.int64) * n, n,
+                                np.tile(np.asarray(pols, dtype=np.int32), n_tr), slots, 0)
+        d_rep = asr.to_device(rep, dev)
+
+        def step():
+            asr.simulate_batched(d_tr, d_rep, n_rep, d_cost, 1, n_rep * n, slots, None, None, d_sum, workspace=d_ws)
+        step()
+        torch.cuda.synchronize()
+        asr.timing_enable(True)
+        asr.timing_reset()
+        ms = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            step()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        kt = asr.timing_read()
+        asr.timing_enable(False)
+        summ = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
+        assert int((summ["n_done"] == n).sum()) == n_rep, "overload sweep: replicas did not finish"
+        # parity sample: evenly spaced replicas against the oracle
+        bad = 0
+        picks = np.linspace(0, n_rep - 1, 48).astype(np.int64)
+        for r in picks:
+            tr_i, pol = int(r) // len(pols), pols[int(r) % len(pols)]
+            tr = orc.gen_trace(int(specs["seed"][tr_i]), int(specs["rate_mhz"][tr_i]), orc.DIST_LOGNORMAL, n, ln, ex)
+            rl, rt, first, end = orc.simulate(tr, pol, orc.cost(*wl.CONFIG_COST), slots)
+            want = (orc.percentile(rl, 50), orc.percentile(rl, 90), orc.percentile(rt, 50), orc.percentile(rt, 90),
+                    first, end, n)
+            got = tuple(int(summ[r][f]) for f in ("p50_e2e_us", "p90_e2e_us", "p50_ttft_us", "p90_ttft_us",
+                                                  "first_arrival_us", "last_done_us", "n_done"))
+            bad += int(got != want)
+        med = statistics.median(ms)
+        out["slots%d" % slots] = {
+            "ms": med, "requests_per_s": n_rep * n / (med / 1e3),
+            "kernel_ms": {k: v[0] / reps for k, v in kt.items() if v[1]},
+            "parity_sample": {"replicas": int(len(picks)), "mismatches": bad}}
+    return out
+
+
 def extension_lines(asr, dev, d_tables, hbm_peak, reps=5):
     """SURVEY.md 8(f) rows, each timed alone (CUDA events through the library's per-kernel timers):
     the two HBM streams against the measured HBM peak, the extended simulator on an overloaded
@@ -438,7 +507,9 @@ def run_ours(args):
         # kernels are taken with; prints its own line, not the bench line
         d_tables = asr.to_device(asr.make_tables(wl.ln_dur_table(), wl.exp_table()), dev)
         if rank == 0:
-            print(json.dumps({"configs": side_configs(asr, dev, d_tables, reps=args.steps)}))
+            side = {} if args.overload_only else side_configs(asr, dev, d_tables, reps=args.steps)
+            side["overload_sweep"] = overload_sweep(asr, dev, d_tables, reps=min(args.steps, 3))
+            print(json.dumps({"configs": side}))
         D.finalize()
         return
 
@@ -623,6 +694,7 @@ def run_ours(args):
         del d_traces, d_ws, d_queues
         torch.cuda.empty_cache()
         side = side_configs(asr, dev, d_tables)
+        side["overload_sweep"] = overload_sweep(asr, dev, d_tables)
         ext_lines = extension_lines(asr, dev, d_tables, hbm_peak)
 
     base = parity = None
@@ -674,6 +746,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-side-configs", action="store_true", help="skip the config 1/2/4 timings")
     ap.add_argument("--side-configs-only", action="store_true", help="time configs 1, 2 and 4 and nothing else")
+    ap.add_argument("--overload-only", action="store_true", help="with --side-configs-only: the overload sweep alone")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
