@@ -358,12 +358,12 @@ __device__ __forceinline__ void sim_warp_replica(const SimArgs &a, const int r, 
                     } else {
                         int64_t b_s = INT64_MAX;
                         uint32_t scanned = 0;   // bit j: my j-th chunk was scanned in this round
+                        const int nj = (c_hi - c_lo + 32) >> 5;   // chunk slots per lane in use (uniform)
                         while (true) {
                             // my most promising chunk among those whose bound reaches the best request so far
                             float best_sc = 0.f;
                             int best_j = -1;
-#pragma unroll
-                            for (int j = 0; j < CHUNK_PER_LANE; ++j) {
+                            for (int j = 0; j < nj; ++j) {
                                 const int c = c_lo + lane + 32 * j;
                                 if (c <= c_hi && !((scanned >> j) & 1u)) {
                                     const ChunkMeta mt = ring[c % CHUNK_RING];
@@ -496,8 +496,11 @@ __device__ __forceinline__ void sim_warp_replica(const SimArgs &a, const int r, 
 // warp-per-replica kernel.  Direct mode: warp w of the grid simulates replica w.
 // Worklist mode (a.defer_list != nullptr): the warps share the replicas that the
 // lane kernel below handed over, defer_list[0 .. *defer_count).
+#ifndef SIM_WARP_MIN_CTAS
+#define SIM_WARP_MIN_CTAS 6
+#endif
 template <int SPL>
-__global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
+__global__ void __launch_bounds__(SIM_WARPS * 32, SPL == 1 ? SIM_WARP_MIN_CTAS : 1) sim_warp_kernel(SimArgs a) {
     __shared__ ChunkMeta s_ring[SIM_WARPS][CHUNK_RING];
     ChunkMeta *ring = s_ring[threadIdx.x >> 5];
     const int gw = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
@@ -505,8 +508,17 @@ __global__ void __launch_bounds__(SIM_WARPS * 32) sim_warp_kernel(SimArgs a) {
         if (gw < a.n_replicas) sim_warp_replica<SPL>(a, gw, ring);
         return;
     }
+    // the hand-over list is in the order the thread tier gave up: replicas that had to choose early -- the long
+    // ones -- first; warps take the next one as they finish (defer_count[4] = the cursor)
     const int cnt = *a.defer_count;
-    for (int w = gw; w < cnt; w += gridDim.x * SIM_WARPS) sim_warp_replica<SPL>(a, a.defer_list[w], ring);
+    while (true) {
+        int w = 0;
+        if (lane_id() == 0) w = atomicAdd(a.defer_count + 4, 1);
+        w = __shfl_sync(ASR_FULL_MASK, w, 0);
+        if (w >= cnt) break;
+        sim_warp_replica<SPL>(a, a.defer_list[w], ring);
+        __syncwarp();
+    }
 }
 
 // ---------------------------------------------------------------------------
@@ -1064,7 +1076,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lan
 // a few dozen sampled requests).  It only steers the schedule -- which replicas share a warp, which are cut into
 // segments -- and never a result.
 constexpr int PLAN_BUCKETS = 32;
-constexpr float PLAN_SPLIT_MAX_LOAD = 4.f;   // beyond it regeneration points (about exp(-load) of the arrivals) are too rare to stitch at
+constexpr float PLAN_SPLIT_MAX_LOAD = 3.5f;   // beyond it regeneration points (about exp(-load) of the arrivals) are too rare to stitch at
 constexpr int PLAN_SAMPLES = 32;
 
 __global__ void __launch_bounds__(256) lane_key_kernel(SimArgs a) {
@@ -1189,6 +1201,7 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
         defer_count[1] = 0;   // warp kernel -> CTA kernel
         defer_count[2] = 0;   // carried-window percentile kernel -> radix kernel, E2E latency
         defer_count[3] = 0;   // the same, TTFT
+        defer_count[4] = 0;   // cursor of the warp kernel over the hand-over list
     }
     __syncthreads();
     const int lane = lane_id(), warp = threadIdx.x >> 5;
