@@ -60,6 +60,7 @@ extern "C" {
 
 #define ASR_SCHED_VERSION 100
 
+#define ASR_SELECT_MAX_K 256
 enum { ASR_FCFS = 0, ASR_SJF = 1, ASR_HRRN = 2 };          /* PAPER.md:287 */
 enum { ASR_ADAPTIVE = 3 };  /* policy switching on queue depth, asr_sched_simulate_batched_ex only */
 enum { ASR_DIST_LOGNORMAL = 0, ASR_DIST_UNIFORM = 1 };
@@ -125,7 +126,8 @@ typedef struct {
 /* One queue of n records.  Writes k indices (positions in `keys`), best
  * first; if k > n the tail is -1.
  *   keys DEVICE [n]; out_idx DEVICE [k]; workspace DEVICE.
- * Limits: 0 <= k <= 32 (else -3); n < 2^31. */
+ * Limits: 0 <= k <= ASR_SELECT_MAX_K = 256 (else -3; the paper's engine admits into up to 256
+ * slots); n < 2^31.  k <= 32 streams the queue once (HBM-bound); 32 < k <= 256 sorts it in shared memory. */
 int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy, int64_t now,
                      int32_t k, int32_t *out_idx, void *workspace,
                      size_t workspace_bytes, void *stream);
@@ -135,7 +137,7 @@ int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy, int64_t n
  * Indices are local to the queue; out_idx[q*k + j] is the j-th best, -1 padded.
  * now_per_queue (nullable) overrides `now` per queue.
  *   keys DEVICE [n_queues*q_len]; q_count, now_per_queue DEVICE [n_queues] or NULL;
- *   out_idx DEVICE [n_queues*k].  Limits: 0 <= k <= 32, q_len < 2^31. */
+ *   out_idx DEVICE [n_queues*k].  Limits: 0 <= k <= ASR_SELECT_MAX_K, q_len < 2^31. */
 int asr_sched_select_batched(const asr_req_t *keys, int32_t n_queues, int32_t q_len,
                              const int32_t *q_count, int32_t policy, int64_t now,
                              const int64_t *now_per_queue, int32_t k, int32_t *out_idx,

@@ -57,7 +57,7 @@ int sm_count() {
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
-    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel", "summary_fast_kernel", "lane_plan_kernels", "sim_lane_kernel(repair)", "sim_lane_kernel(redo)"};
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel", "summary_fast_kernel", "lane_plan_kernels", "sim_lane_kernel(repair)", "sim_lane_kernel(redo)", "select_wide_kernel"};
 struct TimedLaunch {
     int kid;
     cudaEvent_t start, stop;
@@ -671,8 +671,8 @@ extern "C" int asr_sched_select_host(const asr_req_t *keys, int32_t n_queues, in
         set_error("select_host: bad argument");
         return ASR_EINVAL;
     }
-    if (k > 32) {
-        set_error("select_host: k=%d exceeds the limit 32", k);
+    if (k > ASR_SELECT_MAX_K) {
+        set_error("select_host: k=%d exceeds the limit %d", k, ASR_SELECT_MAX_K);
         return ASR_EUNSUPPORTED;
     }
     if (n_queues == 0 || k == 0) return ASR_OK;

@@ -20,7 +20,7 @@ int sm_count();                       // SMs of the current device (queried, cac
 // kernel ids of the per-kernel CUDA-event timing facility (asr_sched_timing_*)
 enum KernelId {
     KID_SELECT = 0, KID_SIM_PREPARE, KID_SIMULATE, KID_SIM_LANE, KID_SUMMARY_PCT, KID_PERCENTILES, KID_GEN_TRACE,
-    KID_GEN_QUEUES, KID_SWEEP_REPLICAS, KID_SIM_CTA, KID_SIM_INIT_LAT, KID_SIM_EX, KID_TPOT, KID_ESTIMATE, KID_ITL_PCT, KID_SUMMARY_FAST, KID_LANE_PLAN, KID_SIM_REPAIR, KID_SIM_REDO, KID_COUNT
+    KID_GEN_QUEUES, KID_SWEEP_REPLICAS, KID_SIM_CTA, KID_SIM_INIT_LAT, KID_SIM_EX, KID_TPOT, KID_ESTIMATE, KID_ITL_PCT, KID_SUMMARY_FAST, KID_LANE_PLAN, KID_SIM_REPAIR, KID_SIM_REDO, KID_SELECT_WIDE, KID_COUNT
 };
 // RAII: counts the launch and, when timing is enabled, brackets it with an
 // event pair recorded on the launching stream.

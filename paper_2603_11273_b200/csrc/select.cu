@@ -1,4 +1,5 @@
-// select.cu -- a2 priority keys + a3 batched top-k select (k <= 32), sm_100a.
+// select.cu -- a2 priority keys + a3 batched top-k select, sm_100a.  The streaming kernel described here serves
+// k <= 32 (config 5); select_wide_kernel near the end serves 32 < k <= 256.
 //
 // One warp owns one queue at a time and STREAMS it from HBM exactly once.  The
 // queue is cut into chunks of SEL_CHUNK records (4 KB); lane 0 of the warp
@@ -536,10 +537,134 @@ static int launch_one(const SelArgs &a, cudaStream_t st) {
     return check_launch("select_topk_kernel");
 }
 
+// ---------------------------------------------------------------------------
+// 32 < k <= 256 (the engine admits into up to 256 slots): one CTA per queue.
+// The queue goes through shared memory in chunks; a chunk joins the k best kept so far, the lot is sorted
+// exactly (bitonic network on the order scalars, equal scalars settled by the full comparator with its
+// (arrival, idx) tie-break), and the first k stay.  Not the streaming design of the k <= 32 kernel above: it
+// trades bandwidth for a selection that needs no candidate buffer sized to k.
+// ---------------------------------------------------------------------------
+constexpr int WIDE_K = 256;
+constexpr int WIDE_CAP = 4096;                 // entries sorted at a time (a power of two)
+constexpr int WIDE_CHUNK = WIDE_CAP - WIDE_K;  // new records per round
+constexpr int WIDE_THREADS = 512;
+
+struct WideSmem {
+    int4 ent[WIDE_CAP];       // (arrival lo, arrival hi, max(est,1), idx)
+    int64_t key[WIDE_CAP];    // order scalar, INT64_MAX = padding
+    uint16_t perm[WIDE_CAP];  // entry of rank i
+    int4 tmp[WIDE_K];
+};
+
+template <int POLICY>
+__global__ void __launch_bounds__(WIDE_THREADS, 1) select_wide_kernel(SelArgs a) {
+    extern __shared__ __align__(128) unsigned char sel_dyn_smem[];
+    WideSmem &sm = *reinterpret_cast<WideSmem *>(sel_dyn_smem);
+    const int tid = threadIdx.x;
+    const int k = a.k;
+    for (int q = blockIdx.x; q < a.n_queues; q += gridDim.x) {
+        const int count = sel_count(a, q);
+        const int64_t now = a.now_per_queue ? a.now_per_queue[q] : a.now;
+        const int64_t qbase = (int64_t)q * a.q_len;
+        const int32_t idx_base = a.global_idx ? (int32_t)qbase : 0;
+        int kept = 0;   // entries [0, kept) = the best so far, best first
+        for (int c0 = 0; c0 < count; c0 += WIDE_CHUNK) {
+            const int nc = min(WIDE_CHUNK, count - c0);
+            for (int j = tid; j < nc; j += WIDE_THREADS) {
+                int4 v;
+                int32_t idx;
+                if (a.src_idx) {
+                    idx = a.src_idx[qbase + c0 + j];
+                    v = __ldg(reinterpret_cast<const int4 *>(a.keys + idx));
+                } else {
+                    idx = idx_base + c0 + j;
+                    v = __ldg(reinterpret_cast<const int4 *>(a.keys + qbase + c0 + j));
+                }
+                sm.ent[kept + j] = make_int4(v.x, v.y, v.w < 1 ? 1 : v.w, idx);
+            }
+            __syncthreads();
+            const int m = kept + nc;
+            int size = 2;   // the power of two that holds m entries
+            while (size < m) size <<= 1;
+            for (int i = tid; i < size; i += WIDE_THREADS) {
+                sm.key[i] = i < m ? order_scalar<POLICY>(sm.ent[i], now) : INT64_MAX;
+                sm.perm[i] = (uint16_t)i;
+            }
+            __syncthreads();
+            for (int kk = 2; kk <= size; kk <<= 1) {
+                for (int j = kk >> 1; j > 0; j >>= 1) {
+                    for (int t = tid; t < (size >> 1); t += WIDE_THREADS) {
+                        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));   // the lower partner
+                        const int l = i | j;
+                        const bool up = (i & kk) == 0;
+                        const int64_t ka = sm.key[i], kb = sm.key[l];
+                        const uint16_t pa = sm.perm[i], pb = sm.perm[l];
+                        // entry at i ranks before the entry at l?  (a padding ranks after everything; its scalar
+                        // INT64_MAX is also that of a real HRRN entry that has not waited)
+                        const bool pad_a = pa >= m, pad_b = pb >= m;
+                        bool a_first;
+                        if (pad_a || pad_b) {
+                            a_first = !pad_a || pad_b;
+                        } else if (ka != kb) {
+                            a_first = ka < kb;
+                        } else {
+                            const int4 ea = sm.ent[pa], eb = sm.ent[pb];
+                            a_first = better<POLICY>(rec_arr(ea), ea.z, ea.w, rec_arr(eb), eb.z, eb.w, now);
+                        }
+                        if (a_first != up) {
+                            sm.key[i] = kb;
+                            sm.key[l] = ka;
+                            sm.perm[i] = pb;
+                            sm.perm[l] = pa;
+                        }
+                    }
+                    __syncthreads();
+                }
+            }
+            kept = m < k ? m : k;
+            if (tid < kept) sm.tmp[tid] = sm.ent[sm.perm[tid]];
+            __syncthreads();
+            if (tid < kept) sm.ent[tid] = sm.tmp[tid];
+            __syncthreads();
+        }
+        int32_t *out = a.out_idx + (int64_t)q * k;
+        for (int j = tid; j < k; j += WIDE_THREADS) out[j] = j < kept ? sm.ent[j].w : -1;
+        __syncthreads();
+    }
+}
+
+template <int POLICY>
+static int launch_wide(const SelArgs &a, cudaStream_t st) {
+    if (a.n_queues <= 0 || a.k <= 0) return ASR_OK;
+    cudaError_t e = cudaFuncSetAttribute(select_wide_kernel<POLICY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(WideSmem));
+    if (e != cudaSuccess) {
+        set_error("select_wide_kernel: cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        return ASR_ECUDA;
+    }
+    const int cap = sm_count() * 2;
+    const int grid = a.n_queues < cap ? a.n_queues : cap;
+    {
+        KernelTimer kt(KID_SELECT_WIDE, st);
+        select_wide_kernel<POLICY><<<grid, WIDE_THREADS, sizeof(WideSmem), st>>>(a);
+    }
+    return check_launch("select_wide_kernel");
+}
+
 int launch_select(const SelArgs &a, int policy, cudaStream_t st) {
     const bool ind = a.src_idx != nullptr;
     if (!ind && (reinterpret_cast<uintptr_t>(a.keys) & 15u) != 0) {
         set_error("select: keys must be 16-byte aligned");
+        return ASR_EINVAL;
+    }
+    if (a.k > 32) {
+        switch (policy) {
+            case ASR_FCFS: return launch_wide<ASR_FCFS>(a, st);
+            case ASR_SJF: return launch_wide<ASR_SJF>(a, st);
+            case ASR_HRRN: return launch_wide<ASR_HRRN>(a, st);
+        }
+        set_error("unknown policy %d", policy);
         return ASR_EINVAL;
     }
     switch (policy) {
@@ -568,8 +693,8 @@ extern "C" int asr_sched_select_batched(const asr_req_t *keys, int32_t n_queues,
         set_error("select_batched: bad argument (n_queues=%d q_len=%d k=%d policy=%d)", n_queues, q_len, k, policy);
         return ASR_EINVAL;
     }
-    if (k > 32) {
-        set_error("select_batched: k=%d exceeds the limit 32", k);
+    if (k > ASR_SELECT_MAX_K) {
+        set_error("select_batched: k=%d exceeds the limit %d", k, ASR_SELECT_MAX_K);
         return ASR_EUNSUPPORTED;
     }
     if (n_queues == 0 || k == 0) return ASR_OK;
@@ -605,8 +730,8 @@ extern "C" int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy
         set_error("select: bad argument (n=%lld k=%d policy=%d)", (long long)n, k, policy);
         return ASR_EINVAL;
     }
-    if (k > 32) {
-        set_error("select: k=%d exceeds the limit 32", k);
+    if (k > ASR_SELECT_MAX_K) {
+        set_error("select: k=%d exceeds the limit %d", k, ASR_SELECT_MAX_K);
         return ASR_EUNSUPPORTED;
     }
     if (k == 0) return ASR_OK;

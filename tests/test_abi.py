@@ -65,9 +65,9 @@ def test_argument_errors_need_no_gpu(asr):
     L = asr.lib()
     assert L.asr_sched_select_batched(None, 4, 16, None, 7, 0, None, 4, None, None) == -1
     assert "policy" in asr.last_error()
-    assert L.asr_sched_select_batched(None, 4, 16, None, 1, 0, None, 33, None, None) == -3
+    assert L.asr_sched_select_batched(None, 4, 16, None, 1, 0, None, 257, None, None) == -3
     assert L.asr_sched_select(None, -1, 0, 0, 1, None, None, 0, None) == -1
-    assert L.asr_sched_select(None, 10, 0, 0, 64, None, None, 0, None) == -3
+    assert L.asr_sched_select(None, 10, 0, 0, 300, None, None, 0, None) == -3
     cm = asr.make_cost(1, 1, 1, 1, 1, 1)
     assert L.asr_sched_simulate(None, 10, 0, cm.ctypes.data, 0, None, None, None, None, 0, None) == -1
     assert L.asr_sched_simulate(None, 10, 0, cm.ctypes.data, 257, None, None, None, None, 0, None) == -3
@@ -77,7 +77,7 @@ def test_argument_errors_need_no_gpu(asr):
     pc9 = np.arange(1, 10, dtype=np.int32)
     assert L.asr_sched_percentiles(None, None, 1, pc9.ctypes.data, 9, None, None, 0, None) == -3
     assert L.asr_sched_gen_trace(0, 0, 0, 10, None, None, None) == -1
-    assert L.asr_sched_select_host(None, 1, 1, 0, 0, 40, None) == -3
+    assert L.asr_sched_select_host(None, 1, 1, 0, 0, 257, None) == -3
     # zero-size work is a no-op that needs no device
     assert L.asr_sched_select_batched(None, 0, 16, None, 1, 0, None, 4, None, None) == 0
     assert L.asr_sched_percentiles(None, None, 0, pc.ctypes.data, 0, None, None, 0, None) == 0

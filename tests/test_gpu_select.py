@@ -40,6 +40,40 @@ def test_batched_stress_kinds(asr, kind, policy):
             assert np.array_equal(got[i], orc.select(q[i], policy, now, k)), (kind, policy, ql, k, i)
 
 
+@pytest.mark.parametrize("kind", ["random", "six", "proportional", "identical", "few_arrivals", "future", "est_edge"])
+@pytest.mark.parametrize("policy", POL)
+def test_wide_k_stress_kinds(asr, kind, policy):
+    """32 < k <= 256 (up to 256 slots to admit into): the shared-memory sort kernel, same tie kinds,
+    queues shorter than k, exactly one round, several rounds with the kept k carried along"""
+    now = 10**9
+    for ql, k, nq in [(20, 33, 3), (64, 64, 4), (300, 100, 5), (3840, 256, 3), (3841, 256, 2), (4096, 33, 3),
+                      (9000, 256, 2), (700, 255, 4)]:
+        q = np.stack([wl.stress_queue(kind, ql, 2000 * ql + i, now) for i in range(nq)])
+        got = gpu_select_batched(asr, q, policy, now, k)
+        for i in range(nq):
+            assert np.array_equal(got[i], orc.select(q[i], policy, now, k)), (kind, policy, ql, k, i)
+
+
+@pytest.mark.parametrize("policy", POL)
+def test_wide_k_ragged_per_queue_now_and_single_queue(asr, policy):
+    import torch
+    rng = np.random.default_rng(50 + policy)
+    nq, ql, k = 24, 900, 100
+    now = 10**8
+    q = np.stack([wl.stress_queue("random" if i % 2 else "six", ql, 977 + i, now) for i in range(nq)])
+    counts = rng.integers(0, ql + 1, size=nq)
+    counts[:4] = [0, 1, ql, 99]
+    nows = rng.integers(1, 2 * now, size=nq)
+    got = gpu_select_batched(asr, q, policy, now, k, q_count=counts, now_pq=nows)
+    for i in range(nq):
+        assert np.array_equal(got[i], orc.select(q[i][:counts[i]], policy, int(nows[i]), k)), i
+    for n, kk in ((5000, 64), (40000, 256)):     # the single-queue call: segments, then the reported positions
+        qq = wl.stress_queue("random", n, n + 3, 10**10)
+        out = asr.select(asr.to_device(qq), n, policy, 10**10, kk)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), orc.select(qq, policy, 10**10, kk)), (policy, n, kk)
+
+
 @pytest.mark.parametrize("policy", POL)
 def test_ragged_counts_and_per_queue_now(asr, policy):
     rng = np.random.default_rng(policy)
