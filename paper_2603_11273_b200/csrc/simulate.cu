@@ -499,8 +499,10 @@ __device__ __forceinline__ void sim_warp_replica(const SimArgs &a, const int r, 
 #ifndef SIM_WARP_MIN_CTAS
 #define SIM_WARP_MIN_CTAS 6
 #endif
-template <int SPL>
-__global__ void __launch_bounds__(SIM_WARPS * 32, SPL == 1 ? SIM_WARP_MIN_CTAS : 1) sim_warp_kernel(SimArgs a) {
+// PACKED: the work-list pass behind the thread tier (thousands of contended replicas: occupancy pays for the
+// registers given up); the direct pass over a few replicas keeps every register
+template <int SPL, bool PACKED>
+__global__ void __launch_bounds__(SIM_WARPS * 32, PACKED ? SIM_WARP_MIN_CTAS : 1) sim_warp_kernel(SimArgs a) {
     __shared__ ChunkMeta s_ring[SIM_WARPS][CHUNK_RING];
     ChunkMeta *ring = s_ring[threadIdx.x >> 5];
     const int gw = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
@@ -1244,11 +1246,14 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
 template <int SPL>
 static void launch_warp(const SimArgs &a, int grid, cudaStream_t st) {
     KernelTimer kt(KID_SIMULATE, st);
-    sim_warp_kernel<SPL><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    sim_warp_kernel<SPL, false><<<grid, SIM_WARPS * 32, 0, st>>>(a);
 }
 
 static void launch_warp_any(const SimArgs &a, int max_slots, int grid, cudaStream_t st) {
-    if (max_slots <= 32) launch_warp<1>(a, grid, st);
+    if (max_slots <= 32 && a.defer_list != nullptr) {
+        KernelTimer kt(KID_SIMULATE, st);
+        sim_warp_kernel<1, true><<<grid, SIM_WARPS * 32, 0, st>>>(a);
+    } else if (max_slots <= 32) launch_warp<1>(a, grid, st);
     else if (max_slots <= 64) launch_warp<2>(a, grid, st);
     else if (max_slots <= 128) launch_warp<4>(a, grid, st);
     else launch_warp<8>(a, grid, st);
