@@ -404,7 +404,7 @@ def overload_sweep(asr, dev, d_tables, reps=3, n_seeds=512, n=3000):
     return out
 
 
-def extension_lines(asr, dev, d_tables, hbm_peak, reps=5):
+def extension_lines(asr, dev, d_tables, hbm_peak, reps=5, consts=None):
     """SURVEY.md 8(f) rows, each timed alone (CUDA events through the library's per-kernel timers):
     the two HBM streams against the measured HBM peak, the extended simulator on an overloaded
     sweep with a KV budget that binds."""
@@ -486,6 +486,12 @@ def extension_lines(asr, dev, d_tables, hbm_peak, reps=5):
                                 "avg_launch_ms": ms / cnt, "requests_per_s": n_rep * n_req / (ms / cnt / 1e3),
                                 "preemptions_per_request": float(d_pre.sum().item()) / (n_rep * n_req),
                                 "replicas_done": int((summ["n_done"] == n_req).sum())}
+        wi = (consts or {}).get("sim_ex_kernel_warp_instr_per_request")
+        if wi:   # issue-slot roofline as for the base simulator (ncu counter from the committed capture)
+            a = wi * n_rep * n_req / (ms / cnt / 1e3)
+            out["sim_ex_kernel"].update({"achieved": a, "peak": ALU_PEAK_WARP_INSTR_PER_S, "unit": "warp-instr/s",
+                                         "frac": a / ALU_PEAK_WARP_INSTR_PER_S, "warp_instr_per_request": wi,
+                                         "constants_stale": bool((consts or {}).get("stale"))})
     return out
 
 
@@ -723,7 +729,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
         side = side_configs(asr, dev, d_tables)
         side["overload_sweep"] = overload_sweep(asr, dev, d_tables)
-        ext_lines = extension_lines(asr, dev, d_tables, hbm_peak)
+        ext_lines = extension_lines(asr, dev, d_tables, hbm_peak, consts=consts)
 
     base = parity = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
