@@ -38,7 +38,7 @@ __device__ __forceinline__ bool ext_ok(const asr_sim_ext_t &ex, int policy) {
 }
 
 template <int SPL>
-__device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) {
+__device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r, ChunkMeta *ring) {
     const int lane = lane_id();
     asr_replica_t rep = a.replicas[r];
     const int n = rep.n, slots = rep.slots, policy = rep.policy;
@@ -76,15 +76,49 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
     int64_t t = 0, M = 0, n_pre = 0;
     int p = 0, lo = 0, nW = 0, nR = 0, done = 0, bm_hi = 0, n_pairs = 0;
     bool blocked = false, bad = false;
+    bool meta_ok = false;   // the chunk bounds (sim_common.cuh) cover the window [lo, p)
     const int64_t first_arrival = n > 0 ? trace[0].arrival_us : 0;
 
     while (done < n) {
         // ---- 1. ingest arrivals <= t (32 at a time)
         while (p < n) {
             const int i = p + lane;
-            const bool in = i < n && ld_cached(trace + i).arrival_us <= t;
+            Rec q;
+            q.arrival_us = 0;
+            q.dur_ms = q.est = 0;
+            if (i < n) q = ld_cached(trace + i);
+            const bool in = i < n && q.arrival_us <= t;
             const uint32_t m = __ballot_sync(ASR_FULL_MASK, in);
             const int cnt = (m == ASR_FULL_MASK) ? 32 : __ffs(~m) - 1;   // arrivals are sorted
+            if (cnt > 0 && meta_ok) {
+                // the newcomers [p, p + cnt) join the bounds of their chunks (at most two; a chunk starts with its
+                // first request)
+                const bool mine = lane < cnt;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int c = (p >> 5) + h;
+                    const bool inc = mine && (i >> 5) == c;
+                    const uint32_t lm = __ballot_sync(ASR_FULL_MASK, inc);
+                    if (lm == 0u) continue;
+                    const int32_t e_new = __reduce_min_sync(ASR_FULL_MASK, inc ? (int32_t)est_of(q.est) : INT32_MAX);
+                    const uint32_t bits = __reduce_or_sync(ASR_FULL_MASK, inc ? 1u << (i & 31) : 0u);
+                    const int64_t a_new = shfl64(q.arrival_us, __ffs(lm) - 1);
+                    if (lane == 0) {
+                        ChunkMeta *slot = ring + (c % CHUNK_RING);
+                        ChunkMeta mt = *slot;
+                        if ((c << 5) >= p) mt.wait = 0u;   // nothing of this chunk was ingested before
+                        if (mt.wait == 0u) {
+                            mt.a_first = a_new;
+                            mt.e_min = e_new;
+                        } else {
+                            mt.e_min = e_new < mt.e_min ? e_new : mt.e_min;
+                        }
+                        mt.wait |= bits;
+                        *slot = mt;
+                    }
+                }
+                __syncwarp();
+            }
             p += cnt;
             nW += cnt;
             if (cnt > 0) blocked = false;
@@ -152,7 +186,23 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
                 }
             freed = (int64_t)shfl64((int64_t)freed, w_slot & 31);
             M -= freed;
-            if (lane == 0) bm[w_idx >> 5] &= ~(1u << (w_idx & 31));   // waits again
+            if (lane == 0) {
+                bm[w_idx >> 5] &= ~(1u << (w_idx & 31));   // waits again
+                if (meta_ok) {
+                    ChunkMeta *slot = ring + ((w_idx >> 5) % CHUNK_RING);
+                    ChunkMeta mt = *slot;
+                    const int32_t e = (int32_t)est_of(w_est);
+                    if (mt.wait == 0u) {
+                        mt.a_first = w_arr;
+                        mt.e_min = e;
+                    } else {
+                        mt.a_first = w_arr < mt.a_first ? w_arr : mt.a_first;
+                        mt.e_min = e < mt.e_min ? e : mt.e_min;
+                    }
+                    mt.wait |= 1u << (w_idx & 31);
+                    *slot = mt;
+                }
+            }
             __syncwarp();
             lo = w_idx < lo ? w_idx : lo;
             --nR;
@@ -167,9 +217,22 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
         uint32_t dur_sum_part = 0;
         int k = 0;
         if (preempted == 0 && !blocked) {
+            // the chunk bounds must cover the window (an eviction may have moved lo back)
+            const int c_lo = lo >> 5, c_hi = (p - 1) >> 5;
+            const bool ringed = nW > 0 && c_hi - c_lo + 1 <= CHUNK_RING - 1;
+            if (!ringed) {
+                meta_ok = false;
+            } else if (!meta_ok && nR < slots) {
+                for (int c = c_lo; c <= c_hi; ++c) chunk_rebuild(trace, bm, ring, c, lo, p, lane);
+                meta_ok = true;
+                __syncwarp();
+            }
             while (nW > 0 && nR < slots) {
                 int64_t b_arr = 0;
                 int32_t b_est = 0, b_dur = 0, b_idx = -1;
+                if (ringed) {
+                    chunk_pick(trace, ring, c_lo, c_hi, pol, t, lane, b_arr, b_est, b_dur, b_idx);
+                } else {
                 for (int c = lo & ~31; c < p; c += 32) {
                     const uint32_t word = bm[c >> 5];
                     const int i = c + lane;
@@ -197,6 +260,7 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
                         b_idx = o_idx;
                     }
                 }
+                }
                 const int64_t kv = B > 0 ? kv_enc(ex, b_dur) : 0;
                 if (B > 0 && M + kv + nR + 1 > B) {   // the head of the line does not fit
                     blocked = true;
@@ -208,6 +272,7 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
                 if (lane == 0) {
                     bm[b_idx >> 5] |= 1u << (b_idx & 31);
                     ever[b_idx >> 5] |= 1u << (b_idx & 31);
+                    if (ringed) ring[(b_idx >> 5) % CHUNK_RING].wait &= ~(1u << (b_idx & 31));
                 }
                 bool seated = false;
 #pragma unroll
@@ -345,8 +410,9 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r) 
 
 template <int SPL>
 __global__ void __launch_bounds__(SIM_WARPS * 32) sim_ex_kernel(SimExArgs a) {
+    __shared__ ChunkMeta s_ring[SIM_WARPS][CHUNK_RING];
     const int gw = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
-    if (gw < a.n_replicas) sim_ex_replica<SPL>(a, gw);
+    if (gw < a.n_replicas) sim_ex_replica<SPL>(a, gw, s_ring[threadIdx.x >> 5]);
 }
 
 template <int SPL>
