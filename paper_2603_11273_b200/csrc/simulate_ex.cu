@@ -409,7 +409,10 @@ __device__ __forceinline__ void sim_ex_replica(const SimExArgs &a, const int r, 
 }
 
 template <int SPL>
-__global__ void __launch_bounds__(SIM_WARPS * 32) sim_ex_kernel(SimExArgs a) {
+#ifndef SIM_EX_MIN_CTAS
+#define SIM_EX_MIN_CTAS 6
+#endif
+__global__ void __launch_bounds__(SIM_WARPS * 32, SPL == 1 ? SIM_EX_MIN_CTAS : 1) sim_ex_kernel(SimExArgs a) {
     __shared__ ChunkMeta s_ring[SIM_WARPS][CHUNK_RING];
     const int gw = (blockIdx.x * SIM_WARPS) + (threadIdx.x >> 5);
     if (gw < a.n_replicas) sim_ex_replica<SPL>(a, gw, s_ring[threadIdx.x >> 5]);
