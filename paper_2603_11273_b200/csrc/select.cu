@@ -554,7 +554,11 @@ struct WideSmem {
     int64_t key[WIDE_CAP];    // order scalar, INT64_MAX = padding
     uint16_t perm[WIDE_CAP];  // entry of rank i
     int4 tmp[WIDE_K];
+    uint32_t hist[256];       // radix select of the k-th order scalar
+    uint32_t wcnt[WIDE_THREADS / 32];
+    uint32_t sel_digit, sel_below, n_cand;
 };
+constexpr int WIDE_SORT_MAX = 1024;   // a round with more entries first drops everything beyond the k-th order scalar
 
 template <int POLICY>
 __global__ void __launch_bounds__(WIDE_THREADS, 1) select_wide_kernel(SelArgs a) {
@@ -591,6 +595,97 @@ __global__ void __launch_bounds__(WIDE_THREADS, 1) select_wide_kernel(SelArgs a)
                 sm.perm[i] = (uint16_t)i;
             }
             __syncthreads();
+            if (m > WIDE_SORT_MAX) {
+                // Radix select (8 x 8 bits, MSB first) of the k-th smallest order scalar T.  Everything with a larger
+                // scalar is worse than k entries (scalars are weakly order-preserving) and is dropped; what is left
+                // (k entries and the ties at T) is compacted to the front and sorted.  Too many ties: sort it all.
+                uint64_t prefix = 0;
+                uint32_t kk = (uint32_t)k;
+                for (int shift = 56; shift >= 0; shift -= 8) {
+                    if (tid < 256) sm.hist[tid] = 0u;
+                    __syncthreads();
+                    for (int i = tid; i < m; i += WIDE_THREADS) {
+                        const uint64_t u = (uint64_t)sm.key[i] ^ 0x8000000000000000ull;
+                        if (shift == 56 || (u >> (shift + 8)) == prefix) atomicAdd(&sm.hist[(u >> shift) & 255u], 1u);
+                    }
+                    __syncthreads();
+                    if (tid < 32) {   // lane L owns bins 8L .. 8L+7
+                        uint32_t c8[8], tot = 0;
+#pragma unroll
+                        for (int b = 0; b < 8; ++b) {
+                            c8[b] = sm.hist[tid * 8 + b];
+                            tot += c8[b];
+                        }
+                        uint32_t incl = tot;
+#pragma unroll
+                        for (int d = 1; d < 32; d <<= 1) {
+                            const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+                            if (tid >= d) incl += y;
+                        }
+                        uint32_t run = incl - tot;
+                        if (run < kk && kk <= incl) {
+#pragma unroll
+                            for (int b = 0; b < 8; ++b) {
+                                if (run < kk && kk <= run + c8[b]) {
+                                    sm.sel_digit = (uint32_t)(tid * 8 + b);
+                                    sm.sel_below = run;
+                                }
+                                run += c8[b];
+                            }
+                        }
+                    }
+                    __syncthreads();
+                    prefix = (prefix << 8) | sm.sel_digit;
+                    kk -= sm.sel_below;
+                }
+                const int64_t T = (int64_t)(prefix ^ 0x8000000000000000ull);
+                // compaction: every thread reads its eight entries, then writes the survivors to the front
+                constexpr int PER = WIDE_CAP / WIDE_THREADS;
+                int64_t ck[PER];
+                uint16_t cp[PER];
+                int nc_mine = 0;
+#pragma unroll
+                for (int j = 0; j < PER; ++j) {
+                    const int i = tid * PER + j;
+                    ck[j] = i < m ? sm.key[i] : INT64_MAX;
+                    cp[j] = sm.perm[i];
+                    if (i < m && ck[j] <= T) ++nc_mine;
+                }
+                uint32_t incl = (uint32_t)nc_mine;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+                    if ((tid & 31) >= d) incl += y;
+                }
+                if ((tid & 31) == 31) sm.wcnt[tid >> 5] = incl;
+                __syncthreads();
+                uint32_t off = incl - (uint32_t)nc_mine, total = 0;
+#pragma unroll
+                for (int w = 0; w < WIDE_THREADS / 32; ++w) {
+                    const uint32_t c = sm.wcnt[w];
+                    if (w < (tid >> 5)) off += c;
+                    total += c;
+                }
+                if (total <= (uint32_t)WIDE_SORT_MAX) {
+                    size = 2;
+                    while (size < (int)total) size <<= 1;
+#pragma unroll
+                    for (int j = 0; j < PER; ++j) {
+                        const int i = tid * PER + j;
+                        if (i < m && ck[j] <= T) {
+                            sm.key[off] = ck[j];
+                            sm.perm[off] = cp[j];
+                            ++off;
+                        }
+                    }
+                    __syncthreads();
+                    for (int i = (int)total + tid; i < size; i += WIDE_THREADS) {
+                        sm.key[i] = INT64_MAX;
+                        sm.perm[i] = 0xFFFFu;   // a padding: ranks after every entry
+                    }
+                }
+                __syncthreads();
+            }
             for (int kk = 2; kk <= size; kk <<= 1) {
                 for (int j = kk >> 1; j > 0; j >>= 1) {
                     for (int t = tid; t < (size >> 1); t += WIDE_THREADS) {
