@@ -78,6 +78,11 @@ def test_argument_errors_need_no_gpu(asr):
     assert L.asr_sched_percentiles(None, None, 1, pc9.ctypes.data, 9, None, None, 0, None) == -3
     assert L.asr_sched_gen_trace(0, 0, 0, 10, None, None, None) == -1
     assert L.asr_sched_select_host(None, 1, 1, 0, 0, 257, None) == -3
+    # tuning options: known ids and value ranges only
+    from paper_2603_11273_b200 import binding as b
+    assert L.asr_sched_set_option(b.OPT_SIM_LANE_SPLIT, 2) == -1
+    assert L.asr_sched_set_option(b.OPT_SIM_LANE_SPLIT, 0) == 0 and L.asr_sched_set_option(b.OPT_SIM_LANE_SPLIT, 1) == 0
+    assert L.asr_sched_set_option(77, 1) == -1
     # zero-size work is a no-op that needs no device
     assert L.asr_sched_select_batched(None, 0, 16, None, 1, 0, None, 4, None, None) == 0
     assert L.asr_sched_percentiles(None, None, 0, pc.ctypes.data, 0, None, None, 0, None) == 0
