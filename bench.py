@@ -335,15 +335,16 @@ def side_configs(asr, dev, d_tables, reps=5):
     return out
 
 
-def overload_sweep(asr, dev, d_tables, reps=3, n_seeds=512, n=3000):
+def overload_sweep(asr, dev, d_tables, reps=3, n_seeds=512, n=3000, check=True):
     """The contended regime of the BASE simulator (Table 1 rows 20-25 req/s):
     n_seeds seeds x 8 arrival rates 16..30 req/s x 3 policies x n lognormal requests, at 16 and at 32 slots,
     through plain asr_sched_simulate_batched (summary-only, default options).  Above ~20 (16 slots) / ~23
     (32 slots) req/s the queue grows and SJF/HRRN choose at every admission.  Reports requests/s, the split
-    of the time over the thread / warp / CTA tiers and the share of replicas each tier finished; a sample of
-    replicas is compared with the oracle (tolerance 0)."""
+    of the time over the thread / warp / CTA tiers.  With `check` (the cpu_baseline / parity leg of the run, never
+    inside a timed region) a sample of replicas is compared with the oracle, tolerance 0."""
     import torch
-    import oracle as orc
+    if check:
+        import oracle as orc
     rates = np.arange(16000, 31000, 2000, dtype=np.int32)                       # mHz
     pols = (wl.FCFS, wl.SJF, wl.HRRN)
     n_tr, n_rep = n_seeds * len(rates), n_seeds * len(rates) * len(pols)
@@ -386,7 +387,7 @@ def overload_sweep(asr, dev, d_tables, reps=3, n_seeds=512, n=3000):
         assert int((summ["n_done"] == n).sum()) == n_rep, "overload sweep: replicas did not finish"
         # parity sample: evenly spaced replicas against the oracle
         bad = 0
-        picks = np.linspace(0, n_rep - 1, 48).astype(np.int64)
+        picks = np.linspace(0, n_rep - 1, 48).astype(np.int64) if check else []
         for r in picks:
             tr_i, pol = int(r) // len(pols), pols[int(r) % len(pols)]
             tr = orc.gen_trace(int(specs["seed"][tr_i]), int(specs["rate_mhz"][tr_i]), orc.DIST_LOGNORMAL, n, ln, ex)
@@ -400,7 +401,7 @@ def overload_sweep(asr, dev, d_tables, reps=3, n_seeds=512, n=3000):
         out["slots%d" % slots] = {
             "ms": med, "requests_per_s": n_rep * n / (med / 1e3),
             "kernel_ms": {k: v[0] / reps for k, v in kt.items() if v[1]},
-            "parity_sample": {"replicas": int(len(picks)), "mismatches": bad}}
+            "parity_sample": {"replicas": int(len(picks)), "mismatches": bad} if check else None}
     return out
 
 
@@ -514,7 +515,8 @@ def run_ours(args):
         d_tables = asr.to_device(asr.make_tables(wl.ln_dur_table(), wl.exp_table()), dev)
         if rank == 0:
             side = {} if args.overload_only else side_configs(asr, dev, d_tables, reps=args.steps)
-            side["overload_sweep"] = overload_sweep(asr, dev, d_tables, reps=min(args.steps, 3))
+            side["overload_sweep"] = overload_sweep(asr, dev, d_tables, reps=min(args.steps, 3),
+                                                    check=not args.no_cpu_baseline)
             print(json.dumps({"configs": side}))
         D.finalize()
         return
@@ -728,7 +730,7 @@ def run_ours(args):
         del d_traces, d_ws, d_queues
         torch.cuda.empty_cache()
         side = side_configs(asr, dev, d_tables)
-        side["overload_sweep"] = overload_sweep(asr, dev, d_tables)
+        side["overload_sweep"] = overload_sweep(asr, dev, d_tables, check=not args.no_cpu_baseline)
         ext_lines = extension_lines(asr, dev, d_tables, hbm_peak, consts=consts)
 
     base = parity = None
@@ -760,6 +762,14 @@ def run_ours(args):
         }
         print(json.dumps(line), flush=True)
     D.finalize()
+    ov_bad = 0
+    if side and side.get("overload_sweep"):
+        for v in side["overload_sweep"].values():
+            if isinstance(v, dict) and v.get("parity_sample"):
+                ov_bad += v["parity_sample"]["mismatches"]
+    if ov_bad:
+        print("bench.py: the overload sweep disagrees with the oracle on %d sampled replicas" % ov_bad, file=sys.stderr)
+        return 3
     if parity is not None and parity["mismatches"] != 0:
         print("bench.py: the timed launches disagree with the oracle: %r" % parity, file=sys.stderr)
         return 3
