@@ -518,6 +518,10 @@ __device__ __forceinline__ void stage_tail(uint32_t *base, int ph, int n, const 
 // Every value that survives comes from a simulation that started in a true state; a boundary that cannot be
 // stitched inside segment s flags the replica, which is then simulated in one piece.
 enum { LANE_SEQ = 0, LANE_UNIT = 1, LANE_REPAIR = 2 };
+#ifndef LANE_REGEN_HEAD_N
+#define LANE_REGEN_HEAD_N 512
+#endif
+constexpr int LANE_REGEN_HEAD = LANE_REGEN_HEAD_N;   // requests at the head of a segment whose regeneration points are recorded
 #ifdef LANE_STATS
 // tuning builds: units run, units flagged, repairs run, repairs that found no common point, replicas redone,
 // requests re-simulated by repairs
@@ -693,16 +697,20 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
                 if (MODE != LANE_SEQ && arr0 >= t && p < n) {
                     // regeneration point: the server is empty when request p arrives, the clock goes to that arrival
                     if (MODE == LANE_UNIT) {
-                        while (wcur < (p >> 5)) {
-                            bm[wcur] = ibits;
-                            ibits = 0;
-                            ++wcur;
+                        // (only the head of the segment is recorded: a repair meets the segment within a few busy
+                        // periods of its start or not at all)
+                        if (p < LANE_REGEN_HEAD) {
+                            while (wcur < (p >> 5)) {
+                                bm[wcur] = ibits;
+                                ibits = 0;
+                                ++wcur;
+                            }
+                            ibits |= 1u << (p & 31);
                         }
-                        ibits |= 1u << (p & 31);
                         q_last = p;
                     } else {
                         const int d = start + p - seg_b;   // position in segment s
-                        if (d >= 0 && ((__ldcg(bm + (d >> 5)) >> (d & 31)) & 1u)) {
+                        if (d >= 0 && d < LANE_REGEN_HEAD && ((__ldcg(bm + (d >> 5)) >> (d & 31)) & 1u)) {
                             merged = true;   // segment s was in this very state: its values are true from here on
                             live = false;
                         }
@@ -796,7 +804,7 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
         if (MODE == LANE_UNIT) {
             stage_tail(ttft32, ph_t, n, sq_t);
             stage_tail(lat32, ph_l, n, sq_l);
-            for (; wcur <= ((n - 1) >> 5); ++wcur) {
+            for (; wcur <= ((min(n, LANE_REGEN_HEAD) - 1) >> 5); ++wcur) {
                 bm[wcur] = ibits;
                 ibits = 0;
             }
