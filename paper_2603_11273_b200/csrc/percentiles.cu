@@ -510,7 +510,7 @@ constexpr int PF_TRIES = 6;
 #define PF_IN_MANY_N 256   // one key per thread: a thread with more than PF_SLOTS - PF_GROUP closes its window
 #endif
 constexpr uint32_t PF_IN_MANY = PF_IN_MANY_N, PF_IN_FEW = PF_IN_MANY / 4;   // keys wanted inside a window
-static_assert(PCT_VPT % PF_GROUP == 0 && PF_SLOTS > PF_GROUP, "slot check granularity");
+static_assert(PCT_VPT % PF_GROUP == 0 && PF_SLOTS >= 2 * PF_GROUP, "slot check granularity");
 
 struct PctFastSmem {
     uint32_t slot[2][PF_SLOTS][PCT_THREADS];
@@ -563,6 +563,22 @@ __device__ __forceinline__ void pf_scan_b(const uint32_t (&c)[8], uint32_t tot, 
     }
 }
 
+// hist[bin] += 1 if p (a predicated shared-memory reduction: no branch, nothing touched when !p)
+__device__ __forceinline__ void pf_inc_if(uint32_t *hist, uint32_t bin, bool p) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred q;\n\t"
+        "setp.ne.u32 q, %1, 0;\n\t"
+        "@q red.shared.add.u32 [%0], 1;\n\t"
+        "}" ::"r"((uint32_t)__cvta_generic_to_shared(hist) + 4u * bin),
+        "r"((uint32_t)p)
+        : "memory");
+}
+#ifndef PF_STRAIGHT_N
+#define PF_STRAIGHT_N 3
+#endif
+constexpr int PF_STRAIGHT = PF_STRAIGHT_N;   // entries per thread and rank handled without a loop (most threads hold 0-2)
+
 // One pass over the keys.  Per key and rank: one compare-and-count below the window's end, one compare for
 // "inside", a predicated store and a predicated pointer bump (written out in PTX: the compiler's version of the
 // same loop took nine instructions per key and rank).  Returns, for rank t, T[t] = keys below the end | keys
@@ -601,14 +617,17 @@ __device__ __forceinline__ void pf_pass(const uint32_t (&key)[PCT_VPT], uint32_t
                 : "r"(key[g * PF_GROUP + j]), "r"(hi0), "r"(lo0), "r"(hi1), "r"(lo1), "n"(ROW)
                 : "memory");
         }
-        // a thread that could run out of slots in the next group closes its window
-        if (p0 > stop0) {
-            lo0 = hi0;
-            over |= 1u;
-        }
-        if (p1 > stop1) {
-            lo1 = hi1;
-            over |= 2u;
+        // a thread that could run out of slots in the next group closes its window (after the first group it holds
+        // at most PF_GROUP keys, after the last one nothing follows)
+        if (g > 0 && g < PCT_VPT / PF_GROUP - 1) {
+            if (p0 > stop0) {
+                lo0 = hi0;
+                over |= 1u;
+            }
+            if (p1 > stop1) {
+                lo1 = hi1;
+                over |= 2u;
+            }
         }
     }
     n[0] = (int)((p0 - b0) / ROW);
@@ -699,13 +718,18 @@ __global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(
             // keys: four consecutive values per 128-bit load; slots past the end read as 2^32-1 (below no window end)
             uint32_t key[PCT_VPT];
             {
-                const uint4 *v128 = reinterpret_cast<const uint4 *>(seg);
+                const uint4 *v128 = reinterpret_cast<const uint4 *>(seg) + tid;
                 const int n4 = N >> 2;
+                const int full_rows = n4 / PCT_THREADS;   // rows of PCT_THREADS quads that every thread loads
 #pragma unroll
                 for (int q = 0; q < PCT_VPT / 4; ++q) {
-                    const int idx = q * PCT_THREADS + tid;
-                    uint4 x = make_uint4(~0u, ~0u, ~0u, ~0u);
-                    if (idx < n4) x = __ldcs(v128 + idx);
+                    uint4 x;
+                    if (q < full_rows) {
+                        x = __ldcs(v128 + q * PCT_THREADS);
+                    } else {
+                        x = make_uint4(~0u, ~0u, ~0u, ~0u);
+                        if (q * PCT_THREADS + tid < n4) x = __ldcs(v128 + q * PCT_THREADS);
+                    }
                     key[4 * q] = x.x, key[4 * q + 1] = x.y, key[4 * q + 2] = x.z, key[4 * q + 3] = x.w;
                 }
             }
@@ -794,7 +818,12 @@ __global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(
                 const uint32_t below0 = (T[0] & 0xFFFFu) - in0, below1 = (T[1] & 0xFFFFu) - in1;
                 // level 1: bins of 2^sh values over the window
                 const int nm = n[0] > n[1] ? n[0] : n[1];
-                for (int e = 0; e < nm; ++e) {
+#pragma unroll
+                for (int e = 0; e < PF_STRAIGHT; ++e) {   // (a slot past the thread's count holds a stale key: never counted)
+                    pf_inc_if(fs.hist[0][0], (fs.slot[0][e][tid] - lo0) >> sh0, e < n[0]);
+                    pf_inc_if(fs.hist[0][1], (fs.slot[1][e][tid] - lo1) >> sh1, e < n[1]);
+                }
+                for (int e = PF_STRAIGHT; e < nm; ++e) {
                     if (e < n[0]) atomicAdd(&fs.hist[0][0][(fs.slot[0][e][tid] - lo0) >> sh0], 1u);
                     if (e < n[1]) atomicAdd(&fs.hist[0][1][(fs.slot[1][e][tid] - lo1) >> sh1], 1u);
                 }
@@ -811,7 +840,13 @@ __global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(
                 if (sh0 > 0 || sh1 > 0) {
                     // level 2: the selected bin, one value per bin
                     const int m0 = sh0 > 0 ? n[0] : 0, m1 = sh1 > 0 ? n[1] : 0, mm = m0 > m1 ? m0 : m1;
-                    for (int e = 0; e < mm; ++e) {
+#pragma unroll
+                    for (int e = 0; e < PF_STRAIGHT; ++e) {
+                        const uint32_t d0 = fs.slot[0][e][tid] - lo0, d1 = fs.slot[1][e][tid] - lo1;
+                        pf_inc_if(fs.hist[1][0], d0 & ((1u << sh0) - 1u), e < m0 && (d0 >> sh0) == bin0);
+                        pf_inc_if(fs.hist[1][1], d1 & ((1u << sh1) - 1u), e < m1 && (d1 >> sh1) == bin1);
+                    }
+                    for (int e = PF_STRAIGHT; e < mm; ++e) {
                         if (e < m0) {
                             const uint32_t d = fs.slot[0][e][tid] - lo0;
                             if ((d >> sh0) == bin0) atomicAdd(&fs.hist[1][0][d & ((1u << sh0) - 1u)], 1u);
