@@ -693,7 +693,6 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
             // B. the boundary of the admission step
             if (nW == 0 && nR == 0) {
                 tb = arr0;   // a new busy period starts with the next arrival
-#ifndef LANE_NO_REGEN
                 if (MODE != LANE_SEQ && arr0 >= t && p < n) {
                     // regeneration point: the server is empty when request p arrives, the clock goes to that arrival
                     if (MODE == LANE_UNIT) {
@@ -716,7 +715,6 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
                         }
                     }
                 }
-#endif
             }
             if (nW == 0 && arr0 > t) {
                 if (nR == 0) {
@@ -891,19 +889,11 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lan
     const int lane = lane_id();
     const int n_items = ((a.n_replicas + 31) / 32) * LANE_MAX_SEG;
     int32_t *next = a.plan.counters + (MODE == LANE_UNIT ? 0 : 1);
-#ifdef LANE_WORK_GRID
-    // tuning build: one item per warp, handed out by the block scheduler
-    for (int once = 0; once < 1; ++once) {
-        const int w = blockIdx.x * (LANE_THREADS / 32) + (threadIdx.x >> 5);
-        (void)next;
-        if (w >= n_items) break;
-#else
     while (true) {
         int w = 0;
         if (lane == 0) w = atomicAdd(next, 1);
         w = __shfl_sync(ASR_FULL_MASK, w, 0);
         if (w >= n_items) break;
-#endif
         const int2 item = make_int2(w / LANE_MAX_SEG, w % LANE_MAX_SEG);
         if (MODE == LANE_REPAIR && item.y == 0) continue;
         const int pos = 32 * item.x + lane;
@@ -960,9 +950,6 @@ __global__ void __launch_bounds__(256) lane_key_kernel(SimArgs a) {
             nseg = nseg > LANE_MAX_SEG ? LANE_MAX_SEG : nseg;
         }
     }
-#ifdef PLAN_NO_SORT
-    bucket = 0;
-#endif
     a.plan.bucket[r] = (uint8_t)bucket;
     a.plan.nseg[r] = (uint8_t)nseg;
     a.plan.failed[r] = 0;
@@ -1120,11 +1107,7 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
             // time-split units, stitched at regeneration points; what could not be stitched, in one piece
             int rc0 = launch_lane_plan(a, st);
             if (rc0) return rc0;
-#ifdef LANE_WORK_GRID
-            const int work_grid = (((a.n_replicas + 31) / 32) * LANE_MAX_SEG + LANE_THREADS / 32 - 1) / (LANE_THREADS / 32);
-#else
             const int work_grid = sm_count() * LANE_WORK_BLOCKS_PER_SM;
-#endif
             {
                 KernelTimer kt(KID_SIM_LANE, st);
                 sim_lane_work_kernel<LANE_UNIT><<<work_grid, LANE_THREADS, 0, st>>>(a);
