@@ -126,3 +126,24 @@ def test_carried_window_percentiles(asr):
     reps = [(t, POL[i % 3], 32) for i, t in enumerate(order)]
     _, _, S = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
     _check_all(traces, reps, S, wl.CONFIG_COST, "windows")
+
+
+def test_warp_tier_window_beyond_the_chunk_ring(asr):
+    """the warp tier with escalation switched off: a burst leaves a window of 7,000 requests, more than the ring of
+    chunk bounds covers (plain scans), which then shrinks back into the ring (bounds rebuilt, branch and bound),
+    while new arrivals keep joining; SJF and HRRN, per-request outputs"""
+    rng = np.random.Generator(np.random.PCG64(99))
+    n = 9000
+    arr = np.concatenate([np.zeros(7000, dtype=np.int64),
+                          np.cumsum(rng.exponential(400000.0, size=n - 7000).astype(np.int64))])
+    tr = _trace(arr, rng.integers(1000, 12001, size=n))
+    big = 2**31 - 1
+    asr.set_option(asr.OPT_SIM_LANE_MIN_REPLICAS, big)
+    asr.set_option(asr.OPT_SIM_ESCALATE_WINDOW, big)
+    try:
+        reps = [(0, orc.SJF, 8), (0, orc.HRRN, 8), (0, orc.HRRN, 32)]
+        L, T, S = run_batched([tr], reps, wl.CONFIG_COST, 32)
+        for i, (t, p, s) in enumerate(reps):
+            check_replica(tr, p, s, wl.CONFIG_COST, L[i], T[i], S[i], "rep %d" % i)
+    finally:
+        asr.set_option(asr.OPT_SIM_ESCALATE_WINDOW, 4096)
