@@ -271,8 +271,7 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
         out_lat = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes);
         out_ttft = (int64_t *)(ws + w.bm_off_bytes + w.bitmap_bytes + w.defer_bytes + w.lat_bytes);
     }
-    int rc = launch_sim_prepare(replicas, n_replicas, total_requests, bm_off, defer, st);
-    if (rc) return rc;
+    int rc = ASR_OK;
     SimArgs a{traces,  replicas, cms,         bm_off,         bitmap,     defer + 64, defer, defer + 64 + n_replicas, defer + 1,
               out_lat, out_ttft, out_summary, total_requests, n_replicas, n_cms, summary_only ? 1 : 0,
               g_opt_escalate.load(), LanePlan{}};
@@ -288,6 +287,10 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
         pl += 2 * w.seg_bytes;
         a.plan.unit_q = (int32_t *)pl;
         a.plan.counters = a.plan.unit_q + (size_t)n_replicas * LANE_MAX_SEG;
+    }
+    if (!a.plan.order) {   // (with a plan its second kernel does this job beside the sort)
+        rc = launch_sim_prepare(replicas, n_replicas, total_requests, bm_off, defer, st);
+        if (rc) return rc;
     }
     rc = launch_simulate(a, max_slots, use_lane, st);
     if (rc) return rc;

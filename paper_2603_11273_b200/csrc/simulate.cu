@@ -981,7 +981,7 @@ __device__ __forceinline__ uint32_t block_excl_scan_1024(uint32_t v, uint32_t *w
 
 // one CTA: stable counting sort of the replicas by load class (thread t owns the replicas [tC, tC + C) and one
 // column of the [class][thread] counters)
-__global__ void __launch_bounds__(1024) lane_sort_kernel(SimArgs a) {
+__device__ __forceinline__ void lane_sort_body(const SimArgs &a) {
     extern __shared__ uint32_t cnt[];   // [PLAN_BUCKETS][1024]
     __shared__ uint32_t wsum[32];
     const int t = threadIdx.x, n = a.n_replicas;
@@ -999,14 +999,18 @@ __global__ void __launch_bounds__(1024) lane_sort_kernel(SimArgs a) {
     for (int r = r0; r < r1; ++r) a.plan.order[cnt[a.plan.bucket[r] * 1024 + t]++] = r;
 }
 
+// block 0 sorts the plan, block 1 lays out the bitmaps and clears the counters (sim_prepare_kernel's job): two
+// single-CTA jobs that do not depend on each other, side by side
+__global__ void lane_plan_prepare_kernel(SimArgs a);
+
 int launch_lane_plan(const SimArgs &a, cudaStream_t st) {
     const int grid = (a.n_replicas + 255) / 256;
     constexpr int SORT_SMEM = PLAN_BUCKETS * 1024 * 4;
-    cudaFuncSetAttribute(lane_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_SMEM);
+    cudaFuncSetAttribute(lane_plan_prepare_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_SMEM);
     {
         KernelTimer kt(KID_LANE_PLAN, st);
         lane_key_kernel<<<grid, 256, 0, st>>>(a);
-        lane_sort_kernel<<<1, 1024, SORT_SMEM, st>>>(a);
+        lane_plan_prepare_kernel<<<2, 1024, SORT_SMEM, st>>>(a);
     }
     count_launch(1);
     return check_launch("lane plan kernels");
@@ -1029,9 +1033,8 @@ __global__ void __launch_bounds__(256) sim_init_lat_kernel(SimArgs a) {
 // A descriptor that replica_ok() will reject (n or out_off out of range) gets the two slack
 // words only, so that one bad descriptor cannot push the bitmaps of the valid replicas past
 // the workspace (which is sized from total_requests: the valid regions are disjoint).
-__global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *replicas, int32_t n_replicas,
-                                                           int64_t total_requests, int64_t *bm_off,
-                                                           int32_t *defer_count) {
+__device__ __forceinline__ void sim_prepare_body(const asr_replica_t *replicas, int32_t n_replicas, int64_t total_requests,
+                                                 int64_t *bm_off, int32_t *defer_count) {
     __shared__ int64_t warp_tot[32];
     __shared__ int64_t carry_s;
     if (threadIdx.x == 0) {
@@ -1078,6 +1081,17 @@ __global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *
         if (threadIdx.x == 1023) carry_s = incl;
         __syncthreads();
     }
+}
+
+__global__ void __launch_bounds__(1024) sim_prepare_kernel(const asr_replica_t *replicas, int32_t n_replicas,
+                                                           int64_t total_requests, int64_t *bm_off,
+                                                           int32_t *defer_count) {
+    sim_prepare_body(replicas, n_replicas, total_requests, bm_off, defer_count);
+}
+
+__global__ void __launch_bounds__(1024) lane_plan_prepare_kernel(SimArgs a) {
+    if (blockIdx.x == 0) lane_sort_body(a);
+    else sim_prepare_body(a.replicas, a.n_replicas, a.total_requests, const_cast<int64_t *>(a.bm_off), a.defer_count);
 }
 
 template <int SPL>
