@@ -502,22 +502,6 @@ __device__ __forceinline__ void stage_tail(uint32_t *base, int ph, int n, const 
 // event order through Stage32.  Exact as long as every value is below 2^32 us, which the
 // kernel proves with the start of the current busy period (every request in the system
 // arrived at or after it); a busy period of 2^32 us sends the replica to the warp kernel.
-// MODE (order-free outputs only):
-//   LANE_SEQ     a thread simulates a whole replica (with a plan: only the replicas flagged `failed`).
-//   LANE_UNIT    a thread simulates one segment [b, b + L) of a replica's trace AS IF it were a trace of its own:
-//                the server is taken to be idle at the segment's first arrival and the trace to end with the
-//                segment.  It records its regeneration points (server empty at an arrival at or after the clock:
-//                the state is then (empty, t = that arrival) whatever came before) in the replica's bitmap, and
-//                the last one in unit_q -- the segment's end itself if everything completed by the next arrival.
-//   LANE_REPAIR  a thread stitches the boundary between segments s-1 and s: unless segment s-1 ended at a
-//                regeneration point, it simulates from the last regeneration point q of segment s-1 (a TRUE state
-//                when the segments before are stitched) across the boundary until it reaches a regeneration point
-//                that segment s recorded too -- from there on segment s's values are the true ones -- and
-//                overwrites the values of the requests [q, that point) in place (positions = request indices for
-//                both streams: at a regeneration point exactly the requests before it have been emitted).
-// Every value that survives comes from a simulation that started in a true state; a boundary that cannot be
-// stitched inside segment s flags the replica, which is then simulated in one piece.
-enum { LANE_SEQ = 0, LANE_UNIT = 1, LANE_REPAIR = 2 };
 #ifndef LANE_REGEN_HEAD_N
 #define LANE_REGEN_HEAD_N 512
 #endif
@@ -532,19 +516,13 @@ __host__ __device__ __forceinline__ int lane_seg_len(int n, int nseg) {
     return (((n + nseg - 1) / nseg) + 31) & ~31;   // whole bitmap words per segment
 }
 
-// one lane's piece; all 32 lanes of a warp call it together (`live` = this lane has a piece).  sbase = the lane's
-// column of the CTA's ring; r = replica; seg / nseg = its segment (units); uq = its unit_q entry
-template <bool FREE, int MODE>
-__device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase, bool live, const int r, const int seg,
-                                         const int nseg, const int uq) {
-    static_assert(FREE || MODE == LANE_SEQ, "units need order-free outputs");
+// a thread simulates replica r from its first request to its last; all 32 lanes of a warp call it together (`live` =
+// this lane has a replica).  sbase = the lane's column of the CTA's ring
+template <bool FREE>
+__device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase, bool live, const int r) {
     // every lane of a warp stays in the loop below until the whole warp is done (the loop
     // re-converges the warp once per admission step); `live` marks the lanes with work
-    if (MODE == LANE_REPAIR && seg == 0) live = false;
     bool valid = live;
-    int start = 0;        // first request of this thread's piece (index in the replica)
-    int seg_b = 0;        // first request of segment `seg`
-    int piece_n = -1;     // requests in the piece (-1: the whole replica)
     asr_replica_t rep;
     rep.trace_off = rep.out_off = 0;
     rep.n = 0;
@@ -553,29 +531,13 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
     if (live) {
         rep = a.replicas[r];
         if (!replica_ok(a, rep, LANE_CAP)) {
-            flag_invalid(a, r);   // (an invalid descriptor is one unit)
+            flag_invalid(a, r);
             live = valid = false;
             rep.cm_id = 0;
             rep.n = 0;
         }
     }
-    if (MODE != LANE_SEQ && live) {
-        const int L = lane_seg_len(rep.n, nseg);
-        seg_b = seg * L;
-        if (MODE == LANE_UNIT) {
-            start = seg_b;
-            piece_n = min(L, rep.n - seg_b);
-        } else {
-            const int q = a.plan.unit_q[uq - 1];   // the entries of a replica are consecutive
-            if (q >= seg_b || a.plan.failed[r] != 0) {
-                live = valid = false;   // segment s-1 ended at a regeneration point (or the replica is flagged already)
-            } else {
-                start = q;
-                piece_n = min(seg_b + L, rep.n) - q;
-            }
-        }
-    }
-    const int n = piece_n >= 0 ? piece_n : rep.n, slots = rep.slots, policy = rep.policy;
+    const int n = rep.n, slots = rep.slots, policy = rep.policy;
     const asr_cost_model_t *cmp = a.cms + rep.cm_id;
     const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
     const int64_t iter_base64 = __ldg(&cmp->iter_base_us), iter_per64 = __ldg(&cmp->iter_per_running_us);
@@ -594,16 +556,9 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
     const uint32_t enc_base = (uint32_t)enc_base64;
     const int32_t enc_per = (int32_t)enc_per64;
     const uint32_t ib = (uint32_t)iter_base64, ip = (uint32_t)iter_per64;
-    const asr_req_t *trace = a.traces + rep.trace_off + start;
+    const asr_req_t *trace = a.traces + rep.trace_off;
     int64_t *lat = a.out_lat + rep.out_off;
     int64_t *ttft = a.out_ttft + rep.out_off;
-    // units: the regeneration points of this piece, one bit per request, in the replica's bitmap (whole words per
-    // segment); `ibits` collects the word `wcur`
-    uint32_t *bm = nullptr;
-    if (MODE != LANE_SEQ && live) bm = a.bitmap + a.bm_off[r] + (seg_b >> 5);
-    uint32_t ibits = 0;
-    int wcur = 0, q_last = 0;
-    bool merged = false;
 
     int64_t t = 0;     // the current iteration boundary
     int64_t tb = 0;    // FREE: start of the current busy period (arrival of its first request)
@@ -634,12 +589,11 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
     const bool staged = (reinterpret_cast<uintptr_t>(ttft) & 15u) == 0;
     // FREE: both outputs through Stage32
     Stage32 sq_t = {0, 0, 0, 0}, sq_l = {0, 0, 0, 0};
-    uint32_t *ttft32 = reinterpret_cast<uint32_t *>(ttft) + start, *lat32 = reinterpret_cast<uint32_t *>(lat) + start;
+    uint32_t *ttft32 = reinterpret_cast<uint32_t *>(ttft), *lat32 = reinterpret_cast<uint32_t *>(lat);
     const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft32) >> 2) & 3u);
     const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat32) >> 2) & 3u);
     // (written now rather than carried through the loop: the kernel sits at its register limit)
-    if (valid && a.out_summary && (MODE == LANE_SEQ || (MODE == LANE_UNIT && seg == 0)))
-        a.out_summary[r].first_arrival_us = n > 0 ? arr0 : 0;
+    if (valid && a.out_summary) a.out_summary[r].first_arrival_us = n > 0 ? arr0 : 0;
     if (n == 0) live = false;
 
     // One trip of the outer loop = one admission step, so that the lanes of a warp (32
@@ -691,31 +645,7 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
         if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
         if (live) {
             // B. the boundary of the admission step
-            if (nW == 0 && nR == 0) {
-                tb = arr0;   // a new busy period starts with the next arrival
-                if (MODE != LANE_SEQ && arr0 >= t && p < n) {
-                    // regeneration point: the server is empty when request p arrives, the clock goes to that arrival
-                    if (MODE == LANE_UNIT) {
-                        // (only the head of the segment is recorded: a repair meets the segment within a few busy
-                        // periods of its start or not at all)
-                        if (p < LANE_REGEN_HEAD) {
-                            while (wcur < (p >> 5)) {
-                                bm[wcur] = ibits;
-                                ibits = 0;
-                                ++wcur;
-                            }
-                            ibits |= 1u << (p & 31);
-                        }
-                        q_last = p;
-                    } else {
-                        const int d = start + p - seg_b;   // position in segment s
-                        if (d >= 0 && d < LANE_REGEN_HEAD && ((__ldcg(bm + (d >> 5)) >> (d & 31)) & 1u)) {
-                            merged = true;   // segment s was in this very state: its values are true from here on
-                            live = false;
-                        }
-                    }
-                }
-            }
+            if (nW == 0 && nR == 0) tb = arr0;   // a new busy period starts with the next arrival
             if (nW == 0 && arr0 > t) {
                 if (nR == 0) {
                     t = arr0;   // idle server: the clock jumps to the next arrival (S14)
@@ -727,7 +657,7 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
                 }
             }
             // C. ingest arrivals <= t
-            while (arr0 <= t && (MODE != LANE_REPAIR || !merged)) {
+            while (arr0 <= t) {
                 last_arr = arr0;
                 last_dur = dur0;
                 ++p;
@@ -748,9 +678,7 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
             // D. admit k >= 1 requests (a slot is free and somebody waits)
             const int free_slots = slots - nR;
             const int k = free_slots < nW ? free_slots : nW;
-            if (MODE == LANE_REPAIR && merged) {
-                // stitched: nothing more to simulate
-            } else if (policy != ASR_FCFS && k < nW) {   // a real choice: hand over to the warp kernel
+            if (policy != ASR_FCFS && k < nW) {   // a real choice: hand over to the warp kernel
                 deferred = true;
                 live = false;
             } else {
@@ -786,52 +714,6 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
             }
         }
     }
-    if (MODE != LANE_SEQ) {
-        if (deferred) {
-            a.plan.failed[r] = 1;   // whatever stopped this piece, the replica is simulated in one piece
-#ifdef LANE_STATS
-            atomicAdd(&g_lane_stats[1], 1ull);
-#endif
-            return;
-        }
-        if (!valid) return;
-#ifdef LANE_STATS
-        atomicAdd(&g_lane_stats[MODE == LANE_UNIT ? 0 : 2], 1ull);
-        if (MODE == LANE_REPAIR) atomicAdd(&g_lane_stats[5], (unsigned long long)p);
-#endif
-        if (MODE == LANE_UNIT) {
-            stage_tail(ttft32, ph_t, n, sq_t);
-            stage_tail(lat32, ph_l, n, sq_l);
-            for (; wcur <= ((min(n, LANE_REGEN_HEAD) - 1) >> 5); ++wcur) {
-                bm[wcur] = ibits;
-                ibits = 0;
-            }
-            // everything completed by the next segment's first arrival: the segment's end is a regeneration point
-            if (start + n < rep.n && t <= ld_arrival(trace + n)) q_last = n;
-            a.plan.unit_q[uq] = start + q_last;
-            asr_summary_t *s = a.out_summary + r;
-            if (seg == nseg - 1) {
-                s->last_done_us = t;
-                s->n_done = rep.n;
-                s->p50_e2e_us = ASR_FMT32;
-                s->p50_ttft_us = ASR_FMT32;
-            }
-        } else {
-            const bool to_end = done >= n && start + n == rep.n;   // the last boundary, simulated to the end of the trace
-            if (!merged && !to_end) {
-                a.plan.failed[r] = 1;   // no common regeneration point inside segment s
-#ifdef LANE_STATS
-                atomicAdd(&g_lane_stats[3], 1ull);
-#endif
-                return;
-            }
-            const int cnt = merged ? p : n;   // at a regeneration point exactly the requests before it have been emitted
-            stage_tail(ttft32, ph_t, cnt, sq_t);
-            stage_tail(lat32, ph_l, cnt, sq_l);
-            if (to_end && !merged) a.out_summary[r].last_done_us = t;
-        }
-        return;
-    }
     if (deferred) {
         const int pos = atomicAdd(a.defer_count, 1);
         a.defer_list[pos] = r;
@@ -862,6 +744,345 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
     }
 }
 
+// ---------------------------------------------------------------------------
+// a piece of a replica in 32-bit times (summary-only calls).
+//   LANE_UNIT    a thread simulates one segment [b, b + L) of a replica's trace AS IF it were a trace of its own:
+//                the server is taken to be idle at the segment's first arrival and the trace to end with the
+//                segment.  It records its regeneration points (server empty at an arrival at or after the clock:
+//                the state is then (empty, t = that arrival) whatever came before) in the replica's bitmap, and
+//                the last one in unit_q -- the segment's end itself if everything completed by the next arrival.
+//   LANE_REPAIR  a thread stitches the boundary between segments s-1 and s: unless segment s-1 ended at a
+//                regeneration point, it simulates from the last regeneration point q of segment s-1 (a TRUE state
+//                when the segments before are stitched) across the boundary until it reaches a regeneration point
+//                that segment s recorded too -- from there on segment s's values are the true ones -- and
+//                overwrites the values of the requests [q, that point) in place (positions = request indices for
+//                both streams: at a regeneration point exactly the requests before it have been emitted).
+// Every value that survives comes from a simulation that started in a true state; a boundary that cannot be
+// stitched inside segment s flags the replica, which lane_run then simulates in one piece.
+//
+// A piece starts with the server empty at one of its arrivals and stays within minutes of it, so every time is kept
+// as a uint32 offset from an EPOCH E (an arrival at which the server was empty): the clock t, the look-ahead
+// arrivals and the ring payloads; iteration costs, token counts and encoder times are 32-bit as well.  Exactness:
+//   * the limits below (computed once per piece) bound what one trip of the loop can add to t by 3 * 2^29, and t is
+//     tested against 2^31 once per trip, so no sum ever wraps; a request outside the limits, a clock beyond 2^31 us
+//     past the epoch or a first arrival before the clock's origin flags the replica, which is then simulated in one
+//     piece by the 64-bit code of lane_run (every emitted value is below 2^32 there too);
+//   * an arrival 2^32 us or more past the epoch reads LANE_FAR, which no clock value reaches; the epoch moves to
+//     the next arrival (read again from the trace, all 64 bits) whenever the server is empty and that arrival is
+//     2^30 us or more past it.
+// ---------------------------------------------------------------------------
+enum { LANE_UNIT = 1, LANE_REPAIR = 2 };
+constexpr uint32_t LANE_FAR = 0xFFFFFFFFu;
+
+__device__ __forceinline__ uint32_t lane_rel(int64_t arrival, int64_t epoch) {
+    const uint64_t d = (uint64_t)(arrival - epoch);
+    return (d >> 32) != 0ull ? LANE_FAR : (uint32_t)d;
+}
+
+template <int MODE>
+__device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbase, bool live, const int r, const int seg,
+                                           const int nseg, const int uq) {
+    static_assert(MODE == LANE_UNIT || MODE == LANE_REPAIR, "pieces only");
+    if (MODE == LANE_REPAIR && seg == 0) live = false;
+    bool valid = live;
+    int start = 0;     // first request of this thread's piece (index in the replica)
+    int seg_b = 0;     // first request of segment `seg`
+    int n = 0;         // requests in the piece
+    asr_replica_t rep;
+    rep.trace_off = rep.out_off = 0;
+    rep.n = 0;
+    rep.policy = rep.cm_id = 0;
+    rep.slots = 1;
+    if (live) {
+        rep = a.replicas[r];
+        if (!replica_ok(a, rep, LANE_CAP)) {
+            flag_invalid(a, r);   // (an invalid descriptor is one unit)
+            live = valid = false;
+            rep.cm_id = 0;
+            rep.n = 0;
+        }
+    }
+    if (live) {
+        const int L = lane_seg_len(rep.n, nseg);
+        seg_b = seg * L;
+        if (MODE == LANE_UNIT) {
+            start = seg_b;
+            n = min(L, rep.n - seg_b);
+        } else {
+            const int q = a.plan.unit_q[uq - 1];   // the entries of a replica are consecutive
+            if (q >= seg_b || a.plan.failed[r] != 0) {
+                live = valid = false;   // segment s-1 ended at a regeneration point (or the replica is flagged already)
+            } else {
+                start = q;
+                n = min(seg_b + L, rep.n) - q;
+            }
+        }
+    }
+    const int slots = rep.slots;
+    const bool chooses = rep.policy != ASR_FCFS;
+    const asr_cost_model_t *cmp = a.cms + rep.cm_id;
+    const int64_t enc_base64 = __ldg(&cmp->enc_base_us), enc_per64 = __ldg(&cmp->enc_per_ms_us);
+    const int64_t iter_base64 = __ldg(&cmp->iter_base_us), iter_per64 = __ldg(&cmp->iter_per_running_us);
+    const int32_t tok_base = __ldg(&cmp->tok_base), tok_per_s_i = __ldg(&cmp->tok_per_s);
+    const uint32_t tok_per_s = (uint32_t)tok_per_s_i;
+    // the limits: one iteration < 2^29 us at 32 running; a request's decode (tokens * that) < 2^29 us; 32 encoder
+    // passes + one iteration < 2^29 us; tok_per_s * dur_ms < 2^32.  dur_lim = the longest audio inside all of them.
+    const int64_t lim29 = ((int64_t)1 << 29) - 1;
+    bool deferred = false;
+    uint32_t dur_lim = 0;
+    {
+        const bool sane = enc_base64 >= 0 && enc_base64 <= lim29 && enc_per64 >= 0 && enc_per64 <= lim29 &&
+                          iter_base64 >= 0 && iter_base64 <= lim29 && iter_per64 >= 0 && iter_per64 <= lim29 &&
+                          tok_per_s_i >= 0 && tok_base > -(1 << 30) && tok_base < (1 << 30);
+        const int64_t cmax = sane ? iter_base64 + iter_per64 * LANE_CAP : lim29 + 1;
+        int64_t dl = -1;
+        if (cmax <= lim29) {
+            const int64_t tok_lim = lim29 / (cmax > 0 ? cmax : 1);             // tokens * cmax < 2^29
+            const int64_t enc_lim = (lim29 - cmax) / LANE_CAP - enc_base64;     // enc_per * dur <= enc_lim
+            dl = (int64_t)1 << 24;                                              // (asr_sched.h: dur_ms <= 2^24)
+            if (tok_per_s_i > 0) {
+                dl = min(dl, (int64_t)0xFFFFFFFFll / tok_per_s_i);
+                dl = tok_lim < tok_base ? -1 : min(dl, ((tok_lim - tok_base) * 1000) / tok_per_s_i);
+            } else if (tok_lim < tok_base) {
+                dl = -1;
+            }
+            if (enc_lim < 0) dl = -1;
+            else if (enc_per64 > 0) dl = min(dl, enc_lim / enc_per64);
+        }
+        if (live && dl < 0) {
+            deferred = true;
+            live = false;
+        }
+        dur_lim = dl < 0 ? 0u : (uint32_t)dl;
+    }
+    const uint32_t enc_base = (uint32_t)enc_base64, enc_per = (uint32_t)enc_per64;
+    const uint32_t ib = (uint32_t)iter_base64, ip = (uint32_t)iter_per64;
+    const asr_req_t *trace = a.traces + rep.trace_off + start;
+    // the regeneration points of segment `seg`, one bit per request, in the replica's bitmap (whole words per
+    // segment); `ibits` collects the word `wcur`
+    uint32_t *bm = nullptr;
+    if (live) bm = a.bitmap + a.bm_off[r] + (seg_b >> 5);
+    uint32_t ibits = 0;
+    int wcur = 0, q_last = 0;
+    bool merged = false;
+
+    int64_t E = 0;      // the epoch
+    uint32_t t = 0;     // the current iteration boundary, us past the epoch
+    int p = 0, lo = 0, nW = 0, nR = 0, done = 0;
+    uint32_t hoff = 0;  // running set = nR ring positions from byte offset hoff, sorted by finish iteration
+    uint32_t it = 0;    // engine iterations so far, mod 2^32
+    // look-ahead window over the trace: records p and p+1 are in registers (one 128-bit load each); the arrival of
+    // p+1 stays as loaded until it becomes arr0 a trip later (a conversion here would wait for the load)
+    uint32_t arr0 = LANE_FAR, last_arr = 0;
+    int64_t raw1 = INT64_MAX;
+    int32_t dur0 = 0, dur1 = 0, last_dur = 0;
+    int32_t est1 = 0;   // (kept live until the record is consumed, see lane_run)
+    bool bad = false;   // a request outside the limits was ingested
+    if (live && n > 0) {
+        const Rec q = ld_cached(trace);
+        E = q.arrival_us;
+        arr0 = 0;
+        dur0 = q.dur_ms;
+        if (MODE == LANE_UNIT && seg == 0) {
+            if (a.out_summary) a.out_summary[r].first_arrival_us = E;
+            if (E < 0) {   // the clock starts at 0, after this arrival: not a piece that starts idle
+                deferred = true;
+                live = false;
+            }
+        }
+    }
+    if (live && n > 1) {
+        const Rec q = ld_cached(trace + 1);
+        raw1 = q.arrival_us;
+        dur1 = q.dur_ms;
+        est1 = q.est;
+    }
+    Stage32 sq_t = {0, 0, 0, 0}, sq_l = {0, 0, 0, 0};
+    uint32_t *ttft32 = reinterpret_cast<uint32_t *>(a.out_ttft + rep.out_off) + start;
+    uint32_t *lat32 = reinterpret_cast<uint32_t *>(a.out_lat + rep.out_off) + start;
+    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft32) >> 2) & 3u);
+    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat32) >> 2) & 3u);
+    if (n == 0) {
+        if (MODE == LANE_UNIT && seg == 0 && valid && a.out_summary) a.out_summary[r].first_arrival_us = 0;
+        live = false;
+    }
+
+    // One trip = one admission step (lane_run): A pops the completions that precede the step, B moves the clock to
+    // its boundary, C ingests, D admits.
+    while (true) {
+        if (live) {
+            // A. completions before the next admission opportunity
+            bool more = nR > 0;
+            const uint32_t a_eff = nW > 0 ? 0u : arr0;   // somebody waiting: admit at the first free slot
+            while (more) {
+                const uint2 e = ring_ld(sbase + hoff);   // sorted: the head finishes first
+                const uint32_t f = e.x;
+                const uint32_t m = f - it;
+                const uint32_t c = ib + ip * (uint32_t)nR;
+                const uint32_t lim = t + (m - 1u) * c;
+                if (m > 0u && nR < slots && a_eff <= lim) {
+                    more = false;
+                } else {
+                    if (m > 0u) {
+                        t = lim + c;
+                        it = f;
+                    }
+                    stage_push(lat32, ph_l, done, t - e.y, sq_l);   // E2E = t - arrival
+                    hoff = (hoff + RING_STEP) & RING_MASK;
+                    --nR;
+                    ++done;
+                    more = nR > 0;
+                }
+            }
+            if (done >= n) live = false;
+            if ((t >> 31) != 0u) {   // too far past the epoch for 32-bit times
+                deferred = true;
+                live = false;
+            }
+        }
+        if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
+        if (live) {
+            // B. the boundary of the admission step
+            if (nW == 0 && nR == 0 && arr0 >= t) {
+                // regeneration point: the server is empty when request p arrives, the clock goes to that arrival
+                if (MODE == LANE_UNIT) {
+                    // (only the head of the segment is recorded: a repair meets the segment within a few busy
+                    // periods of its start or not at all)
+                    if (p < LANE_REGEN_HEAD) {
+                        while (wcur < (p >> 5)) {
+                            bm[wcur] = ibits;
+                            ibits = 0;
+                            ++wcur;
+                        }
+                        ibits |= 1u << (p & 31);
+                    }
+                    q_last = p;
+                } else {
+                    const int d = start + p - seg_b;   // position in segment s
+                    if (d >= 0 && d < LANE_REGEN_HEAD && ((__ldcg(bm + (d >> 5)) >> (d & 31)) & 1u)) {
+                        merged = true;   // segment s was in this very state: its values are true from here on
+                        live = false;
+                    }
+                }
+                if (arr0 >= (1u << 30)) {   // move the epoch to this arrival
+                    E = ld_arrival(trace + p);
+                    arr0 = 0;
+                    t = 0;
+                }
+            }
+            if (nW == 0 && arr0 > t) {
+                if (nR == 0) {
+                    t = arr0;   // idle server: the clock jumps to the next arrival (S14)
+                } else {
+                    const uint32_t c = ib + ip * (uint32_t)nR;
+                    const uint32_t g = arr0 - t;   // c > 0: arr0 <= t + (m-1)*c
+                    const uint32_t q = g / c;
+                    const uint32_t j = q + (g - q * c != 0u ? 1u : 0u);
+                    t += j * c;
+                    it += j;
+                }
+            }
+            // C. ingest arrivals <= t
+            while (arr0 <= t && (MODE != LANE_REPAIR || !merged)) {
+                last_arr = arr0;
+                last_dur = dur0;
+                bad = bad || (uint32_t)dur0 > dur_lim;
+                ++p;
+                ++nW;
+                arr0 = lane_rel(raw1, E);
+                dur0 = dur1;
+                asm volatile("{ .reg .pred p; setp.eq.s32 p, %0, -2147483647; @p prefetch.global.L2 [%1]; }" ::"r"(est1),
+                             "l"(trace));
+                raw1 = INT64_MAX;
+                if (p + 1 < n) {
+                    const Rec q = ld_cached(trace + p + 1);
+                    raw1 = q.arrival_us;
+                    dur1 = q.dur_ms;
+                    est1 = q.est;
+                }
+            }
+            // D. admit k >= 1 requests (a slot is free and somebody waits)
+            const int free_slots = slots - nR;
+            const int k = free_slots < nW ? free_slots : nW;
+            if (MODE == LANE_REPAIR && merged) {
+                // stitched: nothing more to simulate
+            } else if ((chooses && k < nW) || bad) {   // a real choice, or 64-bit arithmetic: the replica is redone in one piece
+                deferred = true;
+                live = false;
+            } else {
+                uint32_t t1 = t + ib + ip * (uint32_t)(nR + k);
+                if (k == 1 && lo == p - 1) {
+                    // the request ingested last: everything needed is in registers
+                    const int32_t tok = tok_base + (int32_t)((tok_per_s * (uint32_t)last_dur) / 1000u);
+                    lane_insert(sbase, hoff, nR, it, (uint32_t)(tok < 1 ? 1 : tok), last_arr);
+                    t1 += enc_per * (uint32_t)last_dur + enc_base;
+                    stage_push(ttft32, ph_t, lo, t1 - last_arr, sq_t);   // first token (S9)
+                } else {
+                    uint32_t dur_sum = 0;
+                    for (int q = 0; q < k; ++q) {
+                        const Rec rq = ld_cached(trace + lo + q);
+                        const int32_t tok = tok_base + (int32_t)((tok_per_s * (uint32_t)rq.dur_ms) / 1000u);
+                        lane_insert(sbase, hoff, nR + q, it, (uint32_t)(tok < 1 ? 1 : tok), lane_rel(rq.arrival_us, E));
+                        dur_sum += (uint32_t)rq.dur_ms;
+                    }
+                    t1 += enc_base * (uint32_t)k + enc_per * dur_sum;
+                    for (int q = 0; q < k; ++q)
+                        stage_push(ttft32, ph_t, lo + q, t1 - lane_rel(ld_arrival(trace + lo + q), E), sq_t);
+                }
+                lo += k;
+                nW -= k;
+                nR += k;
+                t = t1;
+                it += 1u;
+            }
+        }
+    }
+    if (deferred) {
+        a.plan.failed[r] = 1;   // whatever stopped this piece, the replica is simulated in one piece
+#ifdef LANE_STATS
+        atomicAdd(&g_lane_stats[1], 1ull);
+#endif
+        return;
+    }
+    if (!valid) return;
+#ifdef LANE_STATS
+    atomicAdd(&g_lane_stats[MODE == LANE_UNIT ? 0 : 2], 1ull);
+    if (MODE == LANE_REPAIR) atomicAdd(&g_lane_stats[5], (unsigned long long)p);
+#endif
+    const int64_t t_end = E + (int64_t)t;
+    if (MODE == LANE_UNIT) {
+        stage_tail(ttft32, ph_t, n, sq_t);
+        stage_tail(lat32, ph_l, n, sq_l);
+        for (; wcur <= ((min(n, LANE_REGEN_HEAD) - 1) >> 5); ++wcur) {
+            bm[wcur] = ibits;
+            ibits = 0;
+        }
+        // everything completed by the next segment's first arrival: the segment's end is a regeneration point
+        if (start + n < rep.n && t_end <= ld_arrival(trace + n)) q_last = n;
+        a.plan.unit_q[uq] = start + q_last;
+        if (seg == nseg - 1 && a.out_summary) {
+            asr_summary_t *s = a.out_summary + r;
+            s->last_done_us = t_end;
+            s->n_done = rep.n;
+            s->p50_e2e_us = ASR_FMT32;
+            s->p50_ttft_us = ASR_FMT32;
+        }
+    } else {
+        const bool to_end = done >= n && start + n == rep.n;   // the last boundary, simulated to the end of the trace
+        if (!merged && !to_end) {
+            a.plan.failed[r] = 1;   // no common regeneration point inside segment s
+#ifdef LANE_STATS
+            atomicAdd(&g_lane_stats[3], 1ull);
+#endif
+            return;
+        }
+        const int cnt = merged ? p : n;   // at a regeneration point exactly the requests before it have been emitted
+        stage_tail(ttft32, ph_t, cnt, sq_t);
+        stage_tail(lat32, ph_l, cnt, sq_l);
+        if (to_end && !merged && a.out_summary) a.out_summary[r].last_done_us = t_end;
+    }
+}
+
 // a thread simulates a whole replica (with a plan: only the replicas flagged `failed`)
 template <bool FREE>
 __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_kernel(SimArgs a) {
@@ -873,17 +1094,22 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_BLOCKS_PER_SM) sim_lane_ker
 #ifdef LANE_STATS
     if (live && a.plan.failed) atomicAdd(&g_lane_stats[4], 1ull);
 #endif
-    lane_run<FREE, LANE_SEQ>(a, sbase, live, r, 0, 1, 0);
+    lane_run<FREE>(a, sbase, live, r);
 }
 
 // persistent warps work off the plan's items (heaviest load class first): lane j of item (group, seg) takes
 // segment seg of replica order[32*group + j]
 #ifndef LANE_WORK_BLOCKS
-#define LANE_WORK_BLOCKS 12
+#define LANE_WORK_BLOCKS 10
 #endif
-constexpr int LANE_WORK_BLOCKS_PER_SM = LANE_WORK_BLOCKS;   // one CTA less than the replica kernel: the unit's extra state
+// (r02 sweep: 15.8 ms at 10 CTAs and 94 registers, 16.4-16.5 ms at 12 or 13 CTAs squeezed into 80 / 72)
+constexpr int LANE_WORK_BLOCKS_PER_SM = LANE_WORK_BLOCKS;
 template <int MODE>
+#ifdef LANE_WORK_MAXREG
+__global__ void __maxnreg__(LANE_WORK_MAXREG) sim_lane_work_kernel(SimArgs a) {
+#else
 __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lane_work_kernel(SimArgs a) {
+#endif
     __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_ring) + threadIdx.x * 8u;
     const int lane = lane_id();
@@ -906,7 +1132,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lan
         }
         if (!__any_sync(ASR_FULL_MASK, live)) continue;   // no replica of the group has this many segments
         const int uq = pos * LANE_MAX_SEG + item.y;
-        lane_run<true, MODE>(a, sbase, live, r, item.y, nseg, uq);
+        lane_piece<MODE>(a, sbase, live, r, item.y, nseg, uq);
         __syncwarp();
     }
 }
@@ -1118,6 +1344,11 @@ int launch_simulate(const SimArgs &a_in, int max_slots, bool use_lane, cudaStrea
     if (use_lane && max_slots <= LANE_CAP) {
         const int lane_grid = (a.n_replicas + LANE_THREADS - 1) / LANE_THREADS;
         if (a.order_free && a.plan.order) {
+            // (lane_piece: the two value arrays of a summary-only call share the phase of their 16-byte lines)
+            if (((reinterpret_cast<uintptr_t>(a.out_lat) ^ reinterpret_cast<uintptr_t>(a.out_ttft)) & 15u) != 0) {
+                set_error("simulate: workspace value arrays out of phase");
+                return ASR_EINVAL;
+            }
             // time-split units, stitched at regeneration points; what could not be stitched, in one piece
             int rc0 = launch_lane_plan(a, st);
             if (rc0) return rc0;

@@ -100,6 +100,35 @@ def test_bursty_boundaries_and_unstitchable_replicas(asr):
     _check_all(traces, reps, S1, wl.CONFIG_COST, "bursty")
 
 
+def test_pieces_in_32_bit_times(asr):
+    """the 32-bit clock of the pieces (an offset from an epoch that moves at idle arrivals) and the limits that send a
+    replica back to the 64-bit code: (a) gaps of 20 minutes to 3 hours between arrivals (epoch moves; arrivals 2^32 us
+    past the epoch), a trace that starts before t = 0 and one far from it (2^45 us); (b) a cost model whose encoder
+    pass or whose iteration is outside the 32-bit budget, one with 10^5 us iterations, one that costs nothing; (c) a busy period of more than 2^31 us"""
+    rng = np.random.Generator(np.random.PCG64(123))
+    n = 2600
+    gaps = rng.exponential(2.0e6, size=n).astype(np.int64)
+    gaps[::97] += rng.integers(1_200_000_000, 11_000_000_000, size=len(gaps[::97]))   # 20 min .. 3 h
+    arr = np.cumsum(gaps)
+    dur = rng.integers(1000, 35001, size=n)
+    traces = [_trace(arr, dur), _trace(arr - 5_000_000_000, dur), _trace(arr + (1 << 45), dur)]
+    reps = [(t, p, s) for t in range(len(traces)) for p in POL for s in (4, 32)]
+    _, _, S1 = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    _check_all(traces, reps, S1, wl.CONFIG_COST, "gaps")
+    # (b)
+    light = [wl.stress_trace("lognormal", 2700, 500, rate_per_s=0.5), wl.stress_trace("uniform", 5000, 501, rate_per_s=0.2)]
+    reps = [(t, p, 32) for t in range(len(light)) for p in POL]
+    for cost in ((20000, 30000, 8000, 50, 1, 4), (1 << 30, 0, 8000, 50, 1, 4), wl.TOY_COST, (0, 0, 0, 0, 1, 0),
+                 (20000, 2, 1 << 26, 50, 1, 4)):
+        _, _, S1 = run_batched(light, reps, cost, 32, summary_only=True)
+        _check_all(light, reps, S1, cost, "cost %r" % (cost,))
+    # (c) 2,700 requests over 2,700 s, ~20 s of service each under the toy cost model: the server never empties
+    busy = [_trace(np.arange(2700, dtype=np.int64) * 1_000_000, rng.integers(20000, 30001, size=2700))]
+    reps = [(0, p, 32) for p in POL]
+    _, _, S1 = run_batched(busy, reps, wl.TOY_COST, 32, summary_only=True)
+    _check_all(busy, reps, S1, wl.TOY_COST, "busy")
+
+
 def test_carried_window_percentiles(asr):
     """1,500 replicas in runs and alternations of very different traces (the carried window of the percentile
     kernel hits, misses either way, overflows its slots and re-seeds), all values equal, lengths that are
