@@ -873,9 +873,9 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
     uint32_t it = 0;    // engine iterations so far, mod 2^32
     // look-ahead window over the trace: records p and p+1 are in registers (one 128-bit load each); the arrival of
     // p+1 stays as loaded until it becomes arr0 a trip later (a conversion here would wait for the load)
-    uint32_t arr0 = LANE_FAR, last_arr = 0;
+    uint32_t arr0 = LANE_FAR, last_arr = 0, prev_arr = 0;   // last / prev: the two requests ingested last
     int64_t raw1 = INT64_MAX;
-    int32_t dur0 = 0, dur1 = 0, last_dur = 0;
+    int32_t dur0 = 0, dur1 = 0, last_dur = 0, prev_dur = 0;
     int32_t est1 = 0;   // (kept live until the record is consumed, see lane_run)
     bool bad = false;   // a request outside the limits was ingested
     if (live && n > 0) {
@@ -949,6 +949,7 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                     // (only the head of the segment is recorded: a repair meets the segment within a few busy
                     // periods of its start or not at all)
                     if (p < LANE_REGEN_HEAD) {
+#pragma unroll 1
                         while (wcur < (p >> 5)) {
                             bm[wcur] = ibits;
                             ibits = 0;
@@ -984,6 +985,8 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
             }
             // C. ingest arrivals <= t
             while (arr0 <= t && (MODE != LANE_REPAIR || !merged)) {
+                prev_arr = last_arr;
+                prev_dur = last_dur;
                 last_arr = arr0;
                 last_dur = dur0;
                 bad = bad || (uint32_t)dur0 > dur_lim;
@@ -1017,8 +1020,18 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                     lane_insert(sbase, hoff, nR, it, (uint32_t)(tok < 1 ? 1 : tok), last_arr);
                     t1 += enc_per * (uint32_t)last_dur + enc_base;
                     stage_push(ttft32, ph_t, lo, t1 - last_arr, sq_t);   // first token (S9)
+                } else if (k == 2 && nW == 2) {
+                    // the two requests ingested last (two arrivals during one admission step)
+                    const int32_t tok_a = tok_base + (int32_t)((tok_per_s * (uint32_t)prev_dur) / 1000u);
+                    lane_insert(sbase, hoff, nR, it, (uint32_t)(tok_a < 1 ? 1 : tok_a), prev_arr);
+                    const int32_t tok_b = tok_base + (int32_t)((tok_per_s * (uint32_t)last_dur) / 1000u);
+                    lane_insert(sbase, hoff, nR + 1, it, (uint32_t)(tok_b < 1 ? 1 : tok_b), last_arr);
+                    t1 += enc_per * (uint32_t)(prev_dur + last_dur) + 2u * enc_base;
+                    stage_push(ttft32, ph_t, lo, t1 - prev_arr, sq_t);
+                    stage_push(ttft32, ph_t, lo + 1, t1 - last_arr, sq_t);
                 } else {
                     uint32_t dur_sum = 0;
+#pragma unroll 1
                     for (int q = 0; q < k; ++q) {
                         const Rec rq = ld_cached(trace + lo + q);
                         const int32_t tok = tok_base + (int32_t)((tok_per_s * (uint32_t)rq.dur_ms) / 1000u);
@@ -1026,6 +1039,7 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                         dur_sum += (uint32_t)rq.dur_ms;
                     }
                     t1 += enc_base * (uint32_t)k + enc_per * dur_sum;
+#pragma unroll 1
                     for (int q = 0; q < k; ++q)
                         stage_push(ttft32, ph_t, lo + q, t1 - lane_rel(ld_arrival(trace + lo + q), E), sq_t);
                 }
