@@ -519,6 +519,8 @@ struct PctFastSmem {
     uint32_t wovf[2][PCT_THREADS / 32];      // [parity][warp]: bit t = a thread closed its window of rank t
     uint32_t wsum[2][PCT_THREADS / 64];
     uint32_t sel_bin[2][2], sel_rem[2][2];   // [level][rank]
+    uint32_t sel_cnt[2];                     // [rank]: keys in the selected level-1 bin
+    uint32_t lcnt[2], list[2][32];           // [rank]: those keys (their offsets inside the bin) when there are at most 32
 };
 
 __device__ __forceinline__ uint32_t pf_end(uint32_t lo, int sh) {   // saturated: a key 2^32-1 is never inside
@@ -545,7 +547,7 @@ __device__ __forceinline__ void pf_scan_a(const uint32_t *h, int j, uint32_t (&c
 }
 
 __device__ __forceinline__ void pf_scan_b(const uint32_t (&c)[8], uint32_t tot, uint32_t incl, const uint32_t *wsum, int j,
-                                          uint32_t k, uint32_t *sel_bin, uint32_t *sel_rem) {
+                                          uint32_t k, uint32_t *sel_bin, uint32_t *sel_rem, uint32_t *sel_cnt = nullptr) {
     uint32_t excl = incl - tot;
 #pragma unroll
     for (int w = 0; w < PF_HALF / 32; ++w)
@@ -557,6 +559,7 @@ __device__ __forceinline__ void pf_scan_b(const uint32_t (&c)[8], uint32_t tot, 
             if (run < k && k <= run + c[b]) {
                 *sel_bin = (uint32_t)(8 * j + b);
                 *sel_rem = k - run;
+                if (sel_cnt) *sel_cnt = c[b];
             }
             run += c[b];
         }
@@ -733,13 +736,15 @@ __global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(
                     key[4 * q] = x.x, key[4 * q + 1] = x.y, key[4 * q + 2] = x.z, key[4 * q + 3] = x.w;
                 }
             }
-            // clear both histogram levels (their last readers passed the final barrier of the previous segment)
+            // clear the first histogram level and the lists (their last readers passed the final barrier of the
+            // previous segment)
             {
                 uint4 *z = reinterpret_cast<uint4 *>(&fs.hist[0][0][0]);
-                constexpr int n16 = 2 * 2 * PF_BINS / 4;
+                constexpr int n16 = 2 * PF_BINS / 4;
                 static_assert(n16 % PCT_THREADS == 0, "whole passes");
 #pragma unroll
                 for (int q = 0; q < n16 / PCT_THREADS; ++q) z[q * PCT_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
+                if (tid < 2) fs.lcnt[tid] = 0;
             }
             if (!have) {
                 // bisection on the key bits, both ranks at once: bracket [a, a + 2^rem) holds `in` keys, `below` lie under it
@@ -833,35 +838,66 @@ __global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(
                 uint32_t c[8], tot, incl;
                 pf_scan_a(fs.hist[0][tg], j, c, tot, incl, fs.wsum[tg]);
                 __syncthreads();
-                pf_scan_b(c, tot, incl, fs.wsum[tg], j, kw, &fs.sel_bin[0][tg], &fs.sel_rem[0][tg]);
+                pf_scan_b(c, tot, incl, fs.wsum[tg], j, kw, &fs.sel_bin[0][tg], &fs.sel_rem[0][tg], &fs.sel_cnt[tg]);
                 __syncthreads();
                 const uint32_t bin0 = fs.sel_bin[0][0], bin1 = fs.sel_bin[0][1];
                 uint32_t r0 = lo0 + (bin0 << sh0), r1 = lo1 + (bin1 << sh1);
                 if (sh0 > 0 || sh1 > 0) {
-                    // level 2: the selected bin, one value per bin
+                    // level 2: the keys of the selected bin
                     const int m0 = sh0 > 0 ? n[0] : 0, m1 = sh1 > 0 ? n[1] : 0, mm = m0 > m1 ? m0 : m1;
+                    const uint32_t cnt0 = sh0 > 0 ? fs.sel_cnt[0] : 0u, cnt1 = sh1 > 0 ? fs.sel_cnt[1] : 0u;
+                    if (cnt0 <= 32u && cnt1 <= 32u) {
+                        // a handful: listed, and ranked by one warp per rank (any order of equal keys gives the same
+                        // value at every rank)
+                        for (int e = 0; e < mm; ++e) {
+                            if (e < m0) {
+                                const uint32_t dd = fs.slot[0][e][tid] - lo0;
+                                if ((dd >> sh0) == bin0) fs.list[0][atomicAdd(&fs.lcnt[0], 1u)] = dd & ((1u << sh0) - 1u);
+                            }
+                            if (e < m1) {
+                                const uint32_t dd = fs.slot[1][e][tid] - lo1;
+                                if ((dd >> sh1) == bin1) fs.list[1][atomicAdd(&fs.lcnt[1], 1u)] = dd & ((1u << sh1) - 1u);
+                            }
+                        }
+                        __syncthreads();
+                        if (tid < 64) {
+                            const int t = tid >> 5, lane = tid & 31;
+                            const uint32_t cn = t == 0 ? cnt0 : cnt1;
+                            const uint32_t v = (uint32_t)lane < cn ? fs.list[t][lane] : 0xFFFFFFFFu;
+                            uint32_t rank = 0;
+                            for (uint32_t q = 0; q < cn; ++q) {
+                                const uint32_t u = __shfl_sync(ASR_FULL_MASK, v, (int)q);
+                                rank += (u < v || (u == v && q < (uint32_t)lane)) ? 1u : 0u;
+                            }
+                            if ((uint32_t)lane < cn && rank + 1u == fs.sel_rem[0][t]) fs.sel_bin[1][t] = v;
+                        }
+                        __syncthreads();
+                    } else {
+                        // many equal or near-equal keys: a second histogram, one value per bin
+                        {
+                            uint4 *z = reinterpret_cast<uint4 *>(&fs.hist[1][0][0]);
+                            constexpr int n16 = 2 * PF_BINS / 4;
 #pragma unroll
-                    for (int e = 0; e < PF_STRAIGHT; ++e) {
-                        const uint32_t d0 = fs.slot[0][e][tid] - lo0, d1 = fs.slot[1][e][tid] - lo1;
-                        pf_inc_if(fs.hist[1][0], d0 & ((1u << sh0) - 1u), e < m0 && (d0 >> sh0) == bin0);
-                        pf_inc_if(fs.hist[1][1], d1 & ((1u << sh1) - 1u), e < m1 && (d1 >> sh1) == bin1);
-                    }
-                    for (int e = PF_STRAIGHT; e < mm; ++e) {
-                        if (e < m0) {
-                            const uint32_t d = fs.slot[0][e][tid] - lo0;
-                            if ((d >> sh0) == bin0) atomicAdd(&fs.hist[1][0][d & ((1u << sh0) - 1u)], 1u);
+                            for (int q = 0; q < n16 / PCT_THREADS; ++q) z[q * PCT_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
                         }
-                        if (e < m1) {
-                            const uint32_t d = fs.slot[1][e][tid] - lo1;
-                            if ((d >> sh1) == bin1) atomicAdd(&fs.hist[1][1][d & ((1u << sh1) - 1u)], 1u);
+                        __syncthreads();
+                        for (int e = 0; e < mm; ++e) {
+                            if (e < m0) {
+                                const uint32_t dd = fs.slot[0][e][tid] - lo0;
+                                if ((dd >> sh0) == bin0) atomicAdd(&fs.hist[1][0][dd & ((1u << sh0) - 1u)], 1u);
+                            }
+                            if (e < m1) {
+                                const uint32_t dd = fs.slot[1][e][tid] - lo1;
+                                if ((dd >> sh1) == bin1) atomicAdd(&fs.hist[1][1][dd & ((1u << sh1) - 1u)], 1u);
+                            }
                         }
+                        __syncthreads();
+                        const bool act = tg == 0 ? sh0 > 0 : sh1 > 0;
+                        if (act) pf_scan_a(fs.hist[1][tg], j, c, tot, incl, fs.wsum[tg]);
+                        __syncthreads();
+                        if (act) pf_scan_b(c, tot, incl, fs.wsum[tg], j, fs.sel_rem[0][tg], &fs.sel_bin[1][tg], &fs.sel_rem[1][tg]);
+                        __syncthreads();
                     }
-                    __syncthreads();
-                    const bool act = tg == 0 ? sh0 > 0 : sh1 > 0;
-                    if (act) pf_scan_a(fs.hist[1][tg], j, c, tot, incl, fs.wsum[tg]);
-                    __syncthreads();
-                    if (act) pf_scan_b(c, tot, incl, fs.wsum[tg], j, fs.sel_rem[0][tg], &fs.sel_bin[1][tg], &fs.sel_rem[1][tg]);
-                    __syncthreads();
                     if (sh0 > 0) r0 += fs.sel_bin[1][0];
                     if (sh1 > 0) r1 += fs.sel_bin[1][1];
                 }
