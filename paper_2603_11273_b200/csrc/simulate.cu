@@ -497,6 +497,55 @@ __device__ __forceinline__ void stage_tail(uint32_t *base, int ph, int n, const 
     if (cnt >= 1) base[n - 1] = s.v3;
 }
 
+#ifdef LANE_SECTOR_STORES
+// The same with whole 32-byte sectors (pieces): a quad that completes the FIRST half of a sector is parked in shared
+// memory (`park`: 16 bytes of this thread and stream) and written together with the second half, as two 16-byte stores
+// to one sector back to back.  A half-written sector that L2 evicts before its other half arrives costs a read and a
+// second write in DRAM.  r02, config 3: 13.5 GB of DRAM traffic (1.03x the 13.1 GB the kernel has to move) and 16.06 ms
+// this way, 19.0-20.5 GB (1.5x) and 15.4 ms with the 16-byte stores of Stage32 some 6 us apart -- the kernel is bound
+// by its dependent instruction chains, not by HBM, and the parked quad's way back through shared memory sits on
+// them.  Hence an opt-in (-DLANE_SECTOR_STORES), not the default.
+// ph8 = the element phase of base[0] within its 32-byte sector.
+__device__ __forceinline__ void stage8_push(uint32_t *base, int ph8, int pos, uint32_t v, Stage32 &s, uint32_t park) {
+    s.v0 = s.v1;
+    s.v1 = s.v2;
+    s.v2 = s.v3;
+    s.v3 = v;
+    const int k = (ph8 + pos) & 7;
+    if ((k & 3) == 3) {
+        if (pos < 3) {   // short head before the first 16-byte boundary
+            if (pos >= 2) base[pos - 2] = s.v1;
+            if (pos >= 1) base[pos - 1] = s.v2;
+            base[pos] = s.v3;
+        } else if (k == 3) {
+            asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(park), "r"(s.v0), "r"(s.v1), "r"(s.v2), "r"(s.v3) : "memory");
+        } else {
+            if (pos >= 7) {
+                uint4 h;
+                asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(h.x), "=r"(h.y), "=r"(h.z), "=r"(h.w) : "r"(park) : "memory");
+                *reinterpret_cast<uint4 *>(base + pos - 7) = h;
+            }
+            *reinterpret_cast<uint4 *>(base + pos - 3) = make_uint4(s.v0, s.v1, s.v2, s.v3);
+        }
+    }
+}
+
+// after n pushes: a parked quad whose second half never came, and the values after the last whole quad
+__device__ __forceinline__ void stage8_tail(uint32_t *base, int ph8, int n, const Stage32 &s, uint32_t park) {
+    int cnt = (ph8 + n) & 3;
+    cnt = cnt < n ? cnt : n;
+    const int last = n - cnt - 1;   // the last element of the last whole quad (if last >= 3)
+    if (last >= 3 && ((ph8 + last) & 7) == 3) {
+        uint4 h;
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(h.x), "=r"(h.y), "=r"(h.z), "=r"(h.w) : "r"(park) : "memory");
+        *reinterpret_cast<uint4 *>(base + last - 3) = h;
+    }
+    if (cnt >= 3) base[n - 3] = s.v1;
+    if (cnt >= 2) base[n - 2] = s.v2;
+    if (cnt >= 1) base[n - 1] = s.v3;
+}
+#endif
+
 // FREE = order-free outputs: the ring carries the low word of the arrival time instead of
 // the request index, E2E latency is formed at completion and both outputs are emitted in
 // event order through Stage32.  Exact as long as every value is below 2^32 us, which the
@@ -780,8 +829,8 @@ __device__ __forceinline__ uint32_t lane_rel(int64_t arrival, int64_t epoch) {
 }
 
 template <int MODE>
-__device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbase, bool live, const int r, const int seg,
-                                           const int nseg, const int uq) {
+__device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbase, const uint32_t park, bool live, const int r,
+                                           const int seg, const int nseg, const int uq) {
     static_assert(MODE == LANE_UNIT || MODE == LANE_REPAIR, "pieces only");
     if (MODE == LANE_REPAIR && seg == 0) live = false;
     bool valid = live;
@@ -898,10 +947,22 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
         est1 = q.est;
     }
     Stage32 sq_t = {0, 0, 0, 0}, sq_l = {0, 0, 0, 0};
+#ifdef LANE_SECTOR_STORES
+    const uint32_t park_l = park + LANE_THREADS * 16u;
+    const uint32_t ph_mask = 7u;
+#define PIECE_PUSH_T(pos, v) stage8_push(ttft32, ph_t, pos, v, sq_t, park)
+#define PIECE_PUSH_L(pos, v) stage8_push(lat32, ph_l, pos, v, sq_l, park_l)
+#define PIECE_TAIL(cnt) (stage8_tail(ttft32, ph_t, cnt, sq_t, park), stage8_tail(lat32, ph_l, cnt, sq_l, park_l))
+#else
+    const uint32_t ph_mask = 3u;
+#define PIECE_PUSH_T(pos, v) stage_push(ttft32, ph_t, pos, v, sq_t)
+#define PIECE_PUSH_L(pos, v) stage_push(lat32, ph_l, pos, v, sq_l)
+#define PIECE_TAIL(cnt) (stage_tail(ttft32, ph_t, cnt, sq_t), stage_tail(lat32, ph_l, cnt, sq_l))
+#endif
     uint32_t *ttft32 = reinterpret_cast<uint32_t *>(a.out_ttft + rep.out_off) + start;
     uint32_t *lat32 = reinterpret_cast<uint32_t *>(a.out_lat + rep.out_off) + start;
-    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft32) >> 2) & 3u);
-    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat32) >> 2) & 3u);
+    const int ph_t = (int)((reinterpret_cast<uintptr_t>(ttft32) >> 2) & ph_mask);
+    const int ph_l = (int)((reinterpret_cast<uintptr_t>(lat32) >> 2) & ph_mask);
     if (n == 0) {
         if (MODE == LANE_UNIT && seg == 0 && valid && a.out_summary) a.out_summary[r].first_arrival_us = 0;
         live = false;
@@ -927,7 +988,7 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                         t = lim + c;
                         it = f;
                     }
-                    stage_push(lat32, ph_l, done, t - e.y, sq_l);   // E2E = t - arrival
+                    PIECE_PUSH_L(done, t - e.y);   // E2E = t - arrival
                     hoff = (hoff + RING_STEP) & RING_MASK;
                     --nR;
                     ++done;
@@ -1019,7 +1080,7 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                     const int32_t tok = tok_base + (int32_t)((tok_per_s * (uint32_t)last_dur) / 1000u);
                     lane_insert(sbase, hoff, nR, it, (uint32_t)(tok < 1 ? 1 : tok), last_arr);
                     t1 += enc_per * (uint32_t)last_dur + enc_base;
-                    stage_push(ttft32, ph_t, lo, t1 - last_arr, sq_t);   // first token (S9)
+                    PIECE_PUSH_T(lo, t1 - last_arr);   // first token (S9)
                 } else if (k == 2 && nW == 2) {
                     // the two requests ingested last (two arrivals during one admission step)
                     const int32_t tok_a = tok_base + (int32_t)((tok_per_s * (uint32_t)prev_dur) / 1000u);
@@ -1027,8 +1088,8 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                     const int32_t tok_b = tok_base + (int32_t)((tok_per_s * (uint32_t)last_dur) / 1000u);
                     lane_insert(sbase, hoff, nR + 1, it, (uint32_t)(tok_b < 1 ? 1 : tok_b), last_arr);
                     t1 += enc_per * (uint32_t)(prev_dur + last_dur) + 2u * enc_base;
-                    stage_push(ttft32, ph_t, lo, t1 - prev_arr, sq_t);
-                    stage_push(ttft32, ph_t, lo + 1, t1 - last_arr, sq_t);
+                    PIECE_PUSH_T(lo, t1 - prev_arr);
+                    PIECE_PUSH_T(lo + 1, t1 - last_arr);
                 } else {
                     uint32_t dur_sum = 0;
 #pragma unroll 1
@@ -1041,7 +1102,7 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                     t1 += enc_base * (uint32_t)k + enc_per * dur_sum;
 #pragma unroll 1
                     for (int q = 0; q < k; ++q)
-                        stage_push(ttft32, ph_t, lo + q, t1 - lane_rel(ld_arrival(trace + lo + q), E), sq_t);
+                        PIECE_PUSH_T(lo + q, t1 - lane_rel(ld_arrival(trace + lo + q), E));
                 }
                 lo += k;
                 nW -= k;
@@ -1065,8 +1126,7 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
 #endif
     const int64_t t_end = E + (int64_t)t;
     if (MODE == LANE_UNIT) {
-        stage_tail(ttft32, ph_t, n, sq_t);
-        stage_tail(lat32, ph_l, n, sq_l);
+        PIECE_TAIL(n);
         for (; wcur <= ((min(n, LANE_REGEN_HEAD) - 1) >> 5); ++wcur) {
             bm[wcur] = ibits;
             ibits = 0;
@@ -1091,11 +1151,13 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
             return;
         }
         const int cnt = merged ? p : n;   // at a regeneration point exactly the requests before it have been emitted
-        stage_tail(ttft32, ph_t, cnt, sq_t);
-        stage_tail(lat32, ph_l, cnt, sq_l);
+        PIECE_TAIL(cnt);
         if (to_end && !merged && a.out_summary) a.out_summary[r].last_done_us = t_end;
     }
 }
+#undef PIECE_PUSH_T
+#undef PIECE_PUSH_L
+#undef PIECE_TAIL
 
 // a thread simulates a whole replica (with a plan: only the replicas flagged `failed`)
 template <bool FREE>
@@ -1125,6 +1187,12 @@ __global__ void __maxnreg__(LANE_WORK_MAXREG) sim_lane_work_kernel(SimArgs a) {
 __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lane_work_kernel(SimArgs a) {
 #endif
     __shared__ uint2 s_ring[LANE_CAP * LANE_THREADS];
+#ifdef LANE_SECTOR_STORES
+    __shared__ uint4 s_park[2 * LANE_THREADS];   // [stream][thread]: stage8_push
+    const uint32_t park = (uint32_t)__cvta_generic_to_shared(s_park) + threadIdx.x * 16u;
+#else
+    const uint32_t park = 0;
+#endif
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_ring) + threadIdx.x * 8u;
     const int lane = lane_id();
     const int n_items = ((a.n_replicas + 31) / 32) * LANE_MAX_SEG;
@@ -1146,7 +1214,7 @@ __global__ void __launch_bounds__(LANE_THREADS, LANE_WORK_BLOCKS_PER_SM) sim_lan
         }
         if (!__any_sync(ASR_FULL_MASK, live)) continue;   // no replica of the group has this many segments
         const int uq = pos * LANE_MAX_SEG + item.y;
-        lane_piece<MODE>(a, sbase, live, r, item.y, nseg, uq);
+        lane_piece<MODE>(a, sbase, park, live, r, item.y, nseg, uq);
         __syncwarp();
     }
 }
