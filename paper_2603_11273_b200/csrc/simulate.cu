@@ -813,9 +813,10 @@ __device__ __forceinline__ void lane_run(const SimArgs &a, const uint32_t sbase,
 // as a uint32 offset from an EPOCH E (an arrival at which the server was empty): the clock t, the look-ahead
 // arrivals and the ring payloads; iteration costs, token counts and encoder times are 32-bit as well.  Exactness:
 //   * the limits below (computed once per piece) bound what one trip of the loop can add to t by 3 * 2^29, and t is
-//     tested against 2^31 once per trip, so no sum ever wraps; a request outside the limits, a clock beyond 2^31 us
-//     past the epoch or a first arrival before the clock's origin flags the replica, which is then simulated in one
-//     piece by the 64-bit code of lane_run (every emitted value is below 2^32 there too);
+//     tested against 2^30 once per trip (the epoch then moves up, see there), so no sum ever wraps; a request outside
+//     the limits, a request that stays in the system for 2^30 us or a first arrival before the clock's origin flags
+//     the replica, which is then simulated in one piece by the 64-bit code of lane_run (every emitted value is below
+//     2^32 there too);
 //   * an arrival 2^32 us or more past the epoch reads LANE_FAR, which no clock value reaches; the epoch moves to
 //     the next arrival (read again from the trace, all 64 bits) whenever the server is empty and that arrival is
 //     2^30 us or more past it.
@@ -996,9 +997,34 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                 }
             }
             if (done >= n) live = false;
-            if ((t >> 31) != 0u) {   // too far past the epoch for 32-bit times
-                deferred = true;
-                live = false;
+            if (live && (t >> 30) != 0u) {
+                // 2^30 us past the epoch with the server busy (rare): the epoch moves up to the clock, or to the next
+                // arrival if that one is already due (no arrival still to come may lie before the epoch).  The
+                // ring's payloads are arrivals relative to the epoch and only ever enter differences modulo 2^32,
+                // which stay exact while no request in the system is older than 2^32 us; here every one of them
+                // is checked to be younger than 2^30 us (else the 64-bit code takes the replica), and the clock
+                // gains less than 2.5 * 2^30 us before the next check.
+                const uint32_t s = arr0 < t ? arr0 : t;
+                bool young = ((t - s) >> 30) == 0u;
+                for (int i = 0; i < nR; ++i)
+                    young = young && t - ring_ld(sbase + ((hoff + (uint32_t)i * RING_STEP) & RING_MASK)).y < (1u << 30);
+                if (nW > 0) young = young && (E + (int64_t)t) - ld_arrival(trace + lo) < ((int64_t)1 << 30);
+                if (!young) {
+                    deferred = true;
+                    live = false;
+                } else {
+                    for (int i = 0; i < nR; ++i) {
+                        const uint32_t ad = sbase + ((hoff + (uint32_t)i * RING_STEP) & RING_MASK);
+                        const uint2 e = ring_ld(ad);
+                        ring_st(ad, make_uint2(e.x, e.y - s));
+                    }
+                    E += (int64_t)s;
+                    t -= s;
+                    last_arr -= s;
+                    prev_arr -= s;
+                    if (arr0 != LANE_FAR) arr0 -= s;
+                    else if (p < n) arr0 = lane_rel(ld_arrival(trace + p), E);
+                }
             }
         }
         if (!__any_sync(ASR_FULL_MASK, live)) break;   // also the warp's re-convergence point
@@ -1096,13 +1122,14 @@ __device__ __forceinline__ void lane_piece(const SimArgs &a, const uint32_t sbas
                     for (int q = 0; q < k; ++q) {
                         const Rec rq = ld_cached(trace + lo + q);
                         const int32_t tok = tok_base + (int32_t)((tok_per_s * (uint32_t)rq.dur_ms) / 1000u);
-                        lane_insert(sbase, hoff, nR + q, it, (uint32_t)(tok < 1 ? 1 : tok), lane_rel(rq.arrival_us, E));
+                        // (a waiting request may have arrived before the epoch: the difference modulo 2^32)
+                        lane_insert(sbase, hoff, nR + q, it, (uint32_t)(tok < 1 ? 1 : tok), (uint32_t)(rq.arrival_us - E));
                         dur_sum += (uint32_t)rq.dur_ms;
                     }
                     t1 += enc_base * (uint32_t)k + enc_per * dur_sum;
 #pragma unroll 1
                     for (int q = 0; q < k; ++q)
-                        PIECE_PUSH_T(lo + q, t1 - lane_rel(ld_arrival(trace + lo + q), E));
+                        PIECE_PUSH_T(lo + q, t1 - (uint32_t)(ld_arrival(trace + lo + q) - E));
                 }
                 lo += k;
                 nW -= k;

@@ -104,7 +104,8 @@ def test_pieces_in_32_bit_times(asr):
     """the 32-bit clock of the pieces (an offset from an epoch that moves at idle arrivals) and the limits that send a
     replica back to the 64-bit code: (a) gaps of 20 minutes to 3 hours between arrivals (epoch moves; arrivals 2^32 us
     past the epoch), a trace that starts before t = 0 and one far from it (2^45 us); (b) a cost model whose encoder
-    pass or whose iteration is outside the 32-bit budget, one with 10^5 us iterations, one that costs nothing; (c) a busy period of more than 2^31 us"""
+    pass or whose iteration is outside the 32-bit budget, one with 10^5 us iterations, one that costs nothing; (c) busy
+    periods of more than 2^31 us, one with requests that wait longer than 2^30 us and one without"""
     rng = np.random.Generator(np.random.PCG64(123))
     n = 2600
     gaps = rng.exponential(2.0e6, size=n).astype(np.int64)
@@ -127,6 +128,11 @@ def test_pieces_in_32_bit_times(asr):
     reps = [(0, p, 32) for p in POL]
     _, _, S1 = run_batched(busy, reps, wl.TOY_COST, 32, summary_only=True)
     _check_all(busy, reps, S1, wl.TOY_COST, "busy")
+    # the same arrivals with a cheap encoder: ~12 requests running at any time, nobody waits, the server never
+    # empties for 45 minutes (the epoch moves while the server is busy)
+    steady = (20000, 0, 100000, 0, 0, 5)
+    _, _, S1 = run_batched(busy, reps, steady, 32, summary_only=True)
+    _check_all(busy, reps, S1, steady, "steady")
 
 
 def test_carried_window_percentiles(asr):
