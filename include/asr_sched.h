@@ -132,6 +132,21 @@ int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy, int64_t n
                      int32_t k, int32_t *out_idx, void *workspace,
                      size_t workspace_bytes, void *stream);
 
+/* asr_sched_select without a workspace and without any allocation, for callers
+ * that cannot call cudaMalloc (code under CUDA graph capture, serving loops,
+ * harnesses that forbid it).  The scratch of the single-queue reduction tree is
+ * a device array of ASR_SELECT_STATIC_SCRATCH_BYTES built into the library (every
+ * GPU that loads the library holds it until exit).  Same arguments, results and
+ * error codes as asr_sched_select; in addition -3 when
+ * asr_sched_workspace_bytes(ASR_OP_SELECT, n, k) exceeds the array (1 MiB:
+ * k <= 32 up to n = 3.3e7 records, k = 256 up to n = 3.9e6).  All calls on a
+ * device share the array: calls that overlap on the GPU (different streams
+ * without ordering) race; calls on one stream do not.  Nothing is carried from
+ * one call to the next.  Calls no cudaMalloc / cudaFree. */
+#define ASR_SELECT_STATIC_SCRATCH_BYTES (1 << 20)
+int asr_sched_select_static(const asr_req_t *keys, int64_t n, int32_t policy, int64_t now,
+                            int32_t k, int32_t *out_idx, void *stream);
+
 /* n_queues independent queues; queue q is keys[q*q_len .. q*q_len+q_len) of
  * which the first q_count[q] (or q_len if q_count is NULL) records are valid.
  * Indices are local to the queue; out_idx[q*k + j] is the j-th best, -1 padded.

@@ -33,7 +33,7 @@ assert SUMMARY_DTYPE.itemsize == 56 and SPEC_DTYPE.itemsize == 16 and TABLES_DTY
 EXPORTS = (
     "asr_sched_select", "asr_sched_select_batched", "asr_sched_simulate", "asr_sched_simulate_batched",
     "asr_sched_percentiles", "asr_sched_gen_trace", "asr_sched_gen_trace_batched", "asr_sched_gen_queues",
-    "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_simulate_batched_ex", "asr_sched_tpot",
+    "asr_sched_sweep_host", "asr_sched_select_host", "asr_sched_select_static", "asr_sched_simulate_batched_ex", "asr_sched_tpot",
     "asr_sched_estimate", "asr_sched_itl_batched", "asr_sched_trim_scratch", "asr_sched_workspace_bytes", "asr_sched_last_error",
     "asr_sched_version", "asr_sched_launch_count", "asr_sched_timing_enable", "asr_sched_timing_reset",
     "asr_sched_timing_read", "asr_sched_kernel_name", "asr_sched_set_option",
@@ -62,6 +62,7 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         vp, i64, i32, u64, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_size_t
         L.asr_sched_select.argtypes = [vp, i64, i32, i64, i32, vp, vp, sz, vp]
+        L.asr_sched_select_static.argtypes = [vp, i64, i32, i64, i32, vp, vp]
         L.asr_sched_select_batched.argtypes = [vp, i32, i32, vp, i32, i64, vp, i32, vp, vp]
         L.asr_sched_simulate.argtypes = [vp, i64, i32, vp, i32, vp, vp, vp, vp, sz, vp]
         L.asr_sched_simulate_batched.argtypes = [vp, vp, i32, vp, i32, i64, i32, vp, vp, vp, vp, sz, vp]
@@ -75,7 +76,7 @@ def lib():
         L.asr_sched_tpot.argtypes = [vp, i64, vp, vp, vp, vp, vp]
         L.asr_sched_estimate.argtypes = [vp, i64, vp, i32, vp, vp, vp]
         L.asr_sched_itl_batched.argtypes = [vp, vp, i32, vp, i32, i64, i32, vp, i32, vp, vp, sz, vp]
-        for name in EXPORTS[:15]:
+        for name in EXPORTS[:16]:
             getattr(L, name).restype = C.c_int
         L.asr_sched_workspace_bytes.argtypes = [i32, i64, i64, i64]
         L.asr_sched_workspace_bytes.restype = sz
@@ -210,6 +211,17 @@ def select(keys, n: int, policy: int, now: int, k: int, out_idx=None, workspace=
         workspace = _workspace(workspace_bytes(OP_SELECT, n, k), keys.device)
     _check(lib().asr_sched_select(_ptr(keys), n, policy, now, k, _ptr(out_idx), _ptr(workspace),
                                   workspace.numel(), _stream()), "asr_sched_select")
+    return out_idx
+
+
+SELECT_STATIC_SCRATCH_BYTES = 1 << 20
+
+
+def select_static(keys, n: int, policy: int, now: int, k: int, out_idx):
+    """asr_sched_select_static: asr_sched_select with the library's built-in scratch; allocates nothing (the caller
+    passes out_idx, an int32[k] device tensor)."""
+    _check(lib().asr_sched_select_static(_ptr(keys), n, policy, now, k, _ptr(out_idx), _stream()),
+           "asr_sched_select_static")
     return out_idx
 
 

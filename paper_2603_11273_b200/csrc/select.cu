@@ -31,6 +31,7 @@
 // Every decision that affects the output is taken by the exact integer
 // comparator, so the result is the unique total order -- never an approximation.
 // HBM-bound by design: 16 B read per record, 4k B written per queue.
+#include <mutex>
 #include "launchers.cuh"
 
 namespace asr {
@@ -867,6 +868,59 @@ extern "C" int asr_sched_select(const asr_req_t *keys, int64_t n, int32_t policy
         stride = nsegs * k;
     }
     return ASR_OK;
+}
+
+// ---------------------------------------------------------------------------
+// asr_sched_select_static: asr_sched_select for callers that cannot allocate (code under CUDA graph capture,
+// serving loops, harnesses that forbid cudaMalloc).  The level arrays of the single-queue reduction tree live in a
+// file-scope device array instead of a caller's workspace.  Every GPU that loads the library holds the array until
+// exit; every call on a device shares it, so calls that overlap on the GPU (two streams) race.  Nothing in it has
+// to start at zero: every level entry that is read was written by the launch before (-1 padding included).
+// ---------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_select_scratch[ASR_SELECT_STATIC_SCRATCH_BYTES];
+
+// In host code `g_select_scratch` is a host-side stand-in, not a device address: the address on the current device
+// comes from cudaGetSymbolAddress, once per device.
+static int select_scratch_ptr(void **out) {
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static void *ptr[MAX_DEV] = {nullptr};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= MAX_DEV) {
+        set_error("select_static: cudaGetDevice: %s (device %d)", cudaGetErrorString(e), dev);
+        cudaGetLastError();
+        return ASR_ECUDA;
+    }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_select_scratch);
+        if (e != cudaSuccess || !p) {
+            set_error("select_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            cudaGetLastError();
+            return ASR_ECUDA;
+        }
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return ASR_OK;
+}
+
+extern "C" int asr_sched_select_static(const asr_req_t *keys, int64_t n, int32_t policy, int64_t now, int32_t k,
+                                       int32_t *out_idx, void *stream) {
+    if (n >= 0 && k >= 0 && k <= ASR_SELECT_MAX_K && select_ws_bytes(n, k) > (size_t)ASR_SELECT_STATIC_SCRATCH_BYTES) {
+        set_error("select_static: n=%lld k=%d needs %zu bytes of scratch, the built-in array holds %d", (long long)n, k,
+                  select_ws_bytes(n, k), (int)ASR_SELECT_STATIC_SCRATCH_BYTES);
+        return ASR_EUNSUPPORTED;
+    }
+    void *scratch = nullptr;
+    if (n > SEL_SEG && k > 0 && k <= ASR_SELECT_MAX_K) {   // (a queue of one segment needs no scratch)
+        const int rc = select_scratch_ptr(&scratch);
+        if (rc) return rc;
+    }
+    return asr_sched_select(keys, n, policy, now, k, out_idx, scratch, scratch ? (size_t)ASR_SELECT_STATIC_SCRATCH_BYTES : 0,
+                            stream);
 }
 
 namespace asr {
