@@ -182,3 +182,52 @@ def test_warp_tier_window_beyond_the_chunk_ring(asr):
             check_replica(tr, p, s, wl.CONFIG_COST, L[i], T[i], S[i], "rep %d" % i)
     finally:
         asr.set_option(asr.OPT_SIM_ESCALATE_WINDOW, 4096)
+
+
+def test_cost_models_mixed_in_one_batch(asr):
+    """replica.cm_id: neighbouring lanes of a warp run different cost models (one of them outside the 32-bit budget of
+    the pieces, one invalid id) -- summary-only (time-split pieces) and per-request outputs (one thread / one warp per
+    replica), against the oracle replica by replica"""
+    import torch
+    from gpu_util import dev_trace
+    costs = [wl.CONFIG_COST, wl.MEDIUM_COST, (20000, 30000, 8000, 50, 1, 4), (5000, 1, 3000, 20, 2, 7), wl.TOY_COST]
+    traces = [wl.stress_trace("lognormal", 2600, 700, rate_per_s=1.5), wl.stress_trace("uniform", 4100, 701, rate_per_s=3.0),
+              wl.stress_trace("six", 2500, 702, rate_per_s=0.4), wl.stress_trace("lognormal", 3000, 703, rate_per_s=9.0)]
+    reps = [(t, p, s, c) for t in range(len(traces)) for p in POL for s in (8, 32) for c in range(len(costs))]
+    reps.insert(7, (1, orc.SJF, 32, len(costs)))   # cm_id out of range: n_done = -1, nothing else
+    offs = np.concatenate([[0], np.cumsum([len(t) for t in traces])]).astype(np.int64)
+    ns = np.array([len(traces[t]) for t, _, _, _ in reps], dtype=np.int64)
+    out_off = np.concatenate([[0], np.cumsum(ns)]).astype(np.int64)
+    total = int(out_off[-1])
+    rep = asr.make_replicas([offs[t] for t, _, _, _ in reps], out_off[:-1], ns, [p for _, p, _, _ in reps],
+                            [s for _, _, s, _ in reps], [c for _, _, _, c in reps])
+    d_tr, d_rep = dev_trace(np.concatenate(traces)), asr.to_device(rep)
+    d_cm = asr.to_device(np.concatenate([asr.make_cost(*c) for c in costs]))
+    cache = {}
+
+    def want(i):
+        t, p, s, c = reps[i]
+        if (t, p, s, c) not in cache:
+            cache[(t, p, s, c)] = _oracle_summary(traces[t], p, s, costs[c])
+        return cache[(t, p, s, c)]
+
+    fields = ("p50_e2e_us", "p90_e2e_us", "p50_ttft_us", "p90_ttft_us", "first_arrival_us", "last_done_us", "n_done")
+    for summary_only in (True, False):
+        d_sum = torch.zeros(len(reps) * asr.SUMMARY_DTYPE.itemsize, dtype=torch.uint8, device="cuda")
+        lat = None if summary_only else torch.full((total,), -7, dtype=torch.int64, device="cuda")
+        ttft = None if summary_only else torch.full((total,), -7, dtype=torch.int64, device="cuda")
+        asr.simulate_batched(d_tr, d_rep, len(reps), d_cm, len(costs), total, 32, lat, ttft, d_sum)
+        torch.cuda.synchronize()
+        S = d_sum.cpu().numpy().view(asr.SUMMARY_DTYPE)
+        for i in range(len(reps)):
+            if reps[i][3] >= len(costs):
+                assert int(S[i]["n_done"]) == -1
+                continue
+            got = tuple(int(S[i][f]) for f in fields)
+            assert got == want(i), "summary_only=%r replica %d %r: %r != %r" % (summary_only, i, reps[i], got, want(i))
+        if not summary_only:
+            L, T = lat.cpu().numpy(), ttft.cpu().numpy()
+            for i in (0, 13, 31, 58, len(reps) - 1):
+                t, p, s, c = reps[i]
+                rl, rt, _, _ = orc.simulate(traces[t], p, orc.cost(*costs[c]), s)
+                assert np.array_equal(L[out_off[i]:out_off[i + 1]], rl) and np.array_equal(T[out_off[i]:out_off[i + 1]], rt), i
