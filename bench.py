@@ -626,7 +626,7 @@ def run_ours(args):
     sel_avg, sel_cnt, sel_tot = per_launch("select_topk_kernel")
     gen_avg, _, gen_tot = per_launch("gen_trace_kernel")
     # the percentile reduction of a summary-only sweep = carried-window kernel + radix kernel on what it left
-    pf_avg, pf_cnt, pf_tot = per_launch("summary_fast_kernel")
+    pf_avg, pf_cnt, pf_tot = per_launch("summary_stream_kernel")
     pr_avg, pr_cnt, pr_tot = per_launch("summary_percentiles_kernel")
     pct_tot = (pf_tot or 0.0) + (pr_tot or 0.0)
     pct_avg = pct_tot / max(pf_cnt, pr_cnt) if max(pf_cnt, pr_cnt) else None
@@ -640,7 +640,7 @@ def run_ours(args):
             "bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak,
             "traffic": consts.get("select_dram_bytes_per_launch"), "peak_source": peak_src,
             "algorithmic_bytes_per_launch": sel_bytes, "avg_launch_ms": sel_avg, "frac_of_nominal_8TBs": a / 8000.0}
-    stage_ms = {"gen_trace_kernel": gen_tot, "summary_fast_kernel": pct_tot}
+    stage_ms = {"gen_trace_kernel": gen_tot, "summary_stream_kernel": pct_tot}
     for kname in ("sim_lane_kernel", "sim_warp_kernel"):
         k_avg, k_cnt, k_tot = per_launch(kname)
         if not k_avg:
@@ -679,7 +679,7 @@ def run_ours(args):
         # summary-only sweeps hand the reduction uint32 values (the lane kernel proves < 2^32 us): 4 B per value
         pct_bytes = 2 * total * 4
         a = pct_bytes / (pct_avg / 1e3) / 1e9
-        rooflines["summary_fast_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
+        rooflines["summary_stream_kernel"] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s",
                                             "frac": a / hbm_peak,
                                             "traffic": consts.get("summary_percentiles_dram_bytes_per_launch"),
                                             "algorithmic_bytes_per_launch": pct_bytes,

@@ -57,7 +57,7 @@ int sm_count() {
 // ---- per-kernel timing: one CUDA-event pair per launch, on the launch stream
 static const char *const g_kernel_names[KID_COUNT] = {
     "select_topk_kernel", "sim_prepare_kernel", "sim_warp_kernel", "sim_lane_kernel", "summary_percentiles_kernel",
-    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel", "summary_fast_kernel", "lane_plan_kernels", "sim_lane_kernel(repair)", "sim_lane_kernel(redo)", "select_wide_kernel"};
+    "percentiles_kernel", "gen_trace_kernel", "gen_queues_kernel", "build_sweep_replicas_kernel", "sim_cta_kernel", "sim_init_lat_kernel", "sim_ex_kernel", "tpot_kernel", "estimate_kernel", "itl_percentiles_kernel", "summary_stream_kernel", "lane_plan_kernels", "sim_lane_kernel(repair)", "sim_lane_kernel(redo)", "select_wide_kernel"};
 struct TimedLaunch {
     int kid;
     cudaEvent_t start, stop;
@@ -118,7 +118,8 @@ static SimWorkspace sim_ws(int64_t total_requests, int64_t n_replicas, bool summ
     w.plan_off = w.total;
     w.order_bytes = summary_only ? align_up(sizeof(int32_t) * (size_t)n_replicas) : 0;   // also: failed
     w.seg_bytes = summary_only ? align_up((size_t)n_replicas) : 0;                        // load class; segments
-    w.unit_q_bytes = summary_only ? align_up(sizeof(int32_t) * (size_t)n_replicas * LANE_MAX_SEG + 64) : 0;   // + counters
+    // + counters; after the simulation the region is the percentile kernels' scratch (seed list: 2 n + 64 + runs)
+    w.unit_q_bytes = summary_only ? align_up(sizeof(int32_t) * (size_t)n_replicas * LANE_MAX_SEG + 64 + 512) : 0;
     w.total += 2 * w.order_bytes + 2 * w.seg_bytes + w.unit_q_bytes;
     return w;
 }
@@ -294,9 +295,12 @@ extern "C" int asr_sched_simulate_batched(const asr_req_t *traces, const asr_rep
     }
     rc = launch_simulate(a, max_slots, use_lane, st);
     if (rc) return rc;
-    if (out_summary)
+    if (out_summary) {
+        // the hand-over lists are spent: miss lists; so is the plan's unit_q region: seed lists
+        int32_t *scratch = summary_only ? (int32_t *)(ws + w.plan_off + 2 * w.order_bytes + 2 * w.seg_bytes) : nullptr;
         rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, use_lane && summary_only,
-                                        a.plan.order, defer + 64, defer + 2, st);   // the hand-over lists are spent: miss lists
+                                        a.plan.order, defer + 64, defer + 2, scratch, st);
+    }
     return rc;
 }
 
@@ -356,7 +360,7 @@ extern "C" int asr_sched_simulate_batched_ex(const asr_req_t *traces, const asr_
     a.itl_npairs = nullptr;
     rc = launch_simulate_ex(a, max_slots, st);
     if (rc) return rc;
-    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, false, nullptr, nullptr, nullptr, st);
+    if (out_summary) rc = launch_summary_percentiles(replicas, n_replicas, out_lat, out_ttft, out_summary, false, nullptr, nullptr, nullptr, nullptr, st);
     return rc;
 }
 

@@ -82,7 +82,7 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
 constexpr int64_t ASR_FMT32 = INT64_MIN + 32;
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
                                const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, const int32_t *order,
-                               int32_t *miss_list, int32_t *miss_count, cudaStream_t st);
+                               int32_t *miss_list, int32_t *miss_count, int32_t *scratch, cudaStream_t st);
 int launch_gen_trace(const asr_trace_spec_t *specs, asr_trace_spec_t one, int32_t n_traces, int64_t n_per_trace,
                      const asr_tables_t *tables, asr_req_t *out, cudaStream_t st);
 int launch_gen_queues(uint64_t seed, int64_t first, int64_t n, int64_t now, const asr_tables_t *tables,

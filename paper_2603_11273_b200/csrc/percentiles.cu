@@ -472,475 +472,416 @@ __device__ __forceinline__ bool segment_percentiles_reg(const int64_t *__restric
 }
 
 
-// ---------------------------------------------------------------------------
-// carried-window kernel (order-free uint32 segments of a sweep: p50/p90)
-//
-// A CTA walks a run of consecutive segments.  Consecutive segments of a sweep
-// are alike (the same trace under another policy, the neighbouring seed or
-// rate), so the two ranks of segment i are looked for in windows of values
-// around the answers of segment i-1: ONE pass over the register-resident keys
-// counts, per rank, the keys below the window's end and appends the keys
-// inside the window to per-thread private slots (no atomics, no tables to
-// clear); the window is then resolved exactly by a two-level 10-bit histogram
-// over the few hundred collected keys.  Every count is exact and the window is
-// only a guess: a rank that falls outside moves the window that way and
-// doubles it, a thread that runs out of slots halves it, and the pass is
-// repeated on the keys still in registers.  A CTA's first segment finds its
-// windows by bisection on the key bits (count-only passes).  A segment in
-// another format, or one that is not settled after PF_TRIES passes, goes to
-// the miss list, which summary_percentiles_kernel (radix path) works off.
-// No result depends on a guess.
-// ---------------------------------------------------------------------------
-#ifndef PF_SLOTS_N
-#define PF_SLOTS_N 16
-#endif
-#ifndef PF_MIN_CTAS
-#define PF_MIN_CTAS 4
-#endif
 #ifdef PCT_STATS
-__device__ unsigned long long g_pct_stats[8];   // segments, settled, passes, bootstraps, misses, in-window keys, -, -
+__device__ unsigned long long g_pct_stats[8];   // -, settled, passes, above, dense, in-window keys, below, -
 #endif
-constexpr int PF_SLOTS = PF_SLOTS_N;   // private slots per thread and rank
-constexpr int PF_GROUP = 8;            // slots are checked once per group of keys
-constexpr int PF_BINS = 1024;          // bins per histogram level
-constexpr int PF_MAX_SHIFT = 10;       // window = PF_BINS << shift values; the second level resolves 2^shift
-constexpr int PF_HALF = PCT_THREADS / 2;
-constexpr int PF_TRIES = 6;
-#ifndef PF_IN_MANY_N
-#define PF_IN_MANY_N 256   // one key per thread: a thread with more than PF_SLOTS - PF_GROUP closes its window
+// ---------------------------------------------------------------------------
+// summary_stream_kernel: p50/p90 of the uint32 segments of a summary-only sweep, one WARP per segment.
+//
+// Consecutive segments of a sweep are alike (the same trace under another policy, the neighbouring seed), so the
+// two ranks of a segment are looked for in windows of values around the answers of the segment before (round 2
+// first did this with one CTA per segment: 8 barriers and two block scans per segment made the fixed work 60 % of
+// its instructions).  Here a warp walks a run of consecutive work
+// items (segment = one value stream of one replica, in the plan's order) and streams each segment ONCE through its
+// registers, 4 KB at a time with the next 4 KB's loads in flight (a cp.async.bulk ring in shared memory as in
+// select_topk_kernel was measured too: 13 warps per SM fit beside it and run in 2.1 ms, 19 warps without it in
+// 1.96 ms -- the kernel is bound by the latency of its own instruction chains, so warps count for more).
+// Per key and rank: count below the window's end, append to the lane's private slots if inside the window (ten
+// PTX instructions per key for both ranks).  The window is then resolved by a 32-bin radix descent over the ~100 collected keys
+// and a one-warp ranking of the last bin's keys: warp shuffles only, no block barrier anywhere.  A rank outside
+// the window moves and doubles it, a lane that runs out of slots halves it, and the segment is read again
+// (straight from L2); what is not settled after PS_TRIES passes, or has another format, goes to the miss list for
+// summary_percentiles_kernel.  The first streamable segment of every run (the "seed") is computed by that kernel
+// beforehand: its two answers and their distance give the run its first windows.  No result depends on a guess.
+// ---------------------------------------------------------------------------
+#ifndef PS_WARPS_N
+#define PS_WARPS_N 19
 #endif
-constexpr uint32_t PF_IN_MANY = PF_IN_MANY_N, PF_IN_FEW = PF_IN_MANY / 4;   // keys wanted inside a window
-static_assert(PCT_VPT % PF_GROUP == 0 && PF_SLOTS >= 2 * PF_GROUP, "slot check granularity");
+constexpr int PS_WARPS = PS_WARPS_N;
+#ifndef PS_CHUNK_N
+#define PS_CHUNK_N 1024
+#endif
+constexpr int PS_CHUNK = PS_CHUNK_N;   // keys a warp takes at a time (4 KB: one 128-bit load per lane and 512 bytes)
+constexpr int PS_WIN = 32;       // a window is PS_WIN << shift values wide: 32 bins of 2^shift values
+#ifndef PS_SLOTS_N
+#define PS_SLOTS_N 32
+#endif
+constexpr int PS_SLOTS = PS_SLOTS_N;   // private slots per lane and rank
+constexpr int PS_GROUP = 8;      // slots are checked once per group of keys
+constexpr int PS_TRIES = 6;
+constexpr int PS_MAX_SHIFT = 26;
+#ifndef PS_IN_MANY_N
+#define PS_IN_MANY_N 256
+#endif
+constexpr uint32_t PS_IN_MANY = PS_IN_MANY_N, PS_IN_FEW = PS_IN_MANY / 4;   // keys wanted inside a window
+#ifndef PS_RUN_N
+#define PS_RUN_N 24
+#endif
+#ifndef PS_SEED_EVERY_N
+#define PS_SEED_EVERY_N 8
+#endif
+constexpr int PS_SEED_EVERY = PS_SEED_EVERY_N;   // runs that share a seed
+constexpr int PS_RUN = PS_RUN_N;   // consecutive work items per run (each run costs one seed: a radix-kernel segment)
+static_assert(PS_SLOTS >= 2 * PS_GROUP && (PS_CHUNK / 32) % PS_GROUP == 0, "slot check granularity");
 
-struct PctFastSmem {
-    uint32_t slot[2][PF_SLOTS][PCT_THREADS];
-    uint32_t hist[2][2][PF_BINS];            // [level][rank][bin]
-    uint32_t wtot[2][2][PCT_THREADS / 32];   // [parity][rank][warp]: keys below the window's end | keys inside << 16
-    uint32_t wovf[2][PCT_THREADS / 32];      // [parity][warp]: bit t = a thread closed its window of rank t
-    uint32_t wsum[2][PCT_THREADS / 64];
-    uint32_t sel_bin[2][2], sel_rem[2][2];   // [level][rank]
-    uint32_t sel_cnt[2];                     // [rank]: keys in the selected level-1 bin
-    uint32_t lcnt[2], list[2][32];           // [rank]: those keys (their offsets inside the bin) when there are at most 32
+struct __align__(128) PsWarpSmem {
+    uint32_t slot[2][PS_SLOTS][32];   // [rank][slot][lane]
+    uint32_t hist[32];
+    uint32_t list[32];
+    uint32_t lcnt;
+};
+constexpr size_t PS_SMEM_BYTES = sizeof(PsWarpSmem) * PS_WARPS;
+
+// a work item w in [0, 2 * n_replicas): value stream w / n_replicas (0: E2E latency, 1: TTFT) of the replica at
+// position w % n_replicas of the order.  state 0 = nothing to do (invalid replica, or the run's seed: done),
+// 1 = uint32 values in the order-free simulator's format: streamed here, 2 = anything else: miss list
+struct PsDesc {
+    const uint32_t *base;
+    int32_t N, r, y, state;
 };
 
-__device__ __forceinline__ uint32_t pf_end(uint32_t lo, int sh) {   // saturated: a key 2^32-1 is never inside
-    const uint32_t hi = lo + ((uint32_t)PF_BINS << sh);
-    return hi < lo ? 0xFFFFFFFFu : hi;
+struct PsArgs {
+    const asr_replica_t *replicas;
+    const int64_t *lat, *ttft;
+    asr_summary_t *out_summary;
+    const int32_t *order;
+    int32_t *miss_list, *miss_count;   // [2][n_replicas], [2]
+    int32_t *seed_list, *seed_count;   // [2][n_replicas], [2]
+    int32_t *seed_item;                // [groups of PS_SEED_EVERY runs]: the group's seed item, or -1
+    int32_t *cursor;                   // the next run to hand out
+    int32_t n_replicas, run, n_runs;   // run = consecutive work items a warp takes at a time
+    uint32_t one;                      // 1 (see ps_chunk)
+};
+
+__device__ __forceinline__ PsDesc ps_describe(const PsArgs &a, int w, int seed) {
+    PsDesc d;
+    d.y = w >= a.n_replicas ? 1 : 0;
+    const int idx = w - d.y * a.n_replicas;
+    d.r = a.order ? a.order[idx] : idx;
+    const asr_replica_t rp = a.replicas[d.r];
+    const asr_summary_t *s = a.out_summary + d.r;
+    const int64_t flag = d.y == 0 ? s->p50_e2e_us : s->p50_ttft_us;
+    // (only a descriptor the simulator accepted, n_done >= 0, is ever dereferenced)
+    const int64_t *vals = (d.y == 0 ? a.lat : a.ttft) + rp.out_off;
+    d.base = reinterpret_cast<const uint32_t *>(vals);
+    d.N = rp.n;
+    if (w == seed || s->n_done < 0) d.state = 0;
+    else if (flag == ASR_FMT32 && rp.n > 0 && (rp.n & 3) == 0 && (reinterpret_cast<uintptr_t>(vals) & 15u) == 0) d.state = 1;
+    else d.state = 2;
+    return d;
 }
 
-// inclusive scan of the PF_BINS bins of histogram h by the PF_HALF threads of one rank: thread j owns
-// bins 8j .. 8j+7.  Part A leaves the per-warp totals in wsum; after a barrier part B locates rank k.
-__device__ __forceinline__ void pf_scan_a(const uint32_t *h, int j, uint32_t (&c)[8], uint32_t &tot, uint32_t &incl,
-                                          uint32_t *wsum) {
-    static_assert(PF_BINS == PF_HALF * 8, "eight bins per thread");
-    const uint4 a = *reinterpret_cast<const uint4 *>(h + 8 * j), b = *reinterpret_cast<const uint4 *>(h + 8 * j + 4);
-    c[0] = a.x, c[1] = a.y, c[2] = a.z, c[3] = a.w, c[4] = b.x, c[5] = b.y, c[6] = b.z, c[7] = b.w;
-    tot = ((c[0] + c[1]) + (c[2] + c[3])) + ((c[4] + c[5]) + (c[6] + c[7]));
-    incl = tot;
-    const int lane = lane_id();
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
-        if (lane >= d) incl += y;
-    }
-    if (lane == 31) wsum[j >> 5] = incl;
-}
-
-__device__ __forceinline__ void pf_scan_b(const uint32_t (&c)[8], uint32_t tot, uint32_t incl, const uint32_t *wsum, int j,
-                                          uint32_t k, uint32_t *sel_bin, uint32_t *sel_rem, uint32_t *sel_cnt = nullptr) {
-    uint32_t excl = incl - tot;
-#pragma unroll
-    for (int w = 0; w < PF_HALF / 32; ++w)
-        if (w < (j >> 5)) excl += wsum[w];
-    if (excl < k && k <= excl + tot) {
-        uint32_t run = excl;
-#pragma unroll
-        for (int b = 0; b < 8; ++b) {
-            if (run < k && k <= run + c[b]) {
-                *sel_bin = (uint32_t)(8 * j + b);
-                *sel_rem = k - run;
-                if (sel_cnt) *sel_cnt = c[b];
+// one thread per group of PS_SEED_EVERY consecutive runs: the group's first streamable item becomes its seed
+// (computed by summary_percentiles_kernel before summary_stream_kernel starts).  A seed costs as much as four
+// second readings, and all a run needs from it is a first guess, so neighbouring runs share one.
+__global__ void __launch_bounds__(1024) summary_seed_kernel(PsArgs a) {
+    if (threadIdx.x < 2) a.seed_count[threadIdx.x] = 0;
+    if (threadIdx.x == 2) *a.cursor = 0;
+    __syncthreads();
+    const int total = 2 * a.n_replicas;
+    const int n_groups = (a.n_runs + PS_SEED_EVERY - 1) / PS_SEED_EVERY;
+    for (int g = threadIdx.x; g < n_groups; g += 1024) {
+        const int w0 = g * PS_SEED_EVERY * a.run, w1 = (int)min((int64_t)total, (int64_t)w0 + (int64_t)PS_SEED_EVERY * a.run);
+        int seed = -1;
+        for (int w = w0; w < w1 && seed < 0; ++w) {
+            const PsDesc d = ps_describe(a, w, -1);
+            if (d.state == 1) {
+                seed = w;
+                a.seed_list[(size_t)d.y * a.n_replicas + atomicAdd(a.seed_count + d.y, 1)] = d.r;
             }
-            run += c[b];
         }
+        a.seed_item[g] = seed;
     }
 }
 
-// hist[bin] += 1 if p (a predicated shared-memory reduction: no branch, nothing touched when !p)
-__device__ __forceinline__ void pf_inc_if(uint32_t *hist, uint32_t bin, bool p) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred q;\n\t"
-        "setp.ne.u32 q, %1, 0;\n\t"
-        "@q red.shared.add.u32 [%0], 1;\n\t"
-        "}" ::"r"((uint32_t)__cvta_generic_to_shared(hist) + 4u * bin),
-        "r"((uint32_t)p)
-        : "memory");
-}
-#ifndef PF_STRAIGHT_N
-#define PF_STRAIGHT_N 3
-#endif
-constexpr int PF_STRAIGHT = PF_STRAIGHT_N;   // entries per thread and rank handled without a loop (most threads hold 0-2)
+// the lane's state through one pass over a segment
+struct PsPass {
+    uint32_t c0, c1;             // keys below the end of window 0 / 1
+    uint32_t p0, p1;             // next free slot (shared-memory byte address) of rank 0 / 1
+    uint32_t lo0, hi0, lo1, hi1;
+    uint32_t over;               // bit t: this lane closed window t for lack of slots
+};
 
-// One pass over the keys.  Per key and rank: one compare-and-count below the window's end, one compare for
-// "inside", a predicated store and a predicated pointer bump (written out in PTX: the compiler's version of the
-// same loop took nine instructions per key and rank).  Returns, for rank t, T[t] = keys below the end | keys
-// inside << 16 over the whole CTA, and ov = bit t set if some thread closed its window t for lack of slots
-// (then "inside" of rank t is short; "below the end" is always exact).  n[t] = this thread's keys inside.
-__device__ __forceinline__ void pf_pass(const uint32_t (&key)[PCT_VPT], uint32_t lo0, uint32_t hi0, uint32_t lo1,
-                                        uint32_t hi1, PctFastSmem &fs, int par, uint32_t (&T)[2], uint32_t &ov,
-                                        int (&n)[2]) {
-    const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
-    uint32_t c0 = 0, c1 = 0;
-    const uint32_t b0 = (uint32_t)__cvta_generic_to_shared(&fs.slot[0][0][tid]);
-    const uint32_t b1 = (uint32_t)__cvta_generic_to_shared(&fs.slot[1][0][tid]);
-    uint32_t p0 = b0, p1 = b1;
-    constexpr uint32_t ROW = PCT_THREADS * 4;   // bytes between two slots of a thread
-    const uint32_t stop0 = b0 + (PF_SLOTS - PF_GROUP) * ROW, stop1 = b1 + (PF_SLOTS - PF_GROUP) * ROW;
-    uint32_t over = 0;
+// 32 keys of a lane (one chunk): ten instructions per key, slots checked after every PS_GROUP keys.
+// The four predicated increments are written as multiply-adds by `one` (a kernel argument equal to 1, so that
+// ptxas cannot fold them back into additions): IMAD issues to the fma pipe, and the key then costs four
+// instructions on the alu pipe (the compares) and four on the fma pipe, which run side by side at one warp
+// instruction per two cycles each -- as plain additions all eight queue for the alu pipe.
+__device__ __forceinline__ void ps_chunk(const uint32_t (&key)[PS_CHUNK / 32], PsPass &s, uint32_t stop0, uint32_t stop1,
+                                         uint32_t one) {
+    constexpr uint32_t ROW = 32 * 4;   // bytes between two slots of a lane
 #pragma unroll
-    for (int g = 0; g < PCT_VPT / PF_GROUP; ++g) {
+    for (int g = 0; g < PS_CHUNK / 32 / PS_GROUP; ++g) {
 #pragma unroll
-        for (int j = 0; j < PF_GROUP; ++j) {
+        for (int j = 0; j < PS_GROUP; ++j) {
             asm volatile(
                 "{\n\t"
                 ".reg .pred a, b;\n\t"
                 "setp.lt.u32 a, %4, %5;\n\t"
-                "@a add.u32 %0, %0, 1;\n\t"
+                "@a mad.lo.u32 %0, %10, %10, %0;\n\t"
                 "setp.ge.and.u32 b, %4, %6, a;\n\t"
                 "@b st.shared.u32 [%1], %4;\n\t"
-                "@b add.u32 %1, %1, %9;\n\t"
+                "@b mad.lo.u32 %1, %10, %9, %1;\n\t"
                 "setp.lt.u32 a, %4, %7;\n\t"
-                "@a add.u32 %2, %2, 1;\n\t"
+                "@a mad.lo.u32 %2, %10, %10, %2;\n\t"
                 "setp.ge.and.u32 b, %4, %8, a;\n\t"
                 "@b st.shared.u32 [%3], %4;\n\t"
-                "@b add.u32 %3, %3, %9;\n\t"
+                "@b mad.lo.u32 %3, %10, %9, %3;\n\t"
                 "}"
-                : "+r"(c0), "+r"(p0), "+r"(c1), "+r"(p1)
-                : "r"(key[g * PF_GROUP + j]), "r"(hi0), "r"(lo0), "r"(hi1), "r"(lo1), "n"(ROW)
+                : "+r"(s.c0), "+r"(s.p0), "+r"(s.c1), "+r"(s.p1)
+                : "r"(key[g * PS_GROUP + j]), "r"(s.hi0), "r"(s.lo0), "r"(s.hi1), "r"(s.lo1), "n"(ROW), "r"(one)
                 : "memory");
         }
-        // a thread that could run out of slots in the next group closes its window (after the first group it holds
-        // at most PF_GROUP keys, after the last one nothing follows)
-        if (g > 0 && g < PCT_VPT / PF_GROUP - 1) {
-            if (p0 > stop0) {
-                lo0 = hi0;
-                over |= 1u;
+        // a lane that could run out of slots in the next group closes its window (rare: one test for both ranks)
+        if (s.p0 > stop0 || s.p1 > stop1) {
+            if (s.p0 > stop0) {
+                s.lo0 = s.hi0;
+                s.over |= 1u;
             }
-            if (p1 > stop1) {
-                lo1 = hi1;
-                over |= 2u;
+            if (s.p1 > stop1) {
+                s.lo1 = s.hi1;
+                s.over |= 2u;
             }
         }
     }
-    n[0] = (int)((p0 - b0) / ROW);
-    n[1] = (int)((p1 - b1) / ROW);
-    const uint32_t t0 = __reduce_add_sync(ASR_FULL_MASK, c0 | ((uint32_t)n[0] << 16));
-    const uint32_t t1 = __reduce_add_sync(ASR_FULL_MASK, c1 | ((uint32_t)n[1] << 16));
-    const uint32_t wo = __reduce_or_sync(ASR_FULL_MASK, over);
-    if (lane == 0) {
-        fs.wtot[par][0][warp] = t0;
-        fs.wtot[par][1][warp] = t1;
-        fs.wovf[par][warp] = wo;
-    }
-    __syncthreads();
-    T[0] = T[1] = ov = 0;
-#pragma unroll
-    for (int w = 0; w < PCT_THREADS / 32; ++w) {
-        T[0] += fs.wtot[par][0][w];
-        T[1] += fs.wtot[par][1][w];
-        ov |= fs.wovf[par][w];
-    }
 }
 
-// count-only pass: keys below t0 / below t1 over the whole CTA
-__device__ __forceinline__ void pf_count(const uint32_t (&key)[PCT_VPT], uint32_t t0, uint32_t t1, PctFastSmem &fs, int par,
-                                         uint32_t (&C)[2]) {
+__device__ __forceinline__ uint32_t ps_end(uint32_t lo, int sh) {   // saturated: a key 2^32-1 is never inside
+    const uint32_t hi = lo + ((uint32_t)PS_WIN << sh);
+    return hi < lo ? 0xFFFFFFFFu : hi;
+}
+
+// the j-th smallest (j >= 1) of the keys a pass collected for rank t: lane holds n_lane of them in its slots, all
+// inside [lo, lo + (PS_WIN << sh)).  Radix descent, 32 bins (one per lane) per level, until the bin of the rank
+// holds at most 32 keys (ranked by one key per lane) or one value.
+__device__ __forceinline__ uint32_t ps_resolve(PsWarpSmem &sm, int t, int n_lane, uint32_t lo, int sh, uint32_t j) {
+    const int lane = lane_id();
+    const int n_max = (int)__reduce_max_sync(ASR_FULL_MASK, (uint32_t)n_lane);
+    int shift = sh;   // the window is 32 bins of 2^sh values
+    uint32_t cnt_b;
+    for (;;) {
+        sm.hist[lane] = 0;
+        if (lane == 0) sm.lcnt = 0;
+        __syncwarp();
+        for (int e = 0; e < n_max; ++e)
+            if (e < n_lane) {
+                const uint32_t d = (sm.slot[t][e][lane] - lo) >> shift;   // (a key below lo wraps far beyond 32 bins)
+                if (d < 32u) atomicAdd(&sm.hist[d], 1u);
+            }
+        __syncwarp();
+        const uint32_t cnt = sm.hist[lane];
+        uint32_t incl = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t y = __shfl_up_sync(ASR_FULL_MASK, incl, d);
+            if (lane >= d) incl += y;
+        }
+        const int b = __ffs((int)__ballot_sync(ASR_FULL_MASK, incl >= j)) - 1;   // (the rank is inside: b >= 0)
+        j -= __shfl_sync(ASR_FULL_MASK, incl - cnt, b);
+        cnt_b = __shfl_sync(ASR_FULL_MASK, cnt, b);
+        lo += (uint32_t)b << shift;
+        if (shift == 0) return lo;   // one value per bin
+        if (cnt_b <= 32u) break;
+        shift = shift > 5 ? shift - 5 : 0;
+    }
+    // the keys of [lo, lo + 2^shift), one per lane, ranked by comparison (any order of equal keys gives the same
+    // value at every rank)
+    for (int e = 0; e < n_max; ++e)
+        if (e < n_lane) {
+            const uint32_t d = sm.slot[t][e][lane] - lo;
+            if ((d >> shift) == 0u) sm.list[atomicAdd(&sm.lcnt, 1u)] = d;
+        }
+    __syncwarp();
+    const uint32_t v = (uint32_t)lane < cnt_b ? sm.list[lane] : 0xFFFFFFFFu;
+    uint32_t rank = 0;
+    for (uint32_t q = 0; q < cnt_b; ++q) {
+        const uint32_t u = __shfl_sync(ASR_FULL_MASK, v, (int)q);
+        rank += (u < v || (u == v && q < (uint32_t)lane)) ? 1u : 0u;
+    }
+    const uint32_t hit = __ballot_sync(ASR_FULL_MASK, (uint32_t)lane < cnt_b && rank + 1u == j);
+    const uint32_t res = lo + __shfl_sync(ASR_FULL_MASK, v, __ffs((int)hit) - 1);
+    __syncwarp();   // list and hist are rewritten by the next call
+    return res;
+}
+
+__global__ void __launch_bounds__(PS_WARPS * 32, 1) summary_stream_kernel(PsArgs a) {
+    extern __shared__ __align__(128) unsigned char ps_dyn_smem[];
+    PsWarpSmem *smem = reinterpret_cast<PsWarpSmem *>(ps_dyn_smem);
     const int lane = lane_id(), warp = threadIdx.x >> 5;
-    uint32_t c0 = 0, c1 = 0;
-#pragma unroll
-    for (int j = 0; j < PCT_VPT; ++j) {
-        c0 += key[j] < t0 ? 1u : 0u;
-        c1 += key[j] < t1 ? 1u : 0u;
-    }
-    c0 = __reduce_add_sync(ASR_FULL_MASK, c0);
-    c1 = __reduce_add_sync(ASR_FULL_MASK, c1);
-    if (lane == 0) {
-        fs.wtot[par][0][warp] = c0;
-        fs.wtot[par][1][warp] = c1;
-    }
-    __syncthreads();
-    C[0] = C[1] = 0;
-#pragma unroll
-    for (int w = 0; w < PCT_THREADS / 32; ++w) {
-        C[0] += fs.wtot[par][0][w];
-        C[1] += fs.wtot[par][1][w];
-    }
-}
+    PsWarpSmem &sm = smem[warp];
+    // persistent warps take runs from a cursor: a run that needs many second readings does not hold up the rest
+#pragma unroll 1
+  for (;;) {
+    int g = 0;
+    if (lane == 0) g = atomicAdd(a.cursor, 1);
+    g = __shfl_sync(ASR_FULL_MASK, g, 0);
+    if (g >= a.n_runs) break;
+    const int total = 2 * a.n_replicas;
+    const int w0 = g * a.run, w1 = min(total, w0 + a.run);
+    const int seed = a.seed_item[g / PS_SEED_EVERY];
 
-__global__ void __launch_bounds__(PCT_THREADS, PF_MIN_CTAS) summary_fast_kernel(const asr_replica_t *replicas, int32_t n_replicas,
-                                                                                const int64_t *lat, const int64_t *ttft,
-                                                                                asr_summary_t *out_summary,
-                                                                                const int32_t *order, int32_t chunk,
-                                                                                int32_t *miss_list, int32_t *miss_count) {
-    extern __shared__ __align__(16) unsigned char dyn_smem[];
-    PctFastSmem &fs = *reinterpret_cast<PctFastSmem *>(dyn_smem);
-    const int tid = threadIdx.x;
-    const int64_t *vals = blockIdx.y == 0 ? lat : ttft;
-    int32_t *my_miss = miss_list + (size_t)blockIdx.y * n_replicas;
-    bool have = false;
+    // the run's first windows: around the seed's answers, wide enough for ~100 of the keys between them
     uint32_t wlo[2] = {0, 0};
     int wsh[2] = {0, 0};
-    int par = 0;
-    const int i0 = blockIdx.x * chunk, i1 = min(n_replicas, i0 + chunk);
-    for (int i = i0; i < i1; ++i) {
-        const int r = order ? order[i] : i;
-        if (tid == 0 && i + 1 < i1) {
-            // pull the CTA's next segment into L2 while this one is being processed
-            const int rn = order ? order[i + 1] : i + 1;
-            const asr_replica_t nx = replicas[rn];
-            const int64_t flag = blockIdx.y == 0 ? out_summary[rn].p50_e2e_us : out_summary[rn].p50_ttft_us;
-            // only a descriptor the simulator accepted (n_done >= 0) is dereferenced
-            if (out_summary[rn].n_done >= 0 && flag == ASR_FMT32 && nx.n > 0 && nx.n <= PCT_REG_MAX) {
-                const char *src = reinterpret_cast<const char *>(vals + nx.out_off);
-                const uint32_t sz = (uint32_t)(((int64_t)nx.n * 4) & ~15ll);
-                if (sz > 0 && (reinterpret_cast<uintptr_t>(src) & 15u) == 0)
-                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(sz) : "memory");
-            }
-        }
-        if (out_summary[r].n_done < 0) continue;   // invalid descriptor, flagged by the simulator
-        const int64_t flag = blockIdx.y == 0 ? out_summary[r].p50_e2e_us : out_summary[r].p50_ttft_us;
-        const asr_replica_t rep = replicas[r];
-        const int64_t *seg = vals + rep.out_off;
-        const int N = rep.n;
-        bool settled = flag == ASR_FMT32 && N > 0 && N <= PCT_REG_MAX && (N & 3) == 0 &&
-                       (reinterpret_cast<uintptr_t>(seg) & 15u) == 0;
+    bool have = false;
+    if (seed >= 0) {
+        const PsDesc d = ps_describe(a, seed, -1);
+        const asr_summary_t *s = a.out_summary + d.r;
+        const uint32_t r0 = (uint32_t)(d.y == 0 ? s->p50_e2e_us : s->p50_ttft_us);
+        const uint32_t r1 = (uint32_t)(d.y == 0 ? s->p90_e2e_us : s->p90_ttft_us);
+        const uint64_t width = ((uint64_t)(r1 - r0) * 256u) / (uint64_t)d.N;   // 0.4 N keys in r1 - r0: ~100 of them
+        int sh = 0;
+        while (sh < PS_MAX_SHIFT && ((uint64_t)PS_WIN << sh) < width) ++sh;
+        const uint32_t half = (uint32_t)PS_WIN << sh >> 1;
+        wlo[0] = r0 > half ? r0 - half : 0u;
+        wlo[1] = r1 > half ? r1 - half : 0u;
+        wsh[0] = wsh[1] = sh;
+        have = true;
+    }
+
+    constexpr uint32_t ROW = 32 * 4;
+    const uint32_t b0 = smem_u32(&sm.slot[0][0][lane]), b1 = smem_u32(&sm.slot[1][0][lane]);
+    const uint32_t stop0 = b0 + (PS_SLOTS - PS_GROUP) * ROW, stop1 = b1 + (PS_SLOTS - PS_GROUP) * ROW;
+#pragma unroll 1
+    for (int w = w0; w < w1; ++w) {
+        const PsDesc d = ps_describe(a, w, seed);
+        if (d.state == 0) continue;
+        bool settled = d.state == 1 && have;
         uint32_t res[2] = {0, 0};
         if (settled) {
-            const uint32_t k[2] = {(50u * (uint32_t)N + 99u) / 100u, (90u * (uint32_t)N + 99u) / 100u};
-            // keys: four consecutive values per 128-bit load; slots past the end read as 2^32-1 (below no window end)
-            uint32_t key[PCT_VPT];
-            {
-                const uint4 *v128 = reinterpret_cast<const uint4 *>(seg) + tid;
-                const int n4 = N >> 2;
-                const int full_rows = n4 / PCT_THREADS;   // rows of PCT_THREADS quads that every thread loads
-#pragma unroll
-                for (int q = 0; q < PCT_VPT / 4; ++q) {
-                    uint4 x;
-                    if (q < full_rows) {
-                        x = __ldcs(v128 + q * PCT_THREADS);
-                    } else {
-                        x = make_uint4(~0u, ~0u, ~0u, ~0u);
-                        if (q * PCT_THREADS + tid < n4) x = __ldcs(v128 + q * PCT_THREADS);
-                    }
-                    key[4 * q] = x.x, key[4 * q + 1] = x.y, key[4 * q + 2] = x.z, key[4 * q + 3] = x.w;
-                }
-            }
-            // clear the first histogram level and the lists (their last readers passed the final barrier of the
-            // previous segment)
-            {
-                uint4 *z = reinterpret_cast<uint4 *>(&fs.hist[0][0][0]);
-                constexpr int n16 = 2 * PF_BINS / 4;
-                static_assert(n16 % PCT_THREADS == 0, "whole passes");
-#pragma unroll
-                for (int q = 0; q < n16 / PCT_THREADS; ++q) z[q * PCT_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
-                if (tid < 2) fs.lcnt[tid] = 0;
-            }
-            if (!have) {
-                // bisection on the key bits, both ranks at once: bracket [a, a + 2^rem) holds `in` keys, `below` lie under it
-                uint32_t a[2] = {0, 0}, below[2] = {0, 0}, in[2] = {(uint32_t)N, (uint32_t)N};
-                int rem[2] = {32, 32};
-                while (true) {
-                    const bool go0 = rem[0] > PF_MAX_SHIFT + 10 || (in[0] > PF_IN_MANY && rem[0] > 0);
-                    const bool go1 = rem[1] > PF_MAX_SHIFT + 10 || (in[1] > PF_IN_MANY && rem[1] > 0);
-                    if (!go0 && !go1) break;
-                    const uint32_t m0 = go0 ? a[0] + (1u << (rem[0] - 1)) : a[0], m1 = go1 ? a[1] + (1u << (rem[1] - 1)) : a[1];
-                    uint32_t C[2];
-                    pf_count(key, m0, m1, fs, par, C);
-                    par ^= 1;
-                    if (go0) {
-                        --rem[0];
-                        if (k[0] <= C[0]) in[0] = C[0] - below[0];
-                        else in[0] -= C[0] - below[0], below[0] = C[0], a[0] = m0;
-                    }
-                    if (go1) {
-                        --rem[1];
-                        if (k[1] <= C[1]) in[1] = C[1] - below[1];
-                        else in[1] -= C[1] - below[1], below[1] = C[1], a[1] = m1;
-                    }
-                }
-#pragma unroll
-                for (int t = 0; t < 2; ++t) {
-                    wlo[t] = a[t];
-                    wsh[t] = rem[t] > 10 ? rem[t] - 10 : 0;
-                }
-                have = true;
-#ifdef PCT_STATS
-                if (tid == 0) atomicAdd(&g_pct_stats[3], 1ull);
-#endif
-            }
-            uint32_t T[2], ov;
-            int n[2];
+            const uint32_t N = (uint32_t)d.N;
+            const uint32_t k[2] = {(uint32_t)((50ull * N + 99ull) / 100ull), (uint32_t)((90ull * N + 99ull) / 100ull)};
+            const int n4 = d.N >> 2, nch = (d.N + PS_CHUNK - 1) / PS_CHUNK;
             for (int attempt = 0;; ++attempt) {
-                pf_pass(key, wlo[0], pf_end(wlo[0], wsh[0]), wlo[1], pf_end(wlo[1], wsh[1]), fs, par, T, ov, n);
-                par ^= 1;
+                PsPass s;
+                s.c0 = s.c1 = 0;
+                s.p0 = b0, s.p1 = b1;
+                s.lo0 = wlo[0], s.hi0 = ps_end(wlo[0], wsh[0]);
+                s.lo1 = wlo[1], s.hi1 = ps_end(wlo[1], wsh[1]);
+                s.over = 0;
+                // four consecutive keys per 128-bit load, the next chunk's loads in flight under this chunk's pass;
+                // quads past the end read as 2^32-1 (below no window end)
+                {
+                    const uint4 *v = reinterpret_cast<const uint4 *>(d.base) + lane;
+                    uint4 nx[PS_CHUNK / 128];
+#pragma unroll
+                    for (int q = 0; q < PS_CHUNK / 128; ++q) {
+                        nx[q] = make_uint4(~0u, ~0u, ~0u, ~0u);
+                        if (lane + q * 32 < n4) nx[q] = __ldcs(v + q * 32);
+                    }
+#pragma unroll 1
+                    for (int c = 0; c < nch; ++c) {
+                        uint32_t key[PS_CHUNK / 32];
+#pragma unroll
+                        for (int q = 0; q < PS_CHUNK / 128; ++q)
+                            key[4 * q] = nx[q].x, key[4 * q + 1] = nx[q].y, key[4 * q + 2] = nx[q].z, key[4 * q + 3] = nx[q].w;
+                        const int q1 = (c + 1) * (PS_CHUNK / 4) + lane;
+#pragma unroll
+                        for (int q = 0; q < PS_CHUNK / 128; ++q) {
+                            nx[q] = make_uint4(~0u, ~0u, ~0u, ~0u);
+                            if (q1 + q * 32 < n4) nx[q] = __ldcs(v + q1 - lane + q * 32);
+                        }
+                        ps_chunk(key, s, stop0, stop1, a.one);
+                    }
+                }
+                const int n0 = (int)((s.p0 - b0) / ROW), n1 = (int)((s.p1 - b1) / ROW);
+                const uint32_t T[2] = {__reduce_add_sync(ASR_FULL_MASK, s.c0), __reduce_add_sync(ASR_FULL_MASK, s.c1)};
+                const uint32_t in[2] = {__reduce_add_sync(ASR_FULL_MASK, (uint32_t)n0),
+                                        __reduce_add_sync(ASR_FULL_MASK, (uint32_t)n1)};
+                const uint32_t ov = __reduce_or_sync(ASR_FULL_MASK, s.over);
+                __syncwarp();
 #ifdef PCT_STATS
-                if (tid == 0) atomicAdd(&g_pct_stats[2], 1ull);
+                if (lane == 0) atomicAdd(&g_pct_stats[2], 1ull);
 #endif
                 bool ok = true;
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
-                    const uint32_t c = T[t] & 0xFFFFu, in = T[t] >> 16, hi = pf_end(wlo[t], wsh[t]);
-                    if (k[t] > c) {   // above the window (exact even when a thread ran out of slots)
+                    const uint32_t hi = ps_end(wlo[t], wsh[t]);
+                    if (k[t] > T[t]) {   // above the window (exact even when a lane ran out of slots)
                         ok = false;
-                        if (hi == 0xFFFFFFFFu) attempt = PF_TRIES;   // nothing above: keys of 2^32-1, radix path
-                        wlo[t] = hi;
-                        wsh[t] += wsh[t] < PF_MAX_SHIFT ? 1 : 0;
+#ifdef PCT_STATS
+                        if (lane == 0) atomicAdd(&g_pct_stats[3], 1ull);
+#endif
+                        if (hi == 0xFFFFFFFFu) attempt = PS_TRIES;   // nothing above: keys of 2^32-1, radix path
+                        const uint32_t e = k[t] - T[t];   // keys between the window's end and the rank
+                        if (in[t] >= 16u && e <= 2u * in[t]) {
+                            // near: a window of the same width centred where the window's density puts the rank
+                            const uint32_t W = (uint32_t)PS_WIN << wsh[t];
+                            const uint32_t c = hi + (uint32_t)(((uint64_t)e * W) / in[t]);
+                            wlo[t] = c < hi ? 0xFFFFFFFFu - W : c - (W >> 1);
+                        } else {
+                            wlo[t] = hi;
+                            wsh[t] += wsh[t] < PS_MAX_SHIFT ? 1 : 0;
+                        }
                     } else if ((ov >> t) & 1u) {   // too dense for the slots: the upper half, then look again
                         ok = false;
-                        if (wsh[t] == 0) attempt = PF_TRIES;
+#ifdef PCT_STATS
+                        if (lane == 0) atomicAdd(&g_pct_stats[4], 1ull);
+#endif
+                        if (wsh[t] == 0) attempt = PS_TRIES;
                         else {
                             --wsh[t];
-                            wlo[t] = hi - ((uint32_t)PF_BINS << wsh[t]);
+                            wlo[t] = hi - ((uint32_t)PS_WIN << wsh[t]);
                         }
-                    } else if (k[t] <= c - in) {   // below the window
+                    } else if (k[t] <= T[t] - in[t]) {   // below the window
                         ok = false;
-                        wsh[t] += wsh[t] < PF_MAX_SHIFT ? 1 : 0;
-                        const uint32_t W = (uint32_t)PF_BINS << wsh[t];
-                        wlo[t] = wlo[t] > W ? wlo[t] - W : 0u;
+#ifdef PCT_STATS
+                        if (lane == 0) atomicAdd(&g_pct_stats[6], 1ull);
+#endif
+                        const uint32_t e = T[t] - in[t] - k[t] + 1u;   // keys between the rank and the window's start
+                        if (in[t] >= 16u && e <= 2u * in[t]) {
+                            const uint32_t W = (uint32_t)PS_WIN << wsh[t];
+                            const uint32_t back = (uint32_t)(((uint64_t)e * W) / in[t]) + (W >> 1);
+                            wlo[t] = wlo[t] > back ? wlo[t] - back : 0u;
+                        } else {
+                            wsh[t] += wsh[t] < PS_MAX_SHIFT ? 1 : 0;
+                            const uint32_t W = (uint32_t)PS_WIN << wsh[t];
+                            wlo[t] = wlo[t] > W ? wlo[t] - W : 0u;
+                        }
                     }
                 }
-                if (ok) break;
-                if (attempt >= PF_TRIES - 1) {
+                if (ok) {
+#ifdef PCT_STATS
+                    if (lane == 0) {
+                        atomicAdd(&g_pct_stats[1], 1ull);
+                        atomicAdd(&g_pct_stats[5], (unsigned long long)(in[0] + in[1]));
+                    }
+#endif
+                    res[0] = ps_resolve(sm, 0, n0, wlo[0], wsh[0], k[0] - (T[0] - in[0]));
+                    res[1] = ps_resolve(sm, 1, n1, wlo[1], wsh[1], k[1] - (T[1] - in[1]));
+                    // the next segment's windows: centred on these answers, as wide as keeps the slots comfortably filled
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        if (in[t] > PS_IN_MANY) wsh[t] -= wsh[t] > 0 ? 1 : 0;
+                        else if (in[t] < PS_IN_FEW) wsh[t] += wsh[t] < PS_MAX_SHIFT ? 1 : 0;
+                        const uint32_t half = (uint32_t)PS_WIN << wsh[t] >> 1;
+                        wlo[t] = res[t] > half ? res[t] - half : 0u;
+                    }
+                    break;
+                }
+                if (attempt >= PS_TRIES - 1) {
                     settled = false;
                     break;
                 }
             }
-            if (settled) {
-                const int sh0 = wsh[0], sh1 = wsh[1];
-                const uint32_t lo0 = wlo[0], lo1 = wlo[1];
-                const uint32_t in0 = T[0] >> 16, in1 = T[1] >> 16;
-                const uint32_t below0 = (T[0] & 0xFFFFu) - in0, below1 = (T[1] & 0xFFFFu) - in1;
-                // level 1: bins of 2^sh values over the window
-                const int nm = n[0] > n[1] ? n[0] : n[1];
-#pragma unroll
-                for (int e = 0; e < PF_STRAIGHT; ++e) {   // (a slot past the thread's count holds a stale key: never counted)
-                    pf_inc_if(fs.hist[0][0], (fs.slot[0][e][tid] - lo0) >> sh0, e < n[0]);
-                    pf_inc_if(fs.hist[0][1], (fs.slot[1][e][tid] - lo1) >> sh1, e < n[1]);
-                }
-                for (int e = PF_STRAIGHT; e < nm; ++e) {
-                    if (e < n[0]) atomicAdd(&fs.hist[0][0][(fs.slot[0][e][tid] - lo0) >> sh0], 1u);
-                    if (e < n[1]) atomicAdd(&fs.hist[0][1][(fs.slot[1][e][tid] - lo1) >> sh1], 1u);
-                }
-                __syncthreads();
-                const int tg = tid / PF_HALF, j = tid % PF_HALF;
-                const uint32_t kw = tg == 0 ? k[0] - below0 : k[1] - below1;   // rank inside the window
-                uint32_t c[8], tot, incl;
-                pf_scan_a(fs.hist[0][tg], j, c, tot, incl, fs.wsum[tg]);
-                __syncthreads();
-                pf_scan_b(c, tot, incl, fs.wsum[tg], j, kw, &fs.sel_bin[0][tg], &fs.sel_rem[0][tg], &fs.sel_cnt[tg]);
-                __syncthreads();
-                const uint32_t bin0 = fs.sel_bin[0][0], bin1 = fs.sel_bin[0][1];
-                uint32_t r0 = lo0 + (bin0 << sh0), r1 = lo1 + (bin1 << sh1);
-                if (sh0 > 0 || sh1 > 0) {
-                    // level 2: the keys of the selected bin
-                    const int m0 = sh0 > 0 ? n[0] : 0, m1 = sh1 > 0 ? n[1] : 0, mm = m0 > m1 ? m0 : m1;
-                    const uint32_t cnt0 = sh0 > 0 ? fs.sel_cnt[0] : 0u, cnt1 = sh1 > 0 ? fs.sel_cnt[1] : 0u;
-                    if (cnt0 <= 32u && cnt1 <= 32u) {
-                        // a handful: listed, and ranked by one warp per rank (any order of equal keys gives the same
-                        // value at every rank)
-                        for (int e = 0; e < mm; ++e) {
-                            if (e < m0) {
-                                const uint32_t dd = fs.slot[0][e][tid] - lo0;
-                                if ((dd >> sh0) == bin0) fs.list[0][atomicAdd(&fs.lcnt[0], 1u)] = dd & ((1u << sh0) - 1u);
-                            }
-                            if (e < m1) {
-                                const uint32_t dd = fs.slot[1][e][tid] - lo1;
-                                if ((dd >> sh1) == bin1) fs.list[1][atomicAdd(&fs.lcnt[1], 1u)] = dd & ((1u << sh1) - 1u);
-                            }
-                        }
-                        __syncthreads();
-                        if (tid < 64) {
-                            const int t = tid >> 5, lane = tid & 31;
-                            const uint32_t cn = t == 0 ? cnt0 : cnt1;
-                            const uint32_t v = (uint32_t)lane < cn ? fs.list[t][lane] : 0xFFFFFFFFu;
-                            uint32_t rank = 0;
-                            for (uint32_t q = 0; q < cn; ++q) {
-                                const uint32_t u = __shfl_sync(ASR_FULL_MASK, v, (int)q);
-                                rank += (u < v || (u == v && q < (uint32_t)lane)) ? 1u : 0u;
-                            }
-                            if ((uint32_t)lane < cn && rank + 1u == fs.sel_rem[0][t]) fs.sel_bin[1][t] = v;
-                        }
-                        __syncthreads();
-                    } else {
-                        // many equal or near-equal keys: a second histogram, one value per bin
-                        {
-                            uint4 *z = reinterpret_cast<uint4 *>(&fs.hist[1][0][0]);
-                            constexpr int n16 = 2 * PF_BINS / 4;
-#pragma unroll
-                            for (int q = 0; q < n16 / PCT_THREADS; ++q) z[q * PCT_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
-                        }
-                        __syncthreads();
-                        for (int e = 0; e < mm; ++e) {
-                            if (e < m0) {
-                                const uint32_t dd = fs.slot[0][e][tid] - lo0;
-                                if ((dd >> sh0) == bin0) atomicAdd(&fs.hist[1][0][dd & ((1u << sh0) - 1u)], 1u);
-                            }
-                            if (e < m1) {
-                                const uint32_t dd = fs.slot[1][e][tid] - lo1;
-                                if ((dd >> sh1) == bin1) atomicAdd(&fs.hist[1][1][dd & ((1u << sh1) - 1u)], 1u);
-                            }
-                        }
-                        __syncthreads();
-                        const bool act = tg == 0 ? sh0 > 0 : sh1 > 0;
-                        if (act) pf_scan_a(fs.hist[1][tg], j, c, tot, incl, fs.wsum[tg]);
-                        __syncthreads();
-                        if (act) pf_scan_b(c, tot, incl, fs.wsum[tg], j, fs.sel_rem[0][tg], &fs.sel_bin[1][tg], &fs.sel_rem[1][tg]);
-                        __syncthreads();
-                    }
-                    if (sh0 > 0) r0 += fs.sel_bin[1][0];
-                    if (sh1 > 0) r1 += fs.sel_bin[1][1];
-                }
-                res[0] = r0;
-                res[1] = r1;
-                // the next segment's windows: centred on these answers, as wide as keeps the slots comfortably filled
-                const uint32_t inw[2] = {in0, in1};
-#pragma unroll
-                for (int t = 0; t < 2; ++t) {
-                    if (inw[t] > PF_IN_MANY) wsh[t] -= wsh[t] > 0 ? 1 : 0;
-                    else if (inw[t] < PF_IN_FEW) wsh[t] += wsh[t] < PF_MAX_SHIFT ? 1 : 0;
-                    const uint32_t half = (uint32_t)PF_BINS << wsh[t] >> 1;
-                    wlo[t] = res[t] > half ? res[t] - half : 0u;
-                }
-#ifdef PCT_STATS
-                if (tid == 0) {
-                    atomicAdd(&g_pct_stats[1], 1ull);
-                    atomicAdd(&g_pct_stats[5], (unsigned long long)(in0 + in1));
-                }
-#endif
-            }
-            __syncthreads();   // the next segment rewrites slots, totals and histograms
         }
-#ifdef PCT_STATS
-        if (tid == 0) atomicAdd(&g_pct_stats[0], 1ull);
-#endif
-        if (tid == 0) {
+        if (lane == 0) {
+            asr_summary_t *s = a.out_summary + d.r;
             if (settled) {
-                if (blockIdx.y == 0) {
-                    out_summary[r].p50_e2e_us = (int64_t)res[0];
-                    out_summary[r].p90_e2e_us = (int64_t)res[1];
+                if (d.y == 0) {
+                    s->p50_e2e_us = (int64_t)res[0];
+                    s->p90_e2e_us = (int64_t)res[1];
                 } else {
-                    out_summary[r].p50_ttft_us = (int64_t)res[0];
-                    out_summary[r].p90_ttft_us = (int64_t)res[1];
+                    s->p50_ttft_us = (int64_t)res[0];
+                    s->p90_ttft_us = (int64_t)res[1];
                 }
             } else {
-                my_miss[atomicAdd(miss_count + blockIdx.y, 1)] = r;
-#ifdef PCT_STATS
-                atomicAdd(&g_pct_stats[4], 1ull);
-#endif
+                a.miss_list[(size_t)d.y * a.n_replicas + atomicAdd(a.miss_count + d.y, 1)] = d.r;
             }
         }
     }
+    __syncwarp();
+  }
 }
 
 __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) percentiles_kernel(const int64_t *values, const int64_t *seg_off,
@@ -1012,7 +953,6 @@ __global__ void __launch_bounds__(PCT_THREADS, PCT_MIN_CTAS) summary_percentiles
 }
 
 static constexpr size_t PCT_DYN_SMEM = sizeof(PctRegSmem);
-static constexpr size_t PF_DYN_SMEM = sizeof(PctFastSmem);
 
 static int pct_grid(int n_units, const void *fn, size_t smem = PCT_DYN_SMEM) {
     const int n_sm = sm_count();
@@ -1043,41 +983,53 @@ int launch_percentiles(const int64_t *values, const int64_t *seg_off, int32_t n_
 // radix kernel on what it left.  Otherwise the radix kernel on every replica.
 int launch_summary_percentiles(const asr_replica_t *replicas, int32_t n_replicas, const int64_t *lat,
                                const int64_t *ttft, asr_summary_t *out_summary, bool fmt_flags, const int32_t *order,
-                               int32_t *miss_list, int32_t *miss_count, cudaStream_t st) {
+                               int32_t *miss_list, int32_t *miss_count, int32_t *scratch, cudaStream_t st) {
     if (n_replicas <= 0) return ASR_OK;
     cudaFuncSetAttribute(summary_percentiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PCT_DYN_SMEM);
     int gx = pct_grid(n_replicas, (const void *)summary_percentiles_kernel);
     gx = gx > 1 ? (gx + 1) / 2 : 1;
-    const bool fast = fmt_flags && miss_list && miss_count && PCT_THREADS == 256;
-    if (fast) {
-        cudaFuncSetAttribute(summary_fast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PF_DYN_SMEM);
-        int fx = pct_grid(n_replicas, (const void *)summary_fast_kernel, PF_DYN_SMEM);
-        fx = fx > 1 ? (fx + 1) / 2 : 1;
-        // every CTA walks one run of consecutive segments
-        const int chunk = (n_replicas + fx - 1) / fx;
-        fx = (n_replicas + chunk - 1) / chunk;
+    const bool stream = fmt_flags && miss_list && miss_count && scratch;
+    if (stream) {
+        // seeds (radix kernel on the seed list), then one warp per segment; what is left goes to the miss list
+        const int grid = sm_count();
+        const int64_t total = 2 * (int64_t)n_replicas, run = PS_RUN;
+        const int n_runs = (int)((total + run - 1) / run);
+        PsArgs pa{replicas, lat, ttft, out_summary, order, miss_list, miss_count,
+                  scratch + 64, scratch, scratch + 64 + 2 * (size_t)n_replicas, scratch + 2, n_replicas, (int32_t)run, n_runs, 1u};
+        {
+            KernelTimer kt(KID_SUMMARY_PCT, st);
+            summary_seed_kernel<<<1, 1024, 0, st>>>(pa);
+            summary_percentiles_kernel<<<dim3(gx, 2), PCT_THREADS, PCT_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary,
+                                                                                       true, pa.seed_list, pa.seed_count);
+        }
+        int rc = check_launch("summary_percentiles_kernel (seeds)");
+        if (rc) return rc;
+        cudaFuncSetAttribute(summary_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PS_SMEM_BYTES);
         {
             KernelTimer kt(KID_SUMMARY_FAST, st);
-            summary_fast_kernel<<<dim3(fx, 2), PCT_THREADS, PF_DYN_SMEM, st>>>(replicas, n_replicas, lat, ttft, out_summary,
-                                                                               order, chunk, miss_list, miss_count);
+            const int want = (n_runs + PS_WARPS - 1) / PS_WARPS;
+            summary_stream_kernel<<<want < grid ? want : grid, PS_WARPS * 32, PS_SMEM_BYTES, st>>>(pa);
         }
-        int rc = check_launch("summary_fast_kernel");
+        rc = check_launch("summary_stream_kernel");
         if (rc) return rc;
 #ifdef PCT_STATS
         {
-            unsigned long long h[8], z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            int32_t h[4];
             cudaStreamSynchronize(st);
-            cudaMemcpyFromSymbol(h, g_pct_stats, sizeof(h));
+            cudaMemcpy(h, pa.seed_count, 8, cudaMemcpyDeviceToHost);
+            cudaMemcpy(h + 2, miss_count, 8, cudaMemcpyDeviceToHost);
+            unsigned long long g[8], z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            cudaMemcpyFromSymbol(g, g_pct_stats, sizeof(g));
             cudaMemcpyToSymbol(g_pct_stats, z, sizeof(z));
-            fprintf(stderr, "pct stats: segments %llu settled %llu passes %llu bootstraps %llu misses %llu in-window/settled %.0f\n",
-                    h[0], h[1], h[2], h[3], h[4], h[1] ? (double)h[5] / (double)h[1] : 0.0);
+            fprintf(stderr, "stream stats: runs %d x %d items, seeds %d + %d, misses %d + %d, passes %llu settled %llu in-window/settled %.0f above %llu dense %llu below %llu\n",
+                    n_runs, (int)run, h[0], h[1], h[2], h[3], g[2], g[1], g[1] ? (double)g[5] / (double)g[1] : 0.0, g[3], g[4], g[6]);
         }
 #endif
     }
     {
         KernelTimer kt(KID_SUMMARY_PCT, st);
         summary_percentiles_kernel<<<dim3(gx, 2), PCT_THREADS, PCT_DYN_SMEM, st>>>(
-            replicas, n_replicas, lat, ttft, out_summary, fmt_flags, fast ? miss_list : nullptr, fast ? miss_count : nullptr);
+            replicas, n_replicas, lat, ttft, out_summary, fmt_flags, stream ? miss_list : nullptr, stream ? miss_count : nullptr);
     }
     return check_launch("summary_percentiles_kernel");
 }
