@@ -752,6 +752,10 @@ __global__ void __launch_bounds__(PS_WARPS * 32, 1) summary_stream_kernel(PsArgs
             const uint32_t N = (uint32_t)d.N;
             const uint32_t k[2] = {(uint32_t)((50ull * N + 99ull) / 100ull), (uint32_t)((90ull * N + 99ull) / 100ull)};
             const int n4 = d.N >> 2, nch = (d.N + PS_CHUNK - 1) / PS_CHUNK;
+            // the rest of the segment into L2 while its first chunk is on the way: a reading is ten 4 KB loads one
+            // behind the other, and nine of them then come from L2 (1.97 -> 1.87 ms on config 3)
+            if (lane == 0 && d.N > PS_CHUNK)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(d.base + PS_CHUNK), "r"((uint32_t)(d.N - PS_CHUNK) * 4u) : "memory");
             for (int attempt = 0;; ++attempt) {
                 PsPass s;
                 s.c0 = s.c1 = 0;
