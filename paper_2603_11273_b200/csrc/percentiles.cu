@@ -479,20 +479,20 @@ __device__ unsigned long long g_pct_stats[8];   // -, settled, passes, above, de
 // summary_stream_kernel: p50/p90 of the uint32 segments of a summary-only sweep, one WARP per segment.
 //
 // Consecutive segments of a sweep are alike (the same trace under another policy, the neighbouring seed), so the
-// two ranks of a segment are looked for in windows of values around the answers of the segment before (round 2
-// first did this with one CTA per segment: 8 barriers and two block scans per segment made the fixed work 60 % of
-// its instructions).  Here a warp walks a run of consecutive work
-// items (segment = one value stream of one replica, in the plan's order) and streams each segment ONCE through its
-// registers, 4 KB at a time with the next 4 KB's loads in flight (a cp.async.bulk ring in shared memory as in
-// select_topk_kernel was measured too: 13 warps per SM fit beside it and run in 2.1 ms, 19 warps without it in
-// 1.96 ms -- the kernel is bound by the latency of its own instruction chains, so warps count for more).
-// Per key and rank: count below the window's end, append to the lane's private slots if inside the window (ten
-// PTX instructions per key for both ranks).  The window is then resolved by a 32-bin radix descent over the ~100 collected keys
-// and a one-warp ranking of the last bin's keys: warp shuffles only, no block barrier anywhere.  A rank outside
-// the window moves and doubles it, a lane that runs out of slots halves it, and the segment is read again
-// (straight from L2); what is not settled after PS_TRIES passes, or has another format, goes to the miss list for
-// summary_percentiles_kernel.  The first streamable segment of every run (the "seed") is computed by that kernel
-// beforehand: its two answers and their distance give the run its first windows.  No result depends on a guess.
+// two ranks of a segment are looked for in windows of values around the answers of the segment before.  (Round 2
+// first did this with one CTA per segment: eight barriers and two block scans per segment made the fixed work
+// 60 % of its instructions.)  A warp takes a run of consecutive work items -- a work item is one value stream of one
+// replica, in the plan's order -- and streams each segment ONCE through its registers, 4 KB at a time with the next
+// 4 KB's loads in flight and the rest of the segment prefetched into L2.  (A cp.async.bulk ring in shared memory
+// as in select_topk_kernel was measured too: 13 warps per SM fit beside it and run in 2.1 ms, 19 warps without it
+// in 1.96 ms.)  Per key and rank: count below the window's end, append to the lane's private slots if inside the
+// window -- ten PTX instructions per key for both ranks.  The window is then resolved by a radix descent with 32
+// bins over the ~150 collected keys and a one-warp ranking of the last bin's keys: warp shuffles only, no block
+// barrier anywhere.  A rank just outside the window re-centres it, a rank far outside moves and doubles it, a lane
+// that runs out of slots halves it, and the segment is read again (mostly from L2); what is not settled after
+// PS_TRIES passes, or has another format, goes to the miss list for summary_percentiles_kernel.  The first
+// streamable item of every PS_SEED_EVERY runs (the "seed") is computed by that kernel beforehand: its two answers
+// and their distance give the runs their first windows.  No result depends on a guess.
 // ---------------------------------------------------------------------------
 #ifndef PS_WARPS_N
 #define PS_WARPS_N 19
