@@ -235,11 +235,11 @@ def test_cost_models_mixed_in_one_batch(asr):
 
 def test_stream_percentiles_on_long_and_ragged_segments(asr):
     """summary_stream_kernel (one warp per value stream) on segments longer than the register-resident
-    radix path takes (12,000 / 30,004 values: 12 and 30 chunks of 1,024 keys, ragged last chunks), a length that
+    radix path takes (12,000 / 30,004 / 70,000 values: 12 to 69 chunks of 1,024 keys, ragged last chunks), a length that
     is not a multiple of four (radix path through the miss list) and short ones, enough replicas for several runs of
     24 work items with shared seeds"""
     specs = [("lognormal", 12000, 1.0), ("uniform", 30004, 2.0), ("lognormal", 30002, 0.7), ("six", 12000, 0.5),
-             ("lognormal", 2500, 3.0), ("uniform", 1028, 1.0)]
+             ("lognormal", 2500, 3.0), ("uniform", 1028, 1.0), ("lognormal", 70000, 1.5)]
     traces = [wl.stress_trace(k, n, 800 + i, rate_per_s=r) for i, (k, n, r) in enumerate(specs)]
     reps = [(t, p, s) for _ in range(12) for t in range(len(traces)) for p in POL for s in (16, 32)]
     _, _, S = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
