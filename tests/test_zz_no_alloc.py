@@ -43,7 +43,8 @@ def test_select_static_equals_select_on_calls_in_a_row(asr):
             for kk in (k, 200):
                 asr.select_static(dq[(kind, n)], n, policy, NOW, kk, out[kk])
                 torch.cuda.synchronize()
-                assert torch.cuda.mem_get_info()[0] == free0 and torch.cuda.memory_allocated() == alloc0
+                # (device allocations come in 2 MiB pages: anything allocated behind torch's back would show)
+                assert abs(torch.cuda.mem_get_info()[0] - free0) < (1 << 20) and torch.cuda.memory_allocated() == alloc0
                 got.append(((kind, n, policy, kk), out[kk].cpu().numpy().copy()))
     for key, g in got:
         assert np.array_equal(g, want[key]), key
