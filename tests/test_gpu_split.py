@@ -244,3 +244,21 @@ def test_stream_percentiles_on_long_and_ragged_segments(asr):
     reps = [(t, p, s) for _ in range(12) for t in range(len(traces)) for p in POL for s in (16, 32)]
     _, _, S = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
     _check_all(traces, reps, S, wl.CONFIG_COST, "long")
+
+
+def test_stream_percentiles_tiny_segments_and_high_bit_values(asr):
+    """(a) replicas of 4 ... 2,052 requests (segments shorter than a chunk of 1,024 keys, one key per lane or fewer) mixed
+    in one batch; (b) FCFS replicas whose latencies run up to 3.1e9 us in a busy period just short of 2^32 us: uint32 keys with the high bit set (p90 above
+    2^31, p50 below), several runs of them"""
+    rng = np.random.Generator(np.random.PCG64(321))
+    lens = [4, 8, 12, 100, 1000, 1024, 1028, 2048, 2052, 36]
+    traces = [wl.stress_trace("lognormal", n, 900 + i, rate_per_s=1.0 + 0.3 * (i % 4)) for i, n in enumerate(lens)]
+    reps = [(t, p, 32) for _ in range(6) for t in range(len(traces)) for p in POL]
+    _, _, S = run_batched(traces, reps, wl.CONFIG_COST, 32, summary_only=True)
+    _check_all(traces, reps, S, wl.CONFIG_COST, "tiny")
+    # (b) one request per second, ~16 s of service each, 4 slots: the last request waits 3,100 s
+    slow = [_trace(np.arange(1000, dtype=np.int64) * 1_000_000, rng.integers(20000, 30001, size=1000)) for _ in range(3)]
+    reps = [(t, orc.FCFS, 4) for _ in range(12) for t in range(len(slow))]
+    _, _, S = run_batched(slow, reps, wl.TOY_COST, 32, summary_only=True)
+    assert int(S[0]["p90_e2e_us"]) > 2**31 > int(S[0]["p50_e2e_us"]) > 0
+    _check_all(slow, reps, S, wl.TOY_COST, "high bit")
